@@ -1,0 +1,599 @@
+/*
+ * trimeg_oracle.c -- CPU ORACLE for the TRIMEG marker-push hot path.
+ *
+ * THIS FILE IS TEST INFRASTRUCTURE.  It is a plain, slow, fp64 restatement of
+ * what the path computes, written from the paper (/root/reference/PAPER.md,
+ * cited below as PAPER.md:<line>) and from the readings fixed in SURVEY.md
+ * §8(c) / DESIGN.md §3.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may call it.  It shares NO code,
+ * header, table or helper with the CUDA library (paper_2601_14301_b200/csrc);
+ * the only thing both consume is the seeded input generator
+ * (paper_2601_14301_b200/inputs.py), which holds no method arithmetic.
+ *
+ * Build: gcc -O2 -ffp-contract=off -fopenmp -shared -fPIC (see oracle/build.py).
+ * -ffp-contract=off is part of the definition of the locator (rule L2): every
+ * operation of inside() is individually rounded, in the order written here.
+ *
+ * Parity unpinned (defined by SURVEY.md, not by the paper): the form of the
+ * weight equation (G7) and the profile-gradient conventions (G10).  Everything
+ * else is pinned by tests/test_oracle_*.py against closed forms, invariants,
+ * finite differences and brute force.
+ *
+ * What is computed, in the paper's order (push kernel):
+ *   O1 mesh            ring x sector triangulation, local coordinates (xi, eta)
+ *                      with vertices at (0,0),(1,0),(0,1)
+ *   O2 Bell expansion  18 nodal DOFs (6 per vertex)  -> 21 monomial coefficients
+ *                      of the quintic
+ *   O3 locator         brute force and the O(1) candidate search
+ *                      with contains()
+ *   O4 gather (g2p)    dphi, d/dR, d/dZ, d/dphi at the marker PAPER.md:235, 604
+ *   O5 equilibrium     B = grad psi x grad phi + F grad phi PAPER.md:1156-1164
+ *   O6 RHS             A.4-A.6, A.10-A.17 (dA = 0), d ln f_M/dt
+ *                                                     PAPER.md:1204-1269
+ *   O7 RK4             classic 4-stage integrator
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_NCOEF 21
+#define ORC_TWO_PI 6.283185307179586476925286766559
+
+typedef struct {
+    double R0, a, B0, q0, q2;      /* circular equilibrium, q(r) = q0 + q2 (r/a)^2 */
+    double rho0, qs_over_ms;       /* rho_0, q_s/m_s               */
+    double T, kappa_n, kappa_T;    /* Tbar, log-gradients (1/length) */
+    int eom_variant;               /* 0 = b0* as printed (A.4-A.6); 1 = (B/B*par) b + ... (reading G2) */
+    int weight_mode;               /* 0: wdot = -(1-w) L ; 1: wdot = -L (reading G7) */
+} orc_params;
+
+typedef struct {
+    int n_r, n_theta, n_vert, n_tri;
+    double *r_nodes;               /* n_r + 1 */
+    double *Rv, *Zv;               /* n_vert  */
+    int *tri;                      /* [n_tri][3] vertex ids, counter-clockwise */
+    double *geom;                  /* [n_tri][6] R_v0, Z_v0, xi_R, xi_Z, eta_R, eta_Z */
+    double rin2;                   /* squared inscribed radius of the outer polygon */
+    orc_params p;
+    int n_modes;
+    int *mode_n;                   /* toroidal mode numbers n (Def. 19) */
+    double *coef;                  /* [n_tri][n_modes][21][2] (re, im) */
+} orc_ctx;
+
+/* ------------------------------------------------------------------ O1 mesh */
+static int vid(const orc_ctx *c, int i, int j)
+{ /* v(i,j) = 1 + (i-1) n_theta + (j mod n_theta), i = 1..n_r */
+    int jj = ((j % c->n_theta) + c->n_theta) % c->n_theta;
+    return 1 + (i - 1) * c->n_theta + jj;
+}
+
+orc_ctx *orc_create(int n_r, int n_theta, const double *r_nodes,
+                    const double *Rv, const double *Zv, const orc_params *p)
+{
+    if (n_r < 2 || n_theta < 3) return NULL;
+    orc_ctx *c = (orc_ctx *)calloc(1, sizeof(orc_ctx));
+    c->n_r = n_r; c->n_theta = n_theta;
+    c->n_vert = 1 + n_r * n_theta;
+    c->n_tri = (2 * n_r - 1) * n_theta;
+    c->p = *p;
+    c->r_nodes = (double *)malloc(sizeof(double) * (n_r + 1));
+    memcpy(c->r_nodes, r_nodes, sizeof(double) * (n_r + 1));
+    c->Rv = (double *)malloc(sizeof(double) * c->n_vert);
+    c->Zv = (double *)malloc(sizeof(double) * c->n_vert);
+    memcpy(c->Rv, Rv, sizeof(double) * c->n_vert);
+    memcpy(c->Zv, Zv, sizeof(double) * c->n_vert);
+    c->tri = (int *)malloc(sizeof(int) * 3 * c->n_tri);
+    c->geom = (double *)malloc(sizeof(double) * 6 * c->n_tri);
+    /* fan: t = j : (axis, v(1,j), v(1,j+1)) */
+    for (int j = 0; j < n_theta; ++j) {
+        int *t = c->tri + 3 * j;
+        t[0] = 0; t[1] = vid(c, 1, j); t[2] = vid(c, 1, j + 1);
+    }
+    /* rings i = 1..n_r-1, two triangles per ring-sector quad */
+    for (int i = 1; i <= n_r - 1; ++i)
+        for (int j = 0; j < n_theta; ++j) {
+            int base = n_theta + 2 * ((i - 1) * n_theta + j);
+            int *t0 = c->tri + 3 * base, *t1 = c->tri + 3 * (base + 1);
+            t0[0] = vid(c, i, j); t0[1] = vid(c, i + 1, j);     t0[2] = vid(c, i + 1, j + 1);
+            t1[0] = vid(c, i, j); t1[1] = vid(c, i + 1, j + 1); t1[2] = vid(c, i, j + 1);
+        }
+    /* local coordinates: vertices map to (xi,eta) = (0,0),(1,0),(0,1) */
+    for (int t = 0; t < c->n_tri; ++t) {
+        const int *v = c->tri + 3 * t;
+        double R0 = c->Rv[v[0]], Z0 = c->Zv[v[0]];
+        double e1R = c->Rv[v[1]] - R0, e1Z = c->Zv[v[1]] - Z0;
+        double e2R = c->Rv[v[2]] - R0, e2Z = c->Zv[v[2]] - Z0;
+        double D = e1R * e2Z - e2R * e1Z;
+        double *g = c->geom + 6 * t;
+        g[0] = R0; g[1] = Z0;
+        g[2] = e2Z / D;      /* xi_R  */
+        g[3] = -e2R / D;     /* xi_Z  */
+        g[4] = -e1Z / D;     /* eta_R */
+        g[5] = e1R / D;      /* eta_Z */
+    }
+    /* inscribed radius of the outer polygon = distance axis -> midpoint of an outer chord */
+    {
+        int va = vid(c, n_r, 0), vb = vid(c, n_r, 1);
+        double mx = 0.5 * (c->Rv[va] + c->Rv[vb]) - c->Rv[0];
+        double mz = 0.5 * (c->Zv[va] + c->Zv[vb]) - c->Zv[0];
+        c->rin2 = mx * mx + mz * mz;
+    }
+    return c;
+}
+
+void orc_destroy(orc_ctx *c)
+{
+    if (!c) return;
+    free(c->r_nodes); free(c->Rv); free(c->Zv); free(c->tri); free(c->geom);
+    free(c->mode_n); free(c->coef); free(c);
+}
+
+int orc_n_tri(const orc_ctx *c) { return c->n_tri; }
+int orc_n_vert(const orc_ctx *c) { return c->n_vert; }
+void orc_get_tri(const orc_ctx *c, int *out) { memcpy(out, c->tri, sizeof(int) * 3 * c->n_tri); }
+void orc_get_geom(const orc_ctx *c, double *out) { memcpy(out, c->geom, sizeof(double) * 6 * c->n_tri); }
+double orc_get_rin2(const orc_ctx *c) { return c->rin2; }
+void orc_set_params(orc_ctx *c, const orc_params *p) { c->p = *p; }
+
+void orc_set_modes(orc_ctx *c, int n_modes, const int *mode_n)
+{
+    free(c->mode_n); free(c->coef);
+    c->n_modes = n_modes;
+    c->mode_n = (int *)malloc(sizeof(int) * (n_modes > 0 ? n_modes : 1));
+    if (n_modes > 0) memcpy(c->mode_n, mode_n, sizeof(int) * n_modes);
+    c->coef = (double *)calloc((size_t)c->n_tri * (n_modes > 0 ? n_modes : 1) * ORC_NCOEF * 2, sizeof(double));
+}
+void orc_set_coef(orc_ctx *c, const double *coef)
+{ memcpy(c->coef, coef, sizeof(double) * (size_t)c->n_tri * c->n_modes * ORC_NCOEF * 2); }
+void orc_get_coef(const orc_ctx *c, double *coef)
+{ memcpy(coef, c->coef, sizeof(double) * (size_t)c->n_tri * c->n_modes * ORC_NCOEF * 2); }
+
+/* ------------------------------------------------- O2 Bell reduced quintic */
+/* monomial order, degree-major: k = 0..20 <-> (i,j): for d = 0..5, for j = 0..d: (d-j, j) */
+static void mono_ij(int k, int *i, int *j)
+{
+    int d = 0, kk = k;
+    while (kk > d) { kk -= d + 1; ++d; }
+    *j = kk; *i = d - kk;
+}
+static long double ipowl(long double x, int n) { long double r = 1.0L; while (n-- > 0) r *= x; return r; }
+static double ipow(double x, int n) { double r = 1.0; while (n-- > 0) r *= x; return r; }
+static int falling(int i, int a) { int r = 1; for (int q = 0; q < a; ++q) r *= (i - q); return r; }
+/* d^a/dxi^a d^b/deta^b of xi^i eta^j at (xi,eta); 0^0 = 1 */
+static long double mono_derivl(int i, int j, int a, int b, long double xi, long double eta)
+{
+    if (a > i || b > j) return 0.0L;
+    return (long double)falling(i, a) * ipowl(xi, i - a) * (long double)falling(j, b) * ipowl(eta, j - b);
+}
+
+/* Build the 21x21 matrix of one triangle (rows 1-18: six DOFs of PAPER.md:350-353 at the
+ * three vertices; rows 19-21: the quartic term of the normal derivative vanishes on each
+ * edge -- the textbook Bell reduction 21 -> 18, reading O2), row-equilibrate, LU-factor with
+ * partial pivoting in long double. */
+static int bell_factor(const orc_ctx *c, int t, long double A[21][21], long double rowscale[21], int piv[21])
+{
+    const double *g = c->geom + 6 * t;
+    const int *v = c->tri + 3 * t;
+    long double xR = g[2], xZ = g[3], eR = g[4], eZ = g[5];
+    static const long double vx[3] = {0.0L, 1.0L, 0.0L}, ve[3] = {0.0L, 0.0L, 1.0L};
+    for (int pnt = 0; pnt < 3; ++pnt)
+        for (int k = 0; k < 21; ++k) {
+            int i, j; mono_ij(k, &i, &j);
+            long double P   = mono_derivl(i, j, 0, 0, vx[pnt], ve[pnt]);
+            long double Px  = mono_derivl(i, j, 1, 0, vx[pnt], ve[pnt]);
+            long double Pe  = mono_derivl(i, j, 0, 1, vx[pnt], ve[pnt]);
+            long double Pxx = mono_derivl(i, j, 2, 0, vx[pnt], ve[pnt]);
+            long double Pxe = mono_derivl(i, j, 1, 1, vx[pnt], ve[pnt]);
+            long double Pee = mono_derivl(i, j, 0, 2, vx[pnt], ve[pnt]);
+            A[6 * pnt + 0][k] = P;                                              /* f    */
+            A[6 * pnt + 1][k] = xR * Px + eR * Pe;                              /* f_R  */
+            A[6 * pnt + 2][k] = xZ * Px + eZ * Pe;                              /* f_Z  */
+            A[6 * pnt + 3][k] = xR * xR * Pxx + 2.0L * xR * eR * Pxe + eR * eR * Pee;            /* f_RR */
+            A[6 * pnt + 4][k] = xR * xZ * Pxx + (xR * eZ + xZ * eR) * Pxe + eR * eZ * Pee;       /* f_RZ */
+            A[6 * pnt + 5][k] = xZ * xZ * Pxx + 2.0L * xZ * eZ * Pxe + eZ * eZ * Pee;            /* f_ZZ */
+        }
+    /* edges a->b with reference direction (dxi, deta) */
+    static const int ea[3] = {0, 0, 1}, eb[3] = {1, 2, 2};
+    static const long double dxi[3] = {1.0L, 0.0L, -1.0L}, det[3] = {0.0L, 1.0L, 1.0L};
+    for (int e = 0; e < 3; ++e) {
+        long double tR = (long double)c->Rv[v[eb[e]]] - (long double)c->Rv[v[ea[e]]];
+        long double tZ = (long double)c->Zv[v[eb[e]]] - (long double)c->Zv[v[ea[e]]];
+        long double nR = tZ, nZ = -tR;                    /* unnormalised normal */
+        long double alpha = nR * xR + nZ * xZ, beta = nR * eR + nZ * eZ;
+        for (int k = 0; k < 21; ++k) {
+            int i, j; mono_ij(k, &i, &j);
+            long double val = 0.0L;
+            if (i + j == 5) {
+                if (i >= 1) val += alpha * i * ipowl(dxi[e], i - 1) * ipowl(det[e], j);
+                if (j >= 1) val += beta * j * ipowl(dxi[e], i) * ipowl(det[e], j - 1);
+            }
+            A[18 + e][k] = val;
+        }
+    }
+    for (int r = 0; r < 21; ++r) {
+        long double m = 0.0L;
+        for (int k = 0; k < 21; ++k) { long double a = fabsl(A[r][k]); if (a > m) m = a; }
+        if (m == 0.0L) return -1;
+        rowscale[r] = 1.0L / m;
+        for (int k = 0; k < 21; ++k) A[r][k] *= rowscale[r];
+    }
+    for (int k = 0; k < 21; ++k) {
+        int pr = k; long double best = fabsl(A[k][k]);
+        for (int r = k + 1; r < 21; ++r) if (fabsl(A[r][k]) > best) { best = fabsl(A[r][k]); pr = r; }
+        if (best == 0.0L) return -1;
+        piv[k] = pr;
+        if (pr != k) for (int q = 0; q < 21; ++q) { long double tmp = A[k][q]; A[k][q] = A[pr][q]; A[pr][q] = tmp; }
+        for (int r = k + 1; r < 21; ++r) {
+            long double f = A[r][k] / A[k][k];
+            A[r][k] = f;
+            for (int q = k + 1; q < 21; ++q) A[r][q] -= f * A[k][q];
+        }
+    }
+    return 0;
+}
+static void bell_solve(long double A[21][21], const long double rowscale[21], const int piv[21], long double b[21])
+{
+    for (int r = 0; r < 21; ++r) b[r] *= rowscale[r];
+    /* whole rows (multipliers included) were swapped while factoring: permute b first */
+    for (int k = 0; k < 21; ++k)
+        if (piv[k] != k) { long double tmp = b[k]; b[k] = b[piv[k]]; b[piv[k]] = tmp; }
+    for (int k = 0; k < 21; ++k)
+        for (int r = k + 1; r < 21; ++r) b[r] -= A[r][k] * b[k];
+    for (int k = 20; k >= 0; --k) {
+        for (int q = k + 1; q < 21; ++q) b[k] -= A[k][q] * b[q];
+        b[k] /= A[k][k];
+    }
+}
+
+/* dofs: [n_modes][n_vert][6][2] (re,im) in the order f, f_R, f_Z, f_RR, f_RZ, f_ZZ */
+int orc_bell_from_dofs(orc_ctx *c, const double *dofs)
+{
+    int bad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : bad)
+    for (int t = 0; t < c->n_tri; ++t) {
+        long double A[21][21], rs[21]; int piv[21];
+        if (bell_factor(c, t, A, rs, piv)) { bad += 1; continue; }
+        const int *v = c->tri + 3 * t;
+        for (int m = 0; m < c->n_modes; ++m)
+            for (int part = 0; part < 2; ++part) {
+                long double b[21];
+                for (int pnt = 0; pnt < 3; ++pnt)
+                    for (int d = 0; d < 6; ++d)
+                        b[6 * pnt + d] = dofs[(((size_t)m * c->n_vert + v[pnt]) * 6 + d) * 2 + part];
+                b[18] = b[19] = b[20] = 0.0L;
+                bell_solve(A, rs, piv, b);
+                double *out = c->coef + (((size_t)t * c->n_modes + m) * ORC_NCOEF) * 2;
+                for (int k = 0; k < 21; ++k) out[2 * k + part] = (double)b[k];
+            }
+    }
+    return bad ? -1 : 0;
+}
+
+/* --------------------------------------------------------------- O3 locator */
+/* contains(): barycentric test, every operation individually rounded (rule L2). */
+static int inside(const orc_ctx *c, int t, double R, double Z, double *xi, double *eta, double *lam0)
+{
+    const double *g = c->geom + 6 * t;
+    double dx = R - g[0], dz = Z - g[1];
+    double a = g[2] * dx, b = g[3] * dz;
+    *xi = a + b;
+    double cc = g[4] * dx, d = g[5] * dz;
+    *eta = cc + d;
+    double one_m_xi = 1.0 - *xi;
+    *lam0 = one_m_xi - *eta;
+    return (*xi >= 0.0) && (*eta >= 0.0) && (*lam0 >= 0.0);
+}
+static double min3(double a, double b, double c) { double m = a < b ? a : b; return m < c ? m : c; }
+
+/* plain definition: lowest t with inside(t); gap fallback as in SURVEY.md §8(c) O3 */
+static int locate_brute_one(const orc_ctx *c, double R, double Z)
+{
+    double xi, eta, l0;
+    for (int t = 0; t < c->n_tri; ++t)
+        if (inside(c, t, R, Z, &xi, &eta, &l0)) return t;
+    double x = R - c->Rv[0], z = Z - c->Zv[0];
+    double s = x * x + z * z;
+    if (s < c->rin2) {
+        int best = -1; double bm = -INFINITY;
+        for (int t = 0; t < c->n_tri; ++t) {
+            inside(c, t, R, Z, &xi, &eta, &l0);
+            double m = min3(xi, eta, l0);
+            if (m > bm) { bm = m; best = t; }
+        }
+        return best;
+    }
+    return -1;
+}
+
+/* O(1) version: (r, theta) ring/sector guess, 3x3 neighbourhood of cells (<= 18 triangles),
+ * same inside() and same lowest-t rule (rules L1-L4).  r and theta only choose candidates. */
+static int candidates(const orc_ctx *c, double R, double Z, int *cand)
+{
+    double x = R - c->Rv[0], z = Z - c->Zv[0];
+    double r = sqrt(x * x + z * z);
+    double th = atan2(z, x);
+    if (th < 0.0) th += ORC_TWO_PI;
+    int lo = 0, hi = c->n_r;               /* largest i with r_nodes[i] <= r */
+    while (hi - lo > 1) { int mid = (lo + hi) / 2; if (c->r_nodes[mid] <= r) lo = mid; else hi = mid; }
+    int i0 = lo; if (i0 > c->n_r - 1) i0 = c->n_r - 1;
+    double jf = floor(th * c->n_theta / ORC_TWO_PI);
+    if (!(jf >= 0.0 && jf < (double)c->n_theta)) jf = 0.0;   /* also catches NaN */
+    int j0 = (int)jf;
+    int n = 0;
+    for (int ii = i0 - 1; ii <= i0 + 1; ++ii) {
+        if (ii < 0 || ii > c->n_r - 1) continue;
+        for (int dj = -1; dj <= 1; ++dj) {
+            int jj = ((j0 + dj) % c->n_theta + c->n_theta) % c->n_theta;
+            if (ii == 0) cand[n++] = jj;
+            else { int base = c->n_theta + 2 * ((ii - 1) * c->n_theta + jj); cand[n++] = base; cand[n++] = base + 1; }
+        }
+    }
+    /* sort ascending (insertion sort) so that "lowest t" is the first hit */
+    for (int a = 1; a < n; ++a) { int v = cand[a], b = a - 1; while (b >= 0 && cand[b] > v) { cand[b + 1] = cand[b]; --b; } cand[b + 1] = v; }
+    return n;
+}
+static int locate_one(const orc_ctx *c, double R, double Z, double *xi_out, double *eta_out)
+{
+    int cand[18];
+    int n = candidates(c, R, Z, cand);
+    double xi, eta, l0;
+    for (int q = 0; q < n; ++q) {
+        if (q > 0 && cand[q] == cand[q - 1]) continue;
+        if (inside(c, cand[q], R, Z, &xi, &eta, &l0)) { if (xi_out) { *xi_out = xi; *eta_out = eta; } return cand[q]; }
+    }
+    double x = R - c->Rv[0], z = Z - c->Zv[0];
+    double s = x * x + z * z;
+    if (s < c->rin2) {
+        int best = -1; double bm = -INFINITY, bxi = 0, beta_ = 0;
+        for (int q = 0; q < n; ++q) {
+            inside(c, cand[q], R, Z, &xi, &eta, &l0);
+            double m = min3(xi, eta, l0);
+            if (m > bm) { bm = m; best = cand[q]; bxi = xi; beta_ = eta; }
+        }
+        if (xi_out) { *xi_out = bxi; *eta_out = beta_; }
+        return best;
+    }
+    return -1;
+}
+
+void orc_locate_brute(const orc_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell)
+{
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) cell[p] = locate_brute_one(c, R[p], Z[p]);
+}
+void orc_locate(const orc_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell)
+{
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) cell[p] = locate_one(c, R[p], Z[p], NULL, NULL);
+}
+/* (xi, eta, lambda0) of point p in triangle t -- test hook */
+void orc_bary(const orc_ctx *c, size_t n, const int32_t *t, const double *R, const double *Z, double *out)
+{
+    for (size_t p = 0; p < n; ++p) inside(c, t[p], R[p], Z[p], out + 3 * p, out + 3 * p + 1, out + 3 * p + 2);
+}
+
+/* ---------------------------------------------------------------- O4 gather */
+/* Naive monomial sums; E_n = cos(n phi) + i sin(n phi);
+ *   dphi        = sum_n Re(P_n E_n)
+ *   d/dR, d/dZ  = sum_n Re((xi_X dP/dxi + eta_X dP/deta) E_n)
+ *   d/dphi      = sum_n Re(i n P_n E_n)
+ * No factor 2 for n > 0; Im of the n = 0 mode is ignored (reading G15). */
+static void gather_one(const orc_ctx *c, int t, double xi, double eta, double phi, double out[4])
+{
+    const double *g = c->geom + 6 * t;
+    double f = 0.0, fR = 0.0, fZ = 0.0, fp = 0.0;
+    for (int m = 0; m < c->n_modes; ++m) {
+        const double *cf = c->coef + (((size_t)t * c->n_modes + m) * ORC_NCOEF) * 2;
+        double Pr = 0, Pi = 0, Pxr = 0, Pxi_ = 0, Per = 0, Pei = 0;
+        for (int k = 0; k < 21; ++k) {
+            int i, j; mono_ij(k, &i, &j);
+            double mono = ipow(xi, i) * ipow(eta, j);
+            double mx = (i >= 1) ? i * ipow(xi, i - 1) * ipow(eta, j) : 0.0;
+            double me = (j >= 1) ? j * ipow(xi, i) * ipow(eta, j - 1) : 0.0;
+            Pr += cf[2 * k] * mono;  Pi += cf[2 * k + 1] * mono;
+            Pxr += cf[2 * k] * mx;   Pxi_ += cf[2 * k + 1] * mx;
+            Per += cf[2 * k] * me;   Pei += cf[2 * k + 1] * me;
+        }
+        double nn = (double)c->mode_n[m];
+        double Er = cos(nn * phi), Ei = sin(nn * phi);
+        double PRr = g[2] * Pxr + g[4] * Per, PRi = g[2] * Pxi_ + g[4] * Pei;   /* dP/dR */
+        double PZr = g[3] * Pxr + g[5] * Per, PZi = g[3] * Pxi_ + g[5] * Pei;   /* dP/dZ */
+        f  += Pr * Er - Pi * Ei;
+        fR += PRr * Er - PRi * Ei;
+        fZ += PZr * Er - PZi * Ei;
+        fp += nn * (-Pi * Er - Pr * Ei);      /* Re(i n P E) */
+    }
+    out[0] = f; out[1] = fR; out[2] = fZ; out[3] = fp;
+}
+
+/* cell_out[p] = located triangle (or -1, outputs then 0) */
+void orc_gather(const orc_ctx *c, size_t n, const double *R, const double *Z, const double *phi,
+                int32_t *cell_out, double *f, double *fR, double *fZ, double *fphi)
+{
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) {
+        double xi, eta, o[4] = {0, 0, 0, 0};
+        int t = locate_one(c, R[p], Z[p], &xi, &eta);
+        if (t >= 0) gather_one(c, t, xi, eta, phi[p], o);
+        if (cell_out) cell_out[p] = t;
+        f[p] = o[0]; fR[p] = o[1]; fZ[p] = o[2]; if (fphi) fphi[p] = o[3];
+    }
+}
+
+/* ----------------------------------------------------------- O5 equilibrium */
+typedef struct {
+    double B, BR, BZ, Bphi, bR, bZ, bphi, dBdR, dBdZ;
+    double dbR_dZ, dbZ_dR, dbphi_dR, dbphi_dZ, psi;
+} orc_eq;
+
+/* B = grad psi x grad phi + F grad phi; B_R = -psi_Z/R, B_Z = psi_R/R,
+ * B_phi = F/R with psi'(r) = B0 r/q(r) (reading G11), F = B0 R0. */
+static void equilibrium(const orc_params *p, double R, double Z, orc_eq *e)
+{
+    double x = R - p->R0;
+    double s = x * x + Z * Z;
+    double a2 = p->a * p->a;
+    double qs = p->q2 / a2;                         /* d qbar / d s */
+    double qb = p->q0 + qs * s;
+    double g = p->R0 * p->R0 + s / (qb * qb);
+    double gs = 1.0 / (qb * qb) - 2.0 * s * qs / (qb * qb * qb);
+    double sg = sqrt(g);
+    double h = 1.0 / (qb * sg);
+    double hs = -qs / (qb * qb * sg) - gs / (2.0 * qb * g * sg);
+    e->B = p->B0 * sg / R;
+    e->BR = -p->B0 * Z / (R * qb);
+    e->BZ = p->B0 * x / (R * qb);
+    e->Bphi = p->B0 * p->R0 / R;
+    e->bR = -Z * h; e->bZ = x * h; e->bphi = p->R0 / sg;
+    e->dBdR = p->B0 * (gs * x / (sg * R) - sg / (R * R));
+    e->dBdZ = p->B0 * gs * Z / (sg * R);
+    e->dbR_dZ = -h - 2.0 * Z * Z * hs;
+    e->dbZ_dR = h + 2.0 * x * x * hs;
+    e->dbphi_dR = -p->R0 * gs * x / (g * sg);
+    e->dbphi_dZ = -p->R0 * gs * Z / (g * sg);
+    e->psi = (p->q2 != 0.0) ? p->B0 * a2 / (2.0 * p->q2) * log(1.0 + p->q2 * s / (p->q0 * a2))
+                            : p->B0 * s / (2.0 * p->q0);
+}
+void orc_equilibrium(const orc_ctx *c, size_t n, const double *R, const double *Z, double *out /* [n][14] */)
+{
+    for (size_t p = 0; p < n; ++p) {
+        orc_eq e; equilibrium(&c->p, R[p], Z[p], &e);
+        memcpy(out + 14 * p, &e, sizeof(double) * 14);
+    }
+}
+
+/* ------------------------------------------------------------------- O6 RHS */
+/* Electrostatic subset (dA^s = dA^h = 0  =>  u_par = v_par, b* = b0*, dG = dPhi).
+ * eps = (m_s/q_s) rho_0 B_0 (reading G23). */
+static void rhs_point(const orc_params *p, double R, double Z, double vpar, double mu, double w,
+                      const double fld[4] /* dphi, d/dR, d/dZ, d/dphi */, double out[5])
+{
+    orc_eq e; equilibrium(p, R, Z, &e);
+    double eps = p->rho0 * p->B0 / p->qs_over_ms;
+    double cR = -e.dbphi_dZ;                          /* (curl b)_R   , bracket of A.4 */
+    double cZ = e.dbphi_dR + e.bphi / R;              /* (curl b)_Z   , bracket of A.5 */
+    double cP = e.dbR_dZ - e.dbZ_dR;                  /* (curl b)_phi , bracket of A.6 */
+    double bcurlb = e.bR * cR + e.bZ * cZ + e.bphi * cP;
+    double Bsp = e.B + eps * vpar * bcurlb;           /* B*_par */
+    double lead = (p->eom_variant == 1) ? e.B / Bsp : 1.0;
+    double k = eps * vpar / Bsp;
+    double b0R = lead * e.bR + k * cR;                /* A.4 */
+    double b0Z = lead * e.bZ + k * cZ;                /* A.5 */
+    double b0P = lead * e.bphi + k * cP;              /* A.6 */
+    double Cd = eps * mu / (e.B * Bsp);
+    double CE = p->rho0 * p->B0 / Bsp;
+    double R0dot = b0R * vpar + Cd * e.Bphi * e.dBdZ;                            /* A.10 */
+    double Z0dot = b0Z * vpar - Cd * e.Bphi * e.dBdR;                            /* A.11, sign: G1 */
+    double P0dot = b0P * vpar / R + (Cd / R) * (e.BZ * e.dBdR - e.BR * e.dBdZ);  /* A.12 */
+    double v0dot = -mu * (b0R * e.dBdR + b0Z * e.dBdZ);                          /* A.13 */
+    double fR = fld[1], fZ = fld[2], fP = fld[3];
+    double dRdot = CE * (e.bphi * fZ - (e.bZ / R) * fP);                         /* A.14 */
+    double dZdot = CE * (-e.bphi * fR + (e.bR / R) * fP);                        /* A.15 */
+    double dPdot = (CE / R) * (e.bZ * fR - e.bR * fZ);                           /* A.16 */
+    double dvdot = -p->qs_over_ms * (b0R * fR + b0Z * fZ + (b0P / R) * fP);      /* A.17, dA = 0 (G3) */
+    /* d ln f_M / dt, mbar = 1, kappa_X = -kappa_X rhat (G6, G10) */
+    double x = R - p->R0;
+    double r = sqrt(x * x + Z * Z);
+    double drdot = (r > 0.0) ? (dRdot * x + dZdot * Z) / r : 0.0;     /* dRvec . rhat */
+    double en = vpar * vpar / p->T + 2.0 * mu * e.B / p->T - 1.5;
+    double L = drdot * (-p->kappa_n - en * p->kappa_T)
+             - (2.0 * mu / p->T) * (dRdot * e.dBdR + dZdot * e.dBdZ)
+             - (2.0 * vpar / p->T) * dvdot;
+    out[0] = R0dot + dRdot;
+    out[1] = Z0dot + dZdot;
+    out[2] = P0dot + dPdot;
+    out[3] = v0dot + dvdot;
+    out[4] = (p->weight_mode == 0) ? -(1.0 - w) * L : -L;
+}
+
+/* full RHS at a phase-space point: locate -> gather -> equilibrium -> equations.
+ * returns the triangle, or -1 (out[] untouched) if the point is outside the mesh */
+static int rhs_full(const orc_ctx *c, double R, double Z, double phi, double vpar, double mu, double w, double out[5])
+{
+    double xi, eta, fld[4] = {0, 0, 0, 0};
+    int t = locate_one(c, R, Z, &xi, &eta);
+    if (t < 0) return -1;
+    if (c->n_modes > 0) gather_one(c, t, xi, eta, phi, fld);
+    rhs_point(&c->p, R, Z, vpar, mu, w, fld, out);
+    return t;
+}
+
+void orc_rhs(const orc_ctx *c, size_t n, const double *R, const double *Z, const double *phi,
+             const double *vpar, const double *mu, const double *w, int32_t *cell_out,
+             double *dRdt, double *dZdt, double *dphidt, double *dvpardt, double *dwdt)
+{
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) {
+        double o[5] = {0, 0, 0, 0, 0};
+        int t = rhs_full(c, R[p], Z[p], phi[p], vpar[p], mu[p], w[p], o);
+        if (cell_out) cell_out[p] = t;
+        dRdt[p] = o[0]; dZdt[p] = o[1]; dphidt[p] = o[2]; dvpardt[p] = o[3]; dwdt[p] = o[4];
+    }
+}
+/* RHS with the field values handed in (no mesh): test hook for the pointwise identities */
+void orc_rhs_point(const orc_ctx *c, size_t n, const double *R, const double *Z, const double *vpar,
+                   const double *mu, const double *w, const double *fld /* [n][4] */, double *out /* [n][5] */)
+{
+    for (size_t p = 0; p < n; ++p) rhs_point(&c->p, R[p], Z[p], vpar[p], mu[p], w[p], fld + 4 * p, out + 5 * p);
+}
+
+/* ------------------------------------------------------------------- O7 RK4 */
+/* y = (R, Z, phi, v_par, w), mu constant.  phi wrapped to [0, 2 pi) once per step.  A marker
+ * whose any stage position, or final position, is outside the mesh is restored to its
+ * start-of-step state, flagged cell = -1 and skipped from then on.  Field frozen. */
+void orc_push(const orc_ctx *c, size_t n, double *R, double *Z, double *phi, double *vpar,
+              const double *mu, double *w, int32_t *cell, double dt, int nsteps, int nthreads)
+{
+#ifdef _OPENMP
+    if (nthreads > 0) omp_set_num_threads(nthreads);
+#else
+    (void)nthreads;
+#endif
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) {
+        if (cell[p] < 0) continue;          /* already lost */
+        double y[5] = {R[p], Z[p], phi[p], vpar[p], w[p]};
+        int cl = cell[p];
+        for (int s = 0; s < nsteps; ++s) {
+            double k1[5], k2[5], k3[5], k4[5], ys[5];
+            int lost = 0;
+            if (rhs_full(c, y[0], y[1], y[2], y[3], mu[p], y[4], k1) < 0) lost = 1;
+            if (!lost) {
+                for (int q = 0; q < 5; ++q) ys[q] = y[q] + 0.5 * dt * k1[q];
+                if (rhs_full(c, ys[0], ys[1], ys[2], ys[3], mu[p], ys[4], k2) < 0) lost = 1;
+            }
+            if (!lost) {
+                for (int q = 0; q < 5; ++q) ys[q] = y[q] + 0.5 * dt * k2[q];
+                if (rhs_full(c, ys[0], ys[1], ys[2], ys[3], mu[p], ys[4], k3) < 0) lost = 1;
+            }
+            if (!lost) {
+                for (int q = 0; q < 5; ++q) ys[q] = y[q] + dt * k3[q];
+                if (rhs_full(c, ys[0], ys[1], ys[2], ys[3], mu[p], ys[4], k4) < 0) lost = 1;
+            }
+            int newcell = -1;
+            if (!lost) {
+                for (int q = 0; q < 5; ++q) ys[q] = y[q] + (dt / 6.0) * (k1[q] + 2.0 * k2[q] + 2.0 * k3[q] + k4[q]);
+                ys[2] = ys[2] - ORC_TWO_PI * floor(ys[2] / ORC_TWO_PI);
+                newcell = locate_one(c, ys[0], ys[1], NULL, NULL);
+                if (newcell < 0) lost = 1;
+            }
+            if (lost) { cl = -1; break; }       /* y keeps the start-of-step state */
+            for (int q = 0; q < 5; ++q) y[q] = ys[q];
+            cl = newcell;
+        }
+        R[p] = y[0]; Z[p] = y[1]; phi[p] = y[2]; vpar[p] = y[3]; w[p] = y[4]; cell[p] = cl;
+    }
+}
+
+int orc_max_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
