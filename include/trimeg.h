@@ -1,0 +1,191 @@
+/*
+ * trimeg.h -- C ABI of libtrimeg: the B200-native (sm_100a) marker-push hot path of the
+ * TRIMEG gyrokinetic particle-in-cell method (arxiv/paper_2601_14301).
+ *
+ * Citations are /root/reference/PAPER.md:<line> (section / equation); readings of passages
+ * the paper leaves open are numbered G1..G23, L1..L5, O1..O7 in DESIGN.md §3.
+ *
+ * The path, per marker ("particle push kernel"):
+ *   locate the triangle (contains()) ->
+ *   grid-to-particle gather of the perturbed potential dphi and its gradient from C1
+ *   quintic triangle elements x toroidal harmonics e^{i n phi}
+ *   (Def. 19) ->
+ *   analytic equilibrium B = grad psi x grad phi + F grad phi ->
+ *   gyro-centre equations of motion A.4-A.6, A.10-A.17 with dA_par = 0
+ *   and the delta-f weight rate from d ln f_M / dt ->
+ *   classic RK4.
+ *
+ * Conventions common to every call
+ *   - Returns TRIMEG_OK (0) or a negative TRIMEG_ERR_* code; nothing throws or aborts
+ *     across this boundary.  trimeg_strerror() names a code.
+ *   - "_host" pointers are host memory, read during the call and not retained.
+ *     All other data pointers are DEVICE pointers owned by the caller (e.g. PyTorch
+ *     tensors); the library never frees or reallocates them.  fp64 everywhere.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = legacy default stream).  Work is
+ *     enqueued on it and the call returns without synchronising, except where stated.
+ *   - Tables (mesh geometry, coefficient table) are owned by the context, uploaded once
+ *     ("allocate once, upload static data once").
+ *   - One context per GPU (cudaSetDevice before trimeg_mesh_create); a context is not
+ *     thread-safe.  There is no CPU fallback: without a CUDA device calls return
+ *     TRIMEG_ERR_CUDA.
+ */
+#ifndef TRIMEG_H
+#define TRIMEG_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define TRIMEG_OK               0
+#define TRIMEG_ERR_INVALID_ARG (-1)  /* NULL pointer, negative size, bad enum                   */
+#define TRIMEG_ERR_MESH        (-2)  /* nodes not strictly increasing / r_0 != 0 / sagitta rule  */
+#define TRIMEG_ERR_NO_FIELD    (-3)  /* a gather/rhs/push was asked before trimeg_field_upload   */
+#define TRIMEG_ERR_CUDA        (-4)  /* a CUDA runtime call or kernel launch failed              */
+#define TRIMEG_ERR_ALLOC       (-5)  /* device or host allocation failed                         */
+
+#define TRIMEG_NCOEF 21              /* monomials xi^i eta^j, 0 <= i+j <= 5        */
+
+typedef struct trimeg_ctx trimeg_ctx;   /* opaque; owns all device tables */
+typedef void *trimeg_stream;            /* cudaStream_t */
+
+/* Physical parameters (plain data, copied by trimeg_mesh_create / trimeg_set_params).
+ * Normalised units of PAPER.md:1198: length 1 m, ion mass = charge = 1 in the workloads. */
+typedef struct {
+    double R0, a, B0;        /* major radius, minor radius, on-axis field                         */
+    double q0, q2;           /* cylindrical safety factor q(r) = q0 + q2 (r/a)^2; psi' = B0 r/q   */
+    double rho0;             /* rho_0 of A.4-A.6                                  */
+    double qs_over_ms;       /* q_s / m_s                                                         */
+    double T;                /* Tbar of the Maxwellian; sigma_vpar = sqrt(T/2)    */
+    double kappa_n, kappa_T; /* -d ln n0/dr, -d ln T/dr (inverse length)           */
+    int eom_variant;         /* 0: b0* as printed in A.4-A.6; 1: (B/B*par) b + ... (reading G2)   */
+    int weight_mode;         /* 0: dw/dt = -(1-w) d ln f_M/dt; 1: dw/dt = -d ln f_M/dt (G7)       */
+} trimeg_params;
+
+/* Marker arrays, structure of arrays, each of length n.
+ * cell[p] = triangle index of marker p, used as a HINT by the locator (a stale hint costs
+ * time, never correctness); cell[p] < 0 marks a marker outside the mesh: it is skipped. */
+typedef struct {
+    double *R, *Z, *phi;     /* cylindrical position                              */
+    double *vpar;            /* parallel velocity v_par = u_par (electrostatic)                   */
+    double *mu;              /* magnetic moment v_perp^2 / 2B; never written       */
+    double *w;               /* delta-f weight                                 */
+    int32_t *cell;
+} trimeg_markers;
+
+/* ---- mesh (rows a0, a2 of DESIGN.md §1) --------------------------------------------------
+ * Structured ring x sector triangulation of the poloidal plane around the axis (R0, 0):
+ * n_vert = 1 + n_r n_theta vertices, n_tri = (2 n_r - 1) n_theta triangles, numbered as in
+ * DESIGN.md §3 O1 (axis fan first, then two triangles per ring-sector quad), all
+ * counter-clockwise, local coordinates (xi, eta) with the vertices at (0,0),(1,0),(0,1)
+ * (PAPER.md:328).
+ *   r_nodes_host  n_r + 1 radii, r[0] = 0 < r[1] < ... < r[n_r] = a
+ *   vert_R_host, vert_Z_host   n_vert vertex coordinates, or both NULL: the library then
+ *                 places v(i,j) at (R0 + r_i cos(2 pi j/n_theta), r_i sin(2 pi j/n_theta))
+ *                 with the host libm.  Pass them to get bit-identical geometry to another
+ *                 implementation.
+ * Errors: INVALID_ARG (NULL, n_r < 2, n_theta < 3), MESH (nodes not increasing, or the chord
+ * sagitta r_{k+1}(1 - cos(pi/n_theta)) >= r_{k+2} - r_{k+1}: the locator's 3x3 candidate
+ * neighbourhood would not be sufficient, rule L4), CUDA, ALLOC. */
+int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_nodes_host,
+                       const double *vert_R_host, const double *vert_Z_host,
+                       const trimeg_params *params);
+int trimeg_mesh_destroy(trimeg_ctx *ctx);
+int trimeg_mesh_info(const trimeg_ctx *ctx, int *n_vert, int *n_tri);
+int trimeg_set_params(trimeg_ctx *ctx, const trimeg_params *params);
+/* test hook: geometry table [n_tri][6] = (R_v0, Z_v0, xi_R, xi_Z, eta_R, eta_Z) to device memory */
+int trimeg_mesh_download_geom(trimeg_ctx *ctx, double *geom_dev, trimeg_stream stream);
+
+/* ---- field (row a0) -----------------------------------------------------------------------
+ * dphi(R, phi, Z) = sum_n Re( P_n(xi, eta) e^{i n phi} ), P_n the C1 quintic of the triangle
+ * (PAPER.md:338-363, 365-368 with the toroidal basis replaced by harmonics).
+ *   kind 0: data_dev = nodal DOFs [n_modes][n_vert][6] complex128 in the order
+ *           (f, f_R, f_Z, f_RR, f_RZ, f_ZZ) of PAPER.md:350-353; the library expands them on
+ *           the device to the 21 monomial coefficients per triangle and mode with Bell's
+ *           reduction (normal derivative cubic on every edge, reading O2).
+ *   kind 1: data_dev = coefficients [n_tri][n_modes][21] complex128, degree-major monomial
+ *           order k <-> (i, j): for d = 0..5, for j = 0..d: xi^(d-j) eta^j.
+ * mode_n_host: n_modes toroidal mode numbers.  n_modes = 0 is legal (dphi == 0).
+ * Errors: INVALID_ARG, ALLOC, CUDA. */
+int trimeg_field_upload(trimeg_ctx *ctx, int n_modes, const int *mode_n_host,
+                        const void *data_dev, int kind, trimeg_stream stream);
+/* test hook: coefficient table in the kind-1 layout to device memory */
+int trimeg_field_download_coeffs(trimeg_ctx *ctx, void *coeffs_dev, trimeg_stream stream);
+
+/* ---- locator (row a2) ----------------------------------------------
+ * cell[p] = lowest triangle index t whose contains() test passes for (R[p], Z[p]), the test
+ * being xi >= 0, eta >= 0, 1 - xi - eta >= 0 with every operation individually rounded in
+ * the order of DESIGN.md §3 O3 (no fused multiply-add); -1 outside the outer polygon.
+ * The result is bit-identical to the brute-force search over all triangles. */
+int trimeg_locate(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, int32_t *cell,
+                  trimeg_stream stream);
+
+/* ---- gather only (row a3; BASELINE.json configs[3]) ----------------------------------------
+ * dphi, d dphi/dR, d dphi/dZ (and d dphi/dphi if dphi_dphi != NULL) at the markers.
+ * cell_hint may be NULL.  Markers outside the mesh get 0.  NO_FIELD if no field is loaded. */
+int trimeg_gather(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, const double *phi,
+                  const int32_t *cell_hint, double *dphi, double *dphi_dR, double *dphi_dZ,
+                  double *dphi_dphi, trimeg_stream stream);
+
+/* ---- one right-hand-side evaluation (rows a2-a5) -------------------------------------------
+ * The paper's push kernel: five time derivatives per marker
+ * (dRdt, dZdt, dphidt, dvpardt, dwdt), each n doubles.  Markers are not modified; markers
+ * outside the mesh get 0. */
+int trimeg_rhs(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, double *dRdt, double *dZdt,
+               double *dphidt, double *dvpardt, double *dwdt, trimeg_stream stream);
+
+/* ---- cell sort (row a1) ---------------------------------------------------------------------
+ * Counting sort of the markers by cell (markers with cell < 0 go last).  Permutes all seven
+ * arrays in place.  perm_dev (int64[n], may be NULL) receives, for every new position, the
+ * old index.  The order inside one cell is unspecified.  Uses context-owned scratch of
+ * ~60 B/marker, grown on demand (ALLOC if that fails). */
+int trimeg_sort(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_dev,
+                trimeg_stream stream);
+
+/* ---- compaction of the active list (row a6) -------------------------------------------------
+ * Stable partition: markers with cell >= 0 first (original order kept), lost markers after
+ * them.  *n_active_host receives the number of active markers (the call synchronises the
+ * stream to return it).  perm_dev as in trimeg_sort. */
+int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_dev,
+                   size_t *n_active_host, trimeg_stream stream);
+
+/* ---- the push (rows a2-a6) ------------------------------------------------------------------
+ * nsteps classic RK4 steps of size dt on y = (R, Z, phi, vpar, w), mu constant, with the
+ * field frozen; four locate + gather + equilibrium + RHS evaluations per step, all in one
+ * kernel.  After each step phi is wrapped to [0, 2 pi) and cell is set to the triangle of the
+ * new position.  A marker whose any stage position, or new position, is outside the mesh is
+ * restored to its start-of-step state, flagged cell = -1 and skipped from then on; it keeps
+ * its index (use trimeg_compact to drop it).  Markers are not reordered. */
+int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
+                trimeg_stream stream);
+
+/* ---- end-to-end push from HOST buffers -------------------------------------------------------
+ * Same result as: copy the seven arrays to the device, trimeg_locate if locate_first != 0,
+ * trimeg_sort, trimeg_push, undo the sort, copy R, Z, phi, vpar, w, cell back.  `m` holds
+ * HOST pointers (pinned memory makes the copies asynchronous).  Markers are processed in
+ * chunks on several streams so that copies overlap the push.  Synchronises before returning. */
+int trimeg_push_host(trimeg_ctx *ctx, trimeg_markers *m_host, size_t n, double dt, int nsteps,
+                     int locate_first);
+
+/* ---- statistics ------------------------------------------------------------------------------
+ * Totals since context creation (or the last reset): markers flagged lost by trimeg_push,
+ * locator calls that left the hinted triangle, kernels launched by the library.
+ * Synchronises the device.  Any pointer may be NULL. */
+int trimeg_get_stats(trimeg_ctx *ctx, int64_t *n_lost, int64_t *n_relocated, int64_t *n_launches);
+int trimeg_reset_stats(trimeg_ctx *ctx);
+
+/* ---- diagnostics ------------------------------------------------------------------------------
+ * Measured FP64 vector (DFMA) throughput of the current device in TFLOP/s (2 flops per DFMA),
+ * best of 5 launches of a dependency-free DFMA loop: the denominator of the FP64 roofline in
+ * DESIGN.md §6.  Not part of the path.  Synchronises. */
+int trimeg_measure_fp64_peak(trimeg_ctx *ctx, double *tflops_out);
+
+const char *trimeg_strerror(int code);
+const char *trimeg_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TRIMEG_H */

@@ -1,0 +1,315 @@
+// trimeg_device.cuh -- device-side building blocks of the marker push (sm_100a, fp64).
+//
+// Rows of DESIGN.md §1: a2 locator, a3 field gather, a4 equilibrium, a5 RHS assembly.
+// Citations: PAPER.md:<line> = /root/reference/PAPER.md; readings G*/L*/O* = DESIGN.md §3.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace trimeg {
+
+constexpr int NCOEF = 21;
+// A candidate triangle is accepted without looking at any other one only if the marker is
+// inside it by this margin in barycentric units (rule L3).  Rounding errors of the test are
+// <~ 1e-13 even on the thinnest axis-fan triangles, so a triangle passing with this margin is
+// the only one whose contains() test can pass.
+constexpr double LOC_TAU = 1e-9;
+constexpr int LOC_MAX_HOPS = 8;
+
+struct MeshDev {
+    int n_r, n_theta, n_tri;
+    const double *geom;     // [n_tri][6]  R_v0, Z_v0, xi_R, xi_Z, eta_R, eta_Z
+    const double *r_nodes;  // [n_r + 1]
+    double Rax, Zax;        // axis vertex
+    double rin2;            // squared inscribed radius of the outer polygon (gap rule, O3)
+};
+
+struct FieldDev {
+    int n_modes;
+    const double2 *coef;    // [n_tri][n_modes][21] (re, im)
+    const int *mode_n;      // [n_modes] (device)
+    int n_first, n_step;    // arithmetic progression n_k = n_first + k n_step if is_ap
+    int is_ap;
+};
+
+struct PhysDev {
+    double R0, B0, invB0, q0, qs;   // qs = q2 / a^2 = d q / d s,  s = r^2
+    double eps;                     // (m_s/q_s) rho_0 B_0  (reading G23)
+    double rho0B0;                  // numerator of C_E
+    double qom;                     // q_s / m_s
+    double invT, kappa_n, kappa_T;
+    int eom_variant, weight_mode;
+};
+
+// --------------------------------------------------------------------------- a2 locator
+// contains() of PAPER.md:291 in local coordinates, every operation individually rounded
+// in the fixed order of reading O3 / rule L2 (no fused multiply-add).
+struct Bary {
+    double xi, eta, l0;
+    double xR, xZ, eR, eZ;   // xi_R, xi_Z, eta_R, eta_Z of the triangle
+};
+
+__device__ __forceinline__ Bary bary_rn(const MeshDev &M, int t, double R, double Z)
+{
+    const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)t);
+    const double2 v0 = __ldg(g), gx = __ldg(g + 1), ge = __ldg(g + 2);
+    Bary b;
+    const double dx = __dsub_rn(R, v0.x), dz = __dsub_rn(Z, v0.y);
+    b.xi = __dadd_rn(__dmul_rn(gx.x, dx), __dmul_rn(gx.y, dz));
+    b.eta = __dadd_rn(__dmul_rn(ge.x, dx), __dmul_rn(ge.y, dz));
+    b.l0 = __dsub_rn(__dsub_rn(1.0, b.xi), b.eta);
+    b.xR = gx.x; b.xZ = gx.y; b.eR = ge.x; b.eZ = ge.y;
+    return b;
+}
+
+// Triangle across the edge on which barycentric coordinate `which` vanishes
+// (0: lambda0, 1: xi, 2: eta); -1 = across the outer boundary.  Closed form on the
+// ring x sector numbering (O1).
+__device__ __forceinline__ int neighbour(const MeshDev &M, int t, int which)
+{
+    const int nth = M.n_theta;
+    if (t < nth) {                                   // axis fan, sector j = t
+        if (which == 0) return nth + 2 * t + 1;      // outer chord -> ring 1, k = 1
+        if (which == 1) return (t + 1 == nth) ? 0 : t + 1;
+        return (t == 0) ? nth - 1 : t - 1;
+    }
+    const int u = t - nth, k = u & 1, c = u >> 1;
+    const int i = c / nth + 1, j = c - (i - 1) * nth;
+    if (k == 0) {                                    // (v(i,j), v(i+1,j), v(i+1,j+1))
+        if (which == 0) return (i + 1 <= M.n_r - 1) ? nth + 2 * (i * nth + j) + 1 : -1;
+        if (which == 1) return t + 1;
+        const int jm = (j == 0) ? nth - 1 : j - 1;
+        return nth + 2 * ((i - 1) * nth + jm) + 1;
+    }
+    // k == 1: (v(i,j), v(i+1,j+1), v(i,j+1))
+    if (which == 0) { const int jp = (j + 1 == nth) ? 0 : j + 1; return nth + 2 * ((i - 1) * nth + jp); }
+    if (which == 1) return (i >= 2) ? nth + 2 * ((i - 2) * nth + j) : j;
+    return t - 1;
+}
+
+// (r, theta) ring / sector guess: only ever selects CANDIDATES (rule L1).
+static __device__ __noinline__ void ring_sector_guess(const MeshDev &M, double R, double Z, int &i0, int &j0)
+{
+    const double x = R - M.Rax, z = Z - M.Zax;
+    const double r = sqrt(x * x + z * z);
+    double th = atan2(z, x);
+    if (th < 0.0) th += 6.283185307179586476925286766559;
+    int lo = 0, hi = M.n_r;                          // largest i with r_nodes[i] <= r
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (__ldg(M.r_nodes + mid) <= r) lo = mid; else hi = mid; }
+    i0 = lo;
+    double jf = floor(th * (double)M.n_theta * 0.15915494309189533576888376337251);
+    if (!(jf >= 0.0 && jf < (double)M.n_theta)) jf = 0.0;
+    j0 = (int)jf;
+}
+
+// The complete rule of reading O3 on the 3x3 cell neighbourhood of the guess: lowest t whose
+// test passes; if none passes, the gap rule.  Same decisions as a brute-force search.
+static __device__ __noinline__ int locate_full(const MeshDev &M, double R, double Z, Bary &out)
+{
+    int i0, j0;
+    ring_sector_guess(M, R, Z, i0, j0);
+    int best = -1, gap_best = -1;
+    double gap_m = -INFINITY;
+    Bary bb, gb;
+    bb.xi = bb.eta = bb.l0 = bb.xR = bb.xZ = bb.eR = bb.eZ = 0.0;
+    gb = bb;
+    for (int ii = i0 - 1; ii <= i0 + 1; ++ii) {
+        if (ii < 0 || ii > M.n_r - 1) continue;
+        for (int dj = -1; dj <= 1; ++dj) {
+            int jj = j0 + dj;
+            if (jj < 0) jj += M.n_theta;
+            if (jj >= M.n_theta) jj -= M.n_theta;
+            const int base = (ii == 0) ? jj : M.n_theta + 2 * ((ii - 1) * M.n_theta + jj);
+            const int cnt = (ii == 0) ? 1 : 2;
+            for (int k = 0; k < cnt; ++k) {
+                const int t = base + k;
+                const Bary b = bary_rn(M, t, R, Z);
+                const double m = fmin(fmin(b.xi, b.eta), b.l0);
+                if (b.xi >= 0.0 && b.eta >= 0.0 && b.l0 >= 0.0) {
+                    if (best < 0 || t < best) { best = t; bb = b; }
+                }
+                if (m > gap_m || (m == gap_m && t < gap_best)) { gap_m = m; gap_best = t; gb = b; }
+            }
+        }
+    }
+    if (best >= 0) { out = bb; return best; }
+    const double x = __dsub_rn(R, M.Rax), z = __dsub_rn(Z, M.Zax);
+    const double s = __dadd_rn(__dmul_rn(x, x), __dmul_rn(z, z));
+    if (s < M.rin2) { out = gb; return gap_best; }
+    return -1;
+}
+
+// Locator used on the hot path: hinted triangle first, then a walk across the violated
+// edge (closed-form neighbours), complete rule only for markers within LOC_TAU of an edge.
+// Returns the triangle or -1 (outside the outer polygon); `moved` is set when the hint was left.
+__device__ __forceinline__ int locate(const MeshDev &M, double R, double Z, int hint, Bary &out, int &moved)
+{
+    int t = hint;
+    if (t < 0 || t >= M.n_tri) {
+        int i0, j0;
+        ring_sector_guess(M, R, Z, i0, j0);
+        if (i0 > M.n_r - 1) i0 = M.n_r - 1;
+        t = (i0 == 0) ? j0 : M.n_theta + 2 * ((i0 - 1) * M.n_theta + j0);
+    }
+#pragma unroll 1
+    for (int hop = 0; hop < LOC_MAX_HOPS; ++hop) {
+        const Bary b = bary_rn(M, t, R, Z);
+        const double m = fmin(fmin(b.xi, b.eta), b.l0);
+        if (m > LOC_TAU) { out = b; return t; }
+        if (!(m < -LOC_TAU)) break;                   // within TAU of an edge (or NaN): full rule
+        const int which = (b.l0 <= b.xi && b.l0 <= b.eta) ? 0 : ((b.xi <= b.eta) ? 1 : 2);
+        const int tn = neighbour(M, t, which);
+        moved = 1;
+        if (tn < 0) return -1;                        // beyond an outer chord by a clear margin
+        t = tn;
+    }
+    moved = 1;
+    return locate_full(M, R, Z, out);
+}
+
+// --------------------------------------------------------------------------- a3 gather
+// One toroidal mode: complex quintic P and its xi / eta derivatives by bivariate Horner with
+// the product rule (76 real FMAs), coefficients degree-major k(i,j) = d(d+1)/2 + j, d = i+j.
+struct Cplx { double re, im; };
+
+__device__ __forceinline__ constexpr int kidx(int i, int j) { return (i + j) * (i + j + 1) / 2 + j; }
+
+__device__ __forceinline__ void eval_quintic(const double2 *__restrict__ c, double xi, double eta,
+                                             Cplx &P, Cplx &Px, Cplx &Pe)
+{
+    double pr = 0.0, pi = 0.0, pxr = 0.0, pxi = 0.0, per = 0.0, pei = 0.0;
+#pragma unroll
+    for (int j = 5; j >= 0; --j) {
+        // A_j(xi) = sum_i c_ij xi^i and A_j'(xi), i = 0 .. 5-j
+        const int n = 5 - j;
+        double2 top = __ldg(c + kidx(n, j));
+        double ar = top.x, ai = top.y, dr = 0.0, di = 0.0;
+#pragma unroll
+        for (int i = n - 1; i >= 0; --i) {
+            const double2 cc = __ldg(c + kidx(i, j));
+            if (i == n - 1) { dr = ar; di = ai; }
+            else { dr = fma(dr, xi, ar); di = fma(di, xi, ai); }
+            ar = fma(ar, xi, cc.x); ai = fma(ai, xi, cc.y);
+        }
+        if (j == 5) { pr = ar; pi = ai; }
+        else {
+            if (j == 4) { per = pr; pei = pi; pxr = dr; pxi = di; }
+            else {
+                per = fma(per, eta, pr); pei = fma(pei, eta, pi);
+                pxr = fma(pxr, eta, dr); pxi = fma(pxi, eta, di);
+            }
+            pr = fma(pr, eta, ar); pi = fma(pi, eta, ai);
+        }
+    }
+    P.re = pr; P.im = pi; Px.re = pxr; Px.im = pxi; Pe.re = per; Pe.im = pei;
+}
+
+struct FieldVal { double f, fR, fZ, fphi; };   // dphi, d/dR, d/dZ, d/dphi
+
+// dphi = sum_n Re(P_n E_n), E_n = e^{i n phi}; no factor 2, Im of n = 0 ignored (G15).
+__device__ __forceinline__ FieldVal gather(const FieldDev &F, int t, const Bary &b, double phi)
+{
+    double f = 0.0, fx = 0.0, fe = 0.0, fp = 0.0;
+    if (F.n_modes > 0) {
+        const double2 *c = F.coef + (size_t)t * F.n_modes * NCOEF;
+        double Er, Ei, Dr = 1.0, Di = 0.0;
+        if (F.is_ap) {
+            if (F.n_first == 0) { Er = 1.0; Ei = 0.0; }
+            else sincos((double)F.n_first * phi, &Ei, &Er);
+            if (F.n_modes > 1) sincos((double)F.n_step * phi, &Di, &Dr);
+        } else { Er = 1.0; Ei = 0.0; }
+        double nn = (double)F.n_first;
+#pragma unroll 1
+        for (int m = 0; m < F.n_modes; ++m, c += NCOEF) {
+            if (!F.is_ap) { nn = (double)__ldg(F.mode_n + m); sincos(nn * phi, &Ei, &Er); }
+            Cplx P, Px, Pe;
+            eval_quintic(c, b.xi, b.eta, P, Px, Pe);
+            f = fma(P.re, Er, fma(-P.im, Ei, f));
+            fx = fma(Px.re, Er, fma(-Px.im, Ei, fx));
+            fe = fma(Pe.re, Er, fma(-Pe.im, Ei, fe));
+            fp = fma(-nn, fma(P.im, Er, P.re * Ei), fp);          // Re(i n P E)
+            if (F.is_ap) {                                        // E_{n + dn} = E_n E_dn
+                const double tr = fma(Er, Dr, -Ei * Di);
+                Ei = fma(Er, Di, Ei * Dr);
+                Er = tr;
+                nn += (double)F.n_step;
+            }
+        }
+    }
+    FieldVal v;
+    v.f = f;
+    v.fR = fma(b.xR, fx, b.eR * fe);
+    v.fZ = fma(b.xZ, fx, b.eZ * fe);
+    v.fphi = fp;
+    return v;
+}
+
+// ------------------------------------------------------------------- a4 + a5 equilibrium, RHS
+// Analytic circular equilibrium: psi' = B0 r / q(r), F = B0 R0 (G11), B = grad psi x grad phi
+// + F grad phi; b0* (A.4-A.6), equilibrium drifts (A.10-A.13, sign of
+// A.11 per G1), E x B and parallel acceleration (A.14-A.17 with dA = 0, G3), weight rate from
+// d ln f_M/dt (kappa_X along -rhat, G6/G10).
+struct Rates { double R, Z, phi, vpar, w; };
+
+__device__ __forceinline__ Rates rhs_point(const PhysDev &p, double R, double Z, double vpar, double mu,
+                                           double w, const FieldVal &fld)
+{
+    const double x = R - p.R0;
+    const double s = fma(x, x, Z * Z);
+    const double qb = fma(p.qs, s, p.q0);
+    const double iq = 1.0 / qb;
+    const double iq2 = iq * iq;
+    const double g = fma(s, iq2, p.R0 * p.R0);
+    const double gs = iq2 * fma(-2.0 * s * p.qs, iq, 1.0);
+    const double isg = rsqrt(g);
+    const double sg = g * isg;
+    const double ig = isg * isg;
+    const double h = iq * isg;
+    const double hs = -h * fma(0.5 * gs, ig, p.qs * iq);
+    const double iR = 1.0 / R;
+    const double B = p.B0 * sg * iR;
+    const double iB = R * isg * p.invB0;
+    const double BiR = p.B0 * iR;
+    const double BR = -BiR * Z * iq, BZ = BiR * x * iq, Bphi = BiR * p.R0;
+    const double bR = -Z * h, bZ = x * h, bphi = p.R0 * isg;
+    const double dBdR = p.B0 * iR * fma(gs * x, isg, -sg * iR);
+    const double dBdZ = p.B0 * iR * gs * Z * isg;
+    const double dbphi_c = -p.R0 * gs * ig * isg;        // d b_phi / d s * 2 ... times x or Z
+    const double curlR = -dbphi_c * Z;                   // -(d b_phi/dZ)
+    const double curlZ = fma(dbphi_c, x, bphi * iR);     //  d b_phi/dR + b_phi/R
+    const double curlP = -2.0 * (h + s * hs);            //  d b_R/dZ - d b_Z/dR
+    const double bcurlb = fma(bR, curlR, fma(bZ, curlZ, bphi * curlP));
+    const double Bsp = fma(p.eps * vpar, bcurlb, B);     // B*_par
+    const double iBsp = 1.0 / Bsp;
+    const double lead = (p.eom_variant == 1) ? B * iBsp : 1.0;
+    const double k = p.eps * vpar * iBsp;
+    const double b0R = fma(lead, bR, k * curlR);
+    const double b0Z = fma(lead, bZ, k * curlZ);
+    const double b0P = fma(lead, bphi, k * curlP);
+    const double Cd = p.eps * mu * iB * iBsp;
+    const double CE = p.rho0B0 * iBsp;
+    const double CdBphi = Cd * Bphi;
+    const double R0dot = fma(b0R, vpar, CdBphi * dBdZ);
+    const double Z0dot = fma(b0Z, vpar, -CdBphi * dBdR);
+    const double P0dot = iR * fma(b0P, vpar, Cd * fma(BZ, dBdR, -BR * dBdZ));
+    const double v0dot = -mu * fma(b0R, dBdR, b0Z * dBdZ);
+    const double fP_R = fld.fphi * iR;                   // (1/R) d dphi / d phi
+    const double dRdot = CE * fma(bphi, fld.fZ, -bZ * fP_R);
+    const double dZdot = CE * fma(-bphi, fld.fR, bR * fP_R);
+    const double dPdot = CE * iR * fma(bZ, fld.fR, -bR * fld.fZ);
+    const double dvdot = -p.qom * fma(b0R, fld.fR, fma(b0Z, fld.fZ, b0P * fP_R));
+    const double ir = (s > 0.0) ? rsqrt(s) : 0.0;
+    const double drdot = fma(dRdot, x, dZdot * Z) * ir;
+    const double en = fma(vpar * vpar, p.invT, fma(2.0 * mu * B, p.invT, -1.5));
+    const double L = fma(drdot, -fma(en, p.kappa_T, p.kappa_n),
+                         fma(-2.0 * mu * p.invT, fma(dRdot, dBdR, dZdot * dBdZ), -2.0 * vpar * p.invT * dvdot));
+    Rates o;
+    o.R = R0dot + dRdot;
+    o.Z = Z0dot + dZdot;
+    o.phi = P0dot + dPdot;
+    o.vpar = v0dot + dvdot;
+    o.w = (p.weight_mode == 0) ? -(1.0 - w) * L : -L;
+    return o;
+}
+
+}  // namespace trimeg

@@ -1,0 +1,53 @@
+// trimeg_internal.h -- host-side context and launch wrappers shared by the library's
+// translation units (not part of the public ABI).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/trimeg.h"
+#include "trimeg_device.cuh"
+
+namespace trimeg {
+
+struct Stats {                      // device-resident counters
+    unsigned long long n_lost;
+    unsigned long long n_moved;
+};
+
+}  // namespace trimeg
+
+struct trimeg_ctx {
+    int device;
+    int n_sm;
+    int n_r, n_theta, n_vert, n_tri;
+    trimeg_params params;
+    trimeg::MeshDev mesh;
+    trimeg::FieldDev field;
+    trimeg::PhysDev phys;
+    // device tables
+    double *d_geom, *d_r_nodes, *d_vR, *d_vZ;
+    double2 *d_coef;
+    int *d_mode_n;
+    int has_field;
+    trimeg::Stats *d_stats;
+    int64_t n_launches;
+    // scratch for sort / compact / host path (grown on demand)
+    void *d_scratch;
+    size_t scratch_bytes;
+    int *d_bins;                    // n_tri + 2 counters
+    // host path
+    cudaStream_t hstream[3];
+    int hstreams_ready;
+};
+
+namespace trimeg {
+
+// launch wrappers implemented in trimeg_push.cu; each returns the cudaError of the launch
+cudaError_t launch_locate(trimeg_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell, cudaStream_t s);
+cudaError_t launch_gather(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi,
+                          const int32_t *hint, double *f, double *fR, double *fZ, double *fP, cudaStream_t s);
+cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP,
+                       double *dV, double *dW, cudaStream_t s);
+cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
+
+}  // namespace trimeg

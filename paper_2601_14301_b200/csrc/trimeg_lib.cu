@@ -1,0 +1,687 @@
+// trimeg_lib.cu -- C ABI of libtrimeg (include/trimeg.h): context, mesh and field tables
+// (row a0), cell sort (a1), compaction (a6), host-buffer path, statistics.
+#include <math.h>
+#include <stdio.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include <new>
+
+#include "trimeg_internal.h"
+#include "bell_tables.inc"
+
+using namespace trimeg;
+
+#define CU_TRY(expr)                                   \
+    do {                                               \
+        cudaError_t e__ = (expr);                      \
+        if (e__ != cudaSuccess) return TRIMEG_ERR_CUDA; \
+    } while (0)
+
+// ============================================================================ a0: mesh tables
+__device__ __forceinline__ int vertex_id(int n_theta, int i, int j)
+{   // v(i, j) = 1 + (i-1) n_theta + (j mod n_theta), i >= 1
+    if (j >= n_theta) j -= n_theta;
+    return 1 + (i - 1) * n_theta + j;
+}
+__device__ __forceinline__ void tri_vertices(int n_theta, int t, int v[3])
+{
+    if (t < n_theta) { v[0] = 0; v[1] = vertex_id(n_theta, 1, t); v[2] = vertex_id(n_theta, 1, t + 1); return; }
+    const int u = t - n_theta, k = u & 1, c = u >> 1, i = c / n_theta + 1, j = c % n_theta;
+    v[0] = vertex_id(n_theta, i, j);
+    if (k == 0) { v[1] = vertex_id(n_theta, i + 1, j); v[2] = vertex_id(n_theta, i + 1, j + 1); }
+    else { v[1] = vertex_id(n_theta, i + 1, j + 1); v[2] = vertex_id(n_theta, i, j + 1); }
+}
+
+// geometry factors with individually rounded operations (they feed the bit-exact locator)
+__global__ void geom_kernel(int n_r, int n_theta, int n_tri, const double *__restrict__ vR,
+                            const double *__restrict__ vZ, double *__restrict__ geom, double *__restrict__ rin2)
+{
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t == 0) {
+        const int va = vertex_id(n_theta, n_r, 0), vb = vertex_id(n_theta, n_r, 1);
+        const double mx = __dsub_rn(__dmul_rn(0.5, __dadd_rn(vR[va], vR[vb])), vR[0]);
+        const double mz = __dsub_rn(__dmul_rn(0.5, __dadd_rn(vZ[va], vZ[vb])), vZ[0]);
+        *rin2 = __dadd_rn(__dmul_rn(mx, mx), __dmul_rn(mz, mz));
+    }
+    if (t >= n_tri) return;
+    int v[3];
+    tri_vertices(n_theta, t, v);
+    const double R0 = vR[v[0]], Z0 = vZ[v[0]];
+    const double e1R = __dsub_rn(vR[v[1]], R0), e1Z = __dsub_rn(vZ[v[1]], Z0);
+    const double e2R = __dsub_rn(vR[v[2]], R0), e2Z = __dsub_rn(vZ[v[2]], Z0);
+    const double D = __dsub_rn(__dmul_rn(e1R, e2Z), __dmul_rn(e2R, e1Z));
+    double *g = geom + 6 * (size_t)t;
+    g[0] = R0; g[1] = Z0;
+    g[2] = __ddiv_rn(e2Z, D);
+    g[3] = __ddiv_rn(-e2R, D);
+    g[4] = __ddiv_rn(-e1Z, D);
+    g[5] = __ddiv_rn(e1R, D);
+}
+
+// ====================================================================== a0: Bell expansion
+// 18 nodal DOFs -> 21 monomial coefficients, one thread per (triangle, mode).
+// No linear solve: DOFs are mapped to reference coordinates with the edge vectors, multiplied
+// by the fixed right inverse P18 of the vertex conditions, and the three edge bubbles are
+// scaled so that the normal derivative is cubic on every edge (see gen_bell_tables.py).
+__global__ void bell_kernel(int n_theta, int n_tri, int n_vert, int n_modes, const double *__restrict__ vR,
+                            const double *__restrict__ vZ, const double2 *__restrict__ dofs, double2 *__restrict__ coef)
+{
+    const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (idx >= (size_t)n_tri * n_modes) return;
+    const int t = (int)(idx / n_modes), m = (int)(idx % n_modes);
+    int v[3];
+    tri_vertices(n_theta, t, v);
+    const double e1R = vR[v[1]] - vR[v[0]], e1Z = vZ[v[1]] - vZ[v[0]];
+    const double e2R = vR[v[2]] - vR[v[0]], e2Z = vZ[v[2]] - vZ[v[0]];
+    double dr[18], di[18];
+#pragma unroll
+    for (int p = 0; p < 3; ++p) {
+        const double2 *d = dofs + ((size_t)m * n_vert + v[p]) * 6;
+        const double2 f = d[0], fR = d[1], fZ = d[2], fRR = d[3], fRZ = d[4], fZZ = d[5];
+#define TR(dst, X)                                                                                           \
+        dst[6 * p + 0] = f.X;                                                                                \
+        dst[6 * p + 1] = e1R * fR.X + e1Z * fZ.X;                                                            \
+        dst[6 * p + 2] = e2R * fR.X + e2Z * fZ.X;                                                            \
+        dst[6 * p + 3] = e1R * e1R * fRR.X + 2.0 * e1R * e1Z * fRZ.X + e1Z * e1Z * fZZ.X;                    \
+        dst[6 * p + 4] = e1R * e2R * fRR.X + (e1R * e2Z + e1Z * e2R) * fRZ.X + e1Z * e2Z * fZZ.X;            \
+        dst[6 * p + 5] = e2R * e2R * fRR.X + 2.0 * e2R * e2Z * fRZ.X + e2Z * e2Z * fZZ.X;
+        TR(dr, x)
+        TR(di, y)
+#undef TR
+    }
+    double cr[21], ci[21];
+#pragma unroll
+    for (int k = 0; k < 21; ++k) {
+        double sr = 0.0, si = 0.0;
+#pragma unroll
+        for (int q = 0; q < 18; ++q) { sr = fma(c_P18[k][q], dr[q], sr); si = fma(c_P18[k][q], di[q], si); }
+        cr[k] = sr; ci[k] = si;
+    }
+    // degree-5 coefficients c_{i, 5-i} sit at k = 15 + j, j = 5 - i
+    const double e11 = e1R * e1R + e1Z * e1Z, e22 = e2R * e2R + e2Z * e2Z, e12 = e1R * e2R + e1Z * e2Z;
+    const double ett = e11 - 2.0 * e12 + e22;                  // |e2 - e1|^2
+    // edge 0 (eta = 0): G = 5 a c50 + b c41, a = e1.e2, b = -e1.e1, G(bubble) = b
+    // edge 1 (xi = 0) : G = a c14 + 5 b c05, a = e2.e2, b = -e1.e2, G(bubble) = a
+    // edge 2 (l0 = 0) : G = sum c_ij [a i (-1)^(i-1) + b j (-1)^i], a = e22 - e12, b = e11 - e12, G(bubble) = -|t|^2
+    double z[3][2];
+    for (int part = 0; part < 2; ++part) {
+        const double *c = part ? ci : cr;
+        const double G0 = 5.0 * e12 * c[15] - e11 * c[16];
+        const double G1 = e22 * c[19] - 5.0 * e12 * c[20];
+        const double a2 = e22 - e12, b2 = e11 - e12;
+        double G2 = 0.0;
+#pragma unroll
+        for (int j = 0; j <= 5; ++j) {
+            const int i = 5 - j;
+            const double sa = (i >= 1) ? ((i - 1) & 1 ? -(double)i : (double)i) : 0.0;     // i (-1)^(i-1)
+            const double sb = (j >= 1) ? ((i & 1) ? -(double)j : (double)j) : 0.0;         // j (-1)^i
+            G2 += c[15 + j] * (a2 * sa + b2 * sb);
+        }
+        z[0][part] = G0 / e11;
+        z[1][part] = -G1 / e22;
+        z[2][part] = G2 / ett;
+    }
+    double2 *out = coef + ((size_t)t * n_modes + m) * NCOEF;
+#pragma unroll
+    for (int k = 0; k < 21; ++k) {
+        double2 o;
+        o.x = cr[k] + z[0][0] * c_bubble[0][k] + z[1][0] * c_bubble[1][k] + z[2][0] * c_bubble[2][k];
+        o.y = ci[k] + z[0][1] * c_bubble[0][k] + z[1][1] * c_bubble[1][k] + z[2][1] * c_bubble[2][k];
+        out[k] = o;
+    }
+}
+
+// =============================================================================== a1: cell sort
+// Counting sort: histogram over cells (lost markers in the last bin), exclusive scan of the
+// bins, scatter of the marker records to scratch, copy back.
+__global__ void hist_kernel(size_t n, const int32_t *__restrict__ cell, int n_tri, int *__restrict__ bins)
+{
+    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    int c = cell[p];
+    if (c < 0 || c >= n_tri) c = n_tri;
+    atomicAdd(bins + c, 1);
+}
+
+// single-block exclusive scan of nb ints, in place; bins[nb] receives the total
+__global__ void scan_kernel(int *bins, int nb)
+{
+    __shared__ int part[1024];
+    const int tid = threadIdx.x, nt = blockDim.x;
+    const int per = (nb + nt - 1) / nt;
+    const int lo = tid * per, hi = min(lo + per, nb);
+    int sum = 0;
+    for (int k = lo; k < hi; ++k) sum += bins[k];
+    part[tid] = sum;
+    __syncthreads();
+    for (int off = 1; off < nt; off <<= 1) {
+        const int v = (tid >= off) ? part[tid - off] : 0;
+        __syncthreads();
+        part[tid] += v;
+        __syncthreads();
+    }
+    int run = part[tid] - sum;
+    for (int k = lo; k < hi; ++k) { const int c = bins[k]; bins[k] = run; run += c; }
+    if (tid == nt - 1) bins[nb] = part[tid];
+}
+
+struct MarkerScratch { double *R, *Z, *phi, *vpar, *mu, *w; int32_t *cell; };
+
+__global__ void sort_scatter_kernel(size_t n, trimeg_markers m, int n_tri, int *__restrict__ cursor, MarkerScratch o,
+                                    int64_t *__restrict__ perm)
+{
+    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= n) return;
+    const int c0 = m.cell[p];
+    const int c = (c0 < 0 || c0 >= n_tri) ? n_tri : c0;
+    const size_t d = (size_t)atomicAdd(cursor + c, 1);
+    o.R[d] = m.R[p]; o.Z[d] = m.Z[p]; o.phi[d] = m.phi[p]; o.vpar[d] = m.vpar[p];
+    o.mu[d] = m.mu[p]; o.w[d] = m.w[p]; o.cell[d] = c0;
+    if (perm) perm[d] = (int64_t)p;
+}
+
+// ============================================================================== a6: compaction
+// Stable partition (active first) with warp ballots: per-block counts, scan, scatter.
+constexpr int CMP_BLOCK = 256;
+__global__ void compact_count_kernel(size_t n, const int32_t *__restrict__ cell, int *__restrict__ block_cnt)
+{
+    const size_t p = (size_t)blockIdx.x * CMP_BLOCK + threadIdx.x;
+    const int act = (p < n) && (cell[p] >= 0);
+    const int cnt = __syncthreads_count(act);
+    if (threadIdx.x == 0) block_cnt[blockIdx.x] = cnt;
+}
+__global__ void compact_scatter_kernel(size_t n, trimeg_markers m, const int *__restrict__ block_off, int n_blocks,
+                                       MarkerScratch o, int64_t *__restrict__ perm)
+{
+    __shared__ int warp_cnt[CMP_BLOCK / 32];
+    const size_t p = (size_t)blockIdx.x * CMP_BLOCK + threadIdx.x;
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const bool in = p < n;
+    const int c0 = in ? m.cell[p] : -1;
+    const bool act = in && c0 >= 0;
+    const unsigned bal = __ballot_sync(0xffffffffu, act);
+    if (lane == 0) warp_cnt[wid] = __popc(bal);
+    __syncthreads();
+    int before = 0;
+    for (int k = 0; k < wid; ++k) before += warp_cnt[k];
+    const int rank_in_warp = __popc(bal & ((1u << lane) - 1u));
+    if (!in) return;
+    const size_t n_active = (size_t)block_off[n_blocks];
+    size_t d;
+    if (act) d = (size_t)block_off[blockIdx.x] + before + rank_in_warp;
+    else {   // lost markers keep their relative order after the active ones
+        const size_t act_before = (size_t)block_off[blockIdx.x] + before + rank_in_warp;
+        d = n_active + (p - act_before);
+    }
+    o.R[d] = m.R[p]; o.Z[d] = m.Z[p]; o.phi[d] = m.phi[p]; o.vpar[d] = m.vpar[p];
+    o.mu[d] = m.mu[p]; o.w[d] = m.w[p]; o.cell[d] = c0;
+    if (perm) perm[d] = (int64_t)p;
+}
+
+// undo a permutation: dst[perm[d]] = src[d]
+__global__ void unpermute_kernel(size_t n, MarkerScratch src, trimeg_markers dst, const int64_t *__restrict__ perm)
+{
+    const size_t d = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (d >= n) return;
+    const size_t p = (size_t)perm[d];
+    dst.R[p] = src.R[d]; dst.Z[p] = src.Z[d]; dst.phi[p] = src.phi[d]; dst.vpar[p] = src.vpar[d];
+    dst.w[p] = src.w[d]; dst.cell[p] = src.cell[d];
+}
+
+// ================================================================== diagnostics: FP64 roofline
+// Dependent-chain-free DFMA loop: 8 independent accumulators per thread, enough warps to
+// saturate the FP64 pipe.  2 flops per DFMA.
+constexpr int PEAK_ITERS = 2048, PEAK_CHAINS = 8;
+__global__ void __launch_bounds__(256) dfma_peak_kernel(double *out, double a, double b)
+{
+    double acc[PEAK_CHAINS];
+#pragma unroll
+    for (int k = 0; k < PEAK_CHAINS; ++k) acc[k] = (double)(threadIdx.x + k);
+#pragma unroll 4
+    for (int it = 0; it < PEAK_ITERS; ++it) {
+#pragma unroll
+        for (int k = 0; k < PEAK_CHAINS; ++k) acc[k] = fma(acc[k], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < PEAK_CHAINS; ++k) s += acc[k];
+    if (s == 123.456) out[0] = s;          // never true; keeps the loop alive
+}
+
+// ================================================================================ host helpers
+static int ensure_scratch(trimeg_ctx *c, size_t bytes)
+{
+    if (c->scratch_bytes >= bytes) return TRIMEG_OK;
+    if (c->d_scratch) { cudaFree(c->d_scratch); c->d_scratch = nullptr; c->scratch_bytes = 0; }
+    if (cudaMalloc(&c->d_scratch, bytes) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_ALLOC; }
+    c->scratch_bytes = bytes;
+    return TRIMEG_OK;
+}
+static size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+// carve a marker SoA of capacity n out of a byte buffer; returns bytes used
+static size_t carve(char *base, size_t n, MarkerScratch &o)
+{
+    const size_t db = align_up(n * sizeof(double), 256);
+    if (!base) return 6 * db + align_up(n * sizeof(int32_t), 256);     // size query
+    o.R = (double *)base; o.Z = (double *)(base + db); o.phi = (double *)(base + 2 * db);
+    o.vpar = (double *)(base + 3 * db); o.mu = (double *)(base + 4 * db); o.w = (double *)(base + 5 * db);
+    o.cell = (int32_t *)(base + 6 * db);
+    return 6 * db + align_up(n * sizeof(int32_t), 256);
+}
+static void fill_phys(trimeg_ctx *c)
+{
+    const trimeg_params &p = c->params;
+    PhysDev &d = c->phys;
+    d.R0 = p.R0; d.B0 = p.B0; d.invB0 = 1.0 / p.B0; d.q0 = p.q0; d.qs = p.q2 / (p.a * p.a);
+    d.eps = p.rho0 * p.B0 / p.qs_over_ms;
+    d.rho0B0 = p.rho0 * p.B0;
+    d.qom = p.qs_over_ms;
+    d.invT = 1.0 / p.T; d.kappa_n = p.kappa_n; d.kappa_T = p.kappa_T;
+    d.eom_variant = p.eom_variant; d.weight_mode = p.weight_mode;
+}
+static int params_ok(const trimeg_params *p)
+{
+    return p && p->R0 > 0 && p->a > 0 && p->a < p->R0 && p->B0 != 0 && p->q0 > 0 && p->qs_over_ms != 0 && p->T > 0 &&
+           (p->eom_variant == 0 || p->eom_variant == 1) && (p->weight_mode == 0 || p->weight_mode == 1);
+}
+static int markers_ok(const trimeg_markers *m)
+{ return m && m->R && m->Z && m->phi && m->vpar && m->mu && m->w && m->cell; }
+
+// ===================================================================================== C ABI
+extern "C" {
+
+int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_nodes_host,
+                       const double *vert_R_host, const double *vert_Z_host, const trimeg_params *params)
+{
+    if (!out) return TRIMEG_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!r_nodes_host || n_r < 2 || n_theta < 3 || !params_ok(params)) return TRIMEG_ERR_INVALID_ARG;
+    if ((vert_R_host == nullptr) != (vert_Z_host == nullptr)) return TRIMEG_ERR_INVALID_ARG;
+    if ((long long)(2 * (long long)n_r - 1) * n_theta > 0x3fffffffLL) return TRIMEG_ERR_INVALID_ARG;
+    if (r_nodes_host[0] != 0.0) return TRIMEG_ERR_MESH;
+    for (int i = 0; i < n_r; ++i)
+        if (!(r_nodes_host[i + 1] > r_nodes_host[i])) return TRIMEG_ERR_MESH;
+    const double sag = 1.0 - cos(M_PI / n_theta);
+    for (int k = 0; k + 2 <= n_r; ++k)        // rule L4
+        if (!(r_nodes_host[k + 1] * sag < r_nodes_host[k + 2] - r_nodes_host[k + 1])) return TRIMEG_ERR_MESH;
+
+    trimeg_ctx *c = new (std::nothrow) trimeg_ctx;
+    if (!c) return TRIMEG_ERR_ALLOC;
+    memset(c, 0, sizeof(*c));
+    if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
+    cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device);
+    c->n_r = n_r; c->n_theta = n_theta;
+    c->n_vert = 1 + n_r * n_theta;
+    c->n_tri = (2 * n_r - 1) * n_theta;
+    c->params = *params;
+    fill_phys(c);
+
+    double *hR = (double *)malloc(sizeof(double) * c->n_vert), *hZ = (double *)malloc(sizeof(double) * c->n_vert);
+    if (!hR || !hZ) { free(hR); free(hZ); delete c; return TRIMEG_ERR_ALLOC; }
+    if (vert_R_host) {
+        memcpy(hR, vert_R_host, sizeof(double) * c->n_vert);
+        memcpy(hZ, vert_Z_host, sizeof(double) * c->n_vert);
+    } else {
+        hR[0] = params->R0; hZ[0] = 0.0;
+        for (int i = 1; i <= n_r; ++i)
+            for (int j = 0; j < n_theta; ++j) {
+                const double th = 2.0 * M_PI * j / n_theta;
+                hR[1 + (i - 1) * n_theta + j] = params->R0 + r_nodes_host[i] * cos(th);
+                hZ[1 + (i - 1) * n_theta + j] = r_nodes_host[i] * sin(th);
+            }
+    }
+    int rc = TRIMEG_OK;
+    double *d_rin2 = nullptr;
+    do {
+        if (cudaMalloc(&c->d_vR, sizeof(double) * c->n_vert) != cudaSuccess ||
+            cudaMalloc(&c->d_vZ, sizeof(double) * c->n_vert) != cudaSuccess ||
+            cudaMalloc(&c->d_r_nodes, sizeof(double) * (n_r + 1)) != cudaSuccess ||
+            cudaMalloc(&c->d_geom, sizeof(double) * 6 * (size_t)c->n_tri) != cudaSuccess ||
+            cudaMalloc(&c->d_bins, sizeof(int) * ((size_t)c->n_tri + 2)) != cudaSuccess ||
+            cudaMalloc(&c->d_stats, sizeof(Stats)) != cudaSuccess ||
+            cudaMalloc(&d_rin2, sizeof(double)) != cudaSuccess) { rc = TRIMEG_ERR_ALLOC; break; }
+        if (cudaMemcpy(c->d_vR, hR, sizeof(double) * c->n_vert, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_vZ, hZ, sizeof(double) * c->n_vert, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_r_nodes, r_nodes_host, sizeof(double) * (n_r + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemset(c->d_stats, 0, sizeof(Stats)) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        geom_kernel<<<(c->n_tri + 255) / 256, 256>>>(n_r, n_theta, c->n_tri, c->d_vR, c->d_vZ, c->d_geom, d_rin2);
+        c->n_launches++;
+        double rin2 = 0.0;
+        if (cudaGetLastError() != cudaSuccess ||
+            cudaMemcpy(&rin2, d_rin2, sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        c->mesh.n_r = n_r; c->mesh.n_theta = n_theta; c->mesh.n_tri = c->n_tri;
+        c->mesh.geom = c->d_geom; c->mesh.r_nodes = c->d_r_nodes;
+        c->mesh.Rax = hR[0]; c->mesh.Zax = hZ[0]; c->mesh.rin2 = rin2;
+        c->field.n_modes = 0; c->field.coef = nullptr; c->field.mode_n = nullptr;
+        c->field.n_first = 0; c->field.n_step = 0; c->field.is_ap = 1;
+        c->has_field = 0;
+    } while (0);
+    if (d_rin2) cudaFree(d_rin2);
+    free(hR); free(hZ);
+    if (rc != TRIMEG_OK) { cudaGetLastError(); trimeg_mesh_destroy(c); return rc; }
+    *out = c;
+    return TRIMEG_OK;
+}
+
+int trimeg_mesh_destroy(trimeg_ctx *c)
+{
+    if (!c) return TRIMEG_ERR_INVALID_ARG;
+    cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
+    cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch);
+    if (c->hstreams_ready) for (int k = 0; k < 3; ++k) cudaStreamDestroy(c->hstream[k]);
+    cudaGetLastError();
+    delete c;
+    return TRIMEG_OK;
+}
+
+int trimeg_mesh_info(const trimeg_ctx *c, int *n_vert, int *n_tri)
+{
+    if (!c) return TRIMEG_ERR_INVALID_ARG;
+    if (n_vert) *n_vert = c->n_vert;
+    if (n_tri) *n_tri = c->n_tri;
+    return TRIMEG_OK;
+}
+
+int trimeg_set_params(trimeg_ctx *c, const trimeg_params *p)
+{
+    if (!c || !params_ok(p)) return TRIMEG_ERR_INVALID_ARG;
+    c->params = *p;
+    fill_phys(c);
+    return TRIMEG_OK;
+}
+
+int trimeg_mesh_download_geom(trimeg_ctx *c, double *geom_dev, trimeg_stream stream)
+{
+    if (!c || !geom_dev) return TRIMEG_ERR_INVALID_ARG;
+    CU_TRY(cudaMemcpyAsync(geom_dev, c->d_geom, sizeof(double) * 6 * (size_t)c->n_tri, cudaMemcpyDeviceToDevice,
+                           (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, const void *data_dev, int kind,
+                        trimeg_stream stream)
+{
+    if (!c || n_modes < 0 || (kind != 0 && kind != 1)) return TRIMEG_ERR_INVALID_ARG;
+    if (n_modes > 0 && (!mode_n_host || !data_dev)) return TRIMEG_ERR_INVALID_ARG;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (n_modes != c->field.n_modes || !c->d_coef) {
+        // tables may still be in use by kernels enqueued earlier
+        CU_TRY(cudaDeviceSynchronize());
+        cudaFree(c->d_coef); cudaFree(c->d_mode_n);
+        c->d_coef = nullptr; c->d_mode_n = nullptr; c->has_field = 0; c->field.n_modes = 0;
+        if (n_modes > 0) {
+            if (cudaMalloc(&c->d_coef, sizeof(double2) * NCOEF * (size_t)c->n_tri * n_modes) != cudaSuccess ||
+                cudaMalloc(&c->d_mode_n, sizeof(int) * n_modes) != cudaSuccess) {
+                cudaGetLastError();
+                cudaFree(c->d_coef); c->d_coef = nullptr;
+                return TRIMEG_ERR_ALLOC;
+            }
+        }
+    }
+    c->field.n_modes = n_modes; c->field.coef = c->d_coef; c->field.mode_n = c->d_mode_n;
+    c->field.is_ap = 1; c->field.n_first = 0; c->field.n_step = 0;
+    if (n_modes > 0) {
+        c->field.n_first = mode_n_host[0];
+        c->field.n_step = (n_modes > 1) ? mode_n_host[1] - mode_n_host[0] : 0;
+        for (int k = 0; k < n_modes; ++k)
+            if (mode_n_host[k] != c->field.n_first + k * c->field.n_step) c->field.is_ap = 0;
+        CU_TRY(cudaMemcpyAsync(c->d_mode_n, mode_n_host, sizeof(int) * n_modes, cudaMemcpyHostToDevice, s));
+        CU_TRY(cudaStreamSynchronize(s));          // mode_n_host is not retained
+        if (kind == 1) {
+            CU_TRY(cudaMemcpyAsync(c->d_coef, data_dev, sizeof(double2) * NCOEF * (size_t)c->n_tri * n_modes,
+                                   cudaMemcpyDeviceToDevice, s));
+        } else {
+            const size_t work = (size_t)c->n_tri * n_modes;
+            bell_kernel<<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR,
+                                                                       c->d_vZ, (const double2 *)data_dev, c->d_coef);
+            c->n_launches++;
+            CU_TRY(cudaGetLastError());
+        }
+    }
+    c->has_field = 1;
+    return TRIMEG_OK;
+}
+
+int trimeg_field_download_coeffs(trimeg_ctx *c, void *coeffs_dev, trimeg_stream stream)
+{
+    if (!c || !coeffs_dev) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (c->field.n_modes == 0) return TRIMEG_OK;
+    CU_TRY(cudaMemcpyAsync(coeffs_dev, c->d_coef, sizeof(double2) * NCOEF * (size_t)c->n_tri * c->field.n_modes,
+                           cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_locate(trimeg_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell, trimeg_stream stream)
+{
+    if (!c || (n > 0 && (!R || !Z || !cell))) return TRIMEG_ERR_INVALID_ARG;
+    CU_TRY(launch_locate(c, n, R, Z, cell, (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_gather(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi,
+                  const int32_t *cell_hint, double *dphi, double *dphi_dR, double *dphi_dZ, double *dphi_dphi,
+                  trimeg_stream stream)
+{
+    if (!c || (n > 0 && (!R || !Z || !phi || !dphi || !dphi_dR || !dphi_dZ))) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    CU_TRY(launch_gather(c, n, R, Z, phi, cell_hint, dphi, dphi_dR, dphi_dZ, dphi_dphi, (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_rhs(trimeg_ctx *c, const trimeg_markers *m, size_t n, double *dRdt, double *dZdt, double *dphidt,
+               double *dvpardt, double *dwdt, trimeg_stream stream)
+{
+    if (!c || (n > 0 && (!markers_ok(m) || !dRdt || !dZdt || !dphidt || !dvpardt || !dwdt))) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (n == 0) return TRIMEG_OK;
+    CU_TRY(launch_rhs(c, *m, n, dRdt, dZdt, dphidt, dvpardt, dwdt, (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_push(trimeg_ctx *c, trimeg_markers *m, size_t n, double dt, int nsteps, trimeg_stream stream)
+{
+    if (!c || nsteps < 0 || (n > 0 && !markers_ok(m)) || !(dt == dt)) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (n == 0) return TRIMEG_OK;
+    CU_TRY(launch_push(c, *m, n, dt, nsteps, (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+static int copy_back(trimeg_markers *m, const MarkerScratch &o, size_t n, cudaStream_t s)
+{
+    const size_t db = n * sizeof(double);
+    CU_TRY(cudaMemcpyAsync(m->R, o.R, db, cudaMemcpyDeviceToDevice, s));
+    CU_TRY(cudaMemcpyAsync(m->Z, o.Z, db, cudaMemcpyDeviceToDevice, s));
+    CU_TRY(cudaMemcpyAsync(m->phi, o.phi, db, cudaMemcpyDeviceToDevice, s));
+    CU_TRY(cudaMemcpyAsync(m->vpar, o.vpar, db, cudaMemcpyDeviceToDevice, s));
+    CU_TRY(cudaMemcpyAsync(m->mu, o.mu, db, cudaMemcpyDeviceToDevice, s));
+    CU_TRY(cudaMemcpyAsync(m->w, o.w, db, cudaMemcpyDeviceToDevice, s));
+    CU_TRY(cudaMemcpyAsync(m->cell, o.cell, n * sizeof(int32_t), cudaMemcpyDeviceToDevice, s));
+    return TRIMEG_OK;
+}
+
+static int sort_into(trimeg_ctx *c, const trimeg_markers &m, size_t n, const MarkerScratch &o, int64_t *perm,
+                     int *bins, cudaStream_t s)
+{
+    const int nb = c->n_tri + 1;
+    CU_TRY(cudaMemsetAsync(bins, 0, sizeof(int) * (nb + 1), s));
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    hist_kernel<<<grid, 256, 0, s>>>(n, m.cell, c->n_tri, bins);
+    scan_kernel<<<1, 1024, 0, s>>>(bins, nb);
+    sort_scatter_kernel<<<grid, 256, 0, s>>>(n, m, c->n_tri, bins, o, perm);
+    c->n_launches += 3;
+    CU_TRY(cudaGetLastError());
+    return TRIMEG_OK;
+}
+
+int trimeg_sort(trimeg_ctx *c, trimeg_markers *m, size_t n, int64_t *perm_dev, trimeg_stream stream)
+{
+    if (!c || (n > 0 && !markers_ok(m)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    if (n == 0) return TRIMEG_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    MarkerScratch o;
+    const size_t need = carve(nullptr, n, o);
+    int rc = ensure_scratch(c, need);
+    if (rc) return rc;
+    carve((char *)c->d_scratch, n, o);
+    rc = sort_into(c, *m, n, o, perm_dev, c->d_bins, s);
+    if (rc) return rc;
+    return copy_back(m, o, n, s);
+}
+
+int trimeg_compact(trimeg_ctx *c, trimeg_markers *m, size_t n, int64_t *perm_dev, size_t *n_active_host,
+                   trimeg_stream stream)
+{
+    if (!c || (n > 0 && !markers_ok(m)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    if (n == 0) { if (n_active_host) *n_active_host = 0; return TRIMEG_OK; }
+    cudaStream_t s = (cudaStream_t)stream;
+    MarkerScratch o;
+    const size_t nblk = (n + CMP_BLOCK - 1) / CMP_BLOCK;
+    const size_t rec = carve(nullptr, n, o);
+    int rc = ensure_scratch(c, rec + align_up((nblk + 1) * sizeof(int), 256));
+    if (rc) return rc;
+    carve((char *)c->d_scratch, n, o);
+    int *blk = (int *)((char *)c->d_scratch + rec);
+    compact_count_kernel<<<(unsigned)nblk, CMP_BLOCK, 0, s>>>(n, m->cell, blk);
+    scan_kernel<<<1, 1024, 0, s>>>(blk, (int)nblk);
+    compact_scatter_kernel<<<(unsigned)nblk, CMP_BLOCK, 0, s>>>(n, *m, blk, (int)nblk, o, perm_dev);
+    c->n_launches += 3;
+    CU_TRY(cudaGetLastError());
+    rc = copy_back(m, o, n, s);
+    if (rc) return rc;
+    int total = 0;
+    CU_TRY(cudaMemcpyAsync(&total, blk + nblk, sizeof(int), cudaMemcpyDeviceToHost, s));
+    CU_TRY(cudaStreamSynchronize(s));
+    if (n_active_host) *n_active_host = (size_t)total;
+    return TRIMEG_OK;
+}
+
+// Host-buffer path: chunks round-robin over three streams so that the H2D copy of chunk k+1
+// and the D2H copy of chunk k-1 overlap the push of chunk k.
+int trimeg_push_host(trimeg_ctx *c, trimeg_markers *mh, size_t n, double dt, int nsteps, int locate_first)
+{
+    if (!c || nsteps < 0 || (n > 0 && !markers_ok(mh)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (n == 0) return TRIMEG_OK;
+    if (!c->hstreams_ready) {
+        for (int k = 0; k < 3; ++k) CU_TRY(cudaStreamCreateWithFlags(&c->hstream[k], cudaStreamNonBlocking));
+        c->hstreams_ready = 1;
+    }
+    const size_t chunk = (n < ((size_t)1 << 21)) ? n : ((size_t)1 << 21);
+    const size_t n_chunks = (n + chunk - 1) / chunk;
+    const int n_slots = (n_chunks < 3) ? (int)n_chunks : 3;
+    MarkerScratch a, b;
+    const size_t rec = carve(nullptr, chunk, a);
+    const size_t permb = align_up(chunk * sizeof(int64_t), 256);
+    const size_t slot = 2 * rec + permb;
+    // sort scratch is the context scratch; slots live in a separate allocation for this call
+    char *buf = nullptr;
+    if (cudaMalloc(&buf, slot * n_slots) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_ALLOC; }
+    int rc = TRIMEG_OK;
+    int *bins_slot[3] = {nullptr, nullptr, nullptr};
+    for (int k = 0; k < n_slots && rc == TRIMEG_OK; ++k)
+        if (cudaMalloc(&bins_slot[k], sizeof(int) * ((size_t)c->n_tri + 2)) != cudaSuccess) { cudaGetLastError(); rc = TRIMEG_ERR_ALLOC; }
+    for (size_t k = 0; k < n_chunks && rc == TRIMEG_OK; ++k) {
+        const int sl = (int)(k % n_slots);
+        cudaStream_t s = c->hstream[sl];
+        const size_t lo = k * chunk, cnt = (lo + chunk <= n) ? chunk : n - lo;
+        char *base = buf + slot * sl;
+        carve(base, chunk, a);
+        carve(base + rec, chunk, b);
+        int64_t *perm = (int64_t *)(base + 2 * rec);
+        const size_t db = cnt * sizeof(double);
+#define H2D(dst, src, bytes) if (rc == TRIMEG_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA
+#define D2H(dst, src, bytes) if (rc == TRIMEG_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA
+        H2D(a.R, mh->R + lo, db); H2D(a.Z, mh->Z + lo, db); H2D(a.phi, mh->phi + lo, db);
+        H2D(a.vpar, mh->vpar + lo, db); H2D(a.mu, mh->mu + lo, db); H2D(a.w, mh->w + lo, db);
+        if (!locate_first) H2D(a.cell, mh->cell + lo, cnt * sizeof(int32_t));
+        if (rc != TRIMEG_OK) break;
+        trimeg_markers ma = {a.R, a.Z, a.phi, a.vpar, a.mu, a.w, a.cell};
+        trimeg_markers mb = {b.R, b.Z, b.phi, b.vpar, b.mu, b.w, b.cell};
+        if (locate_first && launch_locate(c, cnt, a.R, a.Z, a.cell, s) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        rc = sort_into(c, ma, cnt, b, perm, bins_slot[sl], s);        // a -> b (sorted)
+        if (rc != TRIMEG_OK) break;
+        if (launch_push(c, mb, cnt, dt, nsteps, s) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        unpermute_kernel<<<(unsigned)((cnt + 255) / 256), 256, 0, s>>>(cnt, b, ma, perm);   // b -> a (caller order)
+        c->n_launches++;
+        if (cudaGetLastError() != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        D2H(mh->R + lo, a.R, db); D2H(mh->Z + lo, a.Z, db); D2H(mh->phi + lo, a.phi, db);
+        D2H(mh->vpar + lo, a.vpar, db); D2H(mh->w + lo, a.w, db);
+        D2H(mh->cell + lo, a.cell, cnt * sizeof(int32_t));
+#undef H2D
+#undef D2H
+    }
+    for (int k = 0; k < 3; ++k)
+        if (c->hstreams_ready && cudaStreamSynchronize(c->hstream[k]) != cudaSuccess && rc == TRIMEG_OK) rc = TRIMEG_ERR_CUDA;
+    for (int k = 0; k < 3; ++k) cudaFree(bins_slot[k]);
+    cudaFree(buf);
+    if (rc != TRIMEG_OK) cudaGetLastError();
+    return rc;
+}
+
+int trimeg_get_stats(trimeg_ctx *c, int64_t *n_lost, int64_t *n_relocated, int64_t *n_launches)
+{
+    if (!c) return TRIMEG_ERR_INVALID_ARG;
+    Stats h;
+    CU_TRY(cudaDeviceSynchronize());
+    CU_TRY(cudaMemcpy(&h, c->d_stats, sizeof(Stats), cudaMemcpyDeviceToHost));
+    if (n_lost) *n_lost = (int64_t)h.n_lost;
+    if (n_relocated) *n_relocated = (int64_t)h.n_moved;
+    if (n_launches) *n_launches = c->n_launches;
+    return TRIMEG_OK;
+}
+
+int trimeg_reset_stats(trimeg_ctx *c)
+{
+    if (!c) return TRIMEG_ERR_INVALID_ARG;
+    CU_TRY(cudaDeviceSynchronize());
+    CU_TRY(cudaMemset(c->d_stats, 0, sizeof(Stats)));
+    c->n_launches = 0;
+    return TRIMEG_OK;
+}
+
+int trimeg_measure_fp64_peak(trimeg_ctx *c, double *tflops_out)
+{
+    if (!c || !tflops_out) return TRIMEG_ERR_INVALID_ARG;
+    int rc = ensure_scratch(c, 256);
+    if (rc) return rc;
+    cudaEvent_t e0, e1;
+    CU_TRY(cudaEventCreate(&e0));
+    CU_TRY(cudaEventCreate(&e1));
+    const int blocks = c->n_sm * 32;
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, 0);
+        dfma_peak_kernel<<<blocks, 256>>>((double *)c->d_scratch, 0.999999, 1e-9);
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaGetLastError(); rc = TRIMEG_ERR_CUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double flops = 2.0 * PEAK_ITERS * PEAK_CHAINS * 256.0 * blocks;
+        const double tf = flops / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+        c->n_launches++;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *tflops_out = best;
+    return rc;
+}
+
+const char *trimeg_strerror(int code)
+{
+    switch (code) {
+    case TRIMEG_OK: return "ok";
+    case TRIMEG_ERR_INVALID_ARG: return "invalid argument";
+    case TRIMEG_ERR_MESH: return "invalid mesh (nodes not increasing, r_0 != 0, or sagitta rule violated)";
+    case TRIMEG_ERR_NO_FIELD: return "no field uploaded";
+    case TRIMEG_ERR_CUDA: return "CUDA error";
+    case TRIMEG_ERR_ALLOC: return "allocation failed";
+    default: return "unknown error";
+    }
+}
+
+const char *trimeg_version(void) { return "libtrimeg 0.1 (sm_100a)"; }
+
+}  // extern "C"
