@@ -216,15 +216,16 @@ class Context:
                                  _stream(stream)), "trimeg_rhs")
         return out
 
-    def sort(self, m: Dict[str, torch.Tensor], want_perm: bool = False, stream=None) -> Optional[torch.Tensor]:
-        n = m["R"].numel()
+    def sort(self, m: Dict[str, torch.Tensor], want_perm: bool = False, n: Optional[int] = None,
+             stream=None) -> Optional[torch.Tensor]:
+        n = m["R"].numel() if n is None else int(n)
         ms = _markers(m, n)
         perm = torch.empty(n, dtype=torch.int64, device=m["R"].device) if want_perm else None
         _check(self.L.trimeg_sort(self.h, C.byref(ms), n, _ptr(perm, torch.int64), _stream(stream)), "trimeg_sort")
         return perm
 
-    def compact(self, m: Dict[str, torch.Tensor], want_perm: bool = False, stream=None):
-        n = m["R"].numel()
+    def compact(self, m: Dict[str, torch.Tensor], want_perm: bool = False, n: Optional[int] = None, stream=None):
+        n = m["R"].numel() if n is None else int(n)
         ms = _markers(m, n)
         perm = torch.empty(n, dtype=torch.int64, device=m["R"].device) if want_perm else None
         na = C.c_size_t(0)
