@@ -15,7 +15,7 @@ def _declared_symbols():
     for h in glob.glob(os.path.join(ROOT, "include", "*.h")):
         src = open(h).read()
         src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-        names |= set(re.findall(r"\b(trimeg_[a-z_]+)\s*\(", src))
+        names |= set(re.findall(r"\b(trimeg_[a-z0-9_]+)\s*\(", src))
     return sorted(names)
 
 
