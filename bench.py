@@ -187,6 +187,8 @@ def run_gpu(args, wl):
     sort_every = max(1, min(args.sort_every, wl.nsteps))
     ctx = binding.context_for(wl, inputs)
     ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).to(dev), kind=0)
+    if args.push_kernel >= 0:
+        ctx.set_push_kernel(args.push_kernel)
     m_np = inputs.markers(wl, n=n, seed=D.rank_seed(wl.seed, rank))
     d = binding.markers_to_device(m_np, dev)
     ctx.locate(d["R"], d["Z"], cell=d["cell"])
@@ -316,6 +318,7 @@ def main():
     ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg5"])
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
+    ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()

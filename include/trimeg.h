@@ -160,6 +160,13 @@ int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_d
  * its index (use trimeg_compact to drop it).  Markers are not reordered. */
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
+/* Kernel used by trimeg_push / trimeg_push_host (same results, different schedules):
+ *   0  one thread per marker;
+ *   1..4  triangle-batched tiles: a CTA keeps a tile of markers in shared memory, re-bins them
+ *         by triangle at every RK4 stage and evaluates P markers of one triangle per lane off a
+ *         single load of each coefficient (1: P=2, 192 threads; 2: P=2, 384; 3: P=4, 128; 4: P=4, 256).
+ * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct. */
+int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 
 /* ---- end-to-end push from HOST buffers -------------------------------------------------------
  * Same result as: copy the seven arrays to the device, trimeg_locate if locate_first != 0,

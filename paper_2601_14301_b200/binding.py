@@ -19,7 +19,7 @@ EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_sort", "trimeg_compact",
-    "trimeg_push", "trimeg_push_host", "trimeg_get_stats", "trimeg_reset_stats",
+    "trimeg_push", "trimeg_set_push_kernel", "trimeg_push_host", "trimeg_get_stats", "trimeg_reset_stats",
     "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
 )
 
@@ -70,6 +70,7 @@ def load() -> C.CDLL:
     L.trimeg_sort.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp]
     L.trimeg_compact.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, C.POINTER(sz), vp]
     L.trimeg_push.argtypes = [vp, C.POINTER(trimeg_markers), sz, dbl, i32, vp]
+    L.trimeg_set_push_kernel.argtypes = [vp, i32]
     L.trimeg_push_host.argtypes = [vp, C.POINTER(trimeg_markers), sz, dbl, i32, i32]
     L.trimeg_get_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.trimeg_reset_stats.argtypes = [vp]
@@ -237,6 +238,9 @@ class Context:
         n = m["R"].numel() if n is None else int(n)
         ms = _markers(m, n)
         _check(self.L.trimeg_push(self.h, C.byref(ms), n, float(dt), int(nsteps), _stream(stream)), "trimeg_push")
+
+    def set_push_kernel(self, variant: int):
+        _check(self.L.trimeg_set_push_kernel(self.h, int(variant)), "trimeg_set_push_kernel")
 
     def push_host(self, m_host: Dict[str, torch.Tensor], dt: float, nsteps: int, locate_first: bool = True):
         n = m_host["R"].numel()

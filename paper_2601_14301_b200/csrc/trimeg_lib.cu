@@ -356,6 +356,8 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
         c->field.n_modes = 0; c->field.coef = nullptr; c->field.mode_n = nullptr;
         c->field.n_first = 0; c->field.n_step = 0; c->field.is_ap = 1;
         c->has_field = 0;
+        c->push_kernel = 0;
+        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= 0 && v <= 4) c->push_kernel = v; }
     } while (0);
     if (d_rin2) cudaFree(d_rin2);
     free(hR); free(hZ);
@@ -388,6 +390,13 @@ int trimeg_set_params(trimeg_ctx *c, const trimeg_params *p)
     if (!c || !params_ok(p)) return TRIMEG_ERR_INVALID_ARG;
     c->params = *p;
     fill_phys(c);
+    return TRIMEG_OK;
+}
+
+int trimeg_set_push_kernel(trimeg_ctx *c, int variant)
+{
+    if (!c || variant < 0 || variant > 4) return TRIMEG_ERR_INVALID_ARG;
+    c->push_kernel = variant;
     return TRIMEG_OK;
 }
 

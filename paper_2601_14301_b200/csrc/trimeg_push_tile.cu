@@ -1,0 +1,407 @@
+// trimeg_push_tile.cu -- triangle-batched fused RK4 push (rows a2-a6 of DESIGN.md §1).
+//
+// Why: with one thread per marker every lane fetches every coefficient of its triangle
+// itself (21 x 16-byte loads per mode and stage); on B200 a warp-wide load costs 2-4 cycles
+// of the SM's load/store data pipe even when all lanes read the same address, so the load
+// path, not the FP64 pipe, bounds the kernel (profiles/r01_baseline_push_kernel.md).  The
+// only way to lower load-pipe cycles per FP64 operation is to let one loaded coefficient
+// feed several markers from a REGISTER.  That needs the markers evaluated together to sit
+// in the same triangle, which a cell sort alone cannot keep true for long: markers drift
+// across edges between sorts.
+//
+// How: one CTA owns a tile of NT consecutive markers for the whole call; their RK4 state
+// lives in shared memory.  Every RK4 stage is five block-synchronous phases:
+//   A  locate the stage position of every marker (hinted walk, bit-exact rule O3) and bin
+//      it by triangle in a small open-addressing hash table (warp-aggregated atomics);
+//   B  exclusive scan of the bin counts, each bin padded to a multiple of P slots;
+//   C  scatter (xi, eta, phi, owner) of every marker to its evaluation slot;
+//   D  evaluation: each thread takes P consecutive slots -- by construction the same
+//      triangle -- and runs the bivariate Horner scheme for all P markers off ONE load of
+//      each coefficient; lanes of a warp mostly share the triangle too, so the loads are
+//      warp-uniform L1 hits;
+//   E  each marker reads back its field values, evaluates equilibrium + equations of motion
+//      (a4, a5) and does its RK4 bookkeeping (a6).
+// Markers whose triangle finds no bin (table full) are evaluated by their owner with the
+// one-marker gather of trimeg_device.cuh -- slower, same arithmetic.  The arithmetic of
+// every marker (order of operations, fused multiply-adds) is the same as in push_kernel.
+#include "trimeg_internal.h"
+
+namespace trimeg {
+
+namespace {
+
+constexpr double TWO_PI = 6.283185307179586476925286766559;
+constexpr int NBIN = 64;            // hash bins per stage (distinct triangles of a tile)
+constexpr int NPROBE = 8;
+constexpr int BIN_EMPTY = -1;
+
+enum : unsigned char { FL_ACTIVE = 1, FL_LOST = 2, FL_MOVED = 4, FL_WASACTIVE = 8 };
+
+// indices of the per-marker fp64 state arrays in shared memory
+enum { S_R, S_Z, S_P, S_V, S_W, S_MU, A_R, A_Z, A_P, A_V, A_W, Y_R, Y_Z, Y_P, Y_V, Y_W, N_STATE };
+// S_* = stage position, A_* = RK4 accumulator k1 + 2 k2 + 2 k3, Y_* = start-of-step state
+
+template <int P, int T>
+struct TileCfg {
+    static constexpr int NT = P * T - 12 * P;                 // markers per tile (slack for bin padding)
+    static constexpr int NE = NT + (P - 1) * NBIN;            // evaluation slots, worst case
+    static constexpr size_t smem_bytes()
+    {
+        return sizeof(double) * ((size_t)N_STATE * NT + 4 * (size_t)NE) +
+               sizeof(int) * (3 * (size_t)NT + 2 * (size_t)NE + 3 * NBIN + 8) + NT;
+    }
+};
+
+__device__ __forceinline__ unsigned hash_tri(int t) { return ((unsigned)t * 0x9E3779B1u) >> 26; }   // 6 bits
+
+// P markers, one triangle: complex quintic and its xi / eta derivatives by bivariate Horner
+// (same operation order per marker as eval_quintic), every coefficient loaded once.
+template <int P>
+__device__ __forceinline__ void eval_quintic_multi(const double2 *__restrict__ c, const double (&xi)[P],
+                                                   const double (&eta)[P], double (&pr)[P], double (&pi)[P],
+                                                   double (&pxr)[P], double (&pxi)[P], double (&per)[P],
+                                                   double (&pei)[P])
+{
+    double ar[P], ai[P], dr[P], di[P];
+#pragma unroll
+    for (int j = 5; j >= 0; --j) {
+        const int n = 5 - j;
+#pragma unroll
+        for (int i = n; i >= 0; --i) {
+            const double2 cc = __ldg(c + kidx(i, j));
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                if (i == n) { ar[p] = cc.x; ai[p] = cc.y; dr[p] = 0.0; di[p] = 0.0; }
+                else {
+                    if (i == n - 1) { dr[p] = ar[p]; di[p] = ai[p]; }
+                    else { dr[p] = fma(dr[p], xi[p], ar[p]); di[p] = fma(di[p], xi[p], ai[p]); }
+                    ar[p] = fma(ar[p], xi[p], cc.x); ai[p] = fma(ai[p], xi[p], cc.y);
+                }
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            if (j == 5) { pr[p] = ar[p]; pi[p] = ai[p]; }
+            else {
+                if (j == 4) { per[p] = pr[p]; pei[p] = pi[p]; pxr[p] = dr[p]; pxi[p] = di[p]; }
+                else {
+                    per[p] = fma(per[p], eta[p], pr[p]); pei[p] = fma(pei[p], eta[p], pi[p]);
+                    pxr[p] = fma(pxr[p], eta[p], dr[p]); pxi[p] = fma(pxi[p], eta[p], di[p]);
+                }
+                pr[p] = fma(pr[p], eta[p], ar[p]); pi[p] = fma(pi[p], eta[p], ai[p]);
+            }
+        }
+    }
+}
+
+// dphi, d/dxi, d/deta, d/dphi for P markers of triangle t (same formulas as gather())
+template <int P>
+__device__ __forceinline__ void gather_multi(const FieldDev &F, int t, const double (&xi)[P], const double (&eta)[P],
+                                             const double (&phi)[P], double (&f)[P], double (&fx)[P], double (&fe)[P],
+                                             double (&fp)[P])
+{
+    const double2 *c = F.coef + (size_t)t * F.n_modes * NCOEF;
+    double Er[P], Ei[P], Dr[P], Di[P];
+#pragma unroll
+    for (int p = 0; p < P; ++p) {
+        f[p] = fx[p] = fe[p] = fp[p] = 0.0;
+        Er[p] = 1.0; Ei[p] = 0.0; Dr[p] = 1.0; Di[p] = 0.0;
+        if (F.is_ap) {
+            if (F.n_first != 0) sincos((double)F.n_first * phi[p], &Ei[p], &Er[p]);
+            if (F.n_modes > 1) sincos((double)F.n_step * phi[p], &Di[p], &Dr[p]);
+        }
+    }
+    double nn = (double)F.n_first;
+#pragma unroll 1
+    for (int m = 0; m < F.n_modes; ++m, c += NCOEF) {
+        if (!F.is_ap) {
+            nn = (double)__ldg(F.mode_n + m);
+#pragma unroll
+            for (int p = 0; p < P; ++p) sincos(nn * phi[p], &Ei[p], &Er[p]);
+        }
+        double pr[P], pi[P], pxr[P], pxi[P], per[P], pei[P];
+        eval_quintic_multi<P>(c, xi, eta, pr, pi, pxr, pxi, per, pei);
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            f[p] = fma(pr[p], Er[p], fma(-pi[p], Ei[p], f[p]));
+            fx[p] = fma(pxr[p], Er[p], fma(-pxi[p], Ei[p], fx[p]));
+            fe[p] = fma(per[p], Er[p], fma(-pei[p], Ei[p], fe[p]));
+            fp[p] = fma(-nn, fma(pi[p], Er[p], pr[p] * Ei[p]), fp[p]);          // Re(i n P E)
+            if (F.is_ap) {                                                      // E_{n + dn} = E_n E_dn
+                const double tr = fma(Er[p], Dr[p], -Ei[p] * Di[p]);
+                Ei[p] = fma(Er[p], Di[p], Ei[p] * Dr[p]);
+                Er[p] = tr;
+            }
+        }
+        if (F.is_ap) nn += (double)F.n_step;
+    }
+}
+
+template <int P, int T>
+__global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
+                                                      double dt, int nsteps, Stats *st)
+{
+    using Cfg = TileCfg<P, T>;
+    constexpr int NT = Cfg::NT, NE = Cfg::NE;
+    extern __shared__ double smem_d[];
+    double *S = smem_d;                                   // [N_STATE][NT]
+    double *EV = S + (size_t)N_STATE * NT;                // [4][NE]: in (xi, eta, phi, -) / out (f, fR, fZ, fphi)
+    int *cell = reinterpret_cast<int *>(EV + 4 * (size_t)NE);   // [NT] current triangle (hint)
+    int *binrank = cell + NT;                             // [NT] bin << 16 | rank, -1 = not binned
+    int *slot = binrank + NT;                             // [NT] evaluation slot of the marker
+    int *ev_own = slot + NT;                              // [NE] owner marker of a slot, -1 = padding
+    int *ev_tri = ev_own + NE;                            // [NE] triangle of a slot
+    int *tag = ev_tri + NE;                               // [NBIN] triangle of a bin
+    int *cnt = tag + NBIN;                                // [NBIN]
+    int *off = cnt + NBIN;                                // [NBIN]
+    int *misc = off + NBIN;                               // [0] = number of evaluation slots, [1] lost, [2] moved
+    unsigned char *flags = reinterpret_cast<unsigned char *>(misc + 8);   // [NT]
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const size_t base = (size_t)blockIdx.x * NT;
+    const int nt = (int)((n - base < (size_t)NT) ? (n - base) : (size_t)NT);
+    const bool has_field = F.n_modes > 0;
+    const double hdt = 0.5 * dt, dt6 = dt / 6.0;
+
+    // ---- load the tile
+    for (int q = tid; q < NT; q += T) {
+        unsigned char fl = 0;
+        int c = -1;
+        if (q < nt) {
+            const size_t g = base + q;
+            c = m.cell[g];
+            if (c >= 0) {
+                fl = FL_ACTIVE | FL_WASACTIVE;
+                S[Y_R * NT + q] = m.R[g]; S[Y_Z * NT + q] = m.Z[g]; S[Y_P * NT + q] = m.phi[g];
+                S[Y_V * NT + q] = m.vpar[g]; S[Y_W * NT + q] = m.w[g]; S[S_MU * NT + q] = m.mu[g];
+            }
+        }
+        cell[q] = c; flags[q] = fl;
+    }
+    if (tid < NBIN) { tag[tid] = BIN_EMPTY; cnt[tid] = 0; }
+    if (tid < 8) misc[tid] = 0;
+    __syncthreads();
+
+#pragma unroll 1
+    for (int step = 0; step < nsteps; ++step) {
+#pragma unroll 1
+        for (int stage = 0; stage < 4; ++stage) {
+            // ---------------------------------------------------------------- A: locate + bin
+#pragma unroll 1
+            for (int q0 = 0; q0 < NT; q0 += T) {
+                const int q = q0 + tid;
+                const bool act = (q < NT) && (flags[q] & FL_ACTIVE);
+                int t = -1;
+                if (act) {
+                    if (stage == 0) {
+#pragma unroll
+                        for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
+                    }
+                    Bary b;
+                    int moved = 0;
+                    t = locate(M, S[S_R * NT + q], S[S_Z * NT + q], cell[q], b, moved);
+                    unsigned char fl = flags[q];
+                    if (moved) fl |= FL_MOVED;
+                    if (t < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;     // dropped for the rest of the call
+                    else cell[q] = t;
+                    flags[q] = fl;
+                }
+                if (has_field) {
+                    // warp-aggregated insertion: one probe sequence and one atomicAdd per distinct triangle
+                    const bool ok = act && t >= 0;
+                    const int key = ok ? t : -1 - lane;
+                    const unsigned grp = __match_any_sync(0xffffffffu, key);
+                    const int leader = __ffs(grp) - 1;
+                    int bin = -1, rank0 = 0;
+                    if (ok && lane == leader) {
+                        unsigned h = hash_tri(t);
+#pragma unroll 1
+                        for (int pr = 0; pr < NPROBE; ++pr) {
+                            const int prev = atomicCAS(&tag[h], BIN_EMPTY, t);
+                            if (prev == BIN_EMPTY || prev == t) { bin = (int)h; break; }
+                            h = (h + 1) & (NBIN - 1);
+                        }
+                        if (bin >= 0) rank0 = atomicAdd(&cnt[bin], __popc(grp));
+                    }
+                    bin = __shfl_sync(0xffffffffu, bin, leader);
+                    rank0 = __shfl_sync(0xffffffffu, rank0, leader);
+                    if (q < NT) binrank[q] = (ok && bin >= 0) ? ((bin << 16) | (rank0 + __popc(grp & ((1u << lane) - 1u)))) : -1;
+                }
+            }
+            if (has_field) {
+                __syncthreads();
+                // ------------------------------------------------------------ B: scan of padded bin sizes
+                if (tid < 32) {
+                    int run = 0;
+#pragma unroll
+                    for (int k = 0; k < NBIN / 32; ++k) {
+                        const int b = k * 32 + lane;
+                        const int c = cnt[b];
+                        const int padded = (c + P - 1) / P * P;
+                        int incl = padded;
+#pragma unroll
+                        for (int o = 1; o < 32; o <<= 1) {
+                            const int v = __shfl_up_sync(0xffffffffu, incl, o);
+                            if (lane >= o) incl += v;
+                        }
+                        const int o0 = run + incl - padded;
+                        off[b] = o0;
+                        for (int e = o0 + c; e < o0 + padded; ++e) ev_own[e] = -1;      // padding slots
+                        run += __shfl_sync(0xffffffffu, incl, 31);
+                    }
+                    if (lane == 0) misc[0] = run;
+                }
+                __syncthreads();
+                // ------------------------------------------------------------ C: scatter to evaluation slots
+#pragma unroll 1
+                for (int q = tid; q < NT; q += T) {
+                    const int br = binrank[q];
+                    if (br >= 0) {
+                        const int e = off[br >> 16] + (br & 0xffff);
+                        const int t = cell[q];
+                        const Bary b = bary_rn(M, t, S[S_R * NT + q], S[S_Z * NT + q]);
+                        EV[e] = b.xi; EV[NE + e] = b.eta; EV[2 * NE + e] = S[S_P * NT + q];
+                        ev_own[e] = q; ev_tri[e] = t;
+                        slot[q] = e;
+                    }
+                }
+                __syncthreads();
+                // ------------------------------------------------------------ D: batched evaluation
+                const int n_ev = misc[0];
+                if (tid < NBIN) { tag[tid] = BIN_EMPTY; cnt[tid] = 0; }             // for the next stage
+#pragma unroll 1
+                for (int e0 = tid * P; e0 < n_ev; e0 += T * P) {
+                    const int t = ev_tri[e0];                                        // first slot of a group is real
+                    double xi[P], eta[P], phi[P], f[P], fx[P], fe[P], fp[P];
+                    bool real[P];
+#pragma unroll
+                    for (int p = 0; p < P; ++p) {
+                        real[p] = ev_own[e0 + p] >= 0;
+                        xi[p] = real[p] ? EV[e0 + p] : 0.0;
+                        eta[p] = real[p] ? EV[NE + e0 + p] : 0.0;
+                        phi[p] = real[p] ? EV[2 * NE + e0 + p] : 0.0;
+                    }
+                    gather_multi<P>(F, t, xi, eta, phi, f, fx, fe, fp);
+                    const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)t);
+                    const double2 gx = __ldg(g + 1), ge = __ldg(g + 2);
+#pragma unroll
+                    for (int p = 0; p < P; ++p) {
+                        if (real[p]) {
+                            EV[e0 + p] = f[p];
+                            EV[NE + e0 + p] = fma(gx.x, fx[p], ge.x * fe[p]);        // d/dR
+                            EV[2 * NE + e0 + p] = fma(gx.y, fx[p], ge.y * fe[p]);    // d/dZ
+                            EV[3 * NE + e0 + p] = fp[p];
+                        }
+                    }
+                }
+                __syncthreads();
+            }
+            // ---------------------------------------------------------------- E: equations + RK4
+#pragma unroll 1
+            for (int q = tid; q < NT; q += T) {
+                if (!(flags[q] & FL_ACTIVE)) continue;
+                const double R = S[S_R * NT + q], Z = S[S_Z * NT + q], ph = S[S_P * NT + q];
+                const double v = S[S_V * NT + q], w = S[S_W * NT + q], mu = S[S_MU * NT + q];
+                FieldVal fv;
+                fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
+                if (has_field) {
+                    if (binrank[q] >= 0) {
+                        const int e = slot[q];
+                        fv.f = EV[e]; fv.fR = EV[NE + e]; fv.fZ = EV[2 * NE + e]; fv.fphi = EV[3 * NE + e];
+                    } else {                               // no bin: one-marker gather, same arithmetic
+                        const int t = cell[q];
+                        const Bary b = bary_rn(M, t, R, Z);
+                        fv = gather(F, t, b, ph);
+                    }
+                }
+                const Rates k = rhs_point(Ph, R, Z, v, mu, w, fv);
+                const double yR = S[Y_R * NT + q], yZ = S[Y_Z * NT + q], yP = S[Y_P * NT + q];
+                const double yV = S[Y_V * NT + q], yW = S[Y_W * NT + q];
+                if (stage < 3) {
+                    if (stage == 0) {
+                        S[A_R * NT + q] = k.R; S[A_Z * NT + q] = k.Z; S[A_P * NT + q] = k.phi;
+                        S[A_V * NT + q] = k.vpar; S[A_W * NT + q] = k.w;
+                    } else {
+                        S[A_R * NT + q] = fma(2.0, k.R, S[A_R * NT + q]); S[A_Z * NT + q] = fma(2.0, k.Z, S[A_Z * NT + q]);
+                        S[A_P * NT + q] = fma(2.0, k.phi, S[A_P * NT + q]); S[A_V * NT + q] = fma(2.0, k.vpar, S[A_V * NT + q]);
+                        S[A_W * NT + q] = fma(2.0, k.w, S[A_W * NT + q]);
+                    }
+                    const double c = (stage == 2) ? dt : hdt;
+                    S[S_R * NT + q] = fma(c, k.R, yR); S[S_Z * NT + q] = fma(c, k.Z, yZ); S[S_P * NT + q] = fma(c, k.phi, yP);
+                    S[S_V * NT + q] = fma(c, k.vpar, yV); S[S_W * NT + q] = fma(c, k.w, yW);
+                } else {
+                    const double Rn = fma(dt6, S[A_R * NT + q] + k.R, yR), Zn = fma(dt6, S[A_Z * NT + q] + k.Z, yZ);
+                    double pn = fma(dt6, S[A_P * NT + q] + k.phi, yP);
+                    const double vn = fma(dt6, S[A_V * NT + q] + k.vpar, yV), wn = fma(dt6, S[A_W * NT + q] + k.w, yW);
+                    pn = fma(-TWO_PI, floor(pn * (1.0 / TWO_PI)), pn);
+                    Bary b;
+                    int moved = 0;
+                    const int c = locate(M, Rn, Zn, cell[q], b, moved);
+                    unsigned char fl = flags[q];
+                    if (moved) fl |= FL_MOVED;
+                    if (c < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;            // start-of-step state is kept
+                    else {
+                        cell[q] = c;
+                        S[Y_R * NT + q] = Rn; S[Y_Z * NT + q] = Zn; S[Y_P * NT + q] = pn;
+                        S[Y_V * NT + q] = vn; S[Y_W * NT + q] = wn;
+                    }
+                    flags[q] = fl;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---- write back, statistics
+    int lost = 0, moved = 0;
+    for (int q = tid; q < nt; q += T) {
+        const unsigned char fl = flags[q];
+        if (!(fl & FL_WASACTIVE)) continue;
+        const size_t g = base + q;
+        m.R[g] = S[Y_R * NT + q]; m.Z[g] = S[Y_Z * NT + q]; m.phi[g] = S[Y_P * NT + q];
+        m.vpar[g] = S[Y_V * NT + q]; m.w[g] = S[Y_W * NT + q];
+        m.cell[g] = (fl & FL_LOST) ? -1 : cell[q];
+        lost += (fl & FL_LOST) ? 1 : 0;
+        moved += (fl & FL_MOVED) ? 1 : 0;
+    }
+    lost = __reduce_add_sync(0xffffffffu, lost);
+    moved = __reduce_add_sync(0xffffffffu, moved);
+    if (lane == 0) {
+        if (lost) atomicAdd(&st->n_lost, (unsigned long long)lost);
+        if (moved) atomicAdd(&st->n_moved, (unsigned long long)moved);
+    }
+}
+
+template <int P, int T>
+cudaError_t launch_tile(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
+{
+    using Cfg = TileCfg<P, T>;
+    static bool configured = false;
+    const size_t shm = Cfg::smem_bytes();
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(push_tile_kernel<P, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    const size_t tiles = (n + Cfg::NT - 1) / Cfg::NT;
+    push_tile_kernel<P, T><<<(unsigned)tiles, T, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_push_tile(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
+                             cudaStream_t s)
+{
+    if (n == 0 || nsteps <= 0) return cudaSuccess;
+    switch (variant) {
+    case 1: return launch_tile<2, 192>(c, m, n, dt, nsteps, s);
+    case 2: return launch_tile<2, 384>(c, m, n, dt, nsteps, s);
+    case 3: return launch_tile<4, 128>(c, m, n, dt, nsteps, s);
+    case 4: return launch_tile<4, 256>(c, m, n, dt, nsteps, s);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace trimeg

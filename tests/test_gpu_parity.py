@@ -318,6 +318,76 @@ def test_non_arithmetic_mode_list(B, inputs):
         assert rel_err(got[k].cpu().numpy(), want[k], np.abs(want[k]).max()).max() < 1e-12
 
 
+# ----------------------------------------------------------------------------- tile kernels
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4])
+@pytest.mark.parametrize("name,n,nsteps,sort", [("cfg1", 4096, 20, False), ("cfg1", 1777, 3, True),
+                                                ("cfg2", (1 << 16) + 13, 3, True), ("cfg5", 40009, 5, True),
+                                                ("cfg3", 20011, 2, False)])
+def test_push_kernel_variants_match_oracle(B, inputs, variant, name, n, nsteps, sort):
+    """Every schedule of trimeg_push (trimeg_set_push_kernel) against the oracle: unsorted input
+    (markers of a tile spread over the whole mesh: hash bins overflow, one-marker fallback) and
+    cell-sorted input (the batched path), ragged tile tails, lost markers (cfg5)."""
+    wl, o, ctx, _, _ = _setup(B, inputs, name)
+    ctx.set_push_kernel(variant)
+    m = inputs.markers(wl, n=n)
+    if wl.sigma_w == 0.0:
+        m["w"] = np.random.default_rng(5).standard_normal(n) * 1e-4
+    want = o.push(m, wl.dt, nsteps)
+    d = _dev(B, m)
+    ctx.locate(d["R"], d["Z"], cell=d["cell"])
+    if sort:
+        perm = ctx.sort(d, want_perm=True).cpu().numpy()
+        want = {k: v[perm] for k, v in want.items()}
+        mu0 = m["mu"][perm]
+    else:
+        mu0 = m["mu"]
+    ctx.reset_stats()
+    outside_at_start = int((d["cell"] < 0).sum())
+    ctx.push(d, wl.dt, nsteps)
+    got = _host(d)
+    assert np.array_equal(got["cell"], want["cell"])
+    assert np.array_equal(got["mu"], mu0)
+    _assert_state_close(got, want, 1e-9 if nsteps > 5 else 1e-10, 1e-4)
+    assert ctx.get_stats()["n_lost"] == int((want["cell"] < 0).sum()) - outside_at_start
+
+
+@pytest.mark.parametrize("variant", [1, 4])
+def test_push_tile_kernel_edge_cases(B, inputs, variant):
+    """No field modes (weights bit-identical), already-lost markers on input are left untouched,
+    two calls equal one, non-arithmetic mode list."""
+    wl, o, ctx, _, _ = _setup(B, inputs, "cfg1", modes=())
+    ctx.set_push_kernel(variant)
+    m = inputs.markers(wl, n=1000)
+    m["w"] = np.random.default_rng(1).standard_normal(1000)
+    d = _dev(B, m)
+    ctx.locate(d["R"], d["Z"], cell=d["cell"])
+    d["cell"][::7] = -1
+    before = _host(d)
+    ctx.push(d, 0.05, 10)
+    got = _host(d)
+    assert np.array_equal(got["w"], m["w"])
+    dead = before["cell"] < 0
+    for k in ("R", "Z", "phi", "vpar", "w", "cell"):
+        assert np.array_equal(got[k][dead], before[k][dead]), k
+    want = o.push({k: v[~dead] for k, v in m.items()}, 0.05, 10)
+    _assert_state_close({k: v[~dead] for k, v in got.items()}, want, 1e-10, 1.0)
+    # two calls of 3 + 4 steps equal one call of 7; non-arithmetic mode list
+    wl2, o2, ctx2, dofs, coef = _setup(B, inputs, "cfg1", field=None, modes=(0, 1, 5))
+    ctx2.field_upload(wl2.modes, torch.from_numpy(coef).cuda(), kind=1)
+    ctx2.set_push_kernel(variant)
+    m2 = inputs.markers(wl2, n=3001)
+    want2 = o2.push(m2, wl2.dt, 7)
+    d2 = _dev(B, m2)
+    ctx2.locate(d2["R"], d2["Z"], cell=d2["cell"])
+    ctx2.sort(d2)
+    ctx2.push(d2, wl2.dt, 3)
+    ctx2.push(d2, wl2.dt, 4)
+    got2 = _host(d2)
+    order_got = np.lexsort((got2["mu"], got2["vpar"] * 0))          # mu is a unique, untouched key
+    order_want = np.lexsort((want2["mu"], want2["vpar"] * 0))
+    _assert_state_close({k: v[order_got] for k, v in got2.items()}, {k: v[order_want] for k, v in want2.items()}, 1e-10, 1e-4)
+
+
 # ----------------------------------------------------------------------------- a1 / a6 helpers
 def test_sort_is_a_valid_cell_ordered_permutation(B, inputs):
     wl, o, ctx, _, _ = _setup(B, inputs, "cfg5")
