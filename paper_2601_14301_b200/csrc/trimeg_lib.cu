@@ -356,7 +356,7 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
         c->field.n_modes = 0; c->field.coef = nullptr; c->field.mode_n = nullptr;
         c->field.n_first = 0; c->field.n_step = 0; c->field.is_ap = 1;
         c->has_field = 0;
-        c->push_kernel = 0;
+        c->push_kernel = 2;
         if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= 0 && v <= 4) c->push_kernel = v; }
     } while (0);
     if (d_rin2) cudaFree(d_rin2);
