@@ -240,6 +240,7 @@ def run_gpu(args, wl):
     seconds = t_start.elapsed_time(t_end) * 1e-3
     st1 = ctx.get_stats()
     launches = st1["n_launches"] - st0["n_launches"]
+    tile_counters = ctx.get_tile_counters()
 
     agg = D.aggregate(units, seconds, {"launches": launches}, device=dev)
 
@@ -262,6 +263,7 @@ def run_gpu(args, wl):
         "hbm_time_frac_of_fp64_time": t_hbm / t_fp64, "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
         "launches": n_push, "avg_launch_ms": push_s / max(1, n_push) * 1e3,
         "push_share_of_step": push_s / seconds,
+        "tile_counters": tile_counters,
     }
 
     line = None

@@ -162,10 +162,14 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
                 trimeg_stream stream);
 /* Kernel used by trimeg_push / trimeg_push_host (same results, different schedules):
  *   0  one thread per marker;
- *   1..4  triangle-batched tiles: a CTA keeps a tile of markers in shared memory, re-bins them
- *         by triangle at every RK4 stage and evaluates P markers of one triangle per lane off a
- *         single load of each coefficient (1: P=2, 192 threads; 2: P=2, 384; 3: P=4, 128; 4: P=4, 256).
- * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct. */
+ *   1..TRIMEG_PUSH_KERNEL_MAX  triangle-batched tiles: a CTA keeps a tile of markers in shared
+ *         memory, re-bins them by triangle at every RK4 stage, stages the coefficient records of
+ *         the tile's triangles in shared memory and evaluates P markers of one triangle per lane
+ *         off a single load of each coefficient (1: P=2, 192 threads; 2: P=2, 384; 3: P=4, 128;
+ *         4: P=4, 256; 5: P=3, 256; 6: P=3, 320).
+ * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
+ * INVALID_ARG for a variant outside 0..TRIMEG_PUSH_KERNEL_MAX. */
+#define TRIMEG_PUSH_KERNEL_MAX 6
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 
 /* ---- end-to-end push from HOST buffers -------------------------------------------------------
@@ -182,6 +186,12 @@ int trimeg_push_host(trimeg_ctx *ctx, trimeg_markers *m_host, size_t n, double d
  * Synchronises the device.  Any pointer may be NULL. */
 int trimeg_get_stats(trimeg_ctx *ctx, int64_t *n_lost, int64_t *n_relocated, int64_t *n_launches);
 int trimeg_reset_stats(trimeg_ctx *ctx);
+/* Diagnostics of the tile push kernels since the last reset, out8[0..7] (host): SM cycles that
+ * thread 0 of every CTA spent in phases A (locate + bin), B (records -> shared memory, scan),
+ * C (scatter), D (batched evaluation), E (equations + RK4), summed over CTAs; markers evaluated
+ * by the one-marker fallback; bins used, summed over stages; stages run, summed over CTAs.
+ * Synchronises the device.  DESIGN.md section 5. */
+int trimeg_get_tile_counters(trimeg_ctx *ctx, int64_t *out8_host);
 
 /* ---- diagnostics ------------------------------------------------------------------------------
  * Measured FP64 vector (DFMA) throughput of the current device in TFLOP/s (2 flops per DFMA),

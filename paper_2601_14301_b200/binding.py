@@ -19,7 +19,7 @@ EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_sort", "trimeg_compact",
-    "trimeg_push", "trimeg_set_push_kernel", "trimeg_push_host", "trimeg_get_stats", "trimeg_reset_stats",
+    "trimeg_push", "trimeg_set_push_kernel", "trimeg_push_host", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters",
     "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
 )
 
@@ -74,6 +74,7 @@ def load() -> C.CDLL:
     L.trimeg_push_host.argtypes = [vp, C.POINTER(trimeg_markers), sz, dbl, i32, i32]
     L.trimeg_get_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.trimeg_reset_stats.argtypes = [vp]
+    L.trimeg_get_tile_counters.argtypes = [vp, C.POINTER(C.c_int64)]
     L.trimeg_measure_fp64_peak.argtypes = [vp, dp]
     L.trimeg_strerror.argtypes = [i32]
     L.trimeg_strerror.restype = C.c_char_p
@@ -257,6 +258,12 @@ class Context:
         v = C.c_double(0.0)
         _check(self.L.trimeg_measure_fp64_peak(self.h, C.byref(v)), "trimeg_measure_fp64_peak")
         return float(v.value)
+
+    def get_tile_counters(self) -> Dict[str, int]:
+        a = (C.c_int64 * 8)()
+        _check(self.L.trimeg_get_tile_counters(self.h, a), "trimeg_get_tile_counters")
+        names = ("cyc_A", "cyc_B", "cyc_C", "cyc_D", "cyc_E", "n_fallback", "n_bins", "n_stages")
+        return {k: int(v) for k, v in zip(names, a)}
 
     def reset_stats(self):
         _check(self.L.trimeg_reset_stats(self.h), "trimeg_reset_stats")

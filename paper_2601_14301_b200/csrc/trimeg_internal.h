@@ -12,6 +12,9 @@ namespace trimeg {
 struct Stats {                      // device-resident counters
     unsigned long long n_lost;
     unsigned long long n_moved;
+    // tile-kernel diagnostics (trimeg_get_tile_counters): SM cycles of thread 0 of every CTA spent in
+    // phases A, B, C, D, E; markers evaluated by the one-marker fallback; bins used; stages run
+    unsigned long long tile[8];
 };
 
 }  // namespace trimeg

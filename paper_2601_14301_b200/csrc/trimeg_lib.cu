@@ -357,7 +357,7 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
         c->field.n_first = 0; c->field.n_step = 0; c->field.is_ap = 1;
         c->has_field = 0;
         c->push_kernel = 2;
-        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= 0 && v <= 4) c->push_kernel = v; }
+        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= 0 && v <= TRIMEG_PUSH_KERNEL_MAX) c->push_kernel = v; }
     } while (0);
     if (d_rin2) cudaFree(d_rin2);
     free(hR); free(hZ);
@@ -395,7 +395,7 @@ int trimeg_set_params(trimeg_ctx *c, const trimeg_params *p)
 
 int trimeg_set_push_kernel(trimeg_ctx *c, int variant)
 {
-    if (!c || variant < 0 || variant > 4) return TRIMEG_ERR_INVALID_ARG;
+    if (!c || variant < 0 || variant > TRIMEG_PUSH_KERNEL_MAX) return TRIMEG_ERR_INVALID_ARG;
     c->push_kernel = variant;
     return TRIMEG_OK;
 }
@@ -639,6 +639,16 @@ int trimeg_get_stats(trimeg_ctx *c, int64_t *n_lost, int64_t *n_relocated, int64
     if (n_lost) *n_lost = (int64_t)h.n_lost;
     if (n_relocated) *n_relocated = (int64_t)h.n_moved;
     if (n_launches) *n_launches = c->n_launches;
+    return TRIMEG_OK;
+}
+
+int trimeg_get_tile_counters(trimeg_ctx *c, int64_t *out8)
+{
+    if (!c || !out8) return TRIMEG_ERR_INVALID_ARG;
+    Stats h;
+    CU_TRY(cudaDeviceSynchronize());
+    CU_TRY(cudaMemcpy(&h, c->d_stats, sizeof(Stats), cudaMemcpyDeviceToHost));
+    for (int k = 0; k < 8; ++k) out8[k] = (int64_t)h.tile[k];
     return TRIMEG_OK;
 }
 

@@ -13,15 +13,19 @@
 // lives in shared memory.  Every RK4 stage is five block-synchronous phases:
 //   A  locate the stage position of every marker (hinted walk, bit-exact rule O3) and bin
 //      it by triangle in a small open-addressing hash table (warp-aggregated atomics);
-//   B  exclusive scan of the bin counts, each bin padded to a multiple of P slots;
+//   B  the coefficient records of the stage's triangles (n_modes x 21 complex each) are
+//      copied HBM/L2 -> shared memory with cp.async (no register staging; the copy runs
+//      under phases B and C); exclusive scan of the bin counts, each bin padded to a
+//      multiple of P slots;
 //   C  scatter (xi, eta, phi, owner) of every marker to its evaluation slot;
 //   D  evaluation: each thread takes P consecutive slots -- by construction the same
-//      triangle -- and runs the bivariate Horner scheme for all P markers off ONE load of
-//      each coefficient; lanes of a warp mostly share the triangle too, so the loads are
-//      warp-uniform L1 hits;
+//      triangle -- and runs the bivariate Horner scheme for all P markers off ONE
+//      shared-memory load of each coefficient (warp-uniform address = broadcast, fixed
+//      ~30-cycle latency instead of an L1/L2 round trip that 12 warps per SM cannot hide);
 //   E  each marker reads back its field values, evaluates equilibrium + equations of motion
 //      (a4, a5) and does its RK4 bookkeeping (a6).
-// Markers whose triangle finds no bin (table full) are evaluated by their owner with the
+// Markers whose triangle finds no bin or no shared-memory record (more distinct triangles
+// in the tile than record slots: unsorted input) are evaluated by their owner with the
 // one-marker gather of trimeg_device.cuh -- slower, same arithmetic.  The arithmetic of
 // every marker (order of operations, fused multiply-adds) is the same as in push_kernel.
 #include "trimeg_internal.h"
@@ -45,11 +49,10 @@ template <int P, int T>
 struct TileCfg {
     static constexpr int NT = P * T - 12 * P;                 // markers per tile (slack for bin padding)
     static constexpr int NE = NT + (P - 1) * NBIN;            // evaluation slots, worst case
-    static constexpr size_t smem_bytes()
-    {
-        return sizeof(double) * ((size_t)N_STATE * NT + 4 * (size_t)NE) +
-               sizeof(int) * (3 * (size_t)NT + 2 * (size_t)NE + 3 * NBIN + 8) + NT;
-    }
+    // without the coefficient records, rounded up to 16 bytes
+    static constexpr size_t BASE_BYTES =
+        (sizeof(double) * ((size_t)N_STATE * NT + 4 * (size_t)NE) +
+         sizeof(int) * (3 * (size_t)NT + 2 * (size_t)NE + 5 * NBIN + 8) + NT + 15) / 16 * 16;
 };
 
 __device__ __forceinline__ unsigned hash_tri(int t) { return ((unsigned)t * 0x9E3779B1u) >> 26; }   // 6 bits
@@ -68,7 +71,7 @@ __device__ __forceinline__ void eval_quintic_multi(const double2 *__restrict__ c
         const int n = 5 - j;
 #pragma unroll
         for (int i = n; i >= 0; --i) {
-            const double2 cc = __ldg(c + kidx(i, j));
+            const double2 cc = c[kidx(i, j)];
 #pragma unroll
             for (int p = 0; p < P; ++p) {
                 if (i == n) { ar[p] = cc.x; ai[p] = cc.y; dr[p] = 0.0; di[p] = 0.0; }
@@ -96,11 +99,10 @@ __device__ __forceinline__ void eval_quintic_multi(const double2 *__restrict__ c
 
 // dphi, d/dxi, d/deta, d/dphi for P markers of triangle t (same formulas as gather())
 template <int P>
-__device__ __forceinline__ void gather_multi(const FieldDev &F, int t, const double (&xi)[P], const double (&eta)[P],
+__device__ __forceinline__ void gather_multi(const FieldDev &F, const double2 *c, const double (&xi)[P], const double (&eta)[P],
                                              const double (&phi)[P], double (&f)[P], double (&fx)[P], double (&fe)[P],
                                              double (&fp)[P])
 {
-    const double2 *c = F.coef + (size_t)t * F.n_modes * NCOEF;
     double Er[P], Ei[P], Dr[P], Di[P];
 #pragma unroll
     for (int p = 0; p < P; ++p) {
@@ -139,29 +141,38 @@ __device__ __forceinline__ void gather_multi(const FieldDev &F, int t, const dou
 
 template <int P, int T>
 __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
-                                                      double dt, int nsteps, Stats *st)
+                                                      double dt, int nsteps, Stats *st, int nslot)
 {
     using Cfg = TileCfg<P, T>;
     constexpr int NT = Cfg::NT, NE = Cfg::NE;
-    extern __shared__ double smem_d[];
+    extern __shared__ __align__(16) double smem_d[];
     double *S = smem_d;                                   // [N_STATE][NT]
     double *EV = S + (size_t)N_STATE * NT;                // [4][NE]: in (xi, eta, phi, -) / out (f, fR, fZ, fphi)
     int *cell = reinterpret_cast<int *>(EV + 4 * (size_t)NE);   // [NT] current triangle (hint)
     int *binrank = cell + NT;                             // [NT] bin << 16 | rank, -1 = not binned
     int *slot = binrank + NT;                             // [NT] evaluation slot of the marker
     int *ev_own = slot + NT;                              // [NE] owner marker of a slot, -1 = padding
-    int *ev_tri = ev_own + NE;                            // [NE] triangle of a slot
-    int *tag = ev_tri + NE;                               // [NBIN] triangle of a bin
+    int *ev_rec = ev_own + NE;                            // [NE] coefficient-record slot of an evaluation slot
+    int *tag = ev_rec + NE;                               // [NBIN] triangle of a bin
     int *cnt = tag + NBIN;                                // [NBIN]
     int *off = cnt + NBIN;                                // [NBIN]
-    int *misc = off + NBIN;                               // [0] = number of evaluation slots, [1] lost, [2] moved
+    int *rec_of = off + NBIN;                             // [NBIN] record slot of a bin (order of first claim)
+    int *bin_of = rec_of + NBIN;                          // [NBIN] bin of a record slot
+    int *misc = bin_of + NBIN;                            // [0] = number of evaluation slots, [3] = bins claimed this stage
     unsigned char *flags = reinterpret_cast<unsigned char *>(misc + 8);   // [NT]
+    // coefficient records of the stage's triangles: [nslot][n_modes][21] complex
+    double2 *REC = reinterpret_cast<double2 *>(reinterpret_cast<unsigned char *>(smem_d) + Cfg::BASE_BYTES);
+    const int rec_len = F.n_modes * NCOEF;               // double2 elements per record
 
     const int tid = threadIdx.x, lane = tid & 31;
     const size_t base = (size_t)blockIdx.x * NT;
     const int nt = (int)((n - base < (size_t)NT) ? (n - base) : (size_t)NT);
     const bool has_field = F.n_modes > 0;
     const double hdt = 0.5 * dt, dt6 = dt / 6.0;
+    long long tph[5] = {0, 0, 0, 0, 0}, tlast = 0;      // phase timers (thread 0 only)
+    unsigned n_fallback = 0, n_bins = 0, n_stages = 0;
+#define TILE_TICK(k) do { if (tid == 0) { const long long now_ = clock64(); tph[k] += now_ - tlast; tlast = now_; } } while (0)
+    if (tid == 0) tlast = clock64();
 
     // ---- load the tile
     for (int q = tid; q < NT; q += T) {
@@ -218,6 +229,11 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
 #pragma unroll 1
                         for (int pr = 0; pr < NPROBE; ++pr) {
                             const int prev = atomicCAS(&tag[h], BIN_EMPTY, t);
+                            if (prev == BIN_EMPTY) {                   // first claim: take the next record slot
+                                const int r = atomicAdd(&misc[3], 1);
+                                rec_of[h] = r;
+                                if (r < NBIN) bin_of[r] = (int)h;
+                            }
                             if (prev == BIN_EMPTY || prev == t) { bin = (int)h; break; }
                             h = (h + 1) & (NBIN - 1);
                         }
@@ -230,13 +246,27 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
             }
             if (has_field) {
                 __syncthreads();
+                TILE_TICK(0);
+                // ------------------------------------------------------------ B: records -> shared memory (async)
+                {
+                    const int n_rec = min(misc[3], nslot);
+                    const int total = n_rec * rec_len;
+#pragma unroll 1
+                    for (int idx = tid; idx < total; idx += T) {
+                        const int r = idx / rec_len, k = idx - r * rec_len;
+                        const double2 *src = F.coef + (size_t)tag[bin_of[r]] * rec_len + k;
+                        const unsigned dst = (unsigned)__cvta_generic_to_shared(REC + idx);
+                        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+                    }
+                    asm volatile("cp.async.commit_group;" ::: "memory");
+                }
                 // ------------------------------------------------------------ B: scan of padded bin sizes
                 if (tid < 32) {
                     int run = 0;
 #pragma unroll
                     for (int k = 0; k < NBIN / 32; ++k) {
                         const int b = k * 32 + lane;
-                        const int c = cnt[b];
+                        const int c = (rec_of[b] < nslot) ? cnt[b] : 0;      // no record slot: owner evaluates
                         const int padded = (c + P - 1) / P * P;
                         int incl = padded;
 #pragma unroll
@@ -252,26 +282,31 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
                     if (lane == 0) misc[0] = run;
                 }
                 __syncthreads();
+                TILE_TICK(1);
+                if (tid == 0) { n_bins += (unsigned)misc[3]; ++n_stages; }
                 // ------------------------------------------------------------ C: scatter to evaluation slots
 #pragma unroll 1
                 for (int q = tid; q < NT; q += T) {
                     const int br = binrank[q];
                     if (br >= 0) {
+                        const int r = rec_of[br >> 16];
+                        if (r >= nslot) { binrank[q] = -1; continue; }
                         const int e = off[br >> 16] + (br & 0xffff);
                         const int t = cell[q];
                         const Bary b = bary_rn(M, t, S[S_R * NT + q], S[S_Z * NT + q]);
                         EV[e] = b.xi; EV[NE + e] = b.eta; EV[2 * NE + e] = S[S_P * NT + q];
-                        ev_own[e] = q; ev_tri[e] = t;
+                        ev_own[e] = q; ev_rec[e] = r;
                         slot[q] = e;
                     }
                 }
+                asm volatile("cp.async.wait_group 0;" ::: "memory");
                 __syncthreads();
+                TILE_TICK(2);
                 // ------------------------------------------------------------ D: batched evaluation
                 const int n_ev = misc[0];
-                if (tid < NBIN) { tag[tid] = BIN_EMPTY; cnt[tid] = 0; }             // for the next stage
 #pragma unroll 1
                 for (int e0 = tid * P; e0 < n_ev; e0 += T * P) {
-                    const int t = ev_tri[e0];                                        // first slot of a group is real
+                    const double2 *rec = REC + (size_t)ev_rec[e0] * rec_len;         // first slot of a group is real
                     double xi[P], eta[P], phi[P], f[P], fx[P], fe[P], fp[P];
                     bool real[P];
 #pragma unroll
@@ -281,20 +316,19 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
                         eta[p] = real[p] ? EV[NE + e0 + p] : 0.0;
                         phi[p] = real[p] ? EV[2 * NE + e0 + p] : 0.0;
                     }
-                    gather_multi<P>(F, t, xi, eta, phi, f, fx, fe, fp);
-                    const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)t);
-                    const double2 gx = __ldg(g + 1), ge = __ldg(g + 2);
+                    gather_multi<P>(F, rec, xi, eta, phi, f, fx, fe, fp);
 #pragma unroll
                     for (int p = 0; p < P; ++p) {
-                        if (real[p]) {
-                            EV[e0 + p] = f[p];
-                            EV[NE + e0 + p] = fma(gx.x, fx[p], ge.x * fe[p]);        // d/dR
-                            EV[2 * NE + e0 + p] = fma(gx.y, fx[p], ge.y * fe[p]);    // d/dZ
+                        if (real[p]) {                                               // d/dxi, d/deta: chain rule in E
+                            EV[e0 + p] = f[p]; EV[NE + e0 + p] = fx[p]; EV[2 * NE + e0 + p] = fe[p];
                             EV[3 * NE + e0 + p] = fp[p];
                         }
                     }
                 }
                 __syncthreads();
+                TILE_TICK(3);
+                if (tid < NBIN) { tag[tid] = BIN_EMPTY; cnt[tid] = 0; }             // for the next stage
+                if (tid == 0) misc[3] = 0;
             }
             // ---------------------------------------------------------------- E: equations + RK4
 #pragma unroll 1
@@ -307,11 +341,17 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
                 if (has_field) {
                     if (binrank[q] >= 0) {
                         const int e = slot[q];
-                        fv.f = EV[e]; fv.fR = EV[NE + e]; fv.fZ = EV[2 * NE + e]; fv.fphi = EV[3 * NE + e];
+                        const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)cell[q]);
+                        const double2 gx = __ldg(g + 1), ge = __ldg(g + 2);
+                        const double fx = EV[NE + e], fe = EV[2 * NE + e];
+                        fv.f = EV[e]; fv.fphi = EV[3 * NE + e];
+                        fv.fR = fma(gx.x, fx, ge.x * fe);                            // d/dR
+                        fv.fZ = fma(gx.y, fx, ge.y * fe);                            // d/dZ
                     } else {                               // no bin: one-marker gather, same arithmetic
                         const int t = cell[q];
                         const Bary b = bary_rn(M, t, R, Z);
                         fv = gather(F, t, b, ph);
+                        ++n_fallback;
                     }
                 }
                 const Rates k = rhs_point(Ph, R, Z, v, mu, w, fv);
@@ -349,8 +389,10 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
                 }
             }
             __syncthreads();
+            TILE_TICK(4);
         }
     }
+#undef TILE_TICK
 
     // ---- write back, statistics
     int lost = 0, moved = 0;
@@ -366,6 +408,14 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
     }
     lost = __reduce_add_sync(0xffffffffu, lost);
     moved = __reduce_add_sync(0xffffffffu, moved);
+    n_fallback = __reduce_add_sync(0xffffffffu, n_fallback);
+    if (lane == 0 && n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);
+    if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) atomicAdd(&st->tile[k], (unsigned long long)tph[k]);
+        atomicAdd(&st->tile[6], (unsigned long long)n_bins);
+        atomicAdd(&st->tile[7], (unsigned long long)n_stages);
+    }
     if (lane == 0) {
         if (lost) atomicAdd(&st->n_lost, (unsigned long long)lost);
         if (moved) atomicAdd(&st->n_moved, (unsigned long long)moved);
@@ -377,14 +427,21 @@ cudaError_t launch_tile(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 {
     using Cfg = TileCfg<P, T>;
     static bool configured = false;
-    const size_t shm = Cfg::smem_bytes();
+    constexpr size_t SMEM_MAX = 227 * 1024;                 // per-CTA limit on sm_100
+    constexpr int CTAS = (2 * Cfg::BASE_BYTES + 32 * 1024 <= SMEM_MAX && 2 * T <= 1024) ? 2 : 1;   // CTAs per SM aimed at
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_tile_kernel<P, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+        cudaError_t e = cudaFuncSetAttribute(push_tile_kernel<P, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
         if (e != cudaSuccess) return e;
         configured = true;
     }
+    // record slots: what is left of the SM's shared memory (1 KB per CTA is reserved by the system)
+    const size_t rec_bytes = sizeof(double2) * NCOEF * (size_t)c->field.n_modes;
+    const size_t avail = (SMEM_MAX + 1024) / CTAS - 1024 - Cfg::BASE_BYTES;
+    int nslot = rec_bytes ? (int)(avail / rec_bytes) : 0;
+    if (nslot > NBIN) nslot = NBIN;
+    const size_t shm = Cfg::BASE_BYTES + (size_t)nslot * rec_bytes;
     const size_t tiles = (n + Cfg::NT - 1) / Cfg::NT;
-    push_tile_kernel<P, T><<<(unsigned)tiles, T, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
+    push_tile_kernel<P, T><<<(unsigned)tiles, T, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats, nslot);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -400,6 +457,8 @@ cudaError_t launch_push_tile(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
     case 2: return launch_tile<2, 384>(c, m, n, dt, nsteps, s);
     case 3: return launch_tile<4, 128>(c, m, n, dt, nsteps, s);
     case 4: return launch_tile<4, 256>(c, m, n, dt, nsteps, s);
+    case 5: return launch_tile<3, 256>(c, m, n, dt, nsteps, s);
+    case 6: return launch_tile<3, 320>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }
