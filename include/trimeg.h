@@ -166,10 +166,13 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *         memory, re-bins them by triangle at every RK4 stage, stages the coefficient records of
  *         the tile's triangles in shared memory and evaluates P markers of one triangle per lane
  *         off a single load of each coefficient (1: P=2, 192 threads; 2: P=2, 384; 3: P=4, 128;
- *         4: P=4, 256; 5: P=3, 256; 6: P=3, 320).
+ *         4: P=4, 256; 5: P=3, 256; 6: P=3, 320);
+ *   7..10 warp-autonomous tiles: every warp owns 32 P - 2 P markers, groups them by triangle with
+ *         ballots and evaluates, finishes and re-locates them without any block barrier
+ *         (7: P=2; 8: P=3; 9: P=4, all 4 warps per CTA; 10: P=2, 2 warps per CTA).
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside 0..TRIMEG_PUSH_KERNEL_MAX. */
-#define TRIMEG_PUSH_KERNEL_MAX 6
+#define TRIMEG_PUSH_KERNEL_MAX 10
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 
 /* ---- end-to-end push from HOST buffers -------------------------------------------------------

@@ -57,4 +57,8 @@ cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 cudaError_t launch_push_tile(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                              cudaStream_t s);
 
+// trimeg_push_warp.cu: warp-autonomous variant (no block barriers; variants 7..10)
+cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
+                             cudaStream_t s);
+
 }  // namespace trimeg

@@ -29,6 +29,7 @@
 // one-marker gather of trimeg_device.cuh -- slower, same arithmetic.  The arithmetic of
 // every marker (order of operations, fused multiply-adds) is the same as in push_kernel.
 #include "trimeg_internal.h"
+#include "trimeg_multi.cuh"
 
 namespace trimeg {
 
@@ -56,88 +57,6 @@ struct TileCfg {
 };
 
 __device__ __forceinline__ unsigned hash_tri(int t) { return ((unsigned)t * 0x9E3779B1u) >> 26; }   // 6 bits
-
-// P markers, one triangle: complex quintic and its xi / eta derivatives by bivariate Horner
-// (same operation order per marker as eval_quintic), every coefficient loaded once.
-template <int P>
-__device__ __forceinline__ void eval_quintic_multi(const double2 *__restrict__ c, const double (&xi)[P],
-                                                   const double (&eta)[P], double (&pr)[P], double (&pi)[P],
-                                                   double (&pxr)[P], double (&pxi)[P], double (&per)[P],
-                                                   double (&pei)[P])
-{
-    double ar[P], ai[P], dr[P], di[P];
-#pragma unroll
-    for (int j = 5; j >= 0; --j) {
-        const int n = 5 - j;
-#pragma unroll
-        for (int i = n; i >= 0; --i) {
-            const double2 cc = c[kidx(i, j)];
-#pragma unroll
-            for (int p = 0; p < P; ++p) {
-                if (i == n) { ar[p] = cc.x; ai[p] = cc.y; dr[p] = 0.0; di[p] = 0.0; }
-                else {
-                    if (i == n - 1) { dr[p] = ar[p]; di[p] = ai[p]; }
-                    else { dr[p] = fma(dr[p], xi[p], ar[p]); di[p] = fma(di[p], xi[p], ai[p]); }
-                    ar[p] = fma(ar[p], xi[p], cc.x); ai[p] = fma(ai[p], xi[p], cc.y);
-                }
-            }
-        }
-#pragma unroll
-        for (int p = 0; p < P; ++p) {
-            if (j == 5) { pr[p] = ar[p]; pi[p] = ai[p]; }
-            else {
-                if (j == 4) { per[p] = pr[p]; pei[p] = pi[p]; pxr[p] = dr[p]; pxi[p] = di[p]; }
-                else {
-                    per[p] = fma(per[p], eta[p], pr[p]); pei[p] = fma(pei[p], eta[p], pi[p]);
-                    pxr[p] = fma(pxr[p], eta[p], dr[p]); pxi[p] = fma(pxi[p], eta[p], di[p]);
-                }
-                pr[p] = fma(pr[p], eta[p], ar[p]); pi[p] = fma(pi[p], eta[p], ai[p]);
-            }
-        }
-    }
-}
-
-// dphi, d/dxi, d/deta, d/dphi for P markers of triangle t (same formulas as gather())
-template <int P>
-__device__ __forceinline__ void gather_multi(const FieldDev &F, const double2 *c, const double (&xi)[P], const double (&eta)[P],
-                                             const double (&phi)[P], double (&f)[P], double (&fx)[P], double (&fe)[P],
-                                             double (&fp)[P])
-{
-    double Er[P], Ei[P], Dr[P], Di[P];
-#pragma unroll
-    for (int p = 0; p < P; ++p) {
-        f[p] = fx[p] = fe[p] = fp[p] = 0.0;
-        Er[p] = 1.0; Ei[p] = 0.0; Dr[p] = 1.0; Di[p] = 0.0;
-        if (F.is_ap) {
-            if (F.n_first != 0) sincos((double)F.n_first * phi[p], &Ei[p], &Er[p]);
-            if (F.n_modes > 1) sincos((double)F.n_step * phi[p], &Di[p], &Dr[p]);
-        }
-    }
-    double nn = (double)F.n_first;
-#pragma unroll 1
-    for (int m = 0; m < F.n_modes; ++m, c += NCOEF) {
-        if (!F.is_ap) {
-            nn = (double)__ldg(F.mode_n + m);
-#pragma unroll
-            for (int p = 0; p < P; ++p) sincos(nn * phi[p], &Ei[p], &Er[p]);
-        }
-        double pr[P], pi[P], pxr[P], pxi[P], per[P], pei[P];
-        eval_quintic_multi<P>(c, xi, eta, pr, pi, pxr, pxi, per, pei);
-#pragma unroll
-        for (int p = 0; p < P; ++p) {
-            f[p] = fma(pr[p], Er[p], fma(-pi[p], Ei[p], f[p]));
-            fx[p] = fma(pxr[p], Er[p], fma(-pxi[p], Ei[p], fx[p]));
-            fe[p] = fma(per[p], Er[p], fma(-pei[p], Ei[p], fe[p]));
-            fp[p] = fma(-nn, fma(pi[p], Er[p], pr[p] * Ei[p]), fp[p]);          // Re(i n P E)
-            if (F.is_ap) {                                                      // E_{n + dn} = E_n E_dn
-                const double tr = fma(Er[p], Dr[p], -Ei[p] * Di[p]);
-                Ei[p] = fma(Er[p], Di[p], Ei[p] * Dr[p]);
-                Er[p] = tr;
-            }
-        }
-        if (F.is_ap) nn += (double)F.n_step;
-    }
-}
 
 template <int P, int T>
 __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
@@ -316,7 +235,7 @@ __global__ void __launch_bounds__(T) push_tile_kernel(MeshDev M, FieldDev F, Phy
                         eta[p] = real[p] ? EV[NE + e0 + p] : 0.0;
                         phi[p] = real[p] ? EV[2 * NE + e0 + p] : 0.0;
                     }
-                    gather_multi<P>(F, rec, xi, eta, phi, f, fx, fe, fp);
+                    gather_multi<P, false>(F, rec, xi, eta, phi, f, fx, fe, fp);
 #pragma unroll
                     for (int p = 0; p < P; ++p) {
                         if (real[p]) {                                               // d/dxi, d/deta: chain rule in E
