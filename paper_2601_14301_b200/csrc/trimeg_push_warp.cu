@@ -36,10 +36,10 @@ enum : unsigned char { FL_ACTIVE = 1, FL_LOST = 2, FL_MOVED = 4, FL_WASACTIVE = 
 // per-marker fp64 state: Y = start-of-step state, A = k1 + 2 k2 + 2 k3, S = stage position
 enum { Y_R, Y_Z, Y_P, Y_V, Y_W, S_MU, A_R, A_Z, A_P, A_V, A_W, S_R, S_Z, S_P, S_V, S_W, N_STATE };
 
-template <int P>
+template <int P, int SLACK>
 struct WarpCfg {
-    static constexpr int NW = 32 * P - 2 * P;                       // markers per warp (slack: 2 P padding slots)
-    static constexpr int NE = (NW + (P - 1) * NB_MAX + P - 1) / P * P;   // evaluation slots, worst case
+    static constexpr int NW = 32 * P - SLACK;                       // markers per warp (SLACK slots left for bin padding)
+    static constexpr int NE = 32 * P;                               // evaluation slots: exactly one pass of the warp
     static constexpr size_t WARP_BYTES =
         (sizeof(double) * (size_t)N_STATE * NW + sizeof(int) * ((size_t)NW + 2 * (size_t)NE) + NW + 15) / 16 * 16;
 };
@@ -89,11 +89,11 @@ __device__ __forceinline__ void advance(const MeshDev &M, const PhysDev &Ph, dou
     flags[q] = fl;
 }
 
-template <int P, int WARPS>
+template <int P, int WARPS, int SLACK>
 __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
                                                                double dt, int nsteps, Stats *st)
 {
-    using Cfg = WarpCfg<P>;
+    using Cfg = WarpCfg<P, SLACK>;
     constexpr int NW = Cfg::NW, NE = Cfg::NE;
     constexpr unsigned FULL = 0xffffffffu;
     extern __shared__ __align__(16) unsigned char smem_w[];
@@ -163,7 +163,7 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
             int n_ev = 0, nb = 0;
             if (has_field) {
 #pragma unroll 1
-                while (nb < NB_MAX) {
+                while (nb < NB_MAX && n_ev < NE) {
                     int pl = -1;
 #pragma unroll
                     for (int p = P - 1; p >= 0; --p) if (rem[p]) pl = p;
@@ -173,15 +173,18 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
 #pragma unroll
                     for (int p = 0; p < P; ++p) if (p == pl) { cand = t[p]; rl = rem[p]; }
                     const int tl = __shfl_sync(FULL, cand, __ffs(rl) - 1);
+                    const int room = NE - n_ev;                    // a multiple of P; markers beyond it keep slot -1
                     int count = 0;
 #pragma unroll
                     for (int p = 0; p < P; ++p) {
                         const bool mine = (t[p] == tl);
                         const unsigned mm = __ballot_sync(FULL, mine);
-                        if (mine) slot[p] = n_ev + count + __popc(mm & lt_mask);
+                        const int rank = count + __popc(mm & lt_mask);
+                        if (mine && rank < room) slot[p] = n_ev + rank;
                         count += __popc(mm);
                         rem[p] &= ~mm;
                     }
+                    count = min(count, room);
                     const int padded = (count + P - 1) / P * P;
                     if (lane < padded - count) ev_own[n_ev + count + lane] = -1;
                     n_ev += padded;
@@ -196,7 +199,8 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
 
             // ------------------------------------------------------------ 2 + 3: batched evaluation, equations (slot role)
 #pragma unroll 1
-            for (int e0 = lane * P; e0 < n_ev; e0 += 32 * P) {
+            if (lane * P < n_ev) {
+                const int e0 = lane * P;
                 const int tri = ev_tri[e0];                                          // first slot of a group is real
                 const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)tri);
                 const double2 v0 = __ldg(g), gx = __ldg(g + 1), ge = __ldg(g + 2);
@@ -285,20 +289,20 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
     }
 }
 
-template <int P, int WARPS>
+template <int P, int WARPS, int SLACK>
 cudaError_t launch_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
-    using Cfg = WarpCfg<P>;
+    using Cfg = WarpCfg<P, SLACK>;
     static bool configured = false;
     const size_t shm = Cfg::WARP_BYTES * WARPS;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     const size_t per_cta = (size_t)Cfg::NW * WARPS;
     const size_t ctas = (n + per_cta - 1) / per_cta;
-    push_warp_kernel<P, WARPS><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
+    push_warp_kernel<P, WARPS, SLACK><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -310,10 +314,17 @@ cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
-    case 7: return launch_warp<2, 4>(c, m, n, dt, nsteps, s);
-    case 8: return launch_warp<3, 4>(c, m, n, dt, nsteps, s);
-    case 9: return launch_warp<4, 4>(c, m, n, dt, nsteps, s);
-    case 10: return launch_warp<2, 2>(c, m, n, dt, nsteps, s);
+    case 7: return launch_warp<2, 4, 4>(c, m, n, dt, nsteps, s);
+    case 8: return launch_warp<3, 4, 6>(c, m, n, dt, nsteps, s);
+    case 9: return launch_warp<4, 4, 8>(c, m, n, dt, nsteps, s);
+    case 10: return launch_warp<2, 2, 4>(c, m, n, dt, nsteps, s);
+    case 11: return launch_warp<2, 4, 6>(c, m, n, dt, nsteps, s);
+    case 12: return launch_warp<2, 4, 8>(c, m, n, dt, nsteps, s);
+    case 13: return launch_warp<3, 4, 9>(c, m, n, dt, nsteps, s);
+    case 14: return launch_warp<3, 4, 12>(c, m, n, dt, nsteps, s);
+    case 15: return launch_warp<4, 4, 12>(c, m, n, dt, nsteps, s);
+    case 16: return launch_warp<4, 4, 16>(c, m, n, dt, nsteps, s);
+    case 17: return launch_warp<4, 4, 20>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -319,7 +319,7 @@ def test_non_arithmetic_mode_list(B, inputs):
 
 
 # ----------------------------------------------------------------------------- tile kernels
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17])
 @pytest.mark.parametrize("name,n,nsteps,sort", [("cfg1", 4096, 20, False), ("cfg1", 1777, 3, True),
                                                 ("cfg2", (1 << 16) + 13, 3, True), ("cfg5", 40009, 5, True),
                                                 ("cfg3", 20011, 2, False)])
