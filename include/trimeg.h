@@ -172,7 +172,7 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *         (7: P=2; 8: P=3; 9: P=4, all 4 warps per CTA; 10: P=2, 2 warps per CTA).
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside 0..TRIMEG_PUSH_KERNEL_MAX. */
-#define TRIMEG_PUSH_KERNEL_MAX 17
+#define TRIMEG_PUSH_KERNEL_MAX 33
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 
 /* ---- end-to-end push from HOST buffers -------------------------------------------------------

@@ -61,4 +61,8 @@ cudaError_t launch_push_tile(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                              cudaStream_t s);
 
+// trimeg_push_fused.cu: CTA tiles with resident coefficient records, fused evaluate + finish (variants 28..)
+cudaError_t launch_push_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
+                              cudaStream_t s);
+
 }  // namespace trimeg

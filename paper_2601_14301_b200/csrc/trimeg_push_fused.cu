@@ -1,0 +1,367 @@
+// trimeg_push_fused.cu -- CTA-tile fused RK4 push with resident coefficient records (rows a2-a6 of
+// DESIGN.md §1).
+//
+// What the measurements say (profiles/r01_warp_kernel.md): the batched Horner evaluation is 88 % of
+// the FP64 work; it runs the FP64 pipe at 0.85-0.88 of peak when (a) three warps per scheduler share
+// the pipe and (b) the coefficients come from shared memory (LDS.128: 3.15 SM-cycles per warp-wide
+// load whatever the mix of triangles, fixed 29-cycle latency), but only at ~0.55 when they come
+// through L1 (LDG.128: 4.6+ cycles, more when the lanes sit in several triangles; the records of
+// all resident warps do not fit next to their shared-memory state, so a quarter of the loads go to
+// L2).  The block-synchronous tile kernel had the shared-memory records but idled the pipe during
+// its locate / bin / scatter / equations phases; the warp-autonomous kernel had the overlap but
+// not the records.
+//
+// This kernel: one CTA owns a tile of NT consecutive markers for the whole call (RK4 state in shared
+// memory).  Per RK4 stage
+//   A  bin the markers by their (already known) triangle in a small hash table (warp-aggregated);
+//      the table and the coefficient records behind it STAY between stages and steps -- only a
+//      triangle that no marker of the tile was in before costs a copy (cp.async, 16 B per lane);
+//   B  scan of the bin sizes, each padded to a multiple of P -> evaluation slots, sorted by triangle;
+//   C  every marker writes its index into its slot;
+//   D  one pass, no barrier inside: each thread takes P consecutive slots -- one triangle --, runs
+//      the bivariate Horner scheme for the P markers off ONE shared-memory load of each
+//      coefficient, then finishes the same P markers: chain rule, equilibrium + equations (a4, a5),
+//      RK4 bookkeeping (a6), next stage position and the locate (a2) of that position.  The
+//      latency-bound tails of one warp run under the Horner loops of the others.
+// Markers without a record (more distinct triangles than record slots: unsorted input) or without a
+// slot are evaluated one per thread with the one-marker gather of trimeg_device.cuh: same arithmetic.
+#include "trimeg_internal.h"
+#include "trimeg_multi.cuh"
+#include "trimeg_rk4.cuh"
+
+namespace trimeg {
+
+namespace {
+
+constexpr int NBIN = 64;            // hash bins (distinct triangles the tile can track)
+constexpr int NPROBE = 8;
+constexpr int BIN_EMPTY = -1;
+
+// misc[] slots
+enum { MI_NEV, MI_NREC, MI_NLOAD, MI_NFB, MI_CLEAR, MI_COUNT = 8 };
+
+template <int P, int T>
+struct FusedCfg {
+    static constexpr int NE = P * T;                              // evaluation slots: one pass of the CTA
+    static constexpr int NT = NE - 12 * P;                        // markers per tile (slack for bin padding)
+    static constexpr size_t BASE_BYTES =
+        (sizeof(double) * (size_t)N_STATE * NT +
+         sizeof(int) * (3 * (size_t)NT + (size_t)NE + 5 * NBIN + MI_COUNT) + NT + 15) / 16 * 16;
+};
+
+__device__ __forceinline__ unsigned hash_tri(int t) { return ((unsigned)t * 0x9E3779B1u) >> 26; }   // 6 bits
+
+template <int P, int T, int ILP>
+__global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
+                                                          double dt, int nsteps, Stats *st, int nslot)
+{
+    using Cfg = FusedCfg<P, T>;
+    constexpr int NT = Cfg::NT, NE = Cfg::NE;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(16) double smem_f[];
+    double *S = smem_f;                                   // [N_STATE][NT]
+    int *cell = reinterpret_cast<int *>(S + (size_t)N_STATE * NT);   // [NT] current triangle
+    int *binrank = cell + NT;                             // [NT] bin << 16 | rank, -1 = not binned
+    int *fb_list = binrank + NT;                          // [NT] markers evaluated one per thread
+    int *ev = fb_list + NT;                               // [NE] owner | record slot << 16, -1 = padding
+    int *tag = ev + NE;                                   // [NBIN] triangle of a bin (kept between stages)
+    int *cnt = tag + NBIN;                                // [NBIN] markers in the bin this stage
+    int *off = cnt + NBIN;                                // [NBIN] first evaluation slot, -1 = none
+    int *rec_of = off + NBIN;                             // [NBIN] record slot of the bin, -1 = none
+    int *load_list = rec_of + NBIN;                       // [NBIN] bins whose record must be copied this stage
+    int *misc = load_list + NBIN;                         // [MI_COUNT]
+    unsigned char *flags = reinterpret_cast<unsigned char *>(misc + MI_COUNT);   // [NT]
+    const int rec_len = F.n_modes * NCOEF;                // double2 elements per record
+    const int rec_stride = rec_len + 1;                   // +16 B: records of different triangles in different banks
+    double2 *REC = reinterpret_cast<double2 *>(reinterpret_cast<unsigned char *>(smem_f) + Cfg::BASE_BYTES);
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const size_t base = (size_t)blockIdx.x * NT;
+    const int nt = (int)((n - base < (size_t)NT) ? (n - base) : (size_t)NT);
+    const bool has_field = F.n_modes > 0;
+    const double hdt = 0.5 * dt, dt6 = dt / 6.0;
+    unsigned n_fallback = 0;
+
+    // ---- load the tile, locate the start positions
+    for (int q = tid; q < NT; q += T) {
+        unsigned char fl = 0;
+        int c = -1;
+        if (q < nt) {
+            const size_t g = base + q;
+            c = m.cell[g];
+            if (c >= 0) {
+                const double R = m.R[g], Z = m.Z[g];
+                S[Y_R * NT + q] = R; S[Y_Z * NT + q] = Z; S[Y_P * NT + q] = m.phi[g];
+                S[Y_V * NT + q] = m.vpar[g]; S[Y_W * NT + q] = m.w[g]; S[S_MU * NT + q] = m.mu[g];
+                fl = FL_ACTIVE | FL_WASACTIVE;
+                Bary b;
+                int moved = 0;
+                const int t = locate(M, R, Z, c, b, moved);
+                if (moved) fl |= FL_MOVED;
+                if (t < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;
+                else c = t;
+            }
+        }
+        cell[q] = c; flags[q] = fl;
+    }
+    if (tid < NBIN) { tag[tid] = BIN_EMPTY; cnt[tid] = 0; rec_of[tid] = -1; off[tid] = -1; }
+    if (tid < MI_COUNT) misc[tid] = 0;
+    __syncthreads();
+
+    unsigned n_copied = 0, n_stages = 0;
+#pragma unroll 1
+    for (int step = 0; step < nsteps; ++step) {
+#pragma unroll 1
+        for (int stage = 0; stage < 4; ++stage) {
+            if (!has_field) {                              // no field: equations only, one marker per thread and turn
+#pragma unroll 1
+                for (int q = tid; q < NT; q += T) {
+                    if (!(flags[q] & FL_ACTIVE)) continue;
+                    if (stage == 0) {
+#pragma unroll
+                        for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
+                    }
+                    FieldVal fv;
+                    fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
+                    advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
+                }
+                continue;                                  // a thread only ever touches its own markers here
+            }
+            // ---------------------------------------------------------------- A: bin by triangle
+#pragma unroll 1
+            for (int q0 = 0; q0 < NT; q0 += T) {
+                const int q = q0 + tid;
+                const bool act = (q < NT) && (flags[q] & FL_ACTIVE);
+                int t = -1;
+                if (act) {
+                    t = cell[q];
+                    if (stage == 0) {
+#pragma unroll
+                        for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
+                    }
+                }
+                // warp-aggregated insertion: one probe sequence and one atomicAdd per distinct triangle
+                const int key = act ? t : -1 - lane;
+                const unsigned grp = __match_any_sync(FULL, key);
+                const int leader = __ffs(grp) - 1;
+                int bin = -1, rank0 = 0;
+                if (act && lane == leader) {
+                    unsigned h = hash_tri(t);
+#pragma unroll 1
+                    for (int pr = 0; pr < NPROBE; ++pr) {
+                        const int prev = atomicCAS(&tag[h], BIN_EMPTY, t);
+                        if (prev == BIN_EMPTY) {           // first marker of the tile in this triangle: record slot + copy
+                            const int r = atomicAdd(&misc[MI_NREC], 1);
+                            if (r < nslot) { rec_of[h] = r; load_list[atomicAdd(&misc[MI_NLOAD], 1)] = (int)h; }
+                            else rec_of[h] = -1;
+                        }
+                        if (prev == BIN_EMPTY || prev == t) { bin = (int)h; break; }
+                        h = (h + 1) & (NBIN - 1);
+                    }
+                    if (bin >= 0) rank0 = atomicAdd(&cnt[bin], __popc(grp));
+                }
+                bin = __shfl_sync(FULL, bin, leader);
+                rank0 = __shfl_sync(FULL, rank0, leader);
+                if (q < NT) binrank[q] = (act && bin >= 0) ? ((bin << 16) | (rank0 + __popc(grp & ((1u << lane) - 1u)))) : -1;
+            }
+            __syncthreads();
+            // ---------------------------------------------------------------- B: copy new records, scan the bins
+            {
+                const int n_load = misc[MI_NLOAD];
+                const int total = n_load * rec_len;
+#pragma unroll 1
+                for (int idx = tid; idx < total; idx += T) {
+                    const int i = idx / rec_len, k = idx - i * rec_len;
+                    const int b = load_list[i];
+                    const double2 *src = F.coef + (size_t)tag[b] * rec_len + k;
+                    const unsigned dst = (unsigned)__cvta_generic_to_shared(REC + (size_t)rec_of[b] * rec_stride + k);
+                    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+                }
+                asm volatile("cp.async.commit_group;" ::: "memory");
+                if (tid == 0) n_copied += (unsigned)n_load;
+            }
+            if (tid < 32) {
+                int run = 0, n_ev = 0;
+#pragma unroll
+                for (int k = 0; k < NBIN / 32; ++k) {
+                    const int b = k * 32 + lane;
+                    const int c = (rec_of[b] >= 0) ? cnt[b] : 0;             // no record: one marker per thread
+                    const int padded = (c + P - 1) / P * P;
+                    int incl = padded;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int v = __shfl_up_sync(FULL, incl, o);
+                        if (lane >= o) incl += v;
+                    }
+                    const int o0 = run + incl - padded;
+                    const bool fits = (c > 0) && (o0 + padded <= NE);        // else: no slot, one marker per thread
+                    off[b] = fits ? o0 : -1;
+                    if (fits) {
+                        for (int e = o0 + c; e < o0 + padded; ++e) ev[e] = -1;   // padding slots
+                        n_ev = max(n_ev, o0 + padded);
+                    }
+                    run += __shfl_sync(FULL, incl, 31);
+                }
+                n_ev = __reduce_max_sync(FULL, n_ev);
+                if (lane == 0) { misc[MI_NEV] = n_ev; misc[MI_NFB] = 0; }
+            }
+            __syncthreads();
+            // ---------------------------------------------------------------- C: markers -> evaluation slots
+#pragma unroll 1
+            for (int q = tid; q < NT; q += T) {
+                if (!(flags[q] & FL_ACTIVE)) continue;
+                const int br = binrank[q];
+                const int b = br >> 16;
+                if (br >= 0 && off[b] >= 0) ev[off[b] + (br & 0xffff)] = q | (rec_of[b] << 16);
+                else fb_list[atomicAdd(&misc[MI_NFB], 1)] = q;
+            }
+            if (tid == 0) misc[MI_NLOAD] = 0;
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+            __syncthreads();
+            // ---------------------------------------------------------------- D: evaluate + finish, P slots per thread
+            if (tid < NBIN) cnt[tid] = 0;                                     // for the next stage
+            const int n_ev = misc[MI_NEV];
+            if (tid * P < n_ev) {
+                const int e0 = tid * P;
+                int own[P];
+#pragma unroll
+                for (int p = 0; p < P; ++p) { const int v = ev[e0 + p]; own[p] = (v >= 0) ? (v & 0xffff) : -1; }
+                const int rec = ev[e0] >> 16;                                // first slot of a group is real
+                const int tri = cell[own[0]];
+                const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)tri);
+                const double2 v0 = __ldg(g), gx = __ldg(g + 1), ge = __ldg(g + 2);
+                double xi[P], eta[P], phi[P], f[P], fx[P], fe[P], fp[P];
+#pragma unroll
+                for (int p = 0; p < P; ++p) {
+                    xi[p] = eta[p] = phi[p] = 0.0;
+                    if (own[p] >= 0) {                 // local coordinates exactly as bary_rn() (rule L2)
+                        const double dx = __dsub_rn(S[S_R * NT + own[p]], v0.x), dz = __dsub_rn(S[S_Z * NT + own[p]], v0.y);
+                        xi[p] = __dadd_rn(__dmul_rn(gx.x, dx), __dmul_rn(gx.y, dz));
+                        eta[p] = __dadd_rn(__dmul_rn(ge.x, dx), __dmul_rn(ge.y, dz));
+                        phi[p] = S[S_P * NT + own[p]];
+                    }
+                }
+                gather_multi<P, false>(F, REC + (size_t)rec * rec_stride, xi, eta, phi, f, fx, fe, fp);
+                if constexpr (ILP > 0) {
+#pragma unroll
+                    for (int p0 = 0; p0 < P; p0 += ILP) {
+                        int qs[ILP];
+                        FieldVal fvs[ILP];
+#pragma unroll
+                        for (int i = 0; i < ILP; ++i) {
+                            const int pp = (p0 + i < P) ? p0 + i : P - 1;
+                            qs[i] = (p0 + i < P) ? own[pp] : -1;
+                            fvs[i].f = f[pp]; fvs[i].fphi = fp[pp];
+                            fvs[i].fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
+                            fvs[i].fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
+                        }
+                        advance_multi<ILP>(M, Ph, S, NT, cell, flags, qs, stage, fvs, dt, hdt, dt6);
+                    }
+                } else {
+#pragma unroll 1
+                    for (int p = 0; p < P; ++p) {
+                        int q = -1;                                              // select without dynamic register indexing
+                        FieldVal fv;
+                        fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
+#pragma unroll
+                        for (int pp = 0; pp < P; ++pp)
+                            if (pp == p) {
+                                q = own[pp]; fv.f = f[pp]; fv.fphi = fp[pp];
+                                fv.fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
+                                fv.fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
+                            }
+                        if (q >= 0) advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
+                    }
+                }
+            }
+            // markers without a slot: one per thread, coefficients from global memory
+            {
+                const int n_fb = misc[MI_NFB];
+#pragma unroll 1
+                for (int i = tid; i < n_fb; i += T) {
+                    const int q = fb_list[i];
+                    const int tt = cell[q];
+                    const Bary b = bary_rn(M, tt, S[S_R * NT + q], S[S_Z * NT + q]);
+                    const FieldVal fv = gather(F, tt, b, S[S_P * NT + q]);
+                    ++n_fallback;
+                    advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
+                }
+            }
+            __syncthreads();
+            if (tid == 0) ++n_stages;
+            // the table is nearly full of triangles the markers have left: start it afresh
+            if (stage == 3 && misc[MI_NREC] > min(nslot, NBIN) - 8) {
+                __syncthreads();                                              // everybody has read MI_NREC
+                if (tid < NBIN) { tag[tid] = BIN_EMPTY; rec_of[tid] = -1; }
+                if (tid == 0) misc[MI_NREC] = 0;
+                __syncthreads();
+            }
+        }
+    }
+
+    // ---- write back, statistics
+    int lost = 0, moved = 0;
+    for (int q = tid; q < nt; q += T) {
+        const unsigned char fl = flags[q];
+        if (!(fl & FL_WASACTIVE)) continue;
+        const size_t g = base + q;
+        m.R[g] = S[Y_R * NT + q]; m.Z[g] = S[Y_Z * NT + q]; m.phi[g] = S[Y_P * NT + q];
+        m.vpar[g] = S[Y_V * NT + q]; m.w[g] = S[Y_W * NT + q];
+        m.cell[g] = (fl & FL_LOST) ? -1 : cell[q];
+        lost += (fl & FL_LOST) ? 1 : 0;
+        moved += (fl & FL_MOVED) ? 1 : 0;
+    }
+    lost = __reduce_add_sync(FULL, lost);
+    moved = __reduce_add_sync(FULL, moved);
+    n_fallback = __reduce_add_sync(FULL, n_fallback);
+    if (lane == 0) {
+        if (lost) atomicAdd(&st->n_lost, (unsigned long long)lost);
+        if (moved) atomicAdd(&st->n_moved, (unsigned long long)moved);
+        if (n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);
+    }
+    if (tid == 0) {
+        atomicAdd(&st->tile[6], (unsigned long long)n_copied);
+        atomicAdd(&st->tile[7], (unsigned long long)n_stages);
+    }
+}
+
+template <int P, int T, int ILP>
+cudaError_t launch_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
+{
+    using Cfg = FusedCfg<P, T>;
+    static bool configured = false;
+    constexpr size_t SMEM_MAX = 227 * 1024;                 // per-CTA limit on sm_100
+    if (!configured) {
+        cudaError_t e = cudaFuncSetAttribute(push_fused_kernel<P, T, ILP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+        if (e != cudaSuccess) return e;
+        configured = true;
+    }
+    // record slots: what is left of the CTA's shared memory
+    const size_t rec_bytes = sizeof(double2) * (NCOEF * (size_t)c->field.n_modes + 1);
+    int nslot = c->field.n_modes ? (int)((SMEM_MAX - Cfg::BASE_BYTES) / rec_bytes) : 0;
+    if (nslot > NBIN) nslot = NBIN;
+    const size_t shm = Cfg::BASE_BYTES + (size_t)nslot * rec_bytes;
+    const size_t tiles = (n + Cfg::NT - 1) / Cfg::NT;
+    push_fused_kernel<P, T, ILP><<<(unsigned)tiles, T, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats, nslot);
+    c->n_launches++;
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+cudaError_t launch_push_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
+                              cudaStream_t s)
+{
+    if (n == 0 || nsteps <= 0) return cudaSuccess;
+    switch (variant) {
+    case 28: return launch_fused<2, 384, 0>(c, m, n, dt, nsteps, s);
+    case 29: return launch_fused<2, 384, 2>(c, m, n, dt, nsteps, s);
+    case 30: return launch_fused<3, 288, 0>(c, m, n, dt, nsteps, s);
+    case 31: return launch_fused<3, 288, 3>(c, m, n, dt, nsteps, s);
+    case 32: return launch_fused<2, 320, 0>(c, m, n, dt, nsteps, s);
+    case 33: return launch_fused<4, 256, 0>(c, m, n, dt, nsteps, s);
+    default: return cudaErrorInvalidValue;
+    }
+}
+
+}  // namespace trimeg

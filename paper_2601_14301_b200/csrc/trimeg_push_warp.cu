@@ -24,17 +24,13 @@
 // The arithmetic per marker (order of operations, fused multiply-adds) is that of push_kernel.
 #include "trimeg_internal.h"
 #include "trimeg_multi.cuh"
+#include "trimeg_rk4.cuh"
 
 namespace trimeg {
 
 namespace {
 
-constexpr double TWO_PI = 6.283185307179586476925286766559;
 constexpr int NB_MAX = 12;          // distinct triangles per warp and stage that get evaluation slots
-
-enum : unsigned char { FL_ACTIVE = 1, FL_LOST = 2, FL_MOVED = 4, FL_WASACTIVE = 8 };
-// per-marker fp64 state: Y = start-of-step state, A = k1 + 2 k2 + 2 k3, S = stage position
-enum { Y_R, Y_Z, Y_P, Y_V, Y_W, S_MU, A_R, A_Z, A_P, A_V, A_W, S_R, S_Z, S_P, S_V, S_W, N_STATE };
 
 template <int P, int SLACK>
 struct WarpCfg {
@@ -44,53 +40,8 @@ struct WarpCfg {
         (sizeof(double) * (size_t)N_STATE * NW + sizeof(int) * ((size_t)NW + 2 * (size_t)NE) + NW + 15) / 16 * 16;
 };
 
-// Finish one marker at one stage (slot or home role): equations, RK4 bookkeeping, next position,
-// locate of the next position.  q = index of the marker in the warp's slice.
-__device__ __forceinline__ void advance(const MeshDev &M, const PhysDev &Ph, double *S, int NW, int *cell,
-                                        unsigned char *flags, int q, int stage, const FieldVal &fv, double dt,
-                                        double hdt, double dt6)
-{
-    const double R = S[S_R * NW + q], Z = S[S_Z * NW + q];
-    const double v = S[S_V * NW + q], w = S[S_W * NW + q], mu = S[S_MU * NW + q];
-    const Rates k = rhs_point(Ph, R, Z, v, mu, w, fv);
-    const double yR = S[Y_R * NW + q], yZ = S[Y_Z * NW + q], yP = S[Y_P * NW + q];
-    const double yV = S[Y_V * NW + q], yW = S[Y_W * NW + q];
-    double nR, nZ, nP, nV, nW_;
-    if (stage < 3) {
-        if (stage == 0) {
-            S[A_R * NW + q] = k.R; S[A_Z * NW + q] = k.Z; S[A_P * NW + q] = k.phi;
-            S[A_V * NW + q] = k.vpar; S[A_W * NW + q] = k.w;
-        } else {
-            S[A_R * NW + q] = fma(2.0, k.R, S[A_R * NW + q]); S[A_Z * NW + q] = fma(2.0, k.Z, S[A_Z * NW + q]);
-            S[A_P * NW + q] = fma(2.0, k.phi, S[A_P * NW + q]); S[A_V * NW + q] = fma(2.0, k.vpar, S[A_V * NW + q]);
-            S[A_W * NW + q] = fma(2.0, k.w, S[A_W * NW + q]);
-        }
-        const double c = (stage == 2) ? dt : hdt;
-        nR = fma(c, k.R, yR); nZ = fma(c, k.Z, yZ); nP = fma(c, k.phi, yP);
-        nV = fma(c, k.vpar, yV); nW_ = fma(c, k.w, yW);
-    } else {
-        nR = fma(dt6, S[A_R * NW + q] + k.R, yR); nZ = fma(dt6, S[A_Z * NW + q] + k.Z, yZ);
-        nP = fma(dt6, S[A_P * NW + q] + k.phi, yP);
-        nV = fma(dt6, S[A_V * NW + q] + k.vpar, yV); nW_ = fma(dt6, S[A_W * NW + q] + k.w, yW);
-        nP = fma(-TWO_PI, floor(nP * (1.0 / TWO_PI)), nP);
-    }
-    Bary b;
-    int moved = 0;
-    const int tn = locate(M, nR, nZ, cell[q], b, moved);
-    unsigned char fl = flags[q];
-    if (moved) fl |= FL_MOVED;
-    if (tn < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;        // start-of-step state Y is kept; dropped for the rest of the call
-    else {
-        cell[q] = tn;
-        const int o = (stage < 3) ? S_R : Y_R;             // S_* and Y_* are both (R, Z, phi, vpar, w) in this order
-        S[(o + 0) * NW + q] = nR; S[(o + 1) * NW + q] = nZ; S[(o + 2) * NW + q] = nP;
-        S[(o + 3) * NW + q] = nV; S[(o + 4) * NW + q] = nW_;
-    }
-    flags[q] = fl;
-}
-
-template <int P, int WARPS, int SLACK>
-__global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
+template <int P, int WARPS, int SLACK, int ILP, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
                                                                double dt, int nsteps, Stats *st)
 {
     using Cfg = WarpCfg<P, SLACK>;
@@ -218,6 +169,22 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
                     }
                 }
                 gather_multi<P, true>(F, F.coef + (size_t)tri * F.n_modes * NCOEF, xi, eta, phi, f, fx, fe, fp);
+                if constexpr (ILP > 0) {
+#pragma unroll
+                    for (int p0 = 0; p0 < P; p0 += ILP) {
+                        int qs[ILP];
+                        FieldVal fvs[ILP];
+#pragma unroll
+                        for (int i = 0; i < ILP; ++i) {
+                            const int pp = (p0 + i < P) ? p0 + i : P - 1;
+                            qs[i] = (p0 + i < P) ? own[pp] : -1;
+                            fvs[i].f = f[pp]; fvs[i].fphi = fp[pp];
+                            fvs[i].fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
+                            fvs[i].fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
+                        }
+                        advance_multi<ILP>(M, Ph, S, NW, cell, flags, qs, stage, fvs, dt, hdt, dt6);
+                    }
+                } else
 #pragma unroll 1
                 for (int p = 0; p < P; ++p) {
                     // select without dynamic register indexing
@@ -289,20 +256,20 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
     }
 }
 
-template <int P, int WARPS, int SLACK>
+template <int P, int WARPS, int SLACK, int ILP, int MINB = 1>
 cudaError_t launch_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     using Cfg = WarpCfg<P, SLACK>;
     static bool configured = false;
     const size_t shm = Cfg::WARP_BYTES * WARPS;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK, ILP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     const size_t per_cta = (size_t)Cfg::NW * WARPS;
     const size_t ctas = (n + per_cta - 1) / per_cta;
-    push_warp_kernel<P, WARPS, SLACK><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
+    push_warp_kernel<P, WARPS, SLACK, ILP, MINB><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -314,17 +281,27 @@ cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
-    case 7: return launch_warp<2, 4, 4>(c, m, n, dt, nsteps, s);
-    case 8: return launch_warp<3, 4, 6>(c, m, n, dt, nsteps, s);
-    case 9: return launch_warp<4, 4, 8>(c, m, n, dt, nsteps, s);
-    case 10: return launch_warp<2, 2, 4>(c, m, n, dt, nsteps, s);
-    case 11: return launch_warp<2, 4, 6>(c, m, n, dt, nsteps, s);
-    case 12: return launch_warp<2, 4, 8>(c, m, n, dt, nsteps, s);
-    case 13: return launch_warp<3, 4, 9>(c, m, n, dt, nsteps, s);
-    case 14: return launch_warp<3, 4, 12>(c, m, n, dt, nsteps, s);
-    case 15: return launch_warp<4, 4, 12>(c, m, n, dt, nsteps, s);
-    case 16: return launch_warp<4, 4, 16>(c, m, n, dt, nsteps, s);
-    case 17: return launch_warp<4, 4, 20>(c, m, n, dt, nsteps, s);
+    case 7: return launch_warp<2, 4, 4, 0>(c, m, n, dt, nsteps, s);
+    case 8: return launch_warp<3, 4, 6, 0>(c, m, n, dt, nsteps, s);
+    case 9: return launch_warp<4, 4, 8, 0>(c, m, n, dt, nsteps, s);
+    case 10: return launch_warp<2, 2, 4, 0>(c, m, n, dt, nsteps, s);
+    case 11: return launch_warp<2, 4, 6, 0>(c, m, n, dt, nsteps, s);
+    case 12: return launch_warp<2, 4, 8, 0>(c, m, n, dt, nsteps, s);
+    case 13: return launch_warp<3, 4, 9, 0>(c, m, n, dt, nsteps, s);
+    case 14: return launch_warp<3, 4, 12, 0>(c, m, n, dt, nsteps, s);
+    case 15: return launch_warp<4, 4, 12, 0>(c, m, n, dt, nsteps, s);
+    case 16: return launch_warp<4, 4, 16, 0>(c, m, n, dt, nsteps, s);
+    case 17: return launch_warp<4, 4, 20, 0>(c, m, n, dt, nsteps, s);
+    case 18: return launch_warp<2, 4, 6, 2>(c, m, n, dt, nsteps, s);
+    case 19: return launch_warp<3, 4, 9, 3>(c, m, n, dt, nsteps, s);
+    case 20: return launch_warp<4, 4, 16, 2>(c, m, n, dt, nsteps, s);
+    case 21: return launch_warp<4, 4, 16, 4>(c, m, n, dt, nsteps, s);
+    case 22: return launch_warp<4, 2, 16, 2>(c, m, n, dt, nsteps, s);
+    case 23: return launch_warp<3, 4, 9, 1>(c, m, n, dt, nsteps, s);
+    case 24: return launch_warp<3, 4, 9, 0, 3>(c, m, n, dt, nsteps, s);
+    case 25: return launch_warp<3, 4, 9, 1, 3>(c, m, n, dt, nsteps, s);
+    case 26: return launch_warp<2, 4, 6, 0, 4>(c, m, n, dt, nsteps, s);
+    case 27: return launch_warp<3, 2, 9, 0, 6>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }

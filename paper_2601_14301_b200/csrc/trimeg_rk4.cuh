@@ -1,0 +1,133 @@
+// trimeg_rk4.cuh -- row a6 building blocks shared by the shared-memory push kernels: per-marker RK4
+// state layout, marker flags, and "finish a marker at one stage" (equations a4/a5, RK4 bookkeeping,
+// next stage position, locate of that position).  The arithmetic per marker is that of push_kernel.
+#pragma once
+#include "trimeg_device.cuh"
+
+namespace trimeg {
+
+constexpr double TWO_PI = 6.283185307179586476925286766559;
+
+enum : unsigned char { FL_ACTIVE = 1, FL_LOST = 2, FL_MOVED = 4, FL_WASACTIVE = 8 };
+// per-marker fp64 state: Y = start-of-step state, A = k1 + 2 k2 + 2 k3, S = stage position
+enum { Y_R, Y_Z, Y_P, Y_V, Y_W, S_MU, A_R, A_Z, A_P, A_V, A_W, S_R, S_Z, S_P, S_V, S_W, N_STATE };
+
+// Finish one marker at one stage (slot or home role): equations, RK4 bookkeeping, next position,
+// locate of the next position.  q = index of the marker in the warp's slice.
+__device__ __forceinline__ void advance(const MeshDev &M, const PhysDev &Ph, double *S, int NW, int *cell,
+                                        unsigned char *flags, int q, int stage, const FieldVal &fv, double dt,
+                                        double hdt, double dt6)
+{
+    const double R = S[S_R * NW + q], Z = S[S_Z * NW + q];
+    const double v = S[S_V * NW + q], w = S[S_W * NW + q], mu = S[S_MU * NW + q];
+    const Rates k = rhs_point(Ph, R, Z, v, mu, w, fv);
+    const double yR = S[Y_R * NW + q], yZ = S[Y_Z * NW + q], yP = S[Y_P * NW + q];
+    const double yV = S[Y_V * NW + q], yW = S[Y_W * NW + q];
+    double nR, nZ, nP, nV, nW_;
+    if (stage < 3) {
+        if (stage == 0) {
+            S[A_R * NW + q] = k.R; S[A_Z * NW + q] = k.Z; S[A_P * NW + q] = k.phi;
+            S[A_V * NW + q] = k.vpar; S[A_W * NW + q] = k.w;
+        } else {
+            S[A_R * NW + q] = fma(2.0, k.R, S[A_R * NW + q]); S[A_Z * NW + q] = fma(2.0, k.Z, S[A_Z * NW + q]);
+            S[A_P * NW + q] = fma(2.0, k.phi, S[A_P * NW + q]); S[A_V * NW + q] = fma(2.0, k.vpar, S[A_V * NW + q]);
+            S[A_W * NW + q] = fma(2.0, k.w, S[A_W * NW + q]);
+        }
+        const double c = (stage == 2) ? dt : hdt;
+        nR = fma(c, k.R, yR); nZ = fma(c, k.Z, yZ); nP = fma(c, k.phi, yP);
+        nV = fma(c, k.vpar, yV); nW_ = fma(c, k.w, yW);
+    } else {
+        nR = fma(dt6, S[A_R * NW + q] + k.R, yR); nZ = fma(dt6, S[A_Z * NW + q] + k.Z, yZ);
+        nP = fma(dt6, S[A_P * NW + q] + k.phi, yP);
+        nV = fma(dt6, S[A_V * NW + q] + k.vpar, yV); nW_ = fma(dt6, S[A_W * NW + q] + k.w, yW);
+        nP = fma(-TWO_PI, floor(nP * (1.0 / TWO_PI)), nP);
+    }
+    Bary b;
+    int moved = 0;
+    const int tn = locate(M, nR, nZ, cell[q], b, moved);
+    unsigned char fl = flags[q];
+    if (moved) fl |= FL_MOVED;
+    if (tn < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;        // start-of-step state Y is kept; dropped for the rest of the call
+    else {
+        cell[q] = tn;
+        const int o = (stage < 3) ? S_R : Y_R;             // S_* and Y_* are both (R, Z, phi, vpar, w) in this order
+        S[(o + 0) * NW + q] = nR; S[(o + 1) * NW + q] = nZ; S[(o + 2) * NW + q] = nP;
+        S[(o + 3) * NW + q] = nV; S[(o + 4) * NW + q] = nW_;
+    }
+    flags[q] = fl;
+}
+
+// The same for N markers of one lane at once (q[i] < 0 = padding slot): the N equation chains are
+// independent, so written side by side they give the FP64 pipe N-way instruction-level parallelism
+// (a DFMA has 8 cycles of latency and issues every 2).  Straight-line for the common case (the new
+// position is clearly inside the triangle the marker was in); anything else takes locate().
+template <int N>
+__device__ __forceinline__ void advance_multi(const MeshDev &M, const PhysDev &Ph, double *S, int NW, int *cell,
+                                              unsigned char *flags, const int (&q)[N], int stage, const FieldVal (&fv)[N],
+                                              double dt, double hdt, double dt6)
+{
+    int qq[N], c0[N];
+    Rates k[N];
+    double y[N][5], a[N][5], nw[N][5];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        qq[i] = (q[i] >= 0) ? q[i] : 0;                               // padding: compute on marker 0, store nothing
+        const int j = qq[i];
+        k[i] = rhs_point(Ph, S[S_R * NW + j], S[S_Z * NW + j], S[S_V * NW + j], S[S_MU * NW + j], S[S_W * NW + j], fv[i]);
+        c0[i] = cell[j];
+#pragma unroll
+        for (int v = 0; v < 5; ++v) y[i][v] = S[(Y_R + v) * NW + j];
+    }
+    if (stage > 0) {
+#pragma unroll
+        for (int i = 0; i < N; ++i)
+#pragma unroll
+            for (int v = 0; v < 5; ++v) a[i][v] = S[(A_R + v) * NW + qq[i]];
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const double kk[5] = {k[i].R, k[i].Z, k[i].phi, k[i].vpar, k[i].w};
+        if (stage < 3) {
+            const double c = (stage == 2) ? dt : hdt;
+#pragma unroll
+            for (int v = 0; v < 5; ++v) {
+                a[i][v] = (stage == 0) ? kk[v] : fma(2.0, kk[v], a[i][v]);
+                nw[i][v] = fma(c, kk[v], y[i][v]);
+            }
+        } else {
+#pragma unroll
+            for (int v = 0; v < 5; ++v) nw[i][v] = fma(dt6, a[i][v] + kk[v], y[i][v]);
+            nw[i][2] = fma(-TWO_PI, floor(nw[i][2] * (1.0 / TWO_PI)), nw[i][2]);
+        }
+    }
+    // locate the new positions: hinted triangle first, side by side
+    double marg[N];
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        const Bary b = bary_rn(M, c0[i], nw[i][0], nw[i][1]);
+        marg[i] = fmin(fmin(b.xi, b.eta), b.l0);
+    }
+#pragma unroll
+    for (int i = 0; i < N; ++i) {
+        if (q[i] < 0) continue;
+        const int j = q[i];
+        int tn = c0[i], moved = 0;
+        if (!(marg[i] > LOC_TAU)) { Bary b; tn = locate(M, nw[i][0], nw[i][1], c0[i], b, moved); }
+        unsigned char fl = flags[j];
+        if (moved) fl |= FL_MOVED;
+        if (tn < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;    // start-of-step state Y is kept; dropped for the rest of the call
+        else {
+            cell[j] = tn;
+            const int o = (stage < 3) ? S_R : Y_R;
+#pragma unroll
+            for (int v = 0; v < 5; ++v) S[(o + v) * NW + j] = nw[i][v];
+            if (stage < 3) {
+#pragma unroll
+                for (int v = 0; v < 5; ++v) S[(A_R + v) * NW + j] = a[i][v];
+            }
+        }
+        flags[j] = fl;
+    }
+}
+
+}  // namespace trimeg
