@@ -32,6 +32,8 @@ if ROOT not in sys.path:
 import numpy as np
 
 METRIC = "marker RK4 pushes/sec (incl. field gather)"
+PUSH_KERNEL_NAMES = {0: "push_kernel", 1: "push_warp_kernel<2,4,6>", 2: "push_warp_kernel<4,4,16>", 3: "push_fused_kernel<2,384,1>",
+                     4: "push_fused_kernel<3,288,1>", 5: "push_fused_kernel<4,256,1>", 6: "push_fused_kernel<2,192,2>"}
 UNIT = "marker-steps/s"
 
 
@@ -194,6 +196,7 @@ def run_gpu(args, wl):
     ctx.locate(d["R"], d["Z"], cell=d["cell"])
     torch.cuda.synchronize()
     fp64_peak = ctx.measure_fp64_peak()
+    fp64_peak3 = ctx.measure_fp64_peak_operands(3)     # DFMA stream with three fresh register operands
     hbm_peak, hbm_src = load_peaks()
 
     push_events = []
@@ -253,11 +256,15 @@ def run_gpu(args, wl):
     t_fp64 = flops / (fp64_peak * 1e12)
     t_hbm = byts / (hbm_peak * 1e9)
     roof = {
-        "bound": "alu", "kernel": "push_kernel",
+        "bound": "alu", "kernel": PUSH_KERNEL_NAMES.get(ctx.get_push_kernel(), "push kernel"),
         "achieved": flops / push_s * 1e-12, "peak": fp64_peak, "unit": "TFLOP/s",
         "frac": (flops / push_s * 1e-12) / fp64_peak,
         "peak_source": "FP64 DFMA throughput measured live by trimeg_measure_fp64_peak (nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2)",
         "traffic": None,
+        "peak_three_register_operands": fp64_peak3, "frac_of_three_register_operand_peak": (flops / push_s * 1e-12) / fp64_peak3,
+        "peak_three_register_operands_note": "DFMA stream whose three source operands all change from one instruction to the "
+                                             "next (a Horner step over several markers): the FP64 pipe reads one 64-bit register "
+                                             "operand per cycle, so such a stream issues every 3 cycles instead of 2",
         "algorithmic_flops_per_marker_step": flops_per_marker_step(len(wl.modes)),
         "algorithmic_bytes_per_marker_call": 96.0,
         "hbm_time_frac_of_fp64_time": t_hbm / t_fp64, "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,

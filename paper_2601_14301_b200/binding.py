@@ -19,7 +19,7 @@ EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_sort", "trimeg_compact",
-    "trimeg_push", "trimeg_set_push_kernel", "trimeg_push_host", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters",
+    "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
     "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
 )
 
@@ -75,7 +75,9 @@ def load() -> C.CDLL:
     L.trimeg_get_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.trimeg_reset_stats.argtypes = [vp]
     L.trimeg_get_tile_counters.argtypes = [vp, C.POINTER(C.c_int64)]
+    L.trimeg_get_push_kernel.argtypes = [vp]
     L.trimeg_measure_fp64_peak.argtypes = [vp, dp]
+    L.trimeg_measure_fp64_peak_operands.argtypes = [vp, i32, dp]
     L.trimeg_strerror.argtypes = [i32]
     L.trimeg_strerror.restype = C.c_char_p
     L.trimeg_version.restype = C.c_char_p
@@ -240,6 +242,9 @@ class Context:
         ms = _markers(m, n)
         _check(self.L.trimeg_push(self.h, C.byref(ms), n, float(dt), int(nsteps), _stream(stream)), "trimeg_push")
 
+    def get_push_kernel(self) -> int:
+        return int(self.L.trimeg_get_push_kernel(self.h))
+
     def set_push_kernel(self, variant: int):
         _check(self.L.trimeg_set_push_kernel(self.h, int(variant)), "trimeg_set_push_kernel")
 
@@ -259,10 +264,16 @@ class Context:
         _check(self.L.trimeg_measure_fp64_peak(self.h, C.byref(v)), "trimeg_measure_fp64_peak")
         return float(v.value)
 
+    def measure_fp64_peak_operands(self, n_reg_operands: int) -> float:
+        v = C.c_double(0.0)
+        _check(self.L.trimeg_measure_fp64_peak_operands(self.h, int(n_reg_operands), C.byref(v)),
+               "trimeg_measure_fp64_peak_operands")
+        return float(v.value)
+
     def get_tile_counters(self) -> Dict[str, int]:
         a = (C.c_int64 * 8)()
         _check(self.L.trimeg_get_tile_counters(self.h, a), "trimeg_get_tile_counters")
-        names = ("cyc_A", "cyc_B", "cyc_C", "cyc_D", "cyc_E", "n_fallback", "n_bins", "n_stages")
+        names = ("cyc_head", "cyc_B", "cyc_C", "cyc_modes", "cyc_finish", "n_fallback", "n_records", "n_stages")
         return {k: int(v) for k, v in zip(names, a)}
 
     def reset_stats(self):

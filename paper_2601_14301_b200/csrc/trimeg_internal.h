@@ -32,7 +32,7 @@ struct trimeg_ctx {
     double2 *d_coef;
     int *d_mode_n;
     int has_field;
-    int push_kernel;                // 0 = one thread per marker, 1..4 = triangle-batched tile variants
+    int push_kernel;                // trimeg_set_push_kernel variant
     trimeg::Stats *d_stats;
     int64_t n_launches;
     // scratch for sort / compact / host path (grown on demand)
@@ -53,15 +53,11 @@ cudaError_t launch_gather(trimeg_ctx *c, size_t n, const double *R, const double
 cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP,
                        double *dV, double *dW, cudaStream_t s);
 cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
-// trimeg_push_tile.cu: triangle-batched variant (P markers per lane share each coefficient load)
-cudaError_t launch_push_tile(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
-                             cudaStream_t s);
-
-// trimeg_push_warp.cu: warp-autonomous variant (no block barriers; variants 7..10)
+// trimeg_push_warp.cu: warp-autonomous variant (no block barriers; variants 1, 2)
 cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                              cudaStream_t s);
 
-// trimeg_push_fused.cu: CTA tiles with resident coefficient records, fused evaluate + finish (variants 28..)
+// trimeg_push_fused.cu: CTA tiles with resident coefficient records, fused evaluate + finish (variants 3..6)
 cudaError_t launch_push_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                               cudaStream_t s);
 

@@ -249,6 +249,27 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(double *out, double a, d
     if (s == 123.456) out[0] = s;          // never true; keeps the loop alive
 }
 
+// The same with NREG of the three source operands of every DFMA coming fresh from the register file:
+// 1: acc <- acc * a + b (a, b kernel constants); 2: acc <- acc * y0 + z[k] (y0 stays in the operand reuse
+// cache); 3: acc <- acc * y[k] + z[k] (all three change with every instruction).
+template <int NREG>
+__global__ void __launch_bounds__(256) dfma_operand_kernel(double *out, const double *in, double a, double b)
+{
+    double acc[PEAK_CHAINS], y[PEAK_CHAINS], z[PEAK_CHAINS];
+#pragma unroll
+    for (int k = 0; k < PEAK_CHAINS; ++k) { acc[k] = in[threadIdx.x + k]; y[k] = in[300 + threadIdx.x + k]; z[k] = in[600 + threadIdx.x + k]; }
+#pragma unroll 4
+    for (int it = 0; it < PEAK_ITERS; ++it) {
+#pragma unroll
+        for (int k = 0; k < PEAK_CHAINS; ++k)
+            acc[k] = (NREG == 1) ? fma(acc[k], a, b) : (NREG == 2) ? fma(acc[k], y[0], z[k]) : fma(acc[k], y[k], z[k]);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int k = 0; k < PEAK_CHAINS; ++k) s += acc[k] + y[k] + z[k];
+    if (s == 123.456) out[0] = s;          // never true; keeps the loop alive
+}
+
 // ================================================================================ host helpers
 static int ensure_scratch(trimeg_ctx *c, size_t bytes)
 {
@@ -356,7 +377,7 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
         c->field.n_modes = 0; c->field.coef = nullptr; c->field.mode_n = nullptr;
         c->field.n_first = 0; c->field.n_step = 0; c->field.is_ap = 1;
         c->has_field = 0;
-        c->push_kernel = 2;
+        c->push_kernel = 3;
         if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= 0 && v <= TRIMEG_PUSH_KERNEL_MAX) c->push_kernel = v; }
     } while (0);
     if (d_rin2) cudaFree(d_rin2);
@@ -392,6 +413,8 @@ int trimeg_set_params(trimeg_ctx *c, const trimeg_params *p)
     fill_phys(c);
     return TRIMEG_OK;
 }
+
+int trimeg_get_push_kernel(const trimeg_ctx *c) { return c ? c->push_kernel : -1; }
 
 int trimeg_set_push_kernel(trimeg_ctx *c, int variant)
 {
@@ -680,6 +703,36 @@ int trimeg_measure_fp64_peak(trimeg_ctx *c, double *tflops_out)
         cudaEventElapsedTime(&ms, e0, e1);
         const double flops = 2.0 * PEAK_ITERS * PEAK_CHAINS * 256.0 * blocks;
         const double tf = flops / (ms * 1e-3) * 1e-12;
+        if (rep > 0 && tf > best) best = tf;
+        c->n_launches++;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    *tflops_out = best;
+    return rc;
+}
+
+int trimeg_measure_fp64_peak_operands(trimeg_ctx *c, int n_reg_operands, double *tflops_out)
+{
+    if (!c || !tflops_out || n_reg_operands < 1 || n_reg_operands > 3) return TRIMEG_ERR_INVALID_ARG;
+    if (cudaSetDevice(c->device) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_CUDA; }
+    int rc = ensure_scratch(c, 1024 * sizeof(double));
+    if (rc != TRIMEG_OK) return rc;
+    double *buf = (double *)c->d_scratch;
+    if (cudaMemset(buf, 0, 1024 * sizeof(double)) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_CUDA; }
+    const int blocks = c->n_sm * 32;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    for (int rep = 0; rep < 6; ++rep) {
+        cudaEventRecord(e0, 0);
+        if (n_reg_operands == 1) dfma_operand_kernel<1><<<blocks, 256>>>(buf, buf, 0.999999, 1e-9);
+        else if (n_reg_operands == 2) dfma_operand_kernel<2><<<blocks, 256>>>(buf, buf, 0.999999, 1e-9);
+        else dfma_operand_kernel<3><<<blocks, 256>>>(buf, buf, 0.999999, 1e-9);
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaGetLastError(); rc = TRIMEG_ERR_CUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double tf = 2.0 * PEAK_ITERS * PEAK_CHAINS * 256.0 * blocks / (ms * 1e-3) * 1e-12;
         if (rep > 0 && tf > best) best = tf;
         c->n_launches++;
     }

@@ -48,27 +48,38 @@ __device__ __forceinline__ void eval_quintic_multi(const double2 *__restrict__ c
     }
 }
 
-// dphi, d/dxi, d/deta, d/dphi for P markers of one triangle whose record [n_modes][21] starts at c
-// (same formulas as gather()); GLOBAL: c is global memory (read-only path), else shared memory
-template <int P, bool GLOBAL>
-__device__ __forceinline__ void gather_multi(const FieldDev &F, const double2 *c, const double (&xi)[P], const double (&eta)[P],
-                                             const double (&phi)[P], double (&f)[P], double (&fx)[P], double (&fe)[P],
-                                             double (&fp)[P])
+// Toroidal factors of P markers: E = e^{i n_first phi}, D = e^{i n_step phi} (arithmetic progression of
+// mode numbers; else E is recomputed per mode inside gather_modes).
+template <int P>
+__device__ __forceinline__ void gather_phases(const FieldDev &F, const double (&phi)[P], double (&Er)[P], double (&Ei)[P],
+                                              double (&Dr)[P], double (&Di)[P])
 {
-    double Er[P], Ei[P], Dr[P], Di[P];
 #pragma unroll
     for (int p = 0; p < P; ++p) {
-        f[p] = fx[p] = fe[p] = fp[p] = 0.0;
         Er[p] = 1.0; Ei[p] = 0.0; Dr[p] = 1.0; Di[p] = 0.0;
         if (F.is_ap) {
             if (F.n_first != 0) sincos((double)F.n_first * phi[p], &Ei[p], &Er[p]);
             if (F.n_modes > 1) sincos((double)F.n_step * phi[p], &Di[p], &Dr[p]);
         }
     }
+}
+
+// dphi, d/dxi, d/deta, d/dphi for P markers of one triangle whose record [n_modes][21] starts at c
+// (same formulas as gather()); GLOBAL: c is global memory (read-only path), else shared memory
+template <int P, bool GLOBAL, bool AP>
+__device__ __forceinline__ void gather_modes_impl(const FieldDev &F, const double2 *c, const double (&xi)[P],
+                                                  const double (&eta)[P], const double (&phi)[P], double (&Er)[P],
+                                                  double (&Ei)[P], const double (&Dr)[P], const double (&Di)[P],
+                                                  double (&f)[P], double (&fx)[P], double (&fe)[P], double (&fp)[P])
+{
+#pragma unroll
+    for (int p = 0; p < P; ++p) f[p] = fx[p] = fe[p] = fp[p] = 0.0;
     double nn = (double)F.n_first;
+    const double dn = (double)F.n_step;
+    const int n_modes = F.n_modes;
 #pragma unroll 1
-    for (int m = 0; m < F.n_modes; ++m, c += NCOEF) {
-        if (!F.is_ap) {
+    for (int m = 0; m < n_modes; ++m, c += NCOEF) {
+        if (!AP) {
             nn = (double)__ldg(F.mode_n + m);
 #pragma unroll
             for (int p = 0; p < P; ++p) sincos(nn * phi[p], &Ei[p], &Er[p]);
@@ -81,14 +92,37 @@ __device__ __forceinline__ void gather_multi(const FieldDev &F, const double2 *c
             fx[p] = fma(pxr[p], Er[p], fma(-pxi[p], Ei[p], fx[p]));
             fe[p] = fma(per[p], Er[p], fma(-pei[p], Ei[p], fe[p]));
             fp[p] = fma(-nn, fma(pi[p], Er[p], pr[p] * Ei[p]), fp[p]);          // Re(i n P E)
-            if (F.is_ap) {                                                      // E_{n + dn} = E_n E_dn
+            if (AP) {                                                           // E_{n + dn} = E_n E_dn
                 const double tr = fma(Er[p], Dr[p], -Ei[p] * Di[p]);
                 Ei[p] = fma(Er[p], Di[p], Ei[p] * Dr[p]);
                 Er[p] = tr;
             }
         }
-        if (F.is_ap) nn += (double)F.n_step;
+        if (AP) nn += dn;
     }
+}
+
+// dphi, d/dxi, d/deta, d/dphi for P markers of one triangle whose record [n_modes][21] starts at c
+// (same formulas as gather()); GLOBAL: c is global memory (read-only path), else shared memory.
+// Two copies of the loop, so that the mode loop itself is free of the is_ap branch.
+template <int P, bool GLOBAL>
+__device__ __forceinline__ void gather_modes(const FieldDev &F, const double2 *c, const double (&xi)[P], const double (&eta)[P],
+                                             const double (&phi)[P], double (&Er)[P], double (&Ei)[P], const double (&Dr)[P],
+                                             const double (&Di)[P], double (&f)[P], double (&fx)[P], double (&fe)[P],
+                                             double (&fp)[P])
+{
+    if (F.is_ap) gather_modes_impl<P, GLOBAL, true>(F, c, xi, eta, phi, Er, Ei, Dr, Di, f, fx, fe, fp);
+    else gather_modes_impl<P, GLOBAL, false>(F, c, xi, eta, phi, Er, Ei, Dr, Di, f, fx, fe, fp);
+}
+
+template <int P, bool GLOBAL>
+__device__ __forceinline__ void gather_multi(const FieldDev &F, const double2 *c, const double (&xi)[P], const double (&eta)[P],
+                                             const double (&phi)[P], double (&f)[P], double (&fx)[P], double (&fe)[P],
+                                             double (&fp)[P])
+{
+    double Er[P], Ei[P], Dr[P], Di[P];
+    gather_phases<P>(F, phi, Er, Ei, Dr, Di);
+    gather_modes<P, GLOBAL>(F, c, xi, eta, phi, Er, Ei, Dr, Di, f, fx, fe, fp);
 }
 
 }  // namespace trimeg

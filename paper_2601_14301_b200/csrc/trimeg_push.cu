@@ -163,9 +163,8 @@ cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double 
 cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
-    if (c->push_kernel >= 28) return launch_push_fused(c, m, n, dt, nsteps, c->push_kernel, s);
-    if (c->push_kernel >= 7) return launch_push_warp(c, m, n, dt, nsteps, c->push_kernel, s);
-    if (c->push_kernel > 0) return launch_push_tile(c, m, n, dt, nsteps, c->push_kernel, s);
+    if (c->push_kernel >= 3) return launch_push_fused(c, m, n, dt, nsteps, c->push_kernel, s);
+    if (c->push_kernel >= 1) return launch_push_warp(c, m, n, dt, nsteps, c->push_kernel, s);
     push_kernel<<<grid_for(n, PUSH_BLOCK), PUSH_BLOCK, 0, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;
     return cudaGetLastError();

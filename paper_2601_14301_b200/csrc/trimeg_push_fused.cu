@@ -51,8 +51,8 @@ struct FusedCfg {
 
 __device__ __forceinline__ unsigned hash_tri(int t) { return ((unsigned)t * 0x9E3779B1u) >> 26; }   // 6 bits
 
-template <int P, int T, int ILP>
-__global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
+template <int P, int T, int CTAS>
+__global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
                                                           double dt, int nsteps, Stats *st, int nslot)
 {
     using Cfg = FusedCfg<P, T>;
@@ -93,6 +93,8 @@ __global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F,
                 const double R = m.R[g], Z = m.Z[g];
                 S[Y_R * NT + q] = R; S[Y_Z * NT + q] = Z; S[Y_P * NT + q] = m.phi[g];
                 S[Y_V * NT + q] = m.vpar[g]; S[Y_W * NT + q] = m.w[g]; S[S_MU * NT + q] = m.mu[g];
+#pragma unroll
+                for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
                 fl = FL_ACTIVE | FL_WASACTIVE;
                 Bary b;
                 int moved = 0;
@@ -109,6 +111,46 @@ __global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F,
     __syncthreads();
 
     unsigned n_copied = 0, n_stages = 0;
+    long long tph[6] = {0, 0, 0, 0, 0, 0}, tlast = clock64();       // thread 0: cycles per phase
+#define FUSED_TICK(k) do { if (tid == 0) { const long long now_ = clock64(); tph[k] += now_ - tlast; tlast = now_; } } while (0)
+
+    // Bin marker q (triangle t) for the NEXT evaluation: warp-aggregated -- one probe sequence and one
+    // atomicAdd per distinct triangle of the warp.  Must be called by all 32 lanes (act = false: no marker).
+    auto bin_marker = [&](bool act, int q, int t) {
+        const int key = act ? t : -1 - lane;
+        const unsigned grp = __match_any_sync(FULL, key);
+        const int leader = __ffs(grp) - 1;
+        int bin = -1, rank0 = 0;
+        if (act && lane == leader) {
+            unsigned h = hash_tri(t);
+#pragma unroll 1
+            for (int pr = 0; pr < NPROBE; ++pr) {
+                const int prev = atomicCAS(&tag[h], BIN_EMPTY, t);
+                if (prev == BIN_EMPTY) {                   // first marker of the tile in this triangle: record slot + copy
+                    const int r = atomicAdd(&misc[MI_NREC], 1);
+                    if (r < nslot) { rec_of[h] = r; load_list[atomicAdd(&misc[MI_NLOAD], 1)] = (int)h; }
+                    else rec_of[h] = -1;
+                }
+                if (prev == BIN_EMPTY || prev == t) { bin = (int)h; break; }
+                h = (h + 1) & (NBIN - 1);
+            }
+            if (bin >= 0) rank0 = atomicAdd(&cnt[bin], __popc(grp));
+        }
+        bin = __shfl_sync(FULL, bin, leader);
+        rank0 = __shfl_sync(FULL, rank0, leader);
+        if (act) binrank[q] = (bin >= 0) ? ((bin << 16) | (rank0 + __popc(grp & ((1u << lane) - 1u)))) : -1;
+    };
+
+    if (has_field) {                                       // bins of the first stage
+#pragma unroll 1
+        for (int q0 = 0; q0 < NT; q0 += T) {
+            const int q = q0 + tid;
+            const bool act = (q < NT) && (flags[q] & FL_ACTIVE);
+            bin_marker(act, q, act ? cell[q] : -1);
+        }
+        __syncthreads();
+    }
+
 #pragma unroll 1
     for (int step = 0; step < nsteps; ++step) {
 #pragma unroll 1
@@ -117,54 +159,16 @@ __global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F,
 #pragma unroll 1
                 for (int q = tid; q < NT; q += T) {
                     if (!(flags[q] & FL_ACTIVE)) continue;
-                    if (stage == 0) {
-#pragma unroll
-                        for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
-                    }
                     FieldVal fv;
                     fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
                     advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
-                }
-                continue;                                  // a thread only ever touches its own markers here
-            }
-            // ---------------------------------------------------------------- A: bin by triangle
-#pragma unroll 1
-            for (int q0 = 0; q0 < NT; q0 += T) {
-                const int q = q0 + tid;
-                const bool act = (q < NT) && (flags[q] & FL_ACTIVE);
-                int t = -1;
-                if (act) {
-                    t = cell[q];
-                    if (stage == 0) {
+                    if (stage == 3) {
 #pragma unroll
                         for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
                     }
                 }
-                // warp-aggregated insertion: one probe sequence and one atomicAdd per distinct triangle
-                const int key = act ? t : -1 - lane;
-                const unsigned grp = __match_any_sync(FULL, key);
-                const int leader = __ffs(grp) - 1;
-                int bin = -1, rank0 = 0;
-                if (act && lane == leader) {
-                    unsigned h = hash_tri(t);
-#pragma unroll 1
-                    for (int pr = 0; pr < NPROBE; ++pr) {
-                        const int prev = atomicCAS(&tag[h], BIN_EMPTY, t);
-                        if (prev == BIN_EMPTY) {           // first marker of the tile in this triangle: record slot + copy
-                            const int r = atomicAdd(&misc[MI_NREC], 1);
-                            if (r < nslot) { rec_of[h] = r; load_list[atomicAdd(&misc[MI_NLOAD], 1)] = (int)h; }
-                            else rec_of[h] = -1;
-                        }
-                        if (prev == BIN_EMPTY || prev == t) { bin = (int)h; break; }
-                        h = (h + 1) & (NBIN - 1);
-                    }
-                    if (bin >= 0) rank0 = atomicAdd(&cnt[bin], __popc(grp));
-                }
-                bin = __shfl_sync(FULL, bin, leader);
-                rank0 = __shfl_sync(FULL, rank0, leader);
-                if (q < NT) binrank[q] = (act && bin >= 0) ? ((bin << 16) | (rank0 + __popc(grp & ((1u << lane) - 1u)))) : -1;
+                continue;                                  // a thread only ever touches its own markers here
             }
-            __syncthreads();
             // ---------------------------------------------------------------- B: copy new records, scan the bins
             {
                 const int n_load = misc[MI_NLOAD];
@@ -206,6 +210,7 @@ __global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F,
                 if (lane == 0) { misc[MI_NEV] = n_ev; misc[MI_NFB] = 0; }
             }
             __syncthreads();
+            FUSED_TICK(1);
             // ---------------------------------------------------------------- C: markers -> evaluation slots
 #pragma unroll 1
             for (int q = tid; q < NT; q += T) {
@@ -215,15 +220,25 @@ __global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F,
                 if (br >= 0 && off[b] >= 0) ev[off[b] + (br & 0xffff)] = q | (rec_of[b] << 16);
                 else fb_list[atomicAdd(&misc[MI_NFB], 1)] = q;
             }
+            // the table is nearly full of triangles the markers have left: start it afresh with the bins of the next step
+            const bool clear = (stage == 3) && (misc[MI_NREC] > min(nslot, NBIN) - 8);   // MI_NREC only changes in phase D
+            if (tid < NBIN) cnt[tid] = 0;                                     // phase D counts the bins of the next stage
             if (tid == 0) misc[MI_NLOAD] = 0;
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncthreads();
+            if (clear) {                                                      // uniform; rec_of / tag were read by phase C
+                if (tid < NBIN) { tag[tid] = BIN_EMPTY; rec_of[tid] = -1; }
+                if (tid == 0) misc[MI_NREC] = 0;
+                __syncthreads();
+            }
+            FUSED_TICK(2);
             // ---------------------------------------------------------------- D: evaluate + finish, P slots per thread
-            if (tid < NBIN) cnt[tid] = 0;                                     // for the next stage
             const int n_ev = misc[MI_NEV];
+            int own[P];
+#pragma unroll
+            for (int p = 0; p < P; ++p) own[p] = -1;
             if (tid * P < n_ev) {
                 const int e0 = tid * P;
-                int own[P];
 #pragma unroll
                 for (int p = 0; p < P; ++p) { const int v = ev[e0 + p]; own[p] = (v >= 0) ? (v & 0xffff) : -1; }
                 const int rec = ev[e0] >> 16;                                // first slot of a group is real
@@ -241,64 +256,67 @@ __global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F,
                         phi[p] = S[S_P * NT + own[p]];
                     }
                 }
-                gather_multi<P, false>(F, REC + (size_t)rec * rec_stride, xi, eta, phi, f, fx, fe, fp);
-                if constexpr (ILP > 0) {
-#pragma unroll
-                    for (int p0 = 0; p0 < P; p0 += ILP) {
-                        int qs[ILP];
-                        FieldVal fvs[ILP];
-#pragma unroll
-                        for (int i = 0; i < ILP; ++i) {
-                            const int pp = (p0 + i < P) ? p0 + i : P - 1;
-                            qs[i] = (p0 + i < P) ? own[pp] : -1;
-                            fvs[i].f = f[pp]; fvs[i].fphi = fp[pp];
-                            fvs[i].fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
-                            fvs[i].fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
-                        }
-                        advance_multi<ILP>(M, Ph, S, NT, cell, flags, qs, stage, fvs, dt, hdt, dt6);
-                    }
-                } else {
+                double Er[P], Ei[P], Dr[P], Di[P];
+                gather_phases<P>(F, phi, Er, Ei, Dr, Di);
+                FUSED_TICK(0);
+                gather_modes<P, false>(F, REC + (size_t)rec * rec_stride, xi, eta, phi, Er, Ei, Dr, Di, f, fx, fe, fp);
+                FUSED_TICK(3);
 #pragma unroll 1
-                    for (int p = 0; p < P; ++p) {
-                        int q = -1;                                              // select without dynamic register indexing
-                        FieldVal fv;
-                        fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
+                for (int p = 0; p < P; ++p) {
+                    int q = -1;                                              // select without dynamic register indexing
+                    FieldVal fv;
+                    fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
 #pragma unroll
-                        for (int pp = 0; pp < P; ++pp)
-                            if (pp == p) {
-                                q = own[pp]; fv.f = f[pp]; fv.fphi = fp[pp];
-                                fv.fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
-                                fv.fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
-                            }
-                        if (q >= 0) advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
-                    }
+                    for (int pp = 0; pp < P; ++pp)
+                        if (pp == p) {
+                            q = own[pp]; fv.f = f[pp]; fv.fphi = fp[pp];
+                            fv.fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
+                            fv.fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
+                        }
+                    if (q >= 0) advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
                 }
+            }
+            // the markers this thread finished: start-of-step copy, bin for the next stage (all lanes take part)
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                const int q = own[p];
+                const bool act = (q >= 0) && (flags[q] & FL_ACTIVE);
+                if (act && stage == 3) {
+#pragma unroll
+                    for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
+                }
+                bin_marker(act, q, act ? cell[q] : -1);
             }
             // markers without a slot: one per thread, coefficients from global memory
             {
                 const int n_fb = misc[MI_NFB];
 #pragma unroll 1
-                for (int i = tid; i < n_fb; i += T) {
-                    const int q = fb_list[i];
-                    const int tt = cell[q];
-                    const Bary b = bary_rn(M, tt, S[S_R * NT + q], S[S_Z * NT + q]);
-                    const FieldVal fv = gather(F, tt, b, S[S_P * NT + q]);
-                    ++n_fallback;
-                    advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
+                for (int i0 = 0; i0 < n_fb; i0 += T) {
+                    const int i = i0 + tid;
+                    int q = -1;
+                    if (i < n_fb) {
+                        q = fb_list[i];
+                        const int tt = cell[q];
+                        const Bary b = bary_rn(M, tt, S[S_R * NT + q], S[S_Z * NT + q]);
+                        const FieldVal fv = gather(F, tt, b, S[S_P * NT + q]);
+                        ++n_fallback;
+                        advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
+                    }
+                    const bool act = (q >= 0) && (flags[q] & FL_ACTIVE);
+                    if (act && stage == 3) {
+#pragma unroll
+                        for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
+                    }
+                    bin_marker(act, q, act ? cell[q] : -1);
                 }
             }
+            FUSED_TICK(4);
             __syncthreads();
+            FUSED_TICK(5);
             if (tid == 0) ++n_stages;
-            // the table is nearly full of triangles the markers have left: start it afresh
-            if (stage == 3 && misc[MI_NREC] > min(nslot, NBIN) - 8) {
-                __syncthreads();                                              // everybody has read MI_NREC
-                if (tid < NBIN) { tag[tid] = BIN_EMPTY; rec_of[tid] = -1; }
-                if (tid == 0) misc[MI_NREC] = 0;
-                __syncthreads();
-            }
         }
     }
-
+#undef FUSED_TICK
     // ---- write back, statistics
     int lost = 0, moved = 0;
     for (int q = tid; q < nt; q += T) {
@@ -320,19 +338,21 @@ __global__ void __launch_bounds__(T, 1) push_fused_kernel(MeshDev M, FieldDev F,
         if (n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);
     }
     if (tid == 0) {
+#pragma unroll
+        for (int k = 0; k < 5; ++k) atomicAdd(&st->tile[k], (unsigned long long)(k == 4 ? tph[4] + tph[5] : tph[k]));
         atomicAdd(&st->tile[6], (unsigned long long)n_copied);
         atomicAdd(&st->tile[7], (unsigned long long)n_stages);
     }
 }
 
-template <int P, int T, int ILP>
+template <int P, int T, int CTAS = 1>
 cudaError_t launch_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     using Cfg = FusedCfg<P, T>;
     static bool configured = false;
-    constexpr size_t SMEM_MAX = 227 * 1024;                 // per-CTA limit on sm_100
+    constexpr size_t SMEM_MAX = (228 * 1024) / CTAS - 1024;  // 228 KB per SM, 1 KB per CTA reserved by the system
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_fused_kernel<P, T, ILP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+        cudaError_t e = cudaFuncSetAttribute(push_fused_kernel<P, T, CTAS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
         if (e != cudaSuccess) return e;
         configured = true;
     }
@@ -342,7 +362,7 @@ cudaError_t launch_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, doubl
     if (nslot > NBIN) nslot = NBIN;
     const size_t shm = Cfg::BASE_BYTES + (size_t)nslot * rec_bytes;
     const size_t tiles = (n + Cfg::NT - 1) / Cfg::NT;
-    push_fused_kernel<P, T, ILP><<<(unsigned)tiles, T, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats, nslot);
+    push_fused_kernel<P, T, CTAS><<<(unsigned)tiles, T, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats, nslot);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -354,12 +374,10 @@ cudaError_t launch_push_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, 
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
-    case 28: return launch_fused<2, 384, 0>(c, m, n, dt, nsteps, s);
-    case 29: return launch_fused<2, 384, 2>(c, m, n, dt, nsteps, s);
-    case 30: return launch_fused<3, 288, 0>(c, m, n, dt, nsteps, s);
-    case 31: return launch_fused<3, 288, 3>(c, m, n, dt, nsteps, s);
-    case 32: return launch_fused<2, 320, 0>(c, m, n, dt, nsteps, s);
-    case 33: return launch_fused<4, 256, 0>(c, m, n, dt, nsteps, s);
+    case 3: return launch_fused<2, 384>(c, m, n, dt, nsteps, s);
+    case 4: return launch_fused<3, 288>(c, m, n, dt, nsteps, s);
+    case 5: return launch_fused<4, 256>(c, m, n, dt, nsteps, s);
+    case 6: return launch_fused<2, 192, 2>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -1,10 +1,9 @@
 // trimeg_push_warp.cu -- warp-autonomous, triangle-batched fused RK4 push (rows a2-a6 of DESIGN.md §1).
 //
-// Why (profiles/r01_tile_kernel.md): in the block-synchronous tile kernel the batched evaluation
-// (phase D) runs the FP64 pipe at ~75 %, but locate / binning / scan / scatter / equations are
-// latency-bound chains that the whole CTA waits for between barriers: a third of the time the
-// FP64 pipe idles.  Two CTAs per SM do not help, because each then has too few warps to keep the
-// pipe busy during its own evaluation.
+// Why: with one thread per marker every lane fetches every coefficient itself (21 x 16-byte loads per
+// mode and stage) and the SM's load/store data pipe, not the FP64 pipe, bounds the kernel
+// (profiles/r01_baseline_push_kernel.md).  A coefficient held in a register must serve several markers,
+// which therefore have to sit in the same triangle at the moment of the evaluation.
 //
 // How: every WARP owns NW = 32 P - slack consecutive markers for the whole call (their RK4 state
 // sits in a warp-private slice of shared memory) and runs the stage loop on its own, with
@@ -40,8 +39,8 @@ struct WarpCfg {
         (sizeof(double) * (size_t)N_STATE * NW + sizeof(int) * ((size_t)NW + 2 * (size_t)NE) + NW + 15) / 16 * 16;
 };
 
-template <int P, int WARPS, int SLACK, int ILP, int MINB>
-__global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
+template <int P, int WARPS, int SLACK>
+__global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
                                                                double dt, int nsteps, Stats *st)
 {
     using Cfg = WarpCfg<P, SLACK>;
@@ -169,22 +168,6 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
                     }
                 }
                 gather_multi<P, true>(F, F.coef + (size_t)tri * F.n_modes * NCOEF, xi, eta, phi, f, fx, fe, fp);
-                if constexpr (ILP > 0) {
-#pragma unroll
-                    for (int p0 = 0; p0 < P; p0 += ILP) {
-                        int qs[ILP];
-                        FieldVal fvs[ILP];
-#pragma unroll
-                        for (int i = 0; i < ILP; ++i) {
-                            const int pp = (p0 + i < P) ? p0 + i : P - 1;
-                            qs[i] = (p0 + i < P) ? own[pp] : -1;
-                            fvs[i].f = f[pp]; fvs[i].fphi = fp[pp];
-                            fvs[i].fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
-                            fvs[i].fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
-                        }
-                        advance_multi<ILP>(M, Ph, S, NW, cell, flags, qs, stage, fvs, dt, hdt, dt6);
-                    }
-                } else
 #pragma unroll 1
                 for (int p = 0; p < P; ++p) {
                     // select without dynamic register indexing
@@ -256,20 +239,20 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
     }
 }
 
-template <int P, int WARPS, int SLACK, int ILP, int MINB = 1>
+template <int P, int WARPS, int SLACK>
 cudaError_t launch_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     using Cfg = WarpCfg<P, SLACK>;
     static bool configured = false;
     const size_t shm = Cfg::WARP_BYTES * WARPS;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK, ILP, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     const size_t per_cta = (size_t)Cfg::NW * WARPS;
     const size_t ctas = (n + per_cta - 1) / per_cta;
-    push_warp_kernel<P, WARPS, SLACK, ILP, MINB><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
+    push_warp_kernel<P, WARPS, SLACK><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -281,27 +264,8 @@ cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
-    case 7: return launch_warp<2, 4, 4, 0>(c, m, n, dt, nsteps, s);
-    case 8: return launch_warp<3, 4, 6, 0>(c, m, n, dt, nsteps, s);
-    case 9: return launch_warp<4, 4, 8, 0>(c, m, n, dt, nsteps, s);
-    case 10: return launch_warp<2, 2, 4, 0>(c, m, n, dt, nsteps, s);
-    case 11: return launch_warp<2, 4, 6, 0>(c, m, n, dt, nsteps, s);
-    case 12: return launch_warp<2, 4, 8, 0>(c, m, n, dt, nsteps, s);
-    case 13: return launch_warp<3, 4, 9, 0>(c, m, n, dt, nsteps, s);
-    case 14: return launch_warp<3, 4, 12, 0>(c, m, n, dt, nsteps, s);
-    case 15: return launch_warp<4, 4, 12, 0>(c, m, n, dt, nsteps, s);
-    case 16: return launch_warp<4, 4, 16, 0>(c, m, n, dt, nsteps, s);
-    case 17: return launch_warp<4, 4, 20, 0>(c, m, n, dt, nsteps, s);
-    case 18: return launch_warp<2, 4, 6, 2>(c, m, n, dt, nsteps, s);
-    case 19: return launch_warp<3, 4, 9, 3>(c, m, n, dt, nsteps, s);
-    case 20: return launch_warp<4, 4, 16, 2>(c, m, n, dt, nsteps, s);
-    case 21: return launch_warp<4, 4, 16, 4>(c, m, n, dt, nsteps, s);
-    case 22: return launch_warp<4, 2, 16, 2>(c, m, n, dt, nsteps, s);
-    case 23: return launch_warp<3, 4, 9, 1>(c, m, n, dt, nsteps, s);
-    case 24: return launch_warp<3, 4, 9, 0, 3>(c, m, n, dt, nsteps, s);
-    case 25: return launch_warp<3, 4, 9, 1, 3>(c, m, n, dt, nsteps, s);
-    case 26: return launch_warp<2, 4, 6, 0, 4>(c, m, n, dt, nsteps, s);
-    case 27: return launch_warp<3, 2, 9, 0, 6>(c, m, n, dt, nsteps, s);
+    case 1: return launch_warp<2, 4, 6>(c, m, n, dt, nsteps, s);
+    case 2: return launch_warp<4, 4, 16>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }

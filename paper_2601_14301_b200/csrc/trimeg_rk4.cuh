@@ -57,77 +57,4 @@ __device__ __forceinline__ void advance(const MeshDev &M, const PhysDev &Ph, dou
     flags[q] = fl;
 }
 
-// The same for N markers of one lane at once (q[i] < 0 = padding slot): the N equation chains are
-// independent, so written side by side they give the FP64 pipe N-way instruction-level parallelism
-// (a DFMA has 8 cycles of latency and issues every 2).  Straight-line for the common case (the new
-// position is clearly inside the triangle the marker was in); anything else takes locate().
-template <int N>
-__device__ __forceinline__ void advance_multi(const MeshDev &M, const PhysDev &Ph, double *S, int NW, int *cell,
-                                              unsigned char *flags, const int (&q)[N], int stage, const FieldVal (&fv)[N],
-                                              double dt, double hdt, double dt6)
-{
-    int qq[N], c0[N];
-    Rates k[N];
-    double y[N][5], a[N][5], nw[N][5];
-#pragma unroll
-    for (int i = 0; i < N; ++i) {
-        qq[i] = (q[i] >= 0) ? q[i] : 0;                               // padding: compute on marker 0, store nothing
-        const int j = qq[i];
-        k[i] = rhs_point(Ph, S[S_R * NW + j], S[S_Z * NW + j], S[S_V * NW + j], S[S_MU * NW + j], S[S_W * NW + j], fv[i]);
-        c0[i] = cell[j];
-#pragma unroll
-        for (int v = 0; v < 5; ++v) y[i][v] = S[(Y_R + v) * NW + j];
-    }
-    if (stage > 0) {
-#pragma unroll
-        for (int i = 0; i < N; ++i)
-#pragma unroll
-            for (int v = 0; v < 5; ++v) a[i][v] = S[(A_R + v) * NW + qq[i]];
-    }
-#pragma unroll
-    for (int i = 0; i < N; ++i) {
-        const double kk[5] = {k[i].R, k[i].Z, k[i].phi, k[i].vpar, k[i].w};
-        if (stage < 3) {
-            const double c = (stage == 2) ? dt : hdt;
-#pragma unroll
-            for (int v = 0; v < 5; ++v) {
-                a[i][v] = (stage == 0) ? kk[v] : fma(2.0, kk[v], a[i][v]);
-                nw[i][v] = fma(c, kk[v], y[i][v]);
-            }
-        } else {
-#pragma unroll
-            for (int v = 0; v < 5; ++v) nw[i][v] = fma(dt6, a[i][v] + kk[v], y[i][v]);
-            nw[i][2] = fma(-TWO_PI, floor(nw[i][2] * (1.0 / TWO_PI)), nw[i][2]);
-        }
-    }
-    // locate the new positions: hinted triangle first, side by side
-    double marg[N];
-#pragma unroll
-    for (int i = 0; i < N; ++i) {
-        const Bary b = bary_rn(M, c0[i], nw[i][0], nw[i][1]);
-        marg[i] = fmin(fmin(b.xi, b.eta), b.l0);
-    }
-#pragma unroll
-    for (int i = 0; i < N; ++i) {
-        if (q[i] < 0) continue;
-        const int j = q[i];
-        int tn = c0[i], moved = 0;
-        if (!(marg[i] > LOC_TAU)) { Bary b; tn = locate(M, nw[i][0], nw[i][1], c0[i], b, moved); }
-        unsigned char fl = flags[j];
-        if (moved) fl |= FL_MOVED;
-        if (tn < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;    // start-of-step state Y is kept; dropped for the rest of the call
-        else {
-            cell[j] = tn;
-            const int o = (stage < 3) ? S_R : Y_R;
-#pragma unroll
-            for (int v = 0; v < 5; ++v) S[(o + v) * NW + j] = nw[i][v];
-            if (stage < 3) {
-#pragma unroll
-                for (int v = 0; v < 5; ++v) S[(A_R + v) * NW + j] = a[i][v];
-            }
-        }
-        flags[j] = fl;
-    }
-}
-
 }  // namespace trimeg

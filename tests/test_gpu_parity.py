@@ -318,8 +318,8 @@ def test_non_arithmetic_mode_list(B, inputs):
         assert rel_err(got[k].cpu().numpy(), want[k], np.abs(want[k]).max()).max() < 1e-12
 
 
-# ----------------------------------------------------------------------------- tile kernels
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11, 12, 13, 14, 15, 16, 17, 18, 19, 20, 21, 22, 23, 24, 25, 26, 27, 28, 29, 30, 31, 32, 33])
+# ----------------------------------------------------------------------------- push-kernel schedules
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6])
 @pytest.mark.parametrize("name,n,nsteps,sort", [("cfg1", 4096, 20, False), ("cfg1", 1777, 3, True),
                                                 ("cfg2", (1 << 16) + 13, 3, True), ("cfg5", 40009, 5, True),
                                                 ("cfg3", 20011, 2, False)])
@@ -351,8 +351,8 @@ def test_push_kernel_variants_match_oracle(B, inputs, variant, name, n, nsteps, 
     assert ctx.get_stats()["n_lost"] == int((want["cell"] < 0).sum()) - outside_at_start
 
 
-@pytest.mark.parametrize("variant", [1, 4, 5, 7, 9, 28, 31, 33])
-def test_push_tile_kernel_edge_cases(B, inputs, variant):
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6])
+def test_push_kernel_schedules_edge_cases(B, inputs, variant):
     """No field modes (weights bit-identical), already-lost markers on input are left untouched,
     two calls equal one, non-arithmetic mode list."""
     wl, o, ctx, _, _ = _setup(B, inputs, "cfg1", modes=())
