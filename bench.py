@@ -32,6 +32,9 @@ if ROOT not in sys.path:
 import numpy as np
 
 METRIC = "marker RK4 pushes/sec (incl. field gather)"
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the push kernel, from the committed ncu --set full
+# capture (profiles/r01_fused_push_kernel.md): (workload, push kernel, sort_every, markers) -> bytes; null for anything else
+PROFILED_DRAM_BYTES_PER_LAUNCH = {("cfg5", 3, 10, 1 << 24): 1.936e9}
 PUSH_KERNEL_NAMES = {0: "push_kernel", 1: "push_warp_kernel<2,4,6>", 2: "push_warp_kernel<4,4,16>", 3: "push_fused_kernel<2,384,1>",
                      4: "push_fused_kernel<3,288,1>", 5: "push_fused_kernel<4,256,1>", 6: "push_fused_kernel<2,192,2>"}
 UNIT = "marker-steps/s"
@@ -260,7 +263,7 @@ def run_gpu(args, wl):
         "achieved": flops / push_s * 1e-12, "peak": fp64_peak, "unit": "TFLOP/s",
         "frac": (flops / push_s * 1e-12) / fp64_peak,
         "peak_source": "FP64 DFMA throughput measured live by trimeg_measure_fp64_peak (nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2)",
-        "traffic": None,
+        "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get((wl.name, ctx.get_push_kernel(), sort_every, n)),
         "peak_three_register_operands": fp64_peak3, "frac_of_three_register_operand_peak": (flops / push_s * 1e-12) / fp64_peak3,
         "peak_three_register_operands_note": "DFMA stream whose three source operands all change from one instruction to the "
                                              "next (a Horner step over several markers): the FP64 pipe reads one 64-bit register "

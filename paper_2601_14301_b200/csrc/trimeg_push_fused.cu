@@ -1,28 +1,24 @@
 // trimeg_push_fused.cu -- CTA-tile fused RK4 push with resident coefficient records (rows a2-a6 of
 // DESIGN.md §1).
 //
-// What the measurements say (profiles/r01_warp_kernel.md): the batched Horner evaluation is 88 % of
-// the FP64 work; it runs the FP64 pipe at 0.85-0.88 of peak when (a) three warps per scheduler share
-// the pipe and (b) the coefficients come from shared memory (LDS.128: 3.15 SM-cycles per warp-wide
-// load whatever the mix of triangles, fixed 29-cycle latency), but only at ~0.55 when they come
-// through L1 (LDG.128: 4.6+ cycles, more when the lanes sit in several triangles; the records of
-// all resident warps do not fit next to their shared-memory state, so a quarter of the loads go to
-// L2).  The block-synchronous tile kernel had the shared-memory records but idled the pipe during
-// its locate / bin / scatter / equations phases; the warp-autonomous kernel had the overlap but
-// not the records.
+// Why (profiles/r01_fused_push_kernel.md): the batched Horner evaluation is 88 % of the FP64 work.  Fed
+// through L1 (warp kernel) it is held back by the load path: a warp-wide LDG.128 costs 4.6 cycles of the
+// SM's data pipe -- more when the lanes sit in several triangles --, and the records of all resident warps
+// do not fit in what is left of L1 next to their shared-memory state.  From shared memory a warp-wide
+// LDS.128 costs 3.15 cycles whatever the mix of triangles (records padded by 16 B), with a fixed latency.
 //
 // This kernel: one CTA owns a tile of NT consecutive markers for the whole call (RK4 state in shared
-// memory).  Per RK4 stage
-//   A  bin the markers by their (already known) triangle in a small hash table (warp-aggregated);
-//      the table and the coefficient records behind it STAY between stages and steps -- only a
-//      triangle that no marker of the tile was in before costs a copy (cp.async, 16 B per lane);
-//   B  scan of the bin sizes, each padded to a multiple of P -> evaluation slots, sorted by triangle;
+// memory) and keeps the coefficient records of the tile's triangles in shared memory BETWEEN stages and
+// steps -- only a triangle that no marker of the tile was in before costs a copy.  Per RK4 stage
+//   B  the records of new triangles are copied global -> shared (cp.async, 16 B per lane); one warp scans
+//      the bin sizes, each padded to a multiple of P -> evaluation slots, sorted by triangle;
 //   C  every marker writes its index into its slot;
-//   D  one pass, no barrier inside: each thread takes P consecutive slots -- one triangle --, runs
-//      the bivariate Horner scheme for the P markers off ONE shared-memory load of each
-//      coefficient, then finishes the same P markers: chain rule, equilibrium + equations (a4, a5),
-//      RK4 bookkeeping (a6), next stage position and the locate (a2) of that position.  The
-//      latency-bound tails of one warp run under the Horner loops of the others.
+//   D  one pass, no barrier inside: each thread takes P consecutive slots -- one triangle --, runs the
+//      bivariate Horner scheme for the P markers off ONE shared-memory load of each coefficient, then
+//      finishes the same P markers: chain rule, equilibrium + equations (a4, a5), RK4 bookkeeping (a6),
+//      next stage position and the locate (a2) of that position, and bins them by their new triangle
+//      for the next stage (small hash table, warp-aggregated: one probe sequence and one atomicAdd per
+//      distinct triangle of a warp).
 // Markers without a record (more distinct triangles than record slots: unsorted input) or without a
 // slot are evaluated one per thread with the one-marker gather of trimeg_device.cuh: same arithmetic.
 #include "trimeg_internal.h"
@@ -38,7 +34,7 @@ constexpr int NPROBE = 8;
 constexpr int BIN_EMPTY = -1;
 
 // misc[] slots
-enum { MI_NEV, MI_NREC, MI_NLOAD, MI_NFB, MI_CLEAR, MI_COUNT = 8 };
+enum { MI_NEV, MI_NREC, MI_NLOAD, MI_NFB, MI_COUNT = 8 };
 
 template <int P, int T>
 struct FusedCfg {
