@@ -161,22 +161,24 @@ int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_d
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
 /* Kernel used by trimeg_push / trimeg_push_host (same results, different schedules):
+ *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 3 for a field of 12 or more toroidal modes, else variant 1;
  *   0  one thread per marker, state in registers, coefficients through L1;
  *   1, 2  warp-autonomous: every warp owns 32 P - slack markers (state in shared memory), groups them by
  *         triangle with ballots at every RK4 stage and evaluates P markers of one triangle per lane off a
  *         single load of each coefficient (through L1), finishes and re-locates them without any block
  *         barrier (1: P = 2; 2: P = 4);
- *   3..6  CTA tiles with resident coefficient records (default 3): a CTA owns a tile of markers (state in
+ *   3..6  CTA tiles with resident coefficient records: a CTA owns a tile of markers (state in
  *         shared memory), keeps the coefficient records of the tile's triangles in shared memory between
  *         stages and steps, re-bins the markers by triangle at every stage and evaluates + finishes P
  *         markers of one triangle per thread (3: P = 2, 384 threads; 4: P = 3, 288; 5: P = 4, 256;
  *         6: P = 2, 192 threads, two CTAs per SM).
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
- * INVALID_ARG for a variant outside 0..TRIMEG_PUSH_KERNEL_MAX. */
+ * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX. */
+#define TRIMEG_PUSH_KERNEL_AUTO (-1)
 #define TRIMEG_PUSH_KERNEL_MAX 6
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
-/* The variant trimeg_push will use (the default, the TRIMEG_PUSH_KERNEL environment override at context
- * creation, or the last trimeg_set_push_kernel); -1 for a NULL context. */
+/* The variant trimeg_push will launch (AUTO resolved for the uploaded field; otherwise the TRIMEG_PUSH_KERNEL
+ * environment override at context creation or the last trimeg_set_push_kernel); -2 for a NULL context. */
 int trimeg_get_push_kernel(const trimeg_ctx *ctx);
 
 /* ---- end-to-end push from HOST buffers -------------------------------------------------------
@@ -195,8 +197,8 @@ int trimeg_get_stats(trimeg_ctx *ctx, int64_t *n_lost, int64_t *n_relocated, int
 int trimeg_reset_stats(trimeg_ctx *ctx);
 /* Diagnostics of the shared-memory push kernels since the last reset, out8[0..7] (host).  out8[0..4]: SM
  * cycles of thread 0 of every CTA (lane 0 of every warp for variants 1, 2), summed over CTAs --
- * variants 3..6: [0] evaluation head (geometry, toroidal phases), [1] phase B (record copies, bin scan),
- * [2] phase C (scatter to slots, wait for the copies), [3] the mode loop (batched Horner), [4] finishing
+ * variants 3..6: [0] evaluation head (local coordinates, toroidal phases), [1] phase B (record copies, bin
+ * scan, scatter to slots, barrier), [2] table reset, [3] the mode loop (batched Horner), [4] finishing
  * the markers, binning for the next stage and the wait at the barrier; variants 1, 2: [0] grouping,
  * [3] evaluation + finishing, [4] markers without a slot.  out8[5]: markers evaluated by the one-marker
  * path; out8[6]: coefficient records copied to shared memory (3..6) or bins formed (1, 2); out8[7]: RK4

@@ -7,6 +7,10 @@
 #include "../../include/trimeg.h"
 #include "trimeg_device.cuh"
 
+#ifndef TRIMEG_AUTO_FUSED_MIN_MODES
+#define TRIMEG_AUTO_FUSED_MIN_MODES 12
+#endif
+
 namespace trimeg {
 
 struct Stats {                      // device-resident counters
@@ -45,6 +49,11 @@ struct trimeg_ctx {
 };
 
 namespace trimeg {
+
+// TRIMEG_PUSH_KERNEL_AUTO: with few toroidal modes the per-stage bookkeeping of the CTA-tile kernel (two block
+// barriers, bin scan) outweighs its faster coefficient path and the barrier-free warp kernel wins
+// (cfg2, 3 modes: 4.0e9 vs 3.2e9 marker-steps/s); with many modes it is the other way round (cfg5, 16 modes: 1.43e9 vs 1.52e9).
+inline int auto_push_kernel(int n_modes) { return n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES ? 3 : 1; }
 
 // launch wrappers implemented in trimeg_push.cu; each returns the cudaError of the launch
 cudaError_t launch_locate(trimeg_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell, cudaStream_t s);

@@ -377,8 +377,8 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
         c->field.n_modes = 0; c->field.coef = nullptr; c->field.mode_n = nullptr;
         c->field.n_first = 0; c->field.n_step = 0; c->field.is_ap = 1;
         c->has_field = 0;
-        c->push_kernel = 3;
-        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= 0 && v <= TRIMEG_PUSH_KERNEL_MAX) c->push_kernel = v; }
+        c->push_kernel = TRIMEG_PUSH_KERNEL_AUTO;
+        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= TRIMEG_PUSH_KERNEL_AUTO && v <= TRIMEG_PUSH_KERNEL_MAX) c->push_kernel = v; }
     } while (0);
     if (d_rin2) cudaFree(d_rin2);
     free(hR); free(hZ);
@@ -414,11 +414,16 @@ int trimeg_set_params(trimeg_ctx *c, const trimeg_params *p)
     return TRIMEG_OK;
 }
 
-int trimeg_get_push_kernel(const trimeg_ctx *c) { return c ? c->push_kernel : -1; }
+int trimeg_get_push_kernel(const trimeg_ctx *c)
+{
+    if (!c) return -2;
+    if (c->push_kernel != TRIMEG_PUSH_KERNEL_AUTO) return c->push_kernel;
+    return trimeg::auto_push_kernel(c->field.n_modes);
+}
 
 int trimeg_set_push_kernel(trimeg_ctx *c, int variant)
 {
-    if (!c || variant < 0 || variant > TRIMEG_PUSH_KERNEL_MAX) return TRIMEG_ERR_INVALID_ARG;
+    if (!c || variant < TRIMEG_PUSH_KERNEL_AUTO || variant > TRIMEG_PUSH_KERNEL_MAX) return TRIMEG_ERR_INVALID_ARG;
     c->push_kernel = variant;
     return TRIMEG_OK;
 }

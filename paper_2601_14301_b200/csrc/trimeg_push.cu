@@ -163,8 +163,9 @@ cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double 
 cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
-    if (c->push_kernel >= 3) return launch_push_fused(c, m, n, dt, nsteps, c->push_kernel, s);
-    if (c->push_kernel >= 1) return launch_push_warp(c, m, n, dt, nsteps, c->push_kernel, s);
+    const int variant = (c->push_kernel == TRIMEG_PUSH_KERNEL_AUTO) ? auto_push_kernel(c->field.n_modes) : c->push_kernel;
+    if (variant >= 3) return launch_push_fused(c, m, n, dt, nsteps, variant, s);
+    if (variant >= 1) return launch_push_warp(c, m, n, dt, nsteps, variant, s);
     push_kernel<<<grid_for(n, PUSH_BLOCK), PUSH_BLOCK, 0, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;
     return cudaGetLastError();

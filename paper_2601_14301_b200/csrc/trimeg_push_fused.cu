@@ -9,10 +9,11 @@
 //
 // This kernel: one CTA owns a tile of NT consecutive markers for the whole call (RK4 state in shared
 // memory) and keeps the coefficient records of the tile's triangles in shared memory BETWEEN stages and
-// steps -- only a triangle that no marker of the tile was in before costs a copy.  Per RK4 stage
-//   B  the records of new triangles are copied global -> shared (cp.async, 16 B per lane); one warp scans
-//      the bin sizes, each padded to a multiple of P -> evaluation slots, sorted by triangle;
-//   C  every marker writes its index into its slot;
+// steps -- only a triangle that no marker of the tile was in before costs a copy.  Per RK4 stage (two
+// block barriers)
+//   B  the records of new triangles (coefficients + geometry row) are copied global -> shared (cp.async,
+//      16 B per lane); every warp scans the bin sizes, each padded to a multiple of P, into evaluation
+//      slots sorted by triangle, and every marker writes its index into its slot;
 //   D  one pass, no barrier inside: each thread takes P consecutive slots -- one triangle --, runs the
 //      bivariate Horner scheme for the P markers off ONE shared-memory load of each coefficient, then
 //      finishes the same P markers: chain rule, equilibrium + equations (a4, a5), RK4 bookkeeping (a6),
@@ -34,7 +35,7 @@ constexpr int NPROBE = 8;
 constexpr int BIN_EMPTY = -1;
 
 // misc[] slots
-enum { MI_NEV, MI_NREC, MI_NLOAD, MI_NFB, MI_COUNT = 8 };
+enum { MI_NEV, MI_NREC, MI_NLOAD0, MI_NLOAD1, MI_NFB0, MI_NFB1, MI_COUNT = 8 };   // NLOAD / NFB: one per stage parity
 
 template <int P, int T>
 struct FusedCfg {
@@ -42,7 +43,7 @@ struct FusedCfg {
     static constexpr int NT = NE - 12 * P;                        // markers per tile (slack for bin padding)
     static constexpr size_t BASE_BYTES =
         (sizeof(double) * (size_t)N_STATE * NT +
-         sizeof(int) * (3 * (size_t)NT + (size_t)NE + 5 * NBIN + MI_COUNT) + NT + 15) / 16 * 16;
+         sizeof(int) * (3 * (size_t)NT + (size_t)NE + 6 * NBIN + MI_COUNT) + NT + 15) / 16 * 16;
 };
 
 __device__ __forceinline__ unsigned hash_tri(int t) { return ((unsigned)t * 0x9E3779B1u) >> 26; }   // 6 bits
@@ -61,14 +62,14 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
     int *fb_list = binrank + NT;                          // [NT] markers evaluated one per thread
     int *ev = fb_list + NT;                               // [NE] owner | record slot << 16, -1 = padding
     int *tag = ev + NE;                                   // [NBIN] triangle of a bin (kept between stages)
-    int *cnt = tag + NBIN;                                // [NBIN] markers in the bin this stage
-    int *off = cnt + NBIN;                                // [NBIN] first evaluation slot, -1 = none
-    int *rec_of = off + NBIN;                             // [NBIN] record slot of the bin, -1 = none
-    int *load_list = rec_of + NBIN;                       // [NBIN] bins whose record must be copied this stage
-    int *misc = load_list + NBIN;                         // [MI_COUNT]
+    int *cnt = tag + NBIN;                                // [2][NBIN] markers in the bin, by parity of the stage that evaluates them
+    int *rec_of = cnt + 2 * NBIN;                         // [NBIN] record slot of the bin, -1 = none
+    int *load_list = rec_of + NBIN;                       // [2][NBIN] bins whose record must be copied, same parity rule
+    int *misc = load_list + 2 * NBIN;                     // [MI_COUNT]
     unsigned char *flags = reinterpret_cast<unsigned char *>(misc + MI_COUNT);   // [NT]
     const int rec_len = F.n_modes * NCOEF;                // double2 elements per record
-    const int rec_stride = rec_len + 1;                   // +16 B: records of different triangles in different banks
+    const int rec_copy = rec_len + 3;                     // + the triangle's geometry row (3 double2)
+    const int rec_stride = rec_copy | 1;                  // odd number of 16-byte units: records of different triangles start in different banks
     double2 *REC = reinterpret_cast<double2 *>(reinterpret_cast<unsigned char *>(smem_f) + Cfg::BASE_BYTES);
 
     const int tid = threadIdx.x, lane = tid & 31;
@@ -102,7 +103,7 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
         }
         cell[q] = c; flags[q] = fl;
     }
-    if (tid < NBIN) { tag[tid] = BIN_EMPTY; cnt[tid] = 0; rec_of[tid] = -1; off[tid] = -1; }
+    if (tid < NBIN) { tag[tid] = BIN_EMPTY; cnt[tid] = 0; cnt[NBIN + tid] = 0; rec_of[tid] = -1; }
     if (tid < MI_COUNT) misc[tid] = 0;
     __syncthreads();
 
@@ -112,7 +113,7 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
 
     // Bin marker q (triangle t) for the NEXT evaluation: warp-aggregated -- one probe sequence and one
     // atomicAdd per distinct triangle of the warp.  Must be called by all 32 lanes (act = false: no marker).
-    auto bin_marker = [&](bool act, int q, int t) {
+    auto bin_marker = [&](bool act, int q, int t, int set) {
         const int key = act ? t : -1 - lane;
         const unsigned grp = __match_any_sync(FULL, key);
         const int leader = __ffs(grp) - 1;
@@ -124,13 +125,13 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
                 const int prev = atomicCAS(&tag[h], BIN_EMPTY, t);
                 if (prev == BIN_EMPTY) {                   // first marker of the tile in this triangle: record slot + copy
                     const int r = atomicAdd(&misc[MI_NREC], 1);
-                    if (r < nslot) { rec_of[h] = r; load_list[atomicAdd(&misc[MI_NLOAD], 1)] = (int)h; }
+                    if (r < nslot) { rec_of[h] = r; load_list[set * NBIN + atomicAdd(&misc[MI_NLOAD0 + set], 1)] = (int)h; }
                     else rec_of[h] = -1;
                 }
                 if (prev == BIN_EMPTY || prev == t) { bin = (int)h; break; }
                 h = (h + 1) & (NBIN - 1);
             }
-            if (bin >= 0) rank0 = atomicAdd(&cnt[bin], __popc(grp));
+            if (bin >= 0) rank0 = atomicAdd(&cnt[set * NBIN + bin], __popc(grp));
         }
         bin = __shfl_sync(FULL, bin, leader);
         rank0 = __shfl_sync(FULL, rank0, leader);
@@ -142,7 +143,7 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
         for (int q0 = 0; q0 < NT; q0 += T) {
             const int q = q0 + tid;
             const bool act = (q < NT) && (flags[q] & FL_ACTIVE);
-            bin_marker(act, q, act ? cell[q] : -1);
+            bin_marker(act, q, act ? cell[q] : -1, 0);
         }
         __syncthreads();
     }
@@ -165,68 +166,71 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
                 }
                 continue;                                  // a thread only ever touches its own markers here
             }
-            // ---------------------------------------------------------------- B: copy new records, scan the bins
+            // ------------------------------------------------- B: copy new records; bins -> slots; markers -> slots
+            const int cur = stage & 1, nxt = cur ^ 1;                          // 4 stages per step: parity of the global stage count
             {
-                const int n_load = misc[MI_NLOAD];
-                const int total = n_load * rec_len;
+                const int n_load = misc[MI_NLOAD0 + cur];
+                const int total = n_load * rec_copy;
 #pragma unroll 1
                 for (int idx = tid; idx < total; idx += T) {
-                    const int i = idx / rec_len, k = idx - i * rec_len;
-                    const int b = load_list[i];
-                    const double2 *src = F.coef + (size_t)tag[b] * rec_len + k;
+                    const int i = idx / rec_copy, k = idx - i * rec_copy;
+                    const int b = load_list[cur * NBIN + i];
+                    const double2 *src = (k < rec_len) ? F.coef + (size_t)tag[b] * rec_len + k
+                                                       : reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)tag[b]) + (k - rec_len);
                     const unsigned dst = (unsigned)__cvta_generic_to_shared(REC + (size_t)rec_of[b] * rec_stride + k);
                     asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
                 }
                 asm volatile("cp.async.commit_group;" ::: "memory");
                 if (tid == 0) n_copied += (unsigned)n_load;
             }
-            if (tid < 32) {
-                int run = 0, n_ev = 0;
+            // every warp scans the 64 bin sizes itself (lane l: bins l and l + 32), each padded to a multiple of P
+            int off0, off1;
+            {
+                const int c0 = (rec_of[lane] >= 0) ? cnt[cur * NBIN + lane] : 0;             // no record: one marker per thread
+                const int c1 = (rec_of[32 + lane] >= 0) ? cnt[cur * NBIN + 32 + lane] : 0;
+                const int pad0 = (c0 + P - 1) / P * P, pad1 = (c1 + P - 1) / P * P;
+                int in0 = pad0, in1 = pad1;
 #pragma unroll
-                for (int k = 0; k < NBIN / 32; ++k) {
-                    const int b = k * 32 + lane;
-                    const int c = (rec_of[b] >= 0) ? cnt[b] : 0;             // no record: one marker per thread
-                    const int padded = (c + P - 1) / P * P;
-                    int incl = padded;
-#pragma unroll
-                    for (int o = 1; o < 32; o <<= 1) {
-                        const int v = __shfl_up_sync(FULL, incl, o);
-                        if (lane >= o) incl += v;
-                    }
-                    const int o0 = run + incl - padded;
-                    const bool fits = (c > 0) && (o0 + padded <= NE);        // else: no slot, one marker per thread
-                    off[b] = fits ? o0 : -1;
-                    if (fits) {
-                        for (int e = o0 + c; e < o0 + padded; ++e) ev[e] = -1;   // padding slots
-                        n_ev = max(n_ev, o0 + padded);
-                    }
-                    run += __shfl_sync(FULL, incl, 31);
+                for (int o = 1; o < 32; o <<= 1) {
+                    const int v0 = __shfl_up_sync(FULL, in0, o), v1 = __shfl_up_sync(FULL, in1, o);
+                    if (lane >= o) { in0 += v0; in1 += v1; }
                 }
-                n_ev = __reduce_max_sync(FULL, n_ev);
-                if (lane == 0) { misc[MI_NEV] = n_ev; misc[MI_NFB] = 0; }
+                const int o0 = in0 - pad0, o1 = __shfl_sync(FULL, in0, 31) + in1 - pad1;
+                const bool fit0 = (c0 > 0) && (o0 + pad0 <= NE), fit1 = (c1 > 0) && (o1 + pad1 <= NE);   // else: one marker per thread
+                off0 = fit0 ? o0 : -1; off1 = fit1 ? o1 : -1;
+                if (tid < 32) {
+                    if (fit0) for (int e = o0 + c0; e < o0 + pad0; ++e) ev[e] = -1;            // padding slots
+                    if (fit1) for (int e = o1 + c1; e < o1 + pad1; ++e) ev[e] = -1;
+                    const int n_ev = __reduce_max_sync(FULL, max(fit0 ? o0 + pad0 : 0, fit1 ? o1 + pad1 : 0));
+                    if (lane == 0) { misc[MI_NEV] = n_ev; misc[MI_NFB0 + nxt] = 0; }
+                }
             }
-            __syncthreads();
-            FUSED_TICK(1);
-            // ---------------------------------------------------------------- C: markers -> evaluation slots
 #pragma unroll 1
-            for (int q = tid; q < NT; q += T) {
-                if (!(flags[q] & FL_ACTIVE)) continue;
-                const int br = binrank[q];
-                const int b = br >> 16;
-                if (br >= 0 && off[b] >= 0) ev[off[b] + (br & 0xffff)] = q | (rec_of[b] << 16);
-                else fb_list[atomicAdd(&misc[MI_NFB], 1)] = q;
+            for (int q0 = 0; q0 < NT; q0 += T) {
+                const int q = q0 + tid;
+                const bool act = (q < NT) && (flags[q] & FL_ACTIVE);
+                const int br = act ? binrank[q] : -1;
+                const int b = (br >= 0) ? (br >> 16) : 0;
+                const int oa = __shfl_sync(FULL, off0, b & 31), ob = __shfl_sync(FULL, off1, b & 31);
+                const int o = (b < 32) ? oa : ob;
+                if (act) {
+                    if (br >= 0 && o >= 0) ev[o + (br & 0xffff)] = q | (rec_of[b] << 16);
+                    else fb_list[atomicAdd(&misc[MI_NFB0 + cur], 1)] = q;
+                }
             }
             // the table is nearly full of triangles the markers have left: start it afresh with the bins of the next step
             const bool clear = (stage == 3) && (misc[MI_NREC] > min(nslot, NBIN) - 8);   // MI_NREC only changes in phase D
-            if (tid < NBIN) cnt[tid] = 0;                                     // phase D counts the bins of the next stage
-            if (tid == 0) misc[MI_NLOAD] = 0;
             asm volatile("cp.async.wait_group 0;" ::: "memory");
             __syncthreads();
-            if (clear) {                                                      // uniform; rec_of / tag were read by phase C
+            FUSED_TICK(1);
+            if (clear) {                                                      // uniform; rec_of / tag were read above
                 if (tid < NBIN) { tag[tid] = BIN_EMPTY; rec_of[tid] = -1; }
                 if (tid == 0) misc[MI_NREC] = 0;
                 __syncthreads();
             }
+            // counters of this parity were read above; phase D of the NEXT stage is the first to add to them again
+            if (tid < NBIN) cnt[cur * NBIN + tid] = 0;
+            if (tid == 0) misc[MI_NLOAD0 + cur] = 0;
             FUSED_TICK(2);
             // ---------------------------------------------------------------- D: evaluate + finish, P slots per thread
             const int n_ev = misc[MI_NEV];
@@ -238,9 +242,11 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
 #pragma unroll
                 for (int p = 0; p < P; ++p) { const int v = ev[e0 + p]; own[p] = (v >= 0) ? (v & 0xffff) : -1; }
                 const int rec = ev[e0] >> 16;                                // first slot of a group is real
-                const int tri = cell[own[0]];
-                const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)tri);
-                const double2 v0 = __ldg(g), gx = __ldg(g + 1), ge = __ldg(g + 2);
+                const double2 *recp = REC + (size_t)rec * rec_stride;          // coefficients, then the geometry row
+                TriGeom tg;
+                tg.t = cell[own[0]];
+                tg.v0 = recp[rec_len]; tg.gx = recp[rec_len + 1]; tg.ge = recp[rec_len + 2];
+                const double2 v0 = tg.v0, gx = tg.gx, ge = tg.ge;
                 double xi[P], eta[P], phi[P], f[P], fx[P], fe[P], fp[P];
 #pragma unroll
                 for (int p = 0; p < P; ++p) {
@@ -255,7 +261,7 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
                 double Er[P], Ei[P], Dr[P], Di[P];
                 gather_phases<P>(F, phi, Er, Ei, Dr, Di);
                 FUSED_TICK(0);
-                gather_modes<P, false>(F, REC + (size_t)rec * rec_stride, xi, eta, phi, Er, Ei, Dr, Di, f, fx, fe, fp);
+                gather_modes<P, false>(F, recp, xi, eta, phi, Er, Ei, Dr, Di, f, fx, fe, fp);
                 FUSED_TICK(3);
 #pragma unroll 1
                 for (int p = 0; p < P; ++p) {
@@ -269,7 +275,7 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
                             fv.fR = fma(gx.x, fx[pp], ge.x * fe[pp]);            // d/dR
                             fv.fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);            // d/dZ
                         }
-                    if (q >= 0) advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6);
+                    if (q >= 0) advance(M, Ph, S, NT, cell, flags, q, stage, fv, dt, hdt, dt6, &tg);
                 }
             }
             // the markers this thread finished: start-of-step copy, bin for the next stage (all lanes take part)
@@ -281,11 +287,11 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
 #pragma unroll
                     for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
                 }
-                bin_marker(act, q, act ? cell[q] : -1);
+                bin_marker(act, q, act ? cell[q] : -1, nxt);
             }
             // markers without a slot: one per thread, coefficients from global memory
             {
-                const int n_fb = misc[MI_NFB];
+                const int n_fb = misc[MI_NFB0 + cur];
 #pragma unroll 1
                 for (int i0 = 0; i0 < n_fb; i0 += T) {
                     const int i = i0 + tid;
@@ -303,7 +309,7 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
 #pragma unroll
                         for (int k = 0; k < 5; ++k) S[(S_R + k) * NT + q] = S[(Y_R + k) * NT + q];
                     }
-                    bin_marker(act, q, act ? cell[q] : -1);
+                    bin_marker(act, q, act ? cell[q] : -1, nxt);
                 }
             }
             FUSED_TICK(4);
@@ -334,9 +340,9 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
         if (n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);
     }
     if (tid == 0) {
+        atomicAdd(&st->tile[6], (unsigned long long)n_copied);
 #pragma unroll
         for (int k = 0; k < 5; ++k) atomicAdd(&st->tile[k], (unsigned long long)(k == 4 ? tph[4] + tph[5] : tph[k]));
-        atomicAdd(&st->tile[6], (unsigned long long)n_copied);
         atomicAdd(&st->tile[7], (unsigned long long)n_stages);
     }
 }
@@ -353,7 +359,7 @@ cudaError_t launch_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, doubl
         configured = true;
     }
     // record slots: what is left of the CTA's shared memory
-    const size_t rec_bytes = sizeof(double2) * (NCOEF * (size_t)c->field.n_modes + 1);
+    const size_t rec_bytes = sizeof(double2) * ((NCOEF * (size_t)c->field.n_modes + 3) | 1);   // as rec_stride in the kernel
     int nslot = c->field.n_modes ? (int)((SMEM_MAX - Cfg::BASE_BYTES) / rec_bytes) : 0;
     if (nslot > NBIN) nslot = NBIN;
     const size_t shm = Cfg::BASE_BYTES + (size_t)nslot * rec_bytes;

@@ -154,6 +154,8 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
                 const int tri = ev_tri[e0];                                          // first slot of a group is real
                 const double2 *g = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)tri);
                 const double2 v0 = __ldg(g), gx = __ldg(g + 1), ge = __ldg(g + 2);
+                TriGeom tg;
+                tg.t = tri; tg.v0 = v0; tg.gx = gx; tg.ge = ge;
                 int own[P];
                 double xi[P], eta[P], phi[P], f[P], fx[P], fe[P], fp[P];
 #pragma unroll
@@ -181,7 +183,7 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
                             fv.fR = fma(gx.x, fx[pp], ge.x * fe[pp]);                // d/dR
                             fv.fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);                // d/dZ
                         }
-                    if (q >= 0) advance(M, Ph, S, NW, cell, flags, q, stage, fv, dt, hdt, dt6);
+                    if (q >= 0) advance(M, Ph, S, NW, cell, flags, q, stage, fv, dt, hdt, dt6, &tg);
                 }
             }
             __syncwarp();

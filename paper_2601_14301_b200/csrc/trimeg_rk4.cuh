@@ -12,11 +12,15 @@ enum : unsigned char { FL_ACTIVE = 1, FL_LOST = 2, FL_MOVED = 4, FL_WASACTIVE = 
 // per-marker fp64 state: Y = start-of-step state, A = k1 + 2 k2 + 2 k3, S = stage position
 enum { Y_R, Y_Z, Y_P, Y_V, Y_W, S_MU, A_R, A_Z, A_P, A_V, A_W, S_R, S_Z, S_P, S_V, S_W, N_STATE };
 
+// Geometry row of a triangle held in registers by the caller (R_v0, Z_v0 | xi_R, xi_Z | eta_R, eta_Z).
+struct TriGeom { int t; double2 v0, gx, ge; };
+
 // Finish one marker at one stage (slot or home role): equations, RK4 bookkeeping, next position,
-// locate of the next position.  q = index of the marker in the warp's slice.
+// locate of the next position.  q = index of the marker in the warp's slice.  tg: geometry of the
+// triangle the marker is in, if the caller holds it (saves the locator's loads when the marker stays).
 __device__ __forceinline__ void advance(const MeshDev &M, const PhysDev &Ph, double *S, int NW, int *cell,
                                         unsigned char *flags, int q, int stage, const FieldVal &fv, double dt,
-                                        double hdt, double dt6)
+                                        double hdt, double dt6, const TriGeom *tg = nullptr)
 {
     const double R = S[S_R * NW + q], Z = S[S_Z * NW + q];
     const double v = S[S_V * NW + q], w = S[S_W * NW + q], mu = S[S_MU * NW + q];
@@ -43,8 +47,15 @@ __device__ __forceinline__ void advance(const MeshDev &M, const PhysDev &Ph, dou
         nP = fma(-TWO_PI, floor(nP * (1.0 / TWO_PI)), nP);
     }
     Bary b;
-    int moved = 0;
-    const int tn = locate(M, nR, nZ, cell[q], b, moved);
+    int moved = 0, tn = -2;
+    if (tg != nullptr) {                                   // rule L3 on the current triangle, arithmetic of bary_rn() (rule L2)
+        const double dx = __dsub_rn(nR, tg->v0.x), dz = __dsub_rn(nZ, tg->v0.y);
+        const double xi = __dadd_rn(__dmul_rn(tg->gx.x, dx), __dmul_rn(tg->gx.y, dz));
+        const double eta = __dadd_rn(__dmul_rn(tg->ge.x, dx), __dmul_rn(tg->ge.y, dz));
+        const double l0 = __dsub_rn(__dsub_rn(1.0, xi), eta);
+        if (fmin(fmin(xi, eta), l0) > LOC_TAU) tn = tg->t;
+    }
+    if (tn == -2) tn = locate(M, nR, nZ, cell[q], b, moved);
     unsigned char fl = flags[q];
     if (moved) fl |= FL_MOVED;
     if (tn < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;        // start-of-step state Y is kept; dropped for the rest of the call
