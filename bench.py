@@ -321,16 +321,62 @@ def run_gpu(args, wl):
     return 0
 
 
+def run_gather_sweep(args, wl):
+    """BASELINE.json configs[3]: gather-only sweep (dphi, d/dR, d/dZ at the markers, no push) on the 64 x 256 mesh with
+    modes {0, 5, 10}, marker counts 2^16 .. 2^max in powers of 4, markers as drawn and sorted by triangle.  One JSON line."""
+    import torch
+    from paper_2601_14301_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(0)
+    binding.load()
+    ctx = binding.context_for(wl, inputs)
+    ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
+    hbm_peak, _ = load_peaks()
+    fp64_peak = ctx.measure_fp64_peak()
+    flops = 25 + 170 * len(wl.modes) + 6                       # SURVEY.md 8(d): gather-only work per marker
+    rows = []
+    for lg in range(16, args.max_log2 + 1, 2):
+        n = 1 << lg
+        m = inputs.markers(wl, n=n)
+        R, Z, phi = (torch.from_numpy(m[k]).cuda() for k in ("R", "Z", "phi"))
+        cell = torch.empty(n, dtype=torch.int32, device="cuda")
+        ctx.locate(R, Z, cell=cell)
+        order = torch.argsort(cell, stable=True)
+        out = {k: torch.empty(n, dtype=torch.float64, device="cuda") for k in ("dphi", "dphi_dR", "dphi_dZ")}
+        for name, idx in (("as drawn", None), ("sorted by triangle", order)):
+            r, z, p = (R, Z, phi) if idx is None else (R[idx].contiguous(), Z[idx].contiguous(), phi[idx].contiguous())
+            ts = []
+            for rep in range(3 + max(1, args.steps)):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                ctx.gather(r, z, p, want_dphi=False, out=out)
+                e1.record()
+                torch.cuda.synchronize()
+                if rep >= 3:
+                    ts.append(e0.elapsed_time(e1) * 1e-3)
+            t = sorted(ts)[len(ts) // 2]
+            rows.append({"markers": n, "order": name, "gathers_per_s": n / t, "ms": t * 1e3,
+                         "algorithmic_GBps": 48.0 * n / t * 1e-9, "algorithmic_TFLOPs": flops * n / t * 1e-12})
+        del R, Z, phi, cell, order, out
+    line = {"metric": "field gathers/sec (dphi, d/dR, d/dZ; 3 toroidal modes)", "unit": "gathers/s", "n_gpus": 1,
+            "config": workload_config(wl), "dtype": "f64", "data": "synthetic", "hbm_peak_gbs": hbm_peak, "fp64_peak_tflops": fp64_peak,
+            "algorithmic_bytes_per_gather": 48, "algorithmic_flops_per_gather": flops, "rows": rows}
+    print(json.dumps(line), flush=True)
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg5"])
+    ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
+    ap.add_argument("--max-log2", type=int, default=26, help="cfg4 gather sweep: largest marker count 2^k")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
@@ -340,6 +386,8 @@ def main():
     wl = inputs.WORKLOADS[args.workload]
     if args.markers:
         wl = dataclasses.replace(wl, n_markers=args.markers)
+    if args.workload == "cfg4":
+        return run_gather_sweep(args, wl)
     if args.impl == "reference":
         return run_reference(args, wl)
     return run_gpu(args, wl)

@@ -197,10 +197,14 @@ class Context:
                                     _ptr(cell, torch.int32, n), _stream(stream)), "trimeg_locate")
         return cell
 
-    def gather(self, R, Z, phi, cell_hint=None, want_dphi=True, stream=None) -> Dict[str, torch.Tensor]:
+    def gather(self, R, Z, phi, cell_hint=None, want_dphi=True, stream=None, out=None) -> Dict[str, torch.Tensor]:
+        """out: optional dict of preallocated outputs (dphi, dphi_dR, dphi_dZ[, dphi_dphi]) to write into."""
         n = R.numel()
-        out = {k: torch.empty(n, dtype=torch.float64, device=R.device) for k in ("dphi", "dphi_dR", "dphi_dZ")}
-        fp = torch.empty(n, dtype=torch.float64, device=R.device) if want_dphi else None
+        if out is None:
+            out = {k: torch.empty(n, dtype=torch.float64, device=R.device) for k in ("dphi", "dphi_dR", "dphi_dZ")}
+            fp = torch.empty(n, dtype=torch.float64, device=R.device) if want_dphi else None
+        else:
+            fp = out.get("dphi_dphi") if want_dphi else None
         _check(self.L.trimeg_gather(self.h, n, _ptr(R, torch.float64, n), _ptr(Z, torch.float64, n),
                                     _ptr(phi, torch.float64, n), _ptr(cell_hint, torch.int32, n),
                                     _ptr(out["dphi"], torch.float64), _ptr(out["dphi_dR"], torch.float64),
