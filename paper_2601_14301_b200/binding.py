@@ -24,6 +24,7 @@ EXPORTS = (
 )
 
 OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC = 0, -1, -2, -3, -4, -5
+PUSH_KERNEL_AUTO = -1          # TRIMEG_PUSH_KERNEL_AUTO of include/trimeg.h
 
 
 class TrimegError(RuntimeError):
