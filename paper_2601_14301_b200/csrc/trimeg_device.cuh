@@ -204,6 +204,32 @@ __device__ __forceinline__ void eval_quintic(const double2 *__restrict__ c, doub
     P.re = pr; P.im = pi; Px.re = pxr; Px.im = pxi; Pe.re = per; Pe.im = pei;
 }
 
+// A mode with n = 0: only Re(P) reaches the result (reading G15) -- the real chains of eval_quintic alone.
+__device__ __forceinline__ void eval_quintic_real(const double2 *__restrict__ c, double xi, double eta,
+                                                  double &P, double &Px, double &Pe)
+{
+    double pr = 0.0, pxr = 0.0, per = 0.0;
+#pragma unroll
+    for (int j = 5; j >= 0; --j) {
+        const int n = 5 - j;
+        double ar = __ldg(&c[kidx(n, j)].x), dr = 0.0;
+#pragma unroll
+        for (int i = n - 1; i >= 0; --i) {
+            const double cx = __ldg(&c[kidx(i, j)].x);
+            if (i == n - 1) dr = ar;
+            else dr = fma(dr, xi, ar);
+            ar = fma(ar, xi, cx);
+        }
+        if (j == 5) pr = ar;
+        else {
+            if (j == 4) { per = pr; pxr = dr; }
+            else { per = fma(per, eta, pr); pxr = fma(pxr, eta, dr); }
+            pr = fma(pr, eta, ar);
+        }
+    }
+    P = pr; Px = pxr; Pe = per;
+}
+
 struct FieldVal { double f, fR, fZ, fphi; };   // dphi, d/dR, d/dZ, d/dphi
 
 // dphi = sum_n Re(P_n E_n), E_n = e^{i n phi}; no factor 2, Im of n = 0 ignored (G15).
@@ -219,8 +245,14 @@ __device__ __forceinline__ FieldVal gather(const FieldDev &F, int t, const Bary 
             if (F.n_modes > 1) sincos((double)F.n_step * phi, &Di, &Dr);
         } else { Er = 1.0; Ei = 0.0; }
         double nn = (double)F.n_first;
+        int m = 0;
+        if ((F.is_ap ? F.n_first : __ldg(F.mode_n)) == 0) {      // leading n = 0 mode: E = 1, real part only
+            eval_quintic_real(c, b.xi, b.eta, f, fx, fe);
+            if (F.is_ap) { Er = Dr; Ei = Di; nn += (double)F.n_step; }
+            m = 1; c += NCOEF;
+        }
 #pragma unroll 1
-        for (int m = 0; m < F.n_modes; ++m, c += NCOEF) {
+        for (; m < F.n_modes; ++m, c += NCOEF) {
             if (!F.is_ap) { nn = (double)__ldg(F.mode_n + m); sincos(nn * phi, &Ei, &Er); }
             Cplx P, Px, Pe;
             eval_quintic(c, b.xi, b.eta, P, Px, Pe);

@@ -48,6 +48,42 @@ __device__ __forceinline__ void eval_quintic_multi(const double2 *__restrict__ c
     }
 }
 
+// The same for a mode with n = 0, whose imaginary part never reaches the result (reading G15): real parts only,
+// half the arithmetic.  The real chains are those of eval_quintic_multi, operation for operation.
+template <int P, bool GLOBAL>
+__device__ __forceinline__ void eval_quintic_multi_real(const double2 *__restrict__ c, const double (&xi)[P],
+                                                        const double (&eta)[P], double (&pr)[P], double (&pxr)[P],
+                                                        double (&per)[P])
+{
+    double ar[P], dr[P];
+#pragma unroll
+    for (int j = 5; j >= 0; --j) {
+        const int n = 5 - j;
+#pragma unroll
+        for (int i = n; i >= 0; --i) {
+            const double cx = GLOBAL ? __ldg(&c[kidx(i, j)].x) : c[kidx(i, j)].x;
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                if (i == n) { ar[p] = cx; dr[p] = 0.0; }
+                else {
+                    if (i == n - 1) dr[p] = ar[p];
+                    else dr[p] = fma(dr[p], xi[p], ar[p]);
+                    ar[p] = fma(ar[p], xi[p], cx);
+                }
+            }
+        }
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            if (j == 5) pr[p] = ar[p];
+            else {
+                if (j == 4) { per[p] = pr[p]; pxr[p] = dr[p]; }
+                else { per[p] = fma(per[p], eta[p], pr[p]); pxr[p] = fma(pxr[p], eta[p], dr[p]); }
+                pr[p] = fma(pr[p], eta[p], ar[p]);
+            }
+        }
+    }
+}
+
 // Toroidal factors of P markers: E = e^{i n_first phi}, D = e^{i n_step phi} (arithmetic progression of
 // mode numbers; else E is recomputed per mode inside gather_modes).
 template <int P>
@@ -77,8 +113,20 @@ __device__ __forceinline__ void gather_modes_impl(const FieldDev &F, const doubl
     double nn = (double)F.n_first;
     const double dn = (double)F.n_step;
     const int n_modes = F.n_modes;
+    int m = 0;
+    if (n_modes > 0 && (AP ? F.n_first : __ldg(F.mode_n)) == 0) {      // leading n = 0 mode: E = 1, Re(P) is all that counts
+        double pr[P], pxr[P], per[P];
+        eval_quintic_multi_real<P, GLOBAL>(c, xi, eta, pr, pxr, per);
+#pragma unroll
+        for (int p = 0; p < P; ++p) {
+            f[p] = pr[p]; fx[p] = pxr[p]; fe[p] = per[p];
+            if (AP) { Er[p] = Dr[p]; Ei[p] = Di[p]; }                   // E_{dn} = 1 * D, exactly
+        }
+        if (AP) nn += dn;
+        m = 1; c += NCOEF;
+    }
 #pragma unroll 1
-    for (int m = 0; m < n_modes; ++m, c += NCOEF) {
+    for (; m < n_modes; ++m, c += NCOEF) {
         if (!AP) {
             nn = (double)__ldg(F.mode_n + m);
 #pragma unroll
