@@ -170,7 +170,7 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *   3..6  CTA tiles with resident coefficient records: a CTA owns a tile of markers (state in
  *         shared memory), keeps the coefficient records of the tile's triangles in shared memory between
  *         stages and steps, re-bins the markers by triangle at every stage and evaluates + finishes P
- *         markers of one triangle per thread (3: P = 2, 384 threads; 4: P = 3, 288; 5: P = 4, 256;
+ *         markers of one triangle per thread (3: P = 2, 384 threads; 4: P = 3, 256; 5: P = 4, 256;
  *         6: P = 2, 192 threads, two CTAs per SM).
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX. */

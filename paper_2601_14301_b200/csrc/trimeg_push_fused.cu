@@ -377,7 +377,7 @@ cudaError_t launch_push_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, 
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
     case 3: return launch_fused<2, 384>(c, m, n, dt, nsteps, s);
-    case 4: return launch_fused<3, 288>(c, m, n, dt, nsteps, s);
+    case 4: return launch_fused<3, 256>(c, m, n, dt, nsteps, s);
     case 5: return launch_fused<4, 256>(c, m, n, dt, nsteps, s);
     case 6: return launch_fused<2, 192, 2>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;

@@ -510,3 +510,41 @@ def test_full_size_sampled_parity_in_bench_configuration(B, inputs, name, nsteps
     assert np.array_equal(got["cell"], want["cell"])
     _assert_state_close(got, want, 1e-10, 1e-4)
     assert (want["cell"] < 0).sum() > 0
+
+
+# ----------------------------------------------------------------------------- schedule selection, diagnostics
+def test_automatic_schedule_selection_and_variant_range(B, inputs):
+    """TRIMEG_PUSH_KERNEL_AUTO resolves by the number of uploaded modes (warp kernel below 12, CTA tiles from 12 on);
+    variants outside -1..TRIMEG_PUSH_KERNEL_MAX are rejected; AUTO gives the oracle's result like any fixed variant."""
+    wl, o, ctx, _, _ = _setup(B, inputs, "cfg1")
+    assert ctx.get_push_kernel() == 1
+    for bad in (-2, 7, 100):
+        with pytest.raises(B.TrimegError):
+            ctx.set_push_kernel(bad)
+    ctx.set_push_kernel(3)
+    assert ctx.get_push_kernel() == 3
+    ctx.set_push_kernel(B.PUSH_KERNEL_AUTO)
+    assert ctx.get_push_kernel() == 1
+    wl5, o5, ctx5, _, _ = _setup(B, inputs, "cfg5")
+    assert ctx5.get_push_kernel() == 3
+    m = inputs.markers(wl5, n=30011)
+    want = o5.push(m, wl5.dt, 3)
+    d = _dev(B, m)
+    ctx5.locate(d["R"], d["Z"], cell=d["cell"])
+    ctx5.push(d, wl5.dt, 3)
+    got = _host(d)
+    assert np.array_equal(got["cell"], want["cell"])
+    _assert_state_close(got, want, 1e-10, 1e-4)
+
+
+def test_fp64_peak_depends_on_register_operands(B, inputs):
+    """The roofline denominators of bench.py: a DFMA stream with three fresh register operands per instruction runs at
+    2/3 of the rate of one with a single fresh operand; two fresh operands cost (almost) nothing."""
+    wl, o, ctx, _, _ = _setup(B, inputs, "cfg1")
+    p1, p2, p3 = (ctx.measure_fp64_peak_operands(k) for k in (1, 2, 3))
+    p0 = ctx.measure_fp64_peak()
+    assert 25.0 < p0 < 45.0
+    assert 0.85 < p1 / p0 < 1.05 and 0.80 < p2 / p0 < 1.05
+    assert 0.60 < p3 / p0 < 0.72
+    with pytest.raises(B.TrimegError):
+        ctx.measure_fp64_peak_operands(4)
