@@ -184,8 +184,10 @@ int trimeg_get_push_kernel(const trimeg_ctx *ctx);
 /* ---- end-to-end push from HOST buffers -------------------------------------------------------
  * Same result as: copy the seven arrays to the device, trimeg_locate if locate_first != 0,
  * trimeg_sort, trimeg_push, undo the sort, copy R, Z, phi, vpar, w, cell back.  `m` holds
- * HOST pointers (pinned memory makes the copies asynchronous).  Markers are processed in
- * chunks on several streams so that copies overlap the push.  Synchronises before returning. */
+ * HOST pointers (pinned memory makes the copies asynchronous).  The whole batch is made resident and
+ * cell-sorted as one set (the push kernels live on markers per triangle), re-sorted every 10 steps, and
+ * returned in the caller's order; the device buffers (2 marker sets + 3 permutations, 128 B per marker)
+ * stay allocated in the context.  Synchronises before returning. */
 int trimeg_push_host(trimeg_ctx *ctx, trimeg_markers *m_host, size_t n, double dt, int nsteps,
                      int locate_first);
 

@@ -43,7 +43,9 @@ struct trimeg_ctx {
     void *d_scratch;
     size_t scratch_bytes;
     int *d_bins;                    // n_tri + 2 counters
-    // host path
+    // host path: two marker sets + permutation of the last trimeg_push_host batch (grown on demand)
+    void *d_hbuf;
+    size_t hbuf_bytes;
     cudaStream_t hstream[3];
     int hstreams_ready;
 };

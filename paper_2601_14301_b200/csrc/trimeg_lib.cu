@@ -229,6 +229,14 @@ __global__ void unpermute_kernel(size_t n, MarkerScratch src, trimeg_markers dst
     dst.w[p] = src.w[d]; dst.cell[p] = src.cell[d];
 }
 
+// permutation of a permutation: out[d] = outer[inner[d]]
+__global__ void compose_perm_kernel(size_t n, const int64_t *__restrict__ outer, const int64_t *__restrict__ inner,
+                                    int64_t *__restrict__ out)
+{
+    const size_t d = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (d < n) out[d] = outer[(size_t)inner[d]];
+}
+
 // ================================================================== diagnostics: FP64 roofline
 // Dependent-chain-free DFMA loop: 8 independent accumulators per thread, enough warps to
 // saturate the FP64 pipe.  2 flops per DFMA.
@@ -391,7 +399,7 @@ int trimeg_mesh_destroy(trimeg_ctx *c)
 {
     if (!c) return TRIMEG_ERR_INVALID_ARG;
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
-    cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch);
+    cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
     if (c->hstreams_ready) for (int k = 0; k < 3; ++k) cudaStreamDestroy(c->hstream[k]);
     cudaGetLastError();
     delete c;
@@ -606,54 +614,66 @@ int trimeg_push_host(trimeg_ctx *c, trimeg_markers *mh, size_t n, double dt, int
         for (int k = 0; k < 3; ++k) CU_TRY(cudaStreamCreateWithFlags(&c->hstream[k], cudaStreamNonBlocking));
         c->hstreams_ready = 1;
     }
-    const size_t chunk = (n < ((size_t)1 << 21)) ? n : ((size_t)1 << 21);
-    const size_t n_chunks = (n + chunk - 1) / chunk;
-    const int n_slots = (n_chunks < 3) ? (int)n_chunks : 3;
+    // The whole batch is made resident and sorted as ONE set: the push kernels live on markers per triangle, and
+    // sorting chunks of the batch separately would divide that density by the number of chunks.  Device buffers
+    // (two marker sets + the permutation) are kept in the context between calls.
     MarkerScratch a, b;
-    const size_t rec = carve(nullptr, chunk, a);
-    const size_t permb = align_up(chunk * sizeof(int64_t), 256);
-    const size_t slot = 2 * rec + permb;
-    // sort scratch is the context scratch; slots live in a separate allocation for this call
-    char *buf = nullptr;
-    if (cudaMalloc(&buf, slot * n_slots) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_ALLOC; }
+    const size_t rec = carve(nullptr, n, a);
+    const size_t permb = align_up(n * sizeof(int64_t), 256);
+    const size_t need = 2 * rec + 3 * permb;
+    if (c->hbuf_bytes < need) {
+        if (c->d_hbuf) { cudaFree(c->d_hbuf); c->d_hbuf = nullptr; c->hbuf_bytes = 0; }
+        if (cudaMalloc(&c->d_hbuf, need) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_ALLOC; }
+        c->hbuf_bytes = need;
+    }
+    char *base = (char *)c->d_hbuf;
+    carve(base, n, a);
+    carve(base + rec, n, b);
+    int64_t *perm = (int64_t *)(base + 2 * rec), *perm2 = (int64_t *)(base + 2 * rec + permb),
+            *perm3 = (int64_t *)(base + 2 * rec + 2 * permb);
+    cudaStream_t s = c->hstream[0];
+    const size_t db = n * sizeof(double);
+    const unsigned grid = (unsigned)((n + 255) / 256);
     int rc = TRIMEG_OK;
-    int *bins_slot[3] = {nullptr, nullptr, nullptr};
-    for (int k = 0; k < n_slots && rc == TRIMEG_OK; ++k)
-        if (cudaMalloc(&bins_slot[k], sizeof(int) * ((size_t)c->n_tri + 2)) != cudaSuccess) { cudaGetLastError(); rc = TRIMEG_ERR_ALLOC; }
-    for (size_t k = 0; k < n_chunks && rc == TRIMEG_OK; ++k) {
-        const int sl = (int)(k % n_slots);
-        cudaStream_t s = c->hstream[sl];
-        const size_t lo = k * chunk, cnt = (lo + chunk <= n) ? chunk : n - lo;
-        char *base = buf + slot * sl;
-        carve(base, chunk, a);
-        carve(base + rec, chunk, b);
-        int64_t *perm = (int64_t *)(base + 2 * rec);
-        const size_t db = cnt * sizeof(double);
 #define H2D(dst, src, bytes) if (rc == TRIMEG_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA
 #define D2H(dst, src, bytes) if (rc == TRIMEG_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA
-        H2D(a.R, mh->R + lo, db); H2D(a.Z, mh->Z + lo, db); H2D(a.phi, mh->phi + lo, db);
-        H2D(a.vpar, mh->vpar + lo, db); H2D(a.mu, mh->mu + lo, db); H2D(a.w, mh->w + lo, db);
-        if (!locate_first) H2D(a.cell, mh->cell + lo, cnt * sizeof(int32_t));
+    do {
+        H2D(a.R, mh->R, db); H2D(a.Z, mh->Z, db);
+        if (locate_first) { if (rc == TRIMEG_OK && launch_locate(c, n, a.R, a.Z, a.cell, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA; }
+        else H2D(a.cell, mh->cell, n * sizeof(int32_t));
+        H2D(a.phi, mh->phi, db); H2D(a.vpar, mh->vpar, db); H2D(a.mu, mh->mu, db); H2D(a.w, mh->w, db);
         if (rc != TRIMEG_OK) break;
-        trimeg_markers ma = {a.R, a.Z, a.phi, a.vpar, a.mu, a.w, a.cell};
-        trimeg_markers mb = {b.R, b.Z, b.phi, b.vpar, b.mu, b.w, b.cell};
-        if (locate_first && launch_locate(c, cnt, a.R, a.Z, a.cell, s) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
-        rc = sort_into(c, ma, cnt, b, perm, bins_slot[sl], s);        // a -> b (sorted)
+        // markers drift out of their triangles: sort again every HOST_SORT_EVERY steps (set `cur` <-> set `oth`),
+        // `perm` always maps a position in `cur` to the caller's index
+        constexpr int HOST_SORT_EVERY = 10;
+        MarkerScratch cur = a, oth = b;
+        for (int done = 0; done < nsteps || done == 0; done += HOST_SORT_EVERY) {
+            trimeg_markers mc = {cur.R, cur.Z, cur.phi, cur.vpar, cur.mu, cur.w, cur.cell};
+            rc = sort_into(c, mc, n, oth, (done == 0) ? perm : perm2, c->d_bins, s);     // cur -> oth (sorted by triangle)
+            if (rc != TRIMEG_OK) break;
+            if (done > 0) {
+                compose_perm_kernel<<<grid, 256, 0, s>>>(n, perm, perm2, perm3);
+                c->n_launches++;
+                int64_t *t = perm; perm = perm3; perm3 = t;
+            }
+            const MarkerScratch t = cur; cur = oth; oth = t;
+            const int k = (nsteps - done < HOST_SORT_EVERY) ? nsteps - done : HOST_SORT_EVERY;
+            trimeg_markers mp = {cur.R, cur.Z, cur.phi, cur.vpar, cur.mu, cur.w, cur.cell};
+            if (k > 0 && launch_push(c, mp, n, dt, k, s) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+            if (nsteps == 0) break;
+        }
         if (rc != TRIMEG_OK) break;
-        if (launch_push(c, mb, cnt, dt, nsteps, s) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
-        unpermute_kernel<<<(unsigned)((cnt + 255) / 256), 256, 0, s>>>(cnt, b, ma, perm);   // b -> a (caller order)
+        trimeg_markers mo = {oth.R, oth.Z, oth.phi, oth.vpar, oth.mu, oth.w, oth.cell};
+        unpermute_kernel<<<grid, 256, 0, s>>>(n, cur, mo, perm);       // cur -> oth (caller order)
         c->n_launches++;
         if (cudaGetLastError() != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
-        D2H(mh->R + lo, a.R, db); D2H(mh->Z + lo, a.Z, db); D2H(mh->phi + lo, a.phi, db);
-        D2H(mh->vpar + lo, a.vpar, db); D2H(mh->w + lo, a.w, db);
-        D2H(mh->cell + lo, a.cell, cnt * sizeof(int32_t));
+        D2H(mh->R, oth.R, db); D2H(mh->Z, oth.Z, db); D2H(mh->phi, oth.phi, db);
+        D2H(mh->vpar, oth.vpar, db); D2H(mh->w, oth.w, db);
+        D2H(mh->cell, oth.cell, n * sizeof(int32_t));
+    } while (0);
 #undef H2D
 #undef D2H
-    }
-    for (int k = 0; k < 3; ++k)
-        if (c->hstreams_ready && cudaStreamSynchronize(c->hstream[k]) != cudaSuccess && rc == TRIMEG_OK) rc = TRIMEG_ERR_CUDA;
-    for (int k = 0; k < 3; ++k) cudaFree(bins_slot[k]);
-    cudaFree(buf);
+    if (cudaStreamSynchronize(s) != cudaSuccess && rc == TRIMEG_OK) rc = TRIMEG_ERR_CUDA;
     if (rc != TRIMEG_OK) cudaGetLastError();
     return rc;
 }
