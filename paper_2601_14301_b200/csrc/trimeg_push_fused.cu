@@ -205,7 +205,7 @@ __global__ void __launch_bounds__(T, CTAS) push_fused_kernel(MeshDev M, FieldDev
                     if (lane == 0) { misc[MI_NEV] = n_ev; misc[MI_NFB0 + nxt] = 0; }
                 }
             }
-#pragma unroll 1
+#pragma unroll
             for (int q0 = 0; q0 < NT; q0 += T) {
                 const int q = q0 + tid;
                 const bool act = (q < NT) && (flags[q] & FL_ACTIVE);
