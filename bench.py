@@ -255,7 +255,7 @@ def run_gpu(args, wl):
     push_units = sum(u for _, _, u in push_events)
     n_push = len(push_events)
     flops = flops_per_marker_step(len(wl.modes)) * push_units
-    byts = 96.0 * sum(u / max(1, min(sort_every, wl.nsteps)) for _, _, u in push_events)
+    byts = bytes_per_marker_call(sort_every) * sum(u / max(1, min(sort_every, wl.nsteps)) for _, _, u in push_events)
     t_fp64 = flops / (fp64_peak * 1e12)
     t_hbm = byts / (hbm_peak * 1e9)
     roof = {
@@ -269,7 +269,7 @@ def run_gpu(args, wl):
                                              "next (a Horner step over several markers): the FP64 pipe reads one 64-bit register "
                                              "operand per cycle, so such a stream issues every 3 cycles instead of 2",
         "algorithmic_flops_per_marker_step": flops_per_marker_step(len(wl.modes)),
-        "algorithmic_bytes_per_marker_call": 96.0,
+        "algorithmic_bytes_per_marker_call": bytes_per_marker_call(sort_every),
         "hbm_time_frac_of_fp64_time": t_hbm / t_fp64, "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
         "launches": n_push, "avg_launch_ms": push_s / max(1, n_push) * 1e3,
         "push_share_of_step": push_s / seconds,

@@ -148,7 +148,6 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
             if (lane == 0) { const long long now = clock64(); tph[0] += now - tlast; tlast = now; n_bins += nb; ++n_stages; }
 
             // ------------------------------------------------------------ 2 + 3: batched evaluation, equations (slot role)
-#pragma unroll 1
             if (lane * P < n_ev) {
                 const int e0 = lane * P;
                 const int tri = ev_tri[e0];                                          // first slot of a group is real
