@@ -161,7 +161,7 @@ int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_d
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
 /* Kernel used by trimeg_push / trimeg_push_host (same results, different schedules):
- *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 3 for a field of 12 or more toroidal modes, else variant 1;
+ *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 3 for a field of 12 to 26 toroidal modes, else variant 1;
  *   0  one thread per marker, state in registers, coefficients through L1;
  *   1, 2  warp-autonomous: every warp owns 32 P - slack markers (state in shared memory), groups them by
  *         triangle with ballots at every RK4 stage and evaluates P markers of one triangle per lane off a

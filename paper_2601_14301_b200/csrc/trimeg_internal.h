@@ -10,6 +10,9 @@
 #ifndef TRIMEG_AUTO_FUSED_MIN_MODES
 #define TRIMEG_AUTO_FUSED_MIN_MODES 12
 #endif
+#ifndef TRIMEG_AUTO_FUSED_MAX_MODES
+#define TRIMEG_AUTO_FUSED_MAX_MODES 26
+#endif
 
 namespace trimeg {
 
@@ -54,8 +57,13 @@ namespace trimeg {
 
 // TRIMEG_PUSH_KERNEL_AUTO: with few toroidal modes the per-stage bookkeeping of the CTA-tile kernel (two block
 // barriers, bin scan) outweighs its faster coefficient path and the barrier-free warp kernel wins
-// (cfg2, 3 modes: 4.0e9 vs 3.2e9 marker-steps/s); with many modes it is the other way round (cfg5, 16 modes: 1.43e9 vs 1.52e9).
-inline int auto_push_kernel(int n_modes) { return n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES ? 3 : 1; }
+// (cfg2, 3 modes: 4.2e9 vs 3.2e9 marker-steps/s); with many modes it is the other way round (cfg5, 16 modes: 1.45e9 vs 1.55e9);
+// with very many modes a record (336 B per mode) is so large that the tile kernel has too few record slots in shared
+// memory for the triangles of its tile (14 slots at 26 modes) and the warp kernel, which reads through L1, is used again.
+inline int auto_push_kernel(int n_modes)
+{
+    return (n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES && n_modes <= TRIMEG_AUTO_FUSED_MAX_MODES) ? 3 : 1;
+}
 
 // launch wrappers implemented in trimeg_push.cu; each returns the cudaError of the launch
 cudaError_t launch_locate(trimeg_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell, cudaStream_t s);

@@ -548,3 +548,24 @@ def test_fp64_peak_depends_on_register_operands(B, inputs):
     assert 0.60 < p3 / p0 < 0.72
     with pytest.raises(B.TrimegError):
         ctx.measure_fp64_peak_operands(4)
+
+
+@pytest.mark.parametrize("variant", [1, 3, 6])
+def test_push_many_modes_few_record_slots(B, inputs, variant):
+    """32 toroidal modes: a coefficient record is 10.8 KB, the CTA-tile kernel has room for 11 (variant 6: 4) of them and
+    sends the other triangles' markers down the one-marker path; same results as the oracle either way."""
+    modes = tuple(range(0, 64, 2))
+    wl, o, ctx, _, _ = _setup(B, inputs, "cfg1", modes=modes)
+    assert ctx.get_push_kernel() == 1                       # automatic choice above 26 modes
+    ctx.set_push_kernel(variant)
+    m = inputs.markers(wl, n=6007)
+    m["w"] = np.random.default_rng(7).standard_normal(6007) * 1e-4
+    want = o.push(m, wl.dt, 3)
+    d = _dev(B, m)
+    ctx.locate(d["R"], d["Z"], cell=d["cell"])
+    perm = ctx.sort(d, want_perm=True).cpu().numpy()
+    ctx.push(d, wl.dt, 3)
+    got = _host(d)
+    want = {k: v[perm] for k, v in want.items()}
+    assert np.array_equal(got["cell"], want["cell"])
+    _assert_state_close(got, want, 1e-10, 1e-4)
