@@ -4,7 +4,7 @@
     python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5|cfg2|cfg3] [--impl reference]
 
 One bench "step" = one pass of the whole hot path (DESIGN.md §1 rows a1-a6) over the
-workload's marker batch: [compact lost markers -> cell sort -> fused RK4 push of
+workload's marker batch: compact lost markers, then [cell sort -> fused RK4 push of
 `sort_every` steps] repeated until the workload's nsteps RK4 steps are done, the field
 frozen.  value = marker-RK4-steps of all ranks / max-over-ranks device time.
 
@@ -212,8 +212,9 @@ def run_gpu(args, wl):
         n_act = state["n_active"]
         while done < wl.nsteps:
             k = min(sort_every, wl.nsteps - done)
-            n_act, _ = ctx.compact(d, n=n_act)        # a6: drop lost markers (syncs to return the count)
-            ctx.sort(d, n=n_act)                      # a1
+            if done == 0:
+                n_act, _ = ctx.compact(d, n=n_act)    # a6: drop lost markers once per step (syncs to return the count);
+            ctx.sort(d, n=n_act)                      # a1  (markers lost since sort to the end of the range and are skipped)
             if record:
                 e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
                 e0.record()

@@ -135,13 +135,16 @@ __global__ void bell_kernel(int n_theta, int n_tri, int n_vert, int n_modes, con
 // =============================================================================== a1: cell sort
 // Counting sort: histogram over cells (lost markers in the last bin), exclusive scan of the
 // bins, scatter of the marker records to scratch, copy back.
+// Cell-sorted or nearly sorted input puts the 32 markers of a warp into one or two triangles: one atomic per distinct
+// triangle of the warp (__match_any_sync) instead of 32 serialised atomics on the same address.
 __global__ void hist_kernel(size_t n, const int32_t *__restrict__ cell, int n_tri, int *__restrict__ bins)
 {
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
-    int c = cell[p];
-    if (c < 0 || c >= n_tri) c = n_tri;
-    atomicAdd(bins + c, 1);
+    const int lane = threadIdx.x & 31;
+    int c = -1 - lane;                                   // past the end: a key of its own, nothing counted
+    if (p < n) { c = cell[p]; if (c < 0 || c >= n_tri) c = n_tri; }
+    const unsigned grp = __match_any_sync(0xffffffffu, c);
+    if (c >= 0 && lane == __ffs(grp) - 1) atomicAdd(bins + c, __popc(grp));
 }
 
 // single-block exclusive scan of nb ints, in place; bins[nb] receives the total
@@ -172,10 +175,16 @@ __global__ void sort_scatter_kernel(size_t n, trimeg_markers m, int n_tri, int *
                                     int64_t *__restrict__ perm)
 {
     const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    const int lane = threadIdx.x & 31;
+    int c0 = -1, c = -1 - lane;
+    if (p < n) { c0 = m.cell[p]; c = (c0 < 0 || c0 >= n_tri) ? n_tri : c0; }
+    const unsigned grp = __match_any_sync(0xffffffffu, c);       // one cursor update per distinct triangle of the warp
+    const int leader = __ffs(grp) - 1;
+    int first = 0;
+    if (c >= 0 && lane == leader) first = atomicAdd(cursor + c, __popc(grp));
+    first = __shfl_sync(0xffffffffu, first, leader);
     if (p >= n) return;
-    const int c0 = m.cell[p];
-    const int c = (c0 < 0 || c0 >= n_tri) ? n_tri : c0;
-    const size_t d = (size_t)atomicAdd(cursor + c, 1);
+    const size_t d = (size_t)first + __popc(grp & ((1u << lane) - 1u));
     o.R[d] = m.R[p]; o.Z[d] = m.Z[p]; o.phi[d] = m.phi[p]; o.vpar[d] = m.vpar[p];
     o.mu[d] = m.mu[p]; o.w[d] = m.w[p]; o.cell[d] = c0;
     if (perm) perm[d] = (int64_t)p;
