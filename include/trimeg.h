@@ -175,7 +175,7 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX. */
 #define TRIMEG_PUSH_KERNEL_AUTO (-1)
-#define TRIMEG_PUSH_KERNEL_MAX 6
+#define TRIMEG_PUSH_KERNEL_MAX 8
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 /* The variant trimeg_push will launch (AUTO resolved for the uploaded field; otherwise the TRIMEG_PUSH_KERNEL
  * environment override at context creation or the last trimeg_set_push_kernel); -2 for a NULL context. */

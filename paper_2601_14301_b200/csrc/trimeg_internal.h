@@ -76,6 +76,10 @@ cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                              cudaStream_t s);
 
+// trimeg_push_wcache.cu: warp-autonomous with a CTA-shared record cache in shared memory (variants 7, 8)
+cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
+                               cudaStream_t s);
+
 // trimeg_push_fused.cu: CTA tiles with resident coefficient records, fused evaluate + finish (variants 3..6)
 cudaError_t launch_push_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                               cudaStream_t s);

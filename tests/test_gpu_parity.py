@@ -319,7 +319,7 @@ def test_non_arithmetic_mode_list(B, inputs):
 
 
 # ----------------------------------------------------------------------------- push-kernel schedules
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8])
 @pytest.mark.parametrize("name,n,nsteps,sort", [("cfg1", 4096, 20, False), ("cfg1", 1777, 3, True),
                                                 ("cfg2", (1 << 16) + 13, 3, True), ("cfg5", 40009, 5, True),
                                                 ("cfg3", 20011, 2, False)])
@@ -351,7 +351,7 @@ def test_push_kernel_variants_match_oracle(B, inputs, variant, name, n, nsteps, 
     assert ctx.get_stats()["n_lost"] == int((want["cell"] < 0).sum()) - outside_at_start
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7, 8])
 def test_push_kernel_schedules_edge_cases(B, inputs, variant):
     """No field modes (weights bit-identical), already-lost markers on input are left untouched,
     two calls equal one, non-arithmetic mode list."""
@@ -518,7 +518,7 @@ def test_automatic_schedule_selection_and_variant_range(B, inputs):
     variants outside -1..TRIMEG_PUSH_KERNEL_MAX are rejected; AUTO gives the oracle's result like any fixed variant."""
     wl, o, ctx, _, _ = _setup(B, inputs, "cfg1")
     assert ctx.get_push_kernel() == 1
-    for bad in (-2, 7, 100):
+    for bad in (-2, 9, 100):
         with pytest.raises(B.TrimegError):
             ctx.set_push_kernel(bad)
     ctx.set_push_kernel(3)
@@ -550,7 +550,7 @@ def test_fp64_peak_depends_on_register_operands(B, inputs):
         ctx.measure_fp64_peak_operands(4)
 
 
-@pytest.mark.parametrize("variant", [1, 3, 6])
+@pytest.mark.parametrize("variant", [1, 3, 6, 7])
 def test_push_many_modes_few_record_slots(B, inputs, variant):
     """32 toroidal modes: a coefficient record is 10.8 KB, the CTA-tile kernel has room for 11 (variant 6: 4) of them and
     sends the other triangles' markers down the one-marker path; same results as the oracle either way."""
