@@ -161,7 +161,7 @@ int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_d
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
 /* Kernel used by trimeg_push / trimeg_push_host (same results, different schedules):
- *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 3 for a field of 12 to 26 toroidal modes, else variant 1;
+ *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 7 for a field of 12 to 26 toroidal modes, else variant 1;
  *   0  one thread per marker, state in registers, coefficients through L1;
  *   1, 2  warp-autonomous: every warp owns 32 P - slack markers (state in shared memory), groups them by
  *         triangle with ballots at every RK4 stage and evaluates P markers of one triangle per lane off a
@@ -172,10 +172,13 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *         stages and steps, re-bins the markers by triangle at every stage and evaluates + finishes P
  *         markers of one triangle per thread (3: P = 2, 384 threads; 4: P = 3, 256; 5: P = 4, 256;
  *         6: P = 2, 192 threads, two CTAs per SM).
+ *   7  warp-autonomous like 1 (P = 2, 12 warps per CTA), with the coefficient records of the CTA's triangles in a shared,
+ *         insert-only hash table in shared memory: the first warp that meets a triangle copies its record in, the others
+ *         find it there; the warps meet at a barrier every tenth step only (to empty the table when it is nearly full).
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX. */
 #define TRIMEG_PUSH_KERNEL_AUTO (-1)
-#define TRIMEG_PUSH_KERNEL_MAX 8
+#define TRIMEG_PUSH_KERNEL_MAX 7
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 /* The variant trimeg_push will launch (AUTO resolved for the uploaded field; otherwise the TRIMEG_PUSH_KERNEL
  * environment override at context creation or the last trimeg_set_push_kernel); -2 for a NULL context. */
@@ -202,8 +205,9 @@ int trimeg_reset_stats(trimeg_ctx *ctx);
  * variants 3..6: [0] evaluation head (local coordinates, toroidal phases), [1] phase B (record copies, bin
  * scan, scatter to slots, barrier), [2] table reset, [3] the mode loop (batched Horner), [4] finishing
  * the markers, binning for the next stage and the wait at the barrier; variants 1, 2: [0] grouping,
- * [3] evaluation + finishing, [4] markers without a slot.  out8[5]: markers evaluated by the one-marker
- * path; out8[6]: coefficient records copied to shared memory (3..6) or bins formed (1, 2); out8[7]: RK4
+ * [3] evaluation + finishing, [4] markers without a slot; variant 7 as 1, 2 ([0] includes the record lookups).
+ * out8[5]: markers evaluated by the one-marker
+ * path; out8[6]: coefficient records copied to shared memory (3..7) or bins formed (1, 2); out8[7]: RK4
  * stages run, summed over CTAs (warps).  Synchronises the device.  DESIGN.md section 5. */
 int trimeg_get_tile_counters(trimeg_ctx *ctx, int64_t *out8_host);
 

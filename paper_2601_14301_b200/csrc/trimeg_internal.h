@@ -55,14 +55,14 @@ struct trimeg_ctx {
 
 namespace trimeg {
 
-// TRIMEG_PUSH_KERNEL_AUTO: with few toroidal modes the per-stage bookkeeping of the CTA-tile kernel (two block
-// barriers, bin scan) outweighs its faster coefficient path and the barrier-free warp kernel wins
-// (cfg2, 3 modes: 4.2e9 vs 3.2e9 marker-steps/s); with many modes it is the other way round (cfg5, 16 modes: 1.45e9 vs 1.55e9);
-// with very many modes a record (336 B per mode) is so large that the tile kernel has too few record slots in shared
-// memory for the triangles of its tile (14 slots at 26 modes) and the warp kernel, which reads through L1, is used again.
+// TRIMEG_PUSH_KERNEL_AUTO: with few toroidal modes the coefficient records are small, L1 holds them, and the plain
+// warp-autonomous kernel wins (cfg2, 3 modes: 4.4e9 against 3.7e9 marker-steps/s for variant 7); from about a dozen modes on
+// the records have to sit in shared memory and variant 7 wins (cfg5, 16 modes: 1.66e9 against 1.47e9; the lock-step CTA-tile
+// kernel, variant 3: 1.59e9); with very many modes a record (336 B per mode) is so large that too few of them fit into shared
+// memory for the triangles of a CTA's markers (15 slots at 26 modes) and the plain warp kernel is used again.
 inline int auto_push_kernel(int n_modes)
 {
-    return (n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES && n_modes <= TRIMEG_AUTO_FUSED_MAX_MODES) ? 3 : 1;
+    return (n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES && n_modes <= TRIMEG_AUTO_FUSED_MAX_MODES) ? 7 : 1;
 }
 
 // launch wrappers implemented in trimeg_push.cu; each returns the cudaError of the launch
@@ -76,7 +76,7 @@ cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                              cudaStream_t s);
 
-// trimeg_push_wcache.cu: warp-autonomous with a CTA-shared record cache in shared memory (variants 7, 8)
+// trimeg_push_wcache.cu: warp-autonomous with a CTA-shared record cache in shared memory (variant 7)
 cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                                cudaStream_t s);
 

@@ -12,7 +12,8 @@
 //     row) global -> shared with all its lanes, fences, and publishes it (state READY);
 //   * a warp that finds the bin claimed but not yet READY polls it (bounded; the copying warp never waits for anybody), and
 //     gives the triangle's markers to the one-marker path if the record does not show up or there is no slot left;
-//   * once per RK4 step all warps of the CTA meet at a barrier, and the table is emptied if it is nearly full.
+//   * every tenth RK4 step of a call all warps of the CTA meet at a barrier, and the table is emptied if it is nearly full
+//     (the bench fuses 10 steps per call: no barrier at all; meeting every step costs 4 %, every third step 2 %).
 // Everything else -- the arithmetic per marker, the locator rule, lost-marker handling -- is that of the other push kernels.
 #include "trimeg_internal.h"
 #include "trimeg_multi.cuh"
@@ -26,6 +27,7 @@ constexpr int WC_NBIN = 64;         // hash bins of the CTA's record table
 constexpr int WC_NPROBE = 8;
 constexpr int WC_NB_MAX = 12;       // distinct triangles per warp and stage that get evaluation slots
 constexpr int WC_EMPTY = -1;
+constexpr int WC_SYNC_EVERY = 10;   // RK4 steps between two meetings of the CTA's warps (table check)
 constexpr int WC_MAXSPIN = 400;     // polls of a record another warp is copying (64 ns apart) before giving up
 enum { WC_LOADING = 1, WC_READY = 2 };
 
@@ -279,8 +281,9 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
             __syncwarp();
             if (lane == 0) { const long long now = clock64(); tph[2] += now - tlast; tlast = now; }
         }
-        // ---- once per step: all warps meet; the table is emptied when it is nearly full of triangles the markers have left
-        if (has_field) {
+        // ---- every WC_SYNC_EVERY steps all warps meet; the table is emptied when it is nearly full of triangles the markers
+        // have left (a full table is not an error: triangles without a record go down the one-marker path)
+        if (has_field && step % WC_SYNC_EVERY == WC_SYNC_EVERY - 1 && step + 1 < nsteps) {
             __syncthreads();
             const int claimed = counters[0];
             __syncthreads();                                        // everybody has read the counter before anybody claims again
@@ -355,7 +358,6 @@ cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n,
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
     case 7: return launch_wcache<2, 12, 6>(c, m, n, dt, nsteps, s);
-    case 8: return launch_wcache<2, 8, 6>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }
