@@ -357,7 +357,7 @@ cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n,
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
-    case 7: return launch_wcache<2, 12, 6>(c, m, n, dt, nsteps, s);
+    case 7: return launch_wcache<2, 12, 5>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }
