@@ -5,8 +5,9 @@
 // warps in lock-step (two block barriers per RK4 stage), so its latency-bound phases -- binning, scan, equations -- never
 // hide under the Horner loop of another warp: 30 % of its time.  The warp-autonomous kernel has no barrier but reads the
 // records through L1, which neither holds them all nor delivers them cheaply.  This kernel takes the warp-autonomous
-// schedule (every warp owns 32 P - SLACK markers for the whole call, groups them by triangle with ballots at every stage,
-// evaluates P markers of one triangle per lane, finishes and re-locates them) and gives the CTA's warps ONE shared,
+// schedule (every warp owns 32 P - SLACK markers for the whole call, groups them by triangle with ballots -- anew only at
+// a stage where one of them has changed its triangle, else the slots of the last stage stand --, evaluates P markers of
+// one triangle per lane, finishes and re-locates them) and gives the CTA's warps ONE shared,
 // insert-only hash table of records in shared memory:
 //   * the first warp that meets a triangle claims a bin (atomicCAS on the tag), copies the record (coefficients + geometry
 //     row) global -> shared with all its lanes, fences, and publishes it (state READY);
@@ -128,8 +129,10 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
     long long tph[3] = {0, 0, 0}, tlast = clock64();                // lane 0: grouping (+ lookups), evaluation + finish, one-marker path
     unsigned n_fallback = 0, n_copied = 0, n_stages = 0;
     int t_last[P], r_last[P];                                       // triangle and record slot of the lane's markers at the last stage
+    int slot[P], recp[P], n_ev = 0;                                 // evaluation slot and record of the lane's markers; slots in use
+    unsigned n_regroup = 0;
 #pragma unroll
-    for (int p = 0; p < P; ++p) { t_last[p] = -1; r_last[p] = -1; }
+    for (int p = 0; p < P; ++p) { t_last[p] = -2; r_last[p] = -1; slot[p] = -1; recp[p] = -1; }
 
     if (tid < WC_NBIN) { tag[tid] = WC_EMPTY; state[tid] = 0; rec_of[tid] = -1; }
     if (tid < 4) counters[tid] = 0;
@@ -165,22 +168,30 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
 #pragma unroll 1
         for (int stage = 0; stage < 4; ++stage) {
             // ------------------------------------------------------------ 1: grouping by triangle (home role) + record lookup
-            int t[P], slot[P], recp[P];
+            int t[P];
             unsigned rem[P];
+            bool same = true;
 #pragma unroll
             for (int p = 0; p < P; ++p) {
                 const int q = lane + 32 * p;
                 const bool act = (q < NW) && (flags[q] & FL_ACTIVE);
                 t[p] = act ? cell[q] : -1;
-                slot[p] = -1; recp[p] = -1;
+                same = same && (t[p] == t_last[p]);
                 if (act && stage == 0) {
 #pragma unroll
                     for (int k = 0; k < 5; ++k) S[(S_R + k) * NW + q] = S[(Y_R + k) * NW + q];
                 }
-                rem[p] = __ballot_sync(FULL, act);
             }
-            int n_ev = 0, nb = 0;
-            if (has_field) {
+            // no marker of the warp has changed its triangle since the last stage: the slots of that stage stand
+            if (has_field && !__all_sync(FULL, same)) {
+                int nb = 0;
+                n_ev = 0;
+                ++n_regroup;
+#pragma unroll
+                for (int p = 0; p < P; ++p) { slot[p] = -1; recp[p] = -1; rem[p] = __ballot_sync(FULL, t[p] >= 0); }
+                unsigned kn[P];                                    // markers that stayed in their triangle: they know its record
+#pragma unroll
+                for (int p = 0; p < P; ++p) kn[p] = __ballot_sync(FULL, t[p] >= 0 && t[p] == t_last[p] && r_last[p] >= 0);
 #pragma unroll 1
                 while (nb < WC_NB_MAX && n_ev < NE) {
                     int pl = -1;
@@ -190,7 +201,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                     int cand = 0, known = -1;
                     unsigned rl = 0;
 #pragma unroll
-                    for (int p = 0; p < P; ++p) if (p == pl) { cand = t[p]; rl = rem[p]; known = (t_last[p] == t[p]) ? r_last[p] : -1; }
+                    for (int p = 0; p < P; ++p)
+                        if (p == pl) {
+                            cand = t[p]; known = (t_last[p] == t[p]) ? r_last[p] : -1;
+                            rl = (rem[p] & kn[p]) ? (rem[p] & kn[p]) : rem[p];      // a marker that knows the record leads, if there is one
+                        }
                     const int tl = __shfl_sync(FULL, cand, __ffs(rl) - 1);
                     int rec = __shfl_sync(FULL, known, __ffs(rl) - 1);      // the marker sat in this triangle at the last stage: same record
                     if (rec < 0) rec = wc_lookup(tl, lane, tag, state, rec_of, counters, nslot, M, F, REC, rec_len, rec_stride, n_copied);
@@ -291,7 +306,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                 if (tid < WC_NBIN) { tag[tid] = WC_EMPTY; state[tid] = 0; rec_of[tid] = -1; }
                 if (tid == 0) counters[0] = 0;
 #pragma unroll
-                for (int p = 0; p < P; ++p) { t_last[p] = -1; r_last[p] = -1; }
+                for (int p = 0; p < P; ++p) { t_last[p] = -2; r_last[p] = -1; }
                 __syncthreads();
             }
         }
@@ -319,6 +334,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
         if (lost) atomicAdd(&st->n_lost, (unsigned long long)lost);
         if (moved) atomicAdd(&st->n_moved, (unsigned long long)moved);
         atomicAdd(&st->tile[0], (unsigned long long)tph[0]);
+        atomicAdd(&st->tile[1], (unsigned long long)n_regroup);
         atomicAdd(&st->tile[3], (unsigned long long)tph[1]);
         atomicAdd(&st->tile[4], (unsigned long long)tph[2]);
         if (n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);
