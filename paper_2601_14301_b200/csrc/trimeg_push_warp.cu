@@ -63,6 +63,9 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
     const unsigned lt_mask = (1u << lane) - 1u;
     long long tph[3] = {0, 0, 0}, tlast = clock64();                // lane 0: grouping, evaluation + equations, fallback
     unsigned n_fallback = 0, n_bins = 0, n_stages = 0;
+    int t_last[P], slot[P], n_ev = 0;                               // triangle and evaluation slot of the lane's markers at the last grouping
+#pragma unroll
+    for (int p = 0; p < P; ++p) { t_last[p] = -2; slot[p] = -1; }
 
     // ---- load the warp's markers (home role), locate the start positions
 #pragma unroll
@@ -96,22 +99,26 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
 #pragma unroll 1
         for (int stage = 0; stage < 4; ++stage) {
             // ------------------------------------------------------------ 1: grouping by triangle (home role)
-            int t[P], slot[P];
+            int t[P];
             unsigned rem[P];
+            bool same = true;
 #pragma unroll
             for (int p = 0; p < P; ++p) {
                 const int q = lane + 32 * p;
                 const bool act = (q < NW) && (flags[q] & FL_ACTIVE);
                 t[p] = act ? cell[q] : -1;
-                slot[p] = -1;
+                same = same && (t[p] == t_last[p]);
                 if (act && stage == 0) {
 #pragma unroll
                     for (int k = 0; k < 5; ++k) S[(S_R + k) * NW + q] = S[(Y_R + k) * NW + q];
                 }
-                rem[p] = __ballot_sync(FULL, act);
             }
-            int n_ev = 0, nb = 0;
-            if (has_field) {
+            int nb = 0;
+            // no marker of the warp has changed its triangle since the last stage: the slots of that stage stand
+            if (has_field && !__all_sync(FULL, same)) {
+                n_ev = 0;
+#pragma unroll
+                for (int p = 0; p < P; ++p) { slot[p] = -1; rem[p] = __ballot_sync(FULL, t[p] >= 0); t_last[p] = t[p]; }
 #pragma unroll 1
                 while (nb < NB_MAX && n_ev < NE) {
                     int pl = -1;
