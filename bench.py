@@ -36,7 +36,7 @@ METRIC = "marker RK4 pushes/sec (incl. field gather)"
 # capture (profiles/r01_fused_push_kernel.md): (workload, push kernel, sort_every, markers) -> bytes; null for anything else
 PROFILED_DRAM_BYTES_PER_LAUNCH = {("cfg5", 3, 10, 1 << 24): 1.936e9, ("cfg5", 7, 10, 1 << 24): 1.94e9}
 PUSH_KERNEL_NAMES = {0: "push_kernel", 1: "push_warp_kernel<2,4,6>", 2: "push_warp_kernel<4,4,16>", 3: "push_fused_kernel<2,384,1>",
-                     4: "push_fused_kernel<3,256,1>", 5: "push_fused_kernel<4,256,1>", 6: "push_fused_kernel<2,192,2>", 7: "push_wcache_kernel<2,12,5>"}
+                     4: "push_fused_kernel<3,256,1>", 5: "push_fused_kernel<4,256,1>", 6: "push_fused_kernel<2,192,2>", 7: "push_wcache_kernel<2,12,5>", 8: "push_warp_kernel<2,4,6,4>"}
 UNIT = "marker-steps/s"
 
 

@@ -161,10 +161,11 @@ int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_d
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
 /* Kernel used by trimeg_push / trimeg_push_host (same results, different schedules):
- *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 7 for a field of 12 to 26 toroidal modes, else variant 1;
+ *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 8 for a field of up to 4 toroidal modes, variant 7 for 12 to 26,
+ *      else variant 1;
  *   0  one thread per marker, state in registers, coefficients through L1;
  *   1, 2  warp-autonomous: every warp owns 32 P - slack markers (state in shared memory), groups them by
- *         triangle with ballots at every RK4 stage and evaluates P markers of one triangle per lane off a
+ *         triangle with ballots (anew only at a stage where one of them has changed its triangle) and evaluates P markers of one triangle per lane off a
  *         single load of each coefficient (through L1), finishes and re-locates them without any block
  *         barrier (1: P = 2; 2: P = 4);
  *   3..6  CTA tiles with resident coefficient records: a CTA owns a tile of markers (state in
@@ -175,10 +176,12 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *   7  warp-autonomous like 1 (P = 2, 12 warps per CTA), with the coefficient records of the CTA's triangles in a shared,
  *         insert-only hash table in shared memory: the first warp that meets a triangle copies its record in, the others
  *         find it there; the warps meet at a barrier every tenth step only (to empty the table when it is nearly full).
+ *   8  variant 1 compiled for 128 registers per thread (16 instead of 12 warps per SM): better when the Horner loop is
+ *         short (few modes) and the latency-bound rest of the stage weighs more.
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX. */
 #define TRIMEG_PUSH_KERNEL_AUTO (-1)
-#define TRIMEG_PUSH_KERNEL_MAX 7
+#define TRIMEG_PUSH_KERNEL_MAX 8
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 /* The variant trimeg_push will launch (AUTO resolved for the uploaded field; otherwise the TRIMEG_PUSH_KERNEL
  * environment override at context creation or the last trimeg_set_push_kernel); -2 for a NULL context. */

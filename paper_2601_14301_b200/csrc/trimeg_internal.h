@@ -7,6 +7,9 @@
 #include "../../include/trimeg.h"
 #include "trimeg_device.cuh"
 
+#ifndef TRIMEG_AUTO_SMALL_MAX_MODES
+#define TRIMEG_AUTO_SMALL_MAX_MODES 4
+#endif
 #ifndef TRIMEG_AUTO_FUSED_MIN_MODES
 #define TRIMEG_AUTO_FUSED_MIN_MODES 12
 #endif
@@ -56,12 +59,15 @@ struct trimeg_ctx {
 namespace trimeg {
 
 // TRIMEG_PUSH_KERNEL_AUTO: with few toroidal modes the coefficient records are small, L1 holds them, and the plain
-// warp-autonomous kernel wins (cfg2, 3 modes: 4.4e9 against 3.7e9 marker-steps/s for variant 7); from about a dozen modes on
-// the records have to sit in shared memory and variant 7 wins (cfg5, 16 modes: 1.66e9 against 1.47e9; the lock-step CTA-tile
+// warp-autonomous kernel wins (cfg2, 3 modes: 4.5e9 against 3.7e9 marker-steps/s for variant 7); from about a dozen modes on
+// the records have to sit in shared memory and variant 7 wins (cfg5, 16 modes: 1.74e9 against 1.51e9; the lock-step CTA-tile
 // kernel, variant 3: 1.59e9); with very many modes a record (336 B per mode) is so large that too few of them fit into shared
-// memory for the triangles of a CTA's markers (15 slots at 26 modes) and the plain warp kernel is used again.
+// memory for the triangles of a CTA's markers (15 slots at 26 modes) and the plain warp kernel is used again.  Up to 4 modes
+// the Horner loop is so short that the latency-bound rest of a stage weighs more and 16 warps per SM at 128 registers
+// (variant 8) beat 12 at 168 (cfg2: 4.69e9 against 4.53e9; on the cfg5 mesh the two cross between 4 and 6 modes).
 inline int auto_push_kernel(int n_modes)
 {
+    if (n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES) return 8;
     return (n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES && n_modes <= TRIMEG_AUTO_FUSED_MAX_MODES) ? 7 : 1;
 }
 

@@ -11,7 +11,7 @@
 // under the FP64 work of the others.  Per RK4 stage:
 //   1  grouping (home role: lane l looks after markers l, l + 32, ...): the warp's markers are
 //      partitioned by triangle with ballots; every triangle gets a run of evaluation slots padded
-//      to a multiple of P;
+//      to a multiple of P.  The slots of the last stage stand if no marker has changed its triangle;
 //   2  evaluation (slot role): lane l takes slots [P l, P l + P) -- by construction one triangle --
 //      and runs the bivariate Horner scheme for the P markers off ONE load of each coefficient;
 //      lanes of a warp mostly share the triangle, so the loads are warp-uniform L1 hits;
@@ -39,8 +39,9 @@ struct WarpCfg {
         (sizeof(double) * (size_t)N_STATE * NW + sizeof(int) * ((size_t)NW + 2 * (size_t)NE) + NW + 15) / 16 * 16;
 };
 
-template <int P, int WARPS, int SLACK>
-__global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
+// MINB: CTAs per SM the kernel is compiled for (3 -> 168 registers, 4 -> 128; without it ptxas takes 214 for P = 2)
+template <int P, int WARPS, int SLACK, int MINB>
+__global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
                                                                double dt, int nsteps, Stats *st)
 {
     using Cfg = WarpCfg<P, SLACK>;
@@ -247,20 +248,20 @@ __global__ void __launch_bounds__(32 * WARPS) push_warp_kernel(MeshDev M, FieldD
     }
 }
 
-template <int P, int WARPS, int SLACK>
+template <int P, int WARPS, int SLACK, int MINB>
 cudaError_t launch_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     using Cfg = WarpCfg<P, SLACK>;
     static bool configured = false;
     const size_t shm = Cfg::WARP_BYTES * WARPS;
     if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
         if (e != cudaSuccess) return e;
         configured = true;
     }
     const size_t per_cta = (size_t)Cfg::NW * WARPS;
     const size_t ctas = (n + per_cta - 1) / per_cta;
-    push_warp_kernel<P, WARPS, SLACK><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
+    push_warp_kernel<P, WARPS, SLACK, MINB><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;
     return cudaGetLastError();
 }
@@ -272,8 +273,9 @@ cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
-    case 1: return launch_warp<2, 4, 6>(c, m, n, dt, nsteps, s);
-    case 2: return launch_warp<4, 4, 16>(c, m, n, dt, nsteps, s);
+    case 1: return launch_warp<2, 4, 6, 3>(c, m, n, dt, nsteps, s);
+    case 2: return launch_warp<4, 4, 16, 2>(c, m, n, dt, nsteps, s);
+    case 8: return launch_warp<2, 4, 6, 4>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }

@@ -319,7 +319,7 @@ def test_non_arithmetic_mode_list(B, inputs):
 
 
 # ----------------------------------------------------------------------------- push-kernel schedules
-@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("variant", [0, 1, 2, 3, 4, 5, 6, 7, 8])
 @pytest.mark.parametrize("name,n,nsteps,sort", [("cfg1", 4096, 20, False), ("cfg1", 1777, 3, True),
                                                 ("cfg2", (1 << 16) + 13, 3, True), ("cfg5", 40009, 5, True),
                                                 ("cfg3", 20011, 2, False)])
@@ -351,7 +351,7 @@ def test_push_kernel_variants_match_oracle(B, inputs, variant, name, n, nsteps, 
     assert ctx.get_stats()["n_lost"] == int((want["cell"] < 0).sum()) - outside_at_start
 
 
-@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7])
+@pytest.mark.parametrize("variant", [1, 2, 3, 4, 5, 6, 7, 8])
 def test_push_kernel_schedules_edge_cases(B, inputs, variant):
     """No field modes (weights bit-identical), already-lost markers on input are left untouched,
     two calls equal one, non-arithmetic mode list."""
@@ -514,17 +514,19 @@ def test_full_size_sampled_parity_in_bench_configuration(B, inputs, name, nsteps
 
 # ----------------------------------------------------------------------------- schedule selection, diagnostics
 def test_automatic_schedule_selection_and_variant_range(B, inputs):
-    """TRIMEG_PUSH_KERNEL_AUTO resolves by the number of uploaded modes (plain warp kernel below 12 and above 26, warp kernel with shared-memory records in between);
+    """TRIMEG_PUSH_KERNEL_AUTO resolves by the number of uploaded modes (plain warp kernel below 12 and above 26 -- its 128-register build up to 4 --, warp kernel with shared-memory records in between);
     variants outside -1..TRIMEG_PUSH_KERNEL_MAX are rejected; AUTO gives the oracle's result like any fixed variant."""
     wl, o, ctx, _, _ = _setup(B, inputs, "cfg1")
-    assert ctx.get_push_kernel() == 1
-    for bad in (-2, 8, 100):
+    assert ctx.get_push_kernel() == 8                       # 2 modes
+    for bad in (-2, 9, 100):
         with pytest.raises(B.TrimegError):
             ctx.set_push_kernel(bad)
     ctx.set_push_kernel(3)
     assert ctx.get_push_kernel() == 3
     ctx.set_push_kernel(B.PUSH_KERNEL_AUTO)
-    assert ctx.get_push_kernel() == 1
+    assert ctx.get_push_kernel() == 8
+    _, _, ctx8, _, _ = _setup(B, inputs, "cfg1", modes=tuple(range(0, 16, 2)))
+    assert ctx8.get_push_kernel() == 1                      # 8 modes
     wl5, o5, ctx5, _, _ = _setup(B, inputs, "cfg5")
     assert ctx5.get_push_kernel() == 7
     m = inputs.markers(wl5, n=30011)
@@ -550,7 +552,7 @@ def test_fp64_peak_depends_on_register_operands(B, inputs):
         ctx.measure_fp64_peak_operands(4)
 
 
-@pytest.mark.parametrize("variant", [1, 3, 6, 7])
+@pytest.mark.parametrize("variant", [1, 3, 6, 7, 8])
 def test_push_many_modes_few_record_slots(B, inputs, variant):
     """32 toroidal modes: a coefficient record is 10.8 KB, the CTA-tile kernel has room for 11 (variant 6: 4) of them and
     sends the other triangles' markers down the one-marker path; same results as the oracle either way."""
