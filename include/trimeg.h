@@ -208,8 +208,8 @@ int trimeg_reset_stats(trimeg_ctx *ctx);
  * variants 3..6: [0] evaluation head (local coordinates, toroidal phases), [1] phase B (record copies, bin
  * scan, scatter to slots, barrier), [2] table reset, [3] the mode loop (batched Horner), [4] finishing
  * the markers, binning for the next stage and the wait at the barrier; variants 1, 2: [0] grouping,
- * [3] evaluation + finishing, [4] markers without a slot; variant 7 as 1, 2 ([0] includes the record lookups;
- * [1] is a count, not cycles: the stages at which a warp had to group its markers anew).
+ * [1] a count, not cycles: the stages at which a warp had to group its markers anew,
+ * [3] evaluation + finishing, [4] markers without a slot; variants 7, 8 as 1, 2 (7: [0] includes the record lookups).
  * out8[5]: markers evaluated by the one-marker
  * path; out8[6]: coefficient records copied to shared memory (3..7) or bins formed (1, 2); out8[7]: RK4
  * stages run, summed over CTAs (warps).  Synchronises the device.  DESIGN.md section 5. */

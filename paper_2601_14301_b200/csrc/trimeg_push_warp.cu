@@ -63,7 +63,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
     const double hdt = 0.5 * dt, dt6 = dt / 6.0;
     const unsigned lt_mask = (1u << lane) - 1u;
     long long tph[3] = {0, 0, 0}, tlast = clock64();                // lane 0: grouping, evaluation + equations, fallback
-    unsigned n_fallback = 0, n_bins = 0, n_stages = 0;
+    unsigned n_fallback = 0, n_bins = 0, n_stages = 0, n_regroup = 0;
     int t_last[P], slot[P], n_ev = 0;                               // triangle and evaluation slot of the lane's markers at the last grouping
 #pragma unroll
     for (int p = 0; p < P; ++p) { t_last[p] = -2; slot[p] = -1; }
@@ -118,6 +118,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
             // no marker of the warp has changed its triangle since the last stage: the slots of that stage stand
             if (has_field && !__all_sync(FULL, same)) {
                 n_ev = 0;
+                ++n_regroup;
 #pragma unroll
                 for (int p = 0; p < P; ++p) { slot[p] = -1; rem[p] = __ballot_sync(FULL, t[p] >= 0); t_last[p] = t[p]; }
 #pragma unroll 1
@@ -240,6 +241,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
         if (lost) atomicAdd(&st->n_lost, (unsigned long long)lost);
         if (moved) atomicAdd(&st->n_moved, (unsigned long long)moved);
         atomicAdd(&st->tile[0], (unsigned long long)tph[0]);
+        atomicAdd(&st->tile[1], (unsigned long long)n_regroup);
         atomicAdd(&st->tile[3], (unsigned long long)tph[1]);
         atomicAdd(&st->tile[4], (unsigned long long)tph[2]);
         if (n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);

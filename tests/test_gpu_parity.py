@@ -512,6 +512,33 @@ def test_full_size_sampled_parity_in_bench_configuration(B, inputs, name, nsteps
     assert (want["cell"] < 0).sum() > 0
 
 
+@pytest.mark.parametrize("variant", [1, 7, 8])
+def test_push_keeps_slots_while_markers_stay_in_their_triangles(B, inputs, variant):
+    """The warp-autonomous kernels group their markers by triangle anew only at a stage where a marker of the warp has
+    changed its triangle.  With a tiny time step nobody moves: one grouping per warp in 40 stages; with a large one the
+    grouping runs at most stages; the oracle's result either way (cell-sorted input, 10 RK4 steps)."""
+    wl, o, ctx, _, _ = _setup(B, inputs, "cfg5")
+    ctx.set_push_kernel(variant)
+    n = 12011
+    m = inputs.markers(wl, n=n)
+    frac = {}
+    for dt in (1e-7, 0.2):
+        want = o.push(m, dt, 10)
+        d = _dev(B, m)
+        ctx.locate(d["R"], d["Z"], cell=d["cell"])
+        perm = ctx.sort(d, want_perm=True).cpu().numpy()
+        ctx.reset_stats()
+        ctx.push(d, dt, 10)
+        got = _host(d)
+        assert np.array_equal(got["cell"], want["cell"][perm])
+        _assert_state_close(got, {k: v[perm] for k, v in want.items()}, 1e-9, 1e-4)
+        t = ctx.get_tile_counters()
+        assert t["n_stages"] > 0 and t["n_stages"] % 40 == 0
+        frac[dt] = t["cyc_B"] / t["n_stages"]            # [1] of trimeg_get_tile_counters: groupings per warp and stage
+    assert frac[1e-7] <= 1.5 / 40
+    assert frac[0.2] > 0.5
+
+
 # ----------------------------------------------------------------------------- schedule selection, diagnostics
 def test_automatic_schedule_selection_and_variant_range(B, inputs):
     """TRIMEG_PUSH_KERNEL_AUTO resolves by the number of uploaded modes (plain warp kernel below 12 and above 26 -- its 128-register build up to 4 --, warp kernel with shared-memory records in between);
