@@ -33,10 +33,9 @@ import numpy as np
 
 METRIC = "marker RK4 pushes/sec (incl. field gather)"
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the push kernel, from the committed ncu --set full
-# capture (profiles/r01_fused_push_kernel.md): (workload, push kernel, sort_every, markers) -> bytes; null for anything else
-PROFILED_DRAM_BYTES_PER_LAUNCH = {("cfg5", 3, 10, 1 << 24): 1.936e9, ("cfg5", 7, 10, 1 << 24): 1.94e9}
-PUSH_KERNEL_NAMES = {0: "push_kernel", 1: "push_warp_kernel<2,4,6>", 2: "push_warp_kernel<4,4,16>", 3: "push_fused_kernel<2,384,1>",
-                     4: "push_fused_kernel<3,256,1>", 5: "push_fused_kernel<4,256,1>", 6: "push_fused_kernel<2,192,2>", 7: "push_wcache_kernel<2,12,5>", 8: "push_warp_kernel<2,4,6,4>"}
+# captures under profiles/: (workload, push kernel, sort_every, markers) -> bytes; null for anything else
+PROFILED_DRAM_BYTES_PER_LAUNCH = {("cfg5", 3, 10, 1 << 24): 1.94e9}
+PUSH_KERNEL_NAMES = {0: "push_kernel", 1: "push_warp_kernel<2,4,6,3>", 2: "push_warp_kernel<2,4,6,4>", 3: "push_wcache_kernel<2,12,5>"}
 UNIT = "marker-steps/s"
 
 
@@ -46,9 +45,14 @@ def flops_per_marker_step(n_modes: int) -> int:
     return 4 * (200 + 170 * n_modes)
 
 
+def flops_per_gather(n_modes: int) -> int:
+    """Gather only (configs[3]): locator 25 + 170 per mode + 6 for the chain rule."""
+    return 25 + 170 * n_modes + 6
+
+
 def bytes_per_marker_call(nsteps_fused: int) -> float:
     """Marker stream of one push call: 52 B read + 44 B written per marker, once per call
-    (all fused steps keep the state in registers)."""
+    (all fused steps keep the state on chip)."""
     return 96.0
 
 
@@ -116,49 +120,73 @@ class ClockSampler(threading.Thread):
 
 
 # ------------------------------------------------------------------------------- oracle timing
-def time_oracle(wl, target_seconds: float, steps: int = 1, warmup: int = 0):
-    """Time oracle.push (as it stands) on a bounded strided sample of the workload.
-    Returns (marker-steps/s, cores, description, seconds per timed step, sample size, rk4 steps)."""
+def _strided(m, n_s):
+    n = m["R"].size
+    stride = max(1, n // n_s)
+    return {k: np.ascontiguousarray(v[::stride][:n_s]) for k, v in m.items()}, stride
+
+
+def time_oracle(wl, m_np, target_seconds: float, steps: int = 1, warmup: int = 0, one_core_seconds: float = 0.0):
+    """Time oracle.push (as it stands, never tuned) the way BASELINE.md §4 / SURVEY.md §8(d) plan it: a STRIDED
+    subsample of the workload's seeded marker draw, pushed for the workload's full number of RK4 steps, with OpenMP
+    over markers on all host cores -- and, if one_core_seconds > 0, once more on one core with a smaller strided
+    sample.  The sample is the largest power of two (at most 2^20) that fits `target_seconds`.  Markers are
+    independent, so the rate scales linearly to the full batch.  Returns a dict."""
     import oracle
     from paper_2601_14301_b200 import inputs
     o = oracle.from_workload(wl, inputs)
     o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
     cores = o.max_threads()
-    n_pool = 1 << 16
-    pool = inputs.markers(wl, n=n_pool)
-    probe_n, probe_steps = 2048, 2
-    probe = {k: v[:probe_n] for k, v in pool.items()}
+    nsteps = max(1, wl.nsteps)
+    probe, _ = _strided(m_np, 2048)
     t0 = time.perf_counter()
-    o.push(probe, wl.dt, probe_steps)
-    rate = probe_n * probe_steps / (time.perf_counter() - t0)
-    rk4 = max(1, min(wl.nsteps, 10))
-    n_s = int(min(n_pool, max(1024, rate * target_seconds / rk4)))
-    sample = {k: v[:n_s] for k, v in pool.items()}
+    o.push(probe, wl.dt, 2)
+    rate = probe["R"].size * 2 / (time.perf_counter() - t0)
+    n_s = 1 << int(max(10, min(20, np.floor(np.log2(max(1.0, rate * target_seconds / nsteps))))))
+    n_s = min(n_s, m_np["R"].size)
+    sample, stride = _strided(m_np, n_s)
     for _ in range(warmup):
-        o.push(sample, wl.dt, rk4)
+        o.push(sample, wl.dt, nsteps)
     t0 = time.perf_counter()
     for _ in range(steps):
-        o.push(sample, wl.dt, rk4)
-    dt = (time.perf_counter() - t0) / steps
-    desc = (f"first {n_s} markers of the seeded {wl.name} draw x {rk4} RK4 steps per step, "
-            f"oracle.push with OpenMP over markers ({cores} threads)")
-    return n_s * rk4 / dt, cores, desc, dt, n_s, rk4
+        o.push(sample, wl.dt, nsteps)
+    sec = (time.perf_counter() - t0) / steps
+    out = {"value": n_s * nsteps / sec, "cores": cores, "nproc": os.cpu_count(), "seconds_per_step": sec, "sample_markers": n_s,
+           "rk4_steps": nsteps,
+           "sample": (f"every {stride}-th marker of the seeded {wl.name} draw ({n_s} markers) x the full {nsteps} RK4 steps, "
+                      f"oracle.push with OpenMP over markers on {cores} threads (nproc {os.cpu_count()}); "
+                      "markers are independent: the rate scales linearly to the full batch")}
+    if one_core_seconds > 0:
+        n_1 = 1 << int(max(8, np.floor(np.log2(max(1.0, out["value"] / cores * one_core_seconds / nsteps)))))
+        n_1 = min(n_1, n_s)
+        s1, stride1 = _strided(m_np, n_1)
+        t0 = time.perf_counter()
+        o.push(s1, wl.dt, nsteps, nthreads=1)
+        out["value_one_core"] = n_1 * nsteps / (time.perf_counter() - t0)
+        out["sample_one_core"] = f"every {stride1}-th marker ({n_1} markers) x {nsteps} RK4 steps on 1 thread"
+        o.push(probe, wl.dt, 1, nthreads=cores)           # restore the OpenMP thread count
+    return out
 
 
 def run_reference(args, wl):
     from paper_2601_14301_b200 import dist as D
+    from paper_2601_14301_b200 import inputs
     rank, _, world = D.env_rank()
     if rank != 0:
         return 0
+    m_np = inputs.markers(wl, n=wl.n_markers)
     budget = 150.0 / max(1, args.steps + args.warmup)
-    value, cores, desc, sec, n_s, rk4 = time_oracle(wl, min(20.0, budget), steps=args.steps, warmup=args.warmup)
+    r = time_oracle(wl, m_np, min(20.0, budget), steps=args.steps, warmup=args.warmup)
     line = {
-        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
-        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec * 1e3, "higher_is_better": True,
+        "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": workload_config(wl, extra={"reference_sample_markers": n_s, "reference_rk4_steps_per_step": rk4}),
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
-        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "config": workload_config(wl, extra={"reference_sample_markers": r["sample_markers"], "reference_rk4_steps_per_step": r["rk4_steps"]}),
+        "cpu_baseline": {"value": r["value"], "unit": UNIT, "cores": r["cores"], "nproc": r["nproc"], "kind": "oracle",
+                         "sample": r["sample"],
+                         "note": "the oracle is the unoptimised correctness checker (plain monomial sums, gcc -O2): a baseline, "
+                                 "not a tuned CPU push; the GPU/oracle ratio is not a like-for-like speedup"},
+        "e2e": {"value": r["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
@@ -176,7 +204,171 @@ def workload_config(wl, extra=None):
 
 
 # ----------------------------------------------------------------------------------- GPU arm
+class PushRun:
+    """One workload resident on the current device: context, field, the seeded marker batch (a pristine copy and a
+    working copy).  A bench step = restore the batch to the workload's initial state (device copy), compact, then
+    [cell sort -> fused push of `sort_every` RK4 steps] until the workload's nsteps are done."""
+
+    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True):
+        import torch
+        from paper_2601_14301_b200 import binding, inputs
+        self.torch, self.wl = torch, wl
+        self.n = wl.n_markers
+        self.sort_every = max(1, min(sort_every, wl.nsteps))
+        self.ctx = binding.context_for(wl, inputs)
+        self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
+        if push_kernel >= 0:
+            self.ctx.set_push_kernel(push_kernel)
+        m_np = inputs.markers(wl, n=self.n, seed=seed)
+        self.d0 = binding.markers_to_device(m_np, "cuda")
+        self.ctx.locate(self.d0["R"], self.d0["Z"], cell=self.d0["cell"])
+        self.d = {k: torch.empty_like(v) for k, v in self.d0.items()}
+        self.m_np = m_np if keep_host else None
+        self.push_events = []
+        self.n_start = None
+        torch.cuda.synchronize()
+
+    def step(self, record):
+        wl, ctx, d = self.wl, self.ctx, self.d
+        for k, v in self.d0.items():                      # every step starts from the config's initial state
+            d[k].copy_(v)
+        n_act, _ = ctx.compact(d, n=self.n)               # a6: drop the markers outside the mesh (syncs to return the count)
+        self.n_start = n_act
+        done = 0
+        while done < wl.nsteps:
+            k = min(self.sort_every, wl.nsteps - done)
+            ctx.sort(d, n=n_act)                          # a1 (markers lost since go to the end of the range and are skipped)
+            if record:
+                e0, e1 = self.torch.cuda.Event(enable_timing=True), self.torch.cuda.Event(enable_timing=True)
+                e0.record()
+            ctx.push(d, wl.dt, k, n=n_act)                # a2-a6, fused
+            if record:
+                e1.record()
+                self.push_events.append((e0, e1, n_act * k))
+            done += k
+
+    def run(self, steps, warmup, barrier=lambda: None, device_index=0):
+        torch = self.torch
+        for _ in range(warmup):
+            self.step(False)
+        torch.cuda.synchronize()
+        st0 = self.ctx.get_stats()
+        sampler = ClockSampler(device_index)
+        barrier()
+        torch.cuda.synchronize()
+        sampler.start()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        for _ in range(steps):
+            self.step(True)
+        t1.record()
+        torch.cuda.synchronize()
+        barrier()
+        clocks = sampler.stop()
+        st1 = self.ctx.get_stats()
+        lost = st1["n_lost"] - st0["n_lost"]
+        # unit count: a marker that leaves the mesh during a bench step counts ZERO steps for that step (lower bound)
+        units = self.wl.nsteps * (steps * self.n_start - lost)
+        return {"units": units, "seconds": t0.elapsed_time(t1) * 1e-3, "clocks": clocks, "launches": st1["n_launches"] - st0["n_launches"],
+                "lost_per_step": lost / max(1, steps), "n_start": self.n_start}
+
+    def roofline(self, fp64_peak, seconds):
+        wl = self.wl
+        push_s = sum(a.elapsed_time(b) for a, b, _ in self.push_events) * 1e-3
+        push_units = sum(u for _, _, u in self.push_events)
+        n_push = len(self.push_events)
+        flops = flops_per_marker_step(len(wl.modes)) * push_units
+        return {"bound": "alu", "kernel": PUSH_KERNEL_NAMES.get(self.ctx.get_push_kernel(), "push kernel"),
+                "achieved": flops / push_s * 1e-12, "peak": fp64_peak, "unit": "TFLOP/s",
+                "frac": (flops / push_s * 1e-12) / fp64_peak, "launches": n_push, "avg_launch_ms": push_s / max(1, n_push) * 1e3,
+                "push_share_of_step": push_s / seconds, "units_per_launch": push_units / max(1, n_push)}
+
+    def check_against_oracle(self, stride=4096):
+        """Push a fresh 1/stride strided sample of the batch for the workload's nsteps in the launch pattern that was
+        timed (locate, then [sort -> push sort_every steps] ...) and compare it with the oracle; also: every state
+        array of the batch that was timed is finite."""
+        import oracle
+        torch = self.torch
+        from paper_2601_14301_b200 import binding, inputs
+        wl = self.wl
+        for k in ("R", "Z", "phi", "vpar", "w"):
+            assert bool(torch.isfinite(self.d[k][: self.n_start]).all()), f"non-finite {k} after the timed steps"
+        sample = {k: np.ascontiguousarray(v[::stride]) for k, v in self.m_np.items()}
+        ds = binding.markers_to_device(sample, "cuda")
+        self.ctx.locate(ds["R"], ds["Z"], cell=ds["cell"])
+        ident = torch.arange(ds["R"].numel(), device="cuda")
+        done = 0
+        while done < wl.nsteps:
+            k = min(self.sort_every, wl.nsteps - done)
+            perm = self.ctx.sort(ds, want_perm=True)
+            ident = ident[perm]
+            self.ctx.push(ds, wl.dt, k)
+            done += k
+        got = {k: np.empty_like(v.cpu().numpy()) for k, v in ds.items()}
+        idx = ident.cpu().numpy()
+        for k, v in ds.items():
+            got[k][idx] = v.cpu().numpy()
+        o = oracle.from_workload(wl, inputs)
+        o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
+        want = o.push(sample, wl.dt, wl.nsteps)
+        assert np.array_equal(got["cell"] < 0, want["cell"] < 0), "lost-marker sets differ"
+        worst = 0.0
+        for k, scale in (("R", wl.R0), ("Z", wl.a), ("vpar", 1.0), ("w", max(1e-4, float(np.abs(want["w"]).max())))):
+            worst = max(worst, float((np.abs(got[k] - want[k]) / np.maximum(np.maximum(np.abs(got[k]), np.abs(want[k])), scale)).max()))
+        dphi = np.abs((got["phi"] - want["phi"] + np.pi) % (2 * np.pi) - np.pi).max() / (2 * np.pi)
+        worst = max(worst, float(dphi))
+        cells_differ = int((got["cell"] != want["cell"]).sum())
+        tol = 1e-9 * max(1.0, wl.nsteps / 20.0)
+        assert worst < tol, f"bench parity check failed: {worst} >= {tol}"
+        # note: the library's own Bell expansion (kind 0) vs the oracle's LU: 1e-11 relative per coefficient
+        return {"sample_markers": int(sample["R"].size), "rk4_steps": wl.nsteps, "max_rel_err": worst, "tolerance": tol,
+                "cells_differ": cells_differ, "lost_in_sample": int((want["cell"] < 0).sum()), "finite": True}
+
+    def close(self):
+        self.ctx.close()
+        self.d = self.d0 = None
+        self.torch.cuda.empty_cache()
+
+
+def gather_rows(ctx, wl, log2s, reps, hbm_peak, fp64_peak):
+    """BASELINE.json configs[3]: gather only (dphi, d/dR, d/dZ, no push), markers as drawn and sorted by triangle."""
+    import torch
+    from paper_2601_14301_b200 import inputs
+    flops = flops_per_gather(len(wl.modes))
+    rows = []
+    for lg in log2s:
+        n = 1 << lg
+        pos = inputs.positions(wl, n)
+        R, Z, phi = (torch.from_numpy(pos[k]).cuda() for k in ("R", "Z", "phi"))
+        del pos
+        cell = torch.empty(n, dtype=torch.int32, device="cuda")
+        ctx.locate(R, Z, cell=cell)
+        out = {k: torch.empty(n, dtype=torch.float64, device="cuda") for k in ("dphi", "dphi_dR", "dphi_dZ")}
+        for name in ("as drawn", "sorted by triangle"):
+            if name == "sorted by triangle":
+                order = torch.argsort(cell, stable=True)
+                R, Z, phi, cell = R[order].contiguous(), Z[order].contiguous(), phi[order].contiguous(), cell[order].contiguous()
+                del order
+            ts = []
+            for rep in range(3 + max(1, reps)):
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                ctx.gather(R, Z, phi, cell_hint=cell, want_dphi=False, out=out)
+                e1.record()
+                torch.cuda.synchronize()
+                if rep >= 3:
+                    ts.append(e0.elapsed_time(e1) * 1e-3)
+            t = sorted(ts)[len(ts) // 2]
+            rows.append({"markers": n, "order": name, "gathers_per_s": n / t, "ms": t * 1e3,
+                         "algorithmic_GBps": 52.0 * n / t * 1e-9, "frac_hbm": 52.0 * n / t * 1e-9 / hbm_peak,
+                         "algorithmic_TFLOPs": flops * n / t * 1e-12, "frac_fp64": flops * n / t * 1e-12 / fp64_peak})
+        del R, Z, phi, cell, out
+        torch.cuda.empty_cache()
+    return rows
+
+
 def run_gpu(args, wl):
+    import dataclasses
     import torch
     from paper_2601_14301_b200 import binding, inputs
     from paper_2601_14301_b200 import dist as D
@@ -189,140 +381,117 @@ def run_gpu(args, wl):
     binding.load()
 
     n = wl.n_markers
-    sort_every = max(1, min(args.sort_every, wl.nsteps))
-    ctx = binding.context_for(wl, inputs)
-    ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).to(dev), kind=0)
-    if args.push_kernel >= 0:
-        ctx.set_push_kernel(args.push_kernel)
-    m_np = inputs.markers(wl, n=n, seed=D.rank_seed(wl.seed, rank))
-    d = binding.markers_to_device(m_np, dev)
-    ctx.locate(d["R"], d["Z"], cell=d["cell"])
-    torch.cuda.synchronize()
+    run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank))
+    ctx = run.ctx
     fp64_peak = ctx.measure_fp64_peak()
     fp64_peak3 = ctx.measure_fp64_peak_operands(3)     # DFMA stream with three fresh register operands
     hbm_peak, hbm_src = load_peaks()
 
-    push_events = []
-    state = {"n_active": n}
-
-    def one_step(record: bool):
-        """One pass of the hot path over the batch; returns marker-steps done."""
-        units = 0
-        done = 0
-        n_act = state["n_active"]
-        while done < wl.nsteps:
-            k = min(sort_every, wl.nsteps - done)
-            if done == 0:
-                n_act, _ = ctx.compact(d, n=n_act)    # a6: drop lost markers once per step (syncs to return the count);
-            ctx.sort(d, n=n_act)                      # a1  (markers lost since sort to the end of the range and are skipped)
-            if record:
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record()
-            ctx.push(d, wl.dt, k, n=n_act)            # a2-a6, fused
-            if record:
-                e1.record()
-                push_events.append((e0, e1, n_act * k))
-            units += n_act * k
-            done += k
-        state["n_active"] = n_act
-        return units
-
-    for _ in range(args.warmup):
-        one_step(False)
-    torch.cuda.synchronize()
-    st0 = ctx.get_stats()
-    sampler = ClockSampler(local_rank)
-    D.barrier()
-    torch.cuda.synchronize()
-    sampler.start()
-    t_start, t_end = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    t_start.record()
-    units = 0
-    for _ in range(args.steps):
-        units += one_step(True)
-    t_end.record()
-    torch.cuda.synchronize()
-    D.barrier()
-    clocks = sampler.stop()
-    seconds = t_start.elapsed_time(t_end) * 1e-3
-    st1 = ctx.get_stats()
-    launches = st1["n_launches"] - st0["n_launches"]
+    res = run.run(args.steps, args.warmup, barrier=D.barrier, device_index=local_rank)
+    agg = D.aggregate(res["units"], res["seconds"], {"launches": res["launches"]}, device=dev)
     tile_counters = ctx.get_tile_counters()
 
-    agg = D.aggregate(units, seconds, {"launches": launches}, device=dev)
-
-    # roofline of the dominant kernel (push_kernel), from the live CUDA-event durations
-    push_s = sum(a.elapsed_time(b) for a, b, _ in push_events) * 1e-3
-    push_units = sum(u for _, _, u in push_events)
-    n_push = len(push_events)
-    flops = flops_per_marker_step(len(wl.modes)) * push_units
-    byts = bytes_per_marker_call(sort_every) * sum(u / max(1, min(sort_every, wl.nsteps)) for _, _, u in push_events)
-    t_fp64 = flops / (fp64_peak * 1e12)
-    t_hbm = byts / (hbm_peak * 1e9)
-    roof = {
-        "bound": "alu", "kernel": PUSH_KERNEL_NAMES.get(ctx.get_push_kernel(), "push kernel"),
-        "achieved": flops / push_s * 1e-12, "peak": fp64_peak, "unit": "TFLOP/s",
-        "frac": (flops / push_s * 1e-12) / fp64_peak,
+    roof = run.roofline(fp64_peak, res["seconds"])
+    flops_unit = flops_per_marker_step(len(wl.modes))
+    t_fp64 = flops_unit * roof["units_per_launch"] / (fp64_peak * 1e12)
+    t_hbm = bytes_per_marker_call(run.sort_every) * res["n_start"] / (hbm_peak * 1e9)
+    roof.update({
         "peak_source": "FP64 DFMA throughput measured live by trimeg_measure_fp64_peak (nominal 148 SM x 64 DFMA/clk x 2 x 1.965 GHz = 37.2)",
-        "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get((wl.name, ctx.get_push_kernel(), sort_every, n)),
-        "peak_three_register_operands": fp64_peak3, "frac_of_three_register_operand_peak": (flops / push_s * 1e-12) / fp64_peak3,
-        "peak_three_register_operands_note": "DFMA stream whose three source operands all change from one instruction to the "
-                                             "next (a Horner step over several markers): the FP64 pipe reads one 64-bit register "
-                                             "operand per cycle, so such a stream issues every 3 cycles instead of 2",
-        "algorithmic_flops_per_marker_step": flops_per_marker_step(len(wl.modes)),
-        "algorithmic_bytes_per_marker_call": bytes_per_marker_call(sort_every),
+        "traffic": PROFILED_DRAM_BYTES_PER_LAUNCH.get((wl.name, ctx.get_push_kernel(), run.sort_every, n)),
+        "peak_three_register_operands": fp64_peak3, "frac_of_three_register_operand_peak": roof["achieved"] / fp64_peak3,
+        "algorithmic_flops_per_marker_step": flops_unit,
+        "algorithmic_bytes_per_marker_call": bytes_per_marker_call(run.sort_every),
         "hbm_time_frac_of_fp64_time": t_hbm / t_fp64, "hbm_peak_gbs": hbm_peak, "hbm_peak_source": hbm_src,
-        "launches": n_push, "avg_launch_ms": push_s / max(1, n_push) * 1e3,
-        "push_share_of_step": push_s / seconds,
-        "tile_counters": tile_counters,
-    }
+        "schedule_counters": tile_counters,
+    })
 
-    line = None
-    if True:
-        # ---- e2e: host buffers through the C ABI, copies inside the timed region
-        e2e = None
-        if not args.no_e2e:
-            h = {k: torch.from_numpy(m_np[k]).pin_memory() for k in ("R", "Z", "phi", "vpar", "mu", "w")}
-            h["cell"] = torch.full((n,), -1, dtype=torch.int32).pin_memory()
-            ctx.push_host(h, wl.dt, wl.nsteps, locate_first=True)          # warm-up (also allocates)
+    # ---- the bench checks what it timed: finiteness of the timed batch, a fresh strided sample against the oracle
+    check = None
+    if rank == 0 and not args.no_check:
+        check = run.check_against_oracle(stride=max(1, n // 4096))
+
+    # ---- e2e: host buffers through the C ABI, copies inside the timed region
+    e2e = None
+    if not args.no_e2e:
+        m_np = run.m_np
+        keys = ("R", "Z", "phi", "vpar", "mu", "w")
+        h0 = {k: torch.from_numpy(m_np[k]) for k in keys}
+        h = {k: torch.empty_like(h0[k]).pin_memory() for k in keys}
+        h["cell"] = torch.empty(n, dtype=torch.int32).pin_memory()
+        k_e2e = max(1, min(args.steps, 3))
+        e2e_s, e2e_units = 0.0, 0
+        for it in range(1 + k_e2e):                       # first call: warm-up (also allocates)
+            for k in keys:
+                h[k].copy_(h0[k])                         # every call starts from the config's initial state (untimed)
+            h["cell"].fill_(-1)
             D.barrier()
             torch.cuda.synchronize()
-            k_e2e = max(1, min(args.steps, 3))
-            n_in = int((h["cell"] >= 0).sum())                            # markers still inside after the warm-up call
-            lost0 = ctx.get_stats()["n_lost"]
             t0 = time.perf_counter()
-            e2e_units = 0
-            for _ in range(k_e2e):
-                ctx.push_host(h, wl.dt, wl.nsteps, locate_first=False)     # returns when the results are in the host buffers
-                e2e_units += n_in * wl.nsteps
-                lost1 = ctx.get_stats()["n_lost"]                         # markers flagged lost leave the count of the next step
-                n_in -= lost1 - lost0
-                lost0 = lost1
-            torch.cuda.synchronize()
-            e2e_s = time.perf_counter() - t0
-            ag2 = D.aggregate(e2e_units, e2e_s, {}, device=dev)
-            e2e = {"value": ag2["value"], "unit": UNIT, "h2d_bytes_per_step": n * (6 * 8 + 4),
-                   "d2h_bytes_per_step": n * (5 * 8 + 4), "steps": k_e2e,
-                   "api": "trimeg_push_host (pinned host SoA in: H2D -> locate/sort of the whole batch -> push -> unsort -> D2H)"}
+            ctx.push_host(h, wl.dt, wl.nsteps, locate_first=True)     # returns when the results are in the host buffers
+            dt_call = time.perf_counter() - t0
+            if it > 0:
+                e2e_s += dt_call
+                e2e_units += int((h["cell"] >= 0).sum()) * wl.nsteps  # markers lost on the way count zero steps
+        ag2 = D.aggregate(e2e_units, e2e_s, {}, device=dev)
+        e2e = {"value": ag2["value"], "unit": UNIT, "h2d_bytes_per_step": n * 6 * 8,
+               "d2h_bytes_per_step": n * (5 * 8 + 4), "steps": k_e2e, "frac_of_device_value": ag2["value"] / agg["value"],
+               "api": "trimeg_push_host (pinned host SoA in: chunks of the batch go H2D -> locate -> cell sort -> push, re-sort "
+                      "every 10 steps -> unsort -> D2H on three streams, copies under the push of other chunks)"}
+        del h, h0
+        ctx.release_host_buffers()
 
-        cpu = None
-        if rank == 0 and world == 1 and not args.no_cpu_baseline:
-            v, cores, desc, _, _, _ = time_oracle(wl, 15.0)
-            cpu = {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc}
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        r = time_oracle(wl, run.m_np, 15.0, one_core_seconds=6.0)
+        cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "nproc": r["nproc"], "kind": "oracle", "sample": r["sample"],
+               "value_one_core": r.get("value_one_core"), "sample_one_core": r.get("sample_one_core"),
+               "note": "the oracle is the unoptimised correctness checker (plain monomial sums, gcc -O2): a baseline, not a "
+                       "tuned CPU push; the GPU/oracle ratio is not a like-for-like speedup"}
+    run.close()
 
-        if rank == 0:
-            line = {
-                "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
-                "warmup": args.warmup, "ms_per_step": agg["seconds"] / args.steps * 1e3, "higher_is_better": True,
-                "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-                "config": workload_config(wl, extra={"sort_every": sort_every, "parallelism": f"marker-shard x{world}",
-                                                     "lost_markers": st1["n_lost"]}),
-                "clocks": clocks, "e2e": e2e, "gpu_launches": int(agg["launches"]),
-                "roofline": roof, "cpu_baseline": cpu,
-                "paper_context": "thesis K1 (one RHS eval, EM, B-spline equilibrium): 1.5e8 marker-RHS/s on 1 H100 "
-                                 "(PAPER.md:911) ~ 3.8e7 RK4-step equivalents/s; other hardware, not like-for-like",
-            }
-            print(json.dumps(line), flush=True)
+    # ---- the other configs, device-timed the same way (N = 1 only): short runs, same live peaks
+    sweep = None
+    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers:
+        sweep = {}
+        for name in ("cfg2", "cfg3"):
+            w2 = inputs.WORKLOADS[name]
+            r2 = PushRun(w2, args.sort_every, -1, keep_host=True)
+            out = r2.run(2, 3)
+            rf = r2.roofline(fp64_peak, out["seconds"])
+            chk = None if args.no_check else r2.check_against_oracle(stride=max(1, w2.n_markers // 2048))
+            sweep[name] = {"value": out["units"] / out["seconds"], "unit": UNIT, "steps": 2, "warmup": 3,
+                           "ms_per_step": out["seconds"] / 2 * 1e3, "kernel": rf["kernel"], "frac": rf["frac"],
+                           "achieved_tflops": rf["achieved"], "avg_launch_ms": rf["avg_launch_ms"],
+                           "push_share_of_step": rf["push_share_of_step"], "clocks": out["clocks"],
+                           "config": workload_config(w2, extra={"sort_every": r2.sort_every}), "oracle_check": chk}
+            r2.close()
+            del r2
+        w4 = inputs.WORKLOADS["cfg4"]
+        c4 = binding.context_for(w4, inputs)
+        c4.field_upload(w4.modes, torch.from_numpy(inputs.field_dofs(w4)).cuda(), kind=0)
+        sampler = ClockSampler(local_rank)
+        sampler.start()
+        rows = gather_rows(c4, w4, (24, 28), 2, hbm_peak, fp64_peak)
+        sweep["cfg4"] = {"metric": "field gathers/sec (dphi, d/dR, d/dZ; 3 toroidal modes)", "unit": "gathers/s",
+                         "algorithmic_bytes_per_gather": 52, "algorithmic_flops_per_gather": flops_per_gather(len(w4.modes)),
+                         "rows": rows, "clocks": sampler.stop(), "config": workload_config(w4)}
+        c4.close()
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": agg["seconds"] / args.steps * 1e3, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(wl, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
+                                                 "lost_markers_per_step": res["lost_per_step"],
+                                                 "unit_count": "every bench step restarts from the config's initial state; a marker "
+                                                               "that leaves the mesh during a step counts zero steps for it"}),
+            "clocks": res["clocks"], "e2e": e2e, "gpu_launches": int(agg["launches"]),
+            "roofline": roof, "cpu_baseline": cpu, "oracle_check": check, "config_sweep": sweep,
+            "paper_context": "thesis K1 (one RHS eval, EM, B-spline equilibrium): 1.5e8 marker-RHS/s on 1 H100 "
+                             "(PAPER.md:911) ~ 3.8e7 RK4-step equivalents/s; other hardware, not like-for-like",
+        }
+        print(json.dumps(line), flush=True)
     return 0
 
 
@@ -339,34 +508,10 @@ def run_gather_sweep(args, wl):
     ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
     hbm_peak, _ = load_peaks()
     fp64_peak = ctx.measure_fp64_peak()
-    flops = 25 + 170 * len(wl.modes) + 6                       # gather-only work per marker
-    rows = []
-    for lg in range(16, args.max_log2 + 1, 2):
-        n = 1 << lg
-        m = inputs.markers(wl, n=n)
-        R, Z, phi = (torch.from_numpy(m[k]).cuda() for k in ("R", "Z", "phi"))
-        cell = torch.empty(n, dtype=torch.int32, device="cuda")
-        ctx.locate(R, Z, cell=cell)
-        order = torch.argsort(cell, stable=True)
-        out = {k: torch.empty(n, dtype=torch.float64, device="cuda") for k in ("dphi", "dphi_dR", "dphi_dZ")}
-        for name, idx in (("as drawn", None), ("sorted by triangle", order)):
-            r, z, p = (R, Z, phi) if idx is None else (R[idx].contiguous(), Z[idx].contiguous(), phi[idx].contiguous())
-            ts = []
-            for rep in range(3 + max(1, args.steps)):
-                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-                e0.record()
-                ctx.gather(r, z, p, want_dphi=False, out=out)
-                e1.record()
-                torch.cuda.synchronize()
-                if rep >= 3:
-                    ts.append(e0.elapsed_time(e1) * 1e-3)
-            t = sorted(ts)[len(ts) // 2]
-            rows.append({"markers": n, "order": name, "gathers_per_s": n / t, "ms": t * 1e3,
-                         "algorithmic_GBps": 48.0 * n / t * 1e-9, "algorithmic_TFLOPs": flops * n / t * 1e-12})
-        del R, Z, phi, cell, order, out
+    rows = gather_rows(ctx, wl, range(16, args.max_log2 + 1, 2), args.steps, hbm_peak, fp64_peak)
     line = {"metric": "field gathers/sec (dphi, d/dR, d/dZ; 3 toroidal modes)", "unit": "gathers/s", "n_gpus": 1,
             "config": workload_config(wl), "dtype": "f64", "data": "synthetic", "hbm_peak_gbs": hbm_peak, "fp64_peak_tflops": fp64_peak,
-            "algorithmic_bytes_per_gather": 48, "algorithmic_flops_per_gather": flops, "rows": rows}
+            "algorithmic_bytes_per_gather": 52, "algorithmic_flops_per_gather": flops_per_gather(len(wl.modes)), "rows": rows}
     print(json.dumps(line), flush=True)
     return 0
 
@@ -381,9 +526,11 @@ def main():
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
-    ap.add_argument("--max-log2", type=int, default=26, help="cfg4 gather sweep: largest marker count 2^k")
+    ap.add_argument("--max-log2", type=int, default=28, help="cfg4 gather sweep: largest marker count 2^k")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the short device-timed runs of cfg2, cfg3, cfg4 (config_sweep)")
+    ap.add_argument("--no-check", action="store_true", help="skip the oracle check of a strided sample after the timed steps")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     from paper_2601_14301_b200 import inputs

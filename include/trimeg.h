@@ -25,8 +25,9 @@
  *     enqueued on it and the call returns without synchronising, except where stated.
  *   - Tables (mesh geometry, coefficient table) are owned by the context, uploaded once
  *     ("allocate once, upload static data once").
- *   - One context per GPU (cudaSetDevice before trimeg_mesh_create); a context is not
- *     thread-safe.  There is no CPU fallback: without a CUDA device calls return
+ *   - One context per GPU (cudaSetDevice before trimeg_mesh_create); every later call runs on
+ *     the context's device whatever device is current, and restores the caller's device.  Several
+ *     contexts (on one or several GPUs) may live in one process; a context is not thread-safe.  There is no CPU fallback: without a CUDA device calls return
  *     TRIMEG_ERR_CUDA.
  */
 #ifndef TRIMEG_H
@@ -108,6 +109,10 @@ int trimeg_mesh_download_geom(trimeg_ctx *ctx, double *geom_dev, trimeg_stream s
  *   kind 1: data_dev = coefficients [n_tri][n_modes][21] complex128, degree-major monomial
  *           order k <-> (i, j): for d = 0..5, for j = 0..d: xi^(d-j) eta^j.
  * mode_n_host: n_modes toroidal mode numbers.  n_modes = 0 is legal (dphi == 0).
+ * Ordering: the table is (re)written on `stream`.  A gather / rhs / push that the caller enqueued
+ * earlier on ANOTHER stream may still be reading it: order uploads and pushes on one stream (or
+ * with events).  trimeg_push_host waits for the upload by itself.  A change of n_modes
+ * re-allocates the table and synchronises the device.
  * Errors: INVALID_ARG, ALLOC, CUDA. */
 int trimeg_field_upload(trimeg_ctx *ctx, int n_modes, const int *mode_n_host,
                         const void *data_dev, int kind, trimeg_stream stream);
@@ -123,8 +128,13 @@ int trimeg_locate(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, i
                   trimeg_stream stream);
 
 /* ---- gather only (row a3; BASELINE.json configs[3]) ----------------------------------------
+ * The grid-to-particle interpolation on its own ("field gathering/interpolation";
+ * PAPER.md:608 section 5.1: "the electrostatic scalar potential needs to always be computed"; the
+ * g2p subroutine of the pullback / density / g2p2g kernels):
  * dphi, d dphi/dR, d dphi/dZ (and d dphi/dphi if dphi_dphi != NULL) at the markers.
- * cell_hint may be NULL.  Markers outside the mesh get 0.  NO_FIELD if no field is loaded. */
+ * cell_hint may be NULL.  Markers outside the mesh get 0.  NO_FIELD if no field is loaded.
+ * Any marker order is correct; cell-sorted markers (trimeg_sort) with their cells as hint take the
+ * warp-grouped kernel (several markers of one triangle share each coefficient load). */
 int trimeg_gather(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, const double *phi,
                   const int32_t *cell_hint, double *dphi, double *dphi_dR, double *dphi_dZ,
                   double *dphi_dphi, trimeg_stream stream);
@@ -137,6 +147,9 @@ int trimeg_rhs(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, double *dRdt,
                double *dphidt, double *dvpardt, double *dwdt, trimeg_stream stream);
 
 /* ---- cell sort (row a1) ---------------------------------------------------------------------
+ * Why: the thesis's kernel reads the field tables with 18 % of its accesses coalesced and leaves the
+ * on-chip shared memory unused (section 6.4); with the markers ordered by triangle the
+ * lanes of a warp read the same coefficient record and the record can be staged on chip.
  * Counting sort of the markers by cell (markers with cell < 0 go last).  Permutes all seven
  * arrays in place.  perm_dev (int64[n], may be NULL) receives, for every new position, the
  * old index.  The order inside one cell is unspecified.  Uses context-owned scratch of
@@ -145,57 +158,68 @@ int trimeg_sort(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_dev,
                 trimeg_stream stream);
 
 /* ---- compaction of the active list (row a6) -------------------------------------------------
- * Stable partition: markers with cell >= 0 first (original order kept), lost markers after
- * them.  *n_active_host receives the number of active markers (the call synchronises the
- * stream to return it).  perm_dev as in trimeg_sort. */
+ * Markers evolve independently of each other (section 5.1), so a marker that has left
+ * the mesh (lost-marker rule of trimeg_push, reading G18) can be dropped from the active range
+ * without touching the others.  Stable partition: markers with cell >= 0 first (original order
+ * kept), lost markers after them.  *n_active_host receives the number of active markers (the call
+ * synchronises the stream to return it).  perm_dev as in trimeg_sort. */
 int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_dev,
                    size_t *n_active_host, trimeg_stream stream);
 
 /* ---- the push (rows a2-a6) ------------------------------------------------------------------
- * nsteps classic RK4 steps of size dt on y = (R, Z, phi, vpar, w), mu constant, with the
- * field frozen; four locate + gather + equilibrium + RHS evaluations per step, all in one
- * kernel.  After each step phi is wrapped to [0, 2 pi) and cell is set to the triangle of the
- * new position.  A marker whose any stage position, or new position, is outside the mesh is
- * restored to its start-of-step state, flagged cell = -1 and skipped from then on; it keeps
- * its index (use trimeg_compact to drop it).  Markers are not reordered. */
+ * nsteps classic RK4 steps of size dt on y = (R, Z, phi, vpar, w), mu constant, with
+ * the field frozen; four locate + gather + equilibrium + RHS evaluations per step (the thesis's push
+ * kernel), all in one kernel.  After each step phi is wrapped to [0, 2 pi) and
+ * cell is set to the triangle of the new position.  A marker whose any stage position, or new
+ * position, is outside the mesh is restored to its start-of-step state, flagged cell = -1 and skipped
+ * from then on (reading G18); it keeps its index (use trimeg_compact to drop it).  Markers are not
+ * reordered.  INVALID_ARG for a NaN dt or nsteps < 0. */
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
-/* Kernel used by trimeg_push / trimeg_push_host (same results, different schedules):
- *  -1  (TRIMEG_PUSH_KERNEL_AUTO, the default) variant 8 for a field of up to 4 toroidal modes, variant 7 for 12 to 26,
- *      else variant 1;
- *   0  one thread per marker, state in registers, coefficients through L1;
- *   1, 2  warp-autonomous: every warp owns 32 P - slack markers (state in shared memory), groups them by
- *         triangle with ballots (anew only at a stage where one of them has changed its triangle) and evaluates P markers of one triangle per lane off a
- *         single load of each coefficient (through L1), finishes and re-locates them without any block
- *         barrier (1: P = 2; 2: P = 4);
- *   3..6  CTA tiles with resident coefficient records: a CTA owns a tile of markers (state in
- *         shared memory), keeps the coefficient records of the tile's triangles in shared memory between
- *         stages and steps, re-bins the markers by triangle at every stage and evaluates + finishes P
- *         markers of one triangle per thread (3: P = 2, 384 threads; 4: P = 3, 256; 5: P = 4, 256;
- *         6: P = 2, 192 threads, two CTAs per SM).
- *   7  warp-autonomous like 1 (P = 2, 12 warps per CTA), with the coefficient records of the CTA's triangles in a shared,
- *         insert-only hash table in shared memory: the first warp that meets a triangle copies its record in, the others
- *         find it there; the warps meet at a barrier every tenth step only (to empty the table when it is nearly full).
- *   8  variant 1 compiled for 128 registers per thread (16 instead of 12 warps per SM): better when the Horner loop is
- *         short (few modes) and the latency-bound rest of the stage weighs more.
+/* Schedule used by trimeg_push / trimeg_push_host (same results, different kernels):
+ *  TRIMEG_PUSH_KERNEL_AUTO (the default)  WARP128 for a field of up to 4 toroidal modes, WCACHE for 12 to 26, else WARP;
+ *  TRIMEG_PUSH_KERNEL_THREAD   one thread per marker, state in registers, coefficients through L1 (the plain schedule);
+ *  TRIMEG_PUSH_KERNEL_WARP     warp-autonomous: every warp owns 58 markers (state in shared memory), groups them by
+ *         triangle with ballots (anew only at a stage where one of them has changed its triangle) and evaluates 2 markers
+ *         of one triangle per lane off a single load of each coefficient (through L1), finishes and re-locates them
+ *         without any block barrier;
+ *  TRIMEG_PUSH_KERNEL_WARP128  the same compiled for 128 registers per thread (16 instead of 12 warps per SM): better
+ *         when the Horner loop is short (few modes) and the latency-bound rest of the stage weighs more;
+ *  TRIMEG_PUSH_KERNEL_WCACHE   warp-autonomous like WARP (12 warps per CTA, one CTA per SM), with the coefficient records
+ *         of the CTA's triangles in a shared, insert-only hash table in shared memory: the first warp that meets a
+ *         triangle copies its record in, the others find it there; the warps meet at a barrier every tenth step only.
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
- * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX. */
+ * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX.  (The lock-step CTA-tile schedules of round 1 were
+ * removed: git history, commit 3003ca4, has them.) */
 #define TRIMEG_PUSH_KERNEL_AUTO (-1)
-#define TRIMEG_PUSH_KERNEL_MAX 8
+#define TRIMEG_PUSH_KERNEL_THREAD 0
+#define TRIMEG_PUSH_KERNEL_WARP 1
+#define TRIMEG_PUSH_KERNEL_WARP128 2
+#define TRIMEG_PUSH_KERNEL_WCACHE 3
+#define TRIMEG_PUSH_KERNEL_MAX 3
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 /* The variant trimeg_push will launch (AUTO resolved for the uploaded field; otherwise the TRIMEG_PUSH_KERNEL
- * environment override at context creation or the last trimeg_set_push_kernel); -2 for a NULL context. */
+ * environment override at context creation -- ignored unless it parses as an integer in range -- or the last
+ * trimeg_set_push_kernel); -2 for a NULL context. */
 int trimeg_get_push_kernel(const trimeg_ctx *ctx);
 
 /* ---- end-to-end push from HOST buffers -------------------------------------------------------
- * Same result as: copy the seven arrays to the device, trimeg_locate if locate_first != 0,
- * trimeg_sort, trimeg_push, undo the sort, copy R, Z, phi, vpar, w, cell back.  `m` holds
- * HOST pointers (pinned memory makes the copies asynchronous).  The whole batch is made resident and
- * cell-sorted as one set (the push kernels live on markers per triangle), re-sorted every 10 steps, and
- * returned in the caller's order; the device buffers (2 marker sets + 3 permutations, 128 B per marker)
- * stay allocated in the context.  Synchronises before returning. */
+ * The thesis's offloading strategy (section 5.5): device memory is allocated once and
+ * kept, static tables are uploaded once, only the marker arrays travel.  Same result as: copy the seven
+ * arrays to the device, trimeg_locate if locate_first != 0, trimeg_sort, trimeg_push, undo the sort, copy
+ * R, Z, phi, vpar, w, cell back.  `m` holds HOST pointers (pinned memory makes the copies asynchronous).
+ * The batch is cut into up to 8 chunks of consecutive markers (at least ~100 markers per triangle each);
+ * every chunk is copied in, located, cell-sorted, pushed with a re-sort every 10 steps, unsorted and copied
+ * out on three streams of the context, so that the copies of one chunk run under the push of another.
+ * Results are returned in the caller's order and do not depend on the chunking.  The device buffers
+ * (2 marker sets + 3 permutations, 128 B per marker) stay allocated in the context until
+ * trimeg_release_host_buffers or trimeg_mesh_destroy.  Waits for the last trimeg_field_upload of the
+ * context; synchronises before returning.  INVALID_ARG for a NaN dt. */
 int trimeg_push_host(trimeg_ctx *ctx, trimeg_markers *m_host, size_t n, double dt, int nsteps,
                      int locate_first);
+/* Frees the device buffers kept by trimeg_push_host / trimeg_sort / trimeg_compact (they are
+ * re-allocated on demand).  Synchronises the device. */
+int trimeg_release_host_buffers(trimeg_ctx *ctx);
 
 /* ---- statistics ------------------------------------------------------------------------------
  * Totals since context creation (or the last reset): markers flagged lost by trimeg_push,
@@ -203,16 +227,12 @@ int trimeg_push_host(trimeg_ctx *ctx, trimeg_markers *m_host, size_t n, double d
  * Synchronises the device.  Any pointer may be NULL. */
 int trimeg_get_stats(trimeg_ctx *ctx, int64_t *n_lost, int64_t *n_relocated, int64_t *n_launches);
 int trimeg_reset_stats(trimeg_ctx *ctx);
-/* Diagnostics of the shared-memory push kernels since the last reset, out8[0..7] (host).  out8[0..4]: SM
- * cycles of thread 0 of every CTA (lane 0 of every warp for variants 1, 2), summed over CTAs --
- * variants 3..6: [0] evaluation head (local coordinates, toroidal phases), [1] phase B (record copies, bin
- * scan, scatter to slots, barrier), [2] table reset, [3] the mode loop (batched Horner), [4] finishing
- * the markers, binning for the next stage and the wait at the barrier; variants 1, 2: [0] grouping,
- * [1] a count, not cycles: the stages at which a warp had to group its markers anew,
- * [3] evaluation + finishing, [4] markers without a slot; variants 7, 8 as 1, 2 (7: [0] includes the record lookups).
- * out8[5]: markers evaluated by the one-marker
- * path; out8[6]: coefficient records copied to shared memory (3..7) or bins formed (1, 2); out8[7]: RK4
- * stages run, summed over CTAs (warps).  Synchronises the device.  DESIGN.md section 5. */
+/* Schedule diagnostics of the warp kernels since the last reset, out8[0..7] (host), summed over warps:
+ * [1] stages at which a warp had to group its markers by triangle anew; [5] markers evaluated by the
+ * one-marker path; [6] coefficient records copied to shared memory (WCACHE) or triangle groups formed (WARP);
+ * [7] RK4 stages run.  [0], [3], [4]: SM cycles of lane 0 spent grouping (+ record lookups), evaluating +
+ * finishing, and on markers without a slot -- only in a library built with -DTRIMEG_PROFILE
+ * (python -m paper_2601_14301_b200.build --profile), else 0.  Synchronises the device. */
 int trimeg_get_tile_counters(trimeg_ctx *ctx, int64_t *out8_host);
 
 /* ---- diagnostics ------------------------------------------------------------------------------

@@ -19,12 +19,14 @@ EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_sort", "trimeg_compact",
-    "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
+    "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
     "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
 )
 
 OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC = 0, -1, -2, -3, -4, -5
-PUSH_KERNEL_AUTO = -1          # TRIMEG_PUSH_KERNEL_AUTO of include/trimeg.h
+# TRIMEG_PUSH_KERNEL_* of include/trimeg.h
+PUSH_KERNEL_AUTO, PUSH_KERNEL_THREAD, PUSH_KERNEL_WARP, PUSH_KERNEL_WARP128, PUSH_KERNEL_WCACHE = -1, 0, 1, 2, 3
+PUSH_KERNELS = (PUSH_KERNEL_THREAD, PUSH_KERNEL_WARP, PUSH_KERNEL_WARP128, PUSH_KERNEL_WCACHE)
 
 
 class TrimegError(RuntimeError):
@@ -73,6 +75,7 @@ def load() -> C.CDLL:
     L.trimeg_push.argtypes = [vp, C.POINTER(trimeg_markers), sz, dbl, i32, vp]
     L.trimeg_set_push_kernel.argtypes = [vp, i32]
     L.trimeg_push_host.argtypes = [vp, C.POINTER(trimeg_markers), sz, dbl, i32, i32]
+    L.trimeg_release_host_buffers.argtypes = [vp]
     L.trimeg_get_stats.argtypes = [vp, C.POINTER(C.c_int64), C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
     L.trimeg_reset_stats.argtypes = [vp]
     L.trimeg_get_tile_counters.argtypes = [vp, C.POINTER(C.c_int64)]
@@ -259,6 +262,9 @@ class Context:
         _check(self.L.trimeg_push_host(self.h, C.byref(ms), n, float(dt), int(nsteps), int(bool(locate_first))),
                "trimeg_push_host")
 
+    def release_host_buffers(self):
+        _check(self.L.trimeg_release_host_buffers(self.h), "trimeg_release_host_buffers")
+
     def get_stats(self) -> Dict[str, int]:
         a, b, c = C.c_int64(0), C.c_int64(0), C.c_int64(0)
         _check(self.L.trimeg_get_stats(self.h, C.byref(a), C.byref(b), C.byref(c)), "trimeg_get_stats")
@@ -278,7 +284,7 @@ class Context:
     def get_tile_counters(self) -> Dict[str, int]:
         a = (C.c_int64 * 8)()
         _check(self.L.trimeg_get_tile_counters(self.h, a), "trimeg_get_tile_counters")
-        names = ("cyc_head", "cyc_B", "cyc_C", "cyc_modes", "cyc_finish", "n_fallback", "n_records", "n_stages")
+        names = ("cyc_group", "n_regroup", "unused", "cyc_eval", "cyc_noslot", "n_fallback", "n_records", "n_stages")
         return {k: int(v) for k, v in zip(names, a)}
 
     def reset_stats(self):

@@ -6,7 +6,7 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtrimeg.so")
-SOURCES = ["trimeg_lib.cu", "trimeg_push.cu", "trimeg_push_warp.cu", "trimeg_push_fused.cu", "trimeg_push_wcache.cu"]
+SOURCES = ["trimeg_lib.cu", "trimeg_push.cu", "trimeg_push_warp.cu", "trimeg_push_wcache.cu"]
 DEPS = SOURCES + ["trimeg_device.cuh", "trimeg_multi.cuh", "trimeg_rk4.cuh", "trimeg_internal.h", "bell_tables.inc", os.path.join("..", "..", "include", "trimeg.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-ffp-contract=off", "-shared"]
@@ -19,15 +19,17 @@ def nvcc() -> str:
     raise RuntimeError("nvcc not found")
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, profile: bool = False) -> str:
+    """profile: compile the in-kernel clock64 phase timers of the warp kernels in (-DTRIMEG_PROFILE)."""
     deps = [os.path.join(CSRC, d) for d in DEPS]
-    if not force and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
+    profile = profile or os.environ.get("TRIMEG_PROFILE", "") not in ("", "0")
+    if not force and not profile and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (["-DTRIMEG_PROFILE"] if profile else []) + \
           ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
     return LIB
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv, profile="--profile" in sys.argv))

@@ -38,6 +38,7 @@ struct PhysDev {
     double rho0B0;                  // numerator of C_E
     double qom;                     // q_s / m_s
     double invT, kappa_n, kappa_T;
+    double R0sq, m2qs, invT2;       // R0^2, -2 qs, 2 / T
     int eom_variant, weight_mode;
 };
 
@@ -277,6 +278,25 @@ __device__ __forceinline__ FieldVal gather(const FieldDev &F, int t, const Bary 
 }
 
 // ------------------------------------------------------------------- a4 + a5 equilibrium, RHS
+// Reciprocal and reciprocal square root without the IEEE division sequence: the hardware's 20-bit table seed
+// (MUFU.RCP64H / MUFU.RSQ64H, which runs beside the FP64 pipe) and ONE third-order correction step
+// (2^-20 -> 2^-60 relative), branch-free: 3 (5) FP64 instructions instead of ~12 with a slow-path test.  The result is
+// within ~1.5 ulp of the exact value (parity bar 1e-12).  Arguments are normal positive numbers here (R, q, g, B*_par, s).
+__device__ __forceinline__ double rcp_fast(double x)
+{
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-x, y, 1.0);
+    return fma(y, fma(e, e, e), y);                      // y (1 + e + e^2)
+}
+__device__ __forceinline__ double rsqrt_fast(double x)
+{
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double e = fma(-(x * y), y, 1.0);
+    return fma(y, e * fma(0.375, e, 0.5), y);            // y (1 + e/2 + 3 e^2/8)
+}
+
 // Analytic circular equilibrium: psi' = B0 r / q(r), F = B0 R0 (G11), B = grad psi x grad phi
 // + F grad phi; b0* (A.4-A.6), equilibrium drifts (A.10-A.13, sign of
 // A.11 per G1), E x B and parallel acceleration (A.14-A.17 with dA = 0, G3), weight rate from
@@ -289,58 +309,64 @@ __device__ __forceinline__ Rates rhs_point(const PhysDev &p, double R, double Z,
     const double x = R - p.R0;
     const double s = fma(x, x, Z * Z);
     const double qb = fma(p.qs, s, p.q0);
-    const double iq = 1.0 / qb;
+    const double iq = rcp_fast(qb);
     const double iq2 = iq * iq;
-    const double g = fma(s, iq2, p.R0 * p.R0);
-    const double gs = iq2 * fma(-2.0 * s * p.qs, iq, 1.0);
-    const double isg = rsqrt(g);
+    const double g = fma(s, iq2, p.R0sq);
+    const double gs = iq2 * fma(s * p.m2qs, iq, 1.0);    // dg/ds = 1/q^2 - 2 s q_s/q^3
+    const double isg = rsqrt_fast(g);
     const double sg = g * isg;
     const double ig = isg * isg;
     const double h = iq * isg;
     const double hs = -h * fma(0.5 * gs, ig, p.qs * iq);
-    const double iR = 1.0 / R;
-    const double B = p.B0 * sg * iR;
-    const double iB = R * isg * p.invB0;
-    const double BiR = p.B0 * iR;
-    const double BR = -BiR * Z * iq, BZ = BiR * x * iq, Bphi = BiR * p.R0;
+    const double iR = rcp_fast(R);
+    const double u = p.B0 * iR;                          // B0 / R
+    const double B = u * sg;
+    const double iB = (R * p.invB0) * isg;
+    const double uq = u * iq;                            // B_Z = uq x, B_R = -uq Z
     const double bR = -Z * h, bZ = x * h, bphi = p.R0 * isg;
-    const double dBdR = p.B0 * iR * fma(gs * x, isg, -sg * iR);
-    const double dBdZ = p.B0 * iR * gs * Z * isg;
-    const double dbphi_c = -p.R0 * gs * ig * isg;        // d b_phi / d s * 2 ... times x or Z
-    const double curlR = -dbphi_c * Z;                   // -(d b_phi/dZ)
-    const double curlZ = fma(dbphi_c, x, bphi * iR);     //  d b_phi/dR + b_phi/R
-    const double curlP = -2.0 * (h + s * hs);            //  d b_R/dZ - d b_Z/dR
+    const double gsi = gs * isg;
+    const double ug = u * gsi;
+    const double dBdZ = ug * Z;
+    const double dBdR = fma(ug, x, -(B * iR));
+    const double dc = -(p.R0 * gsi) * ig;                // d b_phi / d s * 2 ... times x or Z
+    const double curlR = -dc * Z;                        // -(d b_phi/dZ)
+    const double curlZ = fma(dc, x, bphi * iR);          //  d b_phi/dR + b_phi/R
+    const double curlP = -2.0 * fma(s, hs, h);           //  d b_R/dZ - d b_Z/dR
     const double bcurlb = fma(bR, curlR, fma(bZ, curlZ, bphi * curlP));
-    const double Bsp = fma(p.eps * vpar, bcurlb, B);     // B*_par
-    const double iBsp = 1.0 / Bsp;
-    const double lead = (p.eom_variant == 1) ? B * iBsp : 1.0;
-    const double k = p.eps * vpar * iBsp;
-    const double b0R = fma(lead, bR, k * curlR);
-    const double b0Z = fma(lead, bZ, k * curlZ);
-    const double b0P = fma(lead, bphi, k * curlP);
-    const double Cd = p.eps * mu * iB * iBsp;
+    const double ev = p.eps * vpar;
+    const double Bsp = fma(ev, bcurlb, B);               // B*_par
+    const double iBsp = rcp_fast(Bsp);
+    const double k = ev * iBsp;
+    double b0R, b0Z, b0P;
+    if (p.eom_variant == 1) {
+        const double lead = B * iBsp;
+        b0R = fma(lead, bR, k * curlR); b0Z = fma(lead, bZ, k * curlZ); b0P = fma(lead, bphi, k * curlP);
+    } else {
+        b0R = fma(k, curlR, bR); b0Z = fma(k, curlZ, bZ); b0P = fma(k, curlP, bphi);
+    }
+    const double Cd = ((p.eps * mu) * iB) * iBsp;
     const double CE = p.rho0B0 * iBsp;
-    const double CdBphi = Cd * Bphi;
+    const double CdBphi = Cd * (u * p.R0);
     const double R0dot = fma(b0R, vpar, CdBphi * dBdZ);
     const double Z0dot = fma(b0Z, vpar, -CdBphi * dBdR);
-    const double P0dot = iR * fma(b0P, vpar, Cd * fma(BZ, dBdR, -BR * dBdZ));
+    const double P0 = fma(b0P, vpar, (Cd * uq) * fma(x, dBdR, Z * dBdZ));     // R dphi/dt, equilibrium part (B_Z dB/dR - B_R dB/dZ = uq (x dB/dR + Z dB/dZ))
     const double v0dot = -mu * fma(b0R, dBdR, b0Z * dBdZ);
     const double fP_R = fld.fphi * iR;                   // (1/R) d dphi / d phi
     const double dRdot = CE * fma(bphi, fld.fZ, -bZ * fP_R);
     const double dZdot = CE * fma(-bphi, fld.fR, bR * fP_R);
-    const double dPdot = CE * iR * fma(bZ, fld.fR, -bR * fld.fZ);
+    const double dP = fma(bZ, fld.fR, -bR * fld.fZ);     // R dphi/dt / C_E, perturbed part
     const double dvdot = -p.qom * fma(b0R, fld.fR, fma(b0Z, fld.fZ, b0P * fP_R));
-    const double ir = (s > 0.0) ? rsqrt(s) : 0.0;
+    const double ir = (s > 1e-300) ? rsqrt_fast(s) : 0.0;
     const double drdot = fma(dRdot, x, dZdot * Z) * ir;
-    const double en = fma(vpar * vpar, p.invT, fma(2.0 * mu * B, p.invT, -1.5));
+    const double en = fma(vpar * vpar, p.invT, fma(mu * B, p.invT2, -1.5));
     const double L = fma(drdot, -fma(en, p.kappa_T, p.kappa_n),
-                         fma(-2.0 * mu * p.invT, fma(dRdot, dBdR, dZdot * dBdZ), -2.0 * vpar * p.invT * dvdot));
+                         fma(-(mu * p.invT2), fma(dRdot, dBdR, dZdot * dBdZ), -(vpar * p.invT2) * dvdot));
     Rates o;
     o.R = R0dot + dRdot;
     o.Z = Z0dot + dZdot;
-    o.phi = P0dot + dPdot;
+    o.phi = iR * fma(CE, dP, P0);
     o.vpar = v0dot + dvdot;
-    o.w = (p.weight_mode == 0) ? -(1.0 - w) * L : -L;
+    o.w = (p.weight_mode == 0) ? (w - 1.0) * L : -L;
     return o;
 }
 

@@ -22,8 +22,7 @@ namespace trimeg {
 struct Stats {                      // device-resident counters
     unsigned long long n_lost;
     unsigned long long n_moved;
-    // tile-kernel diagnostics (trimeg_get_tile_counters): SM cycles of thread 0 of every CTA spent in
-    // phases A, B, C, D, E; markers evaluated by the one-marker fallback; bins used; stages run
+    // schedule diagnostics of the warp kernels (trimeg_get_tile_counters)
     unsigned long long tile[8];
 };
 
@@ -52,23 +51,25 @@ struct trimeg_ctx {
     // host path: two marker sets + permutation of the last trimeg_push_host batch (grown on demand)
     void *d_hbuf;
     size_t hbuf_bytes;
-    cudaStream_t hstream[3];
+    cudaStream_t hstream[3];        // compute, H2D, D2H
+    cudaEvent_t hevent[16];         // per chunk: inputs landed (0..7), results ready (8..15)
     int hstreams_ready;
+    cudaEvent_t ev_upload;          // recorded after the last trimeg_field_upload on its stream
 };
 
 namespace trimeg {
 
 // TRIMEG_PUSH_KERNEL_AUTO: with few toroidal modes the coefficient records are small, L1 holds them, and the plain
-// warp-autonomous kernel wins (cfg2, 3 modes: 4.5e9 against 3.7e9 marker-steps/s for variant 7); from about a dozen modes on
-// the records have to sit in shared memory and variant 7 wins (cfg5, 16 modes: 1.74e9 against 1.51e9; the lock-step CTA-tile
-// kernel, variant 3: 1.59e9); with very many modes a record (336 B per mode) is so large that too few of them fit into shared
-// memory for the triangles of a CTA's markers (15 slots at 26 modes) and the plain warp kernel is used again.  Up to 4 modes
-// the Horner loop is so short that the latency-bound rest of a stage weighs more and 16 warps per SM at 128 registers
-// (variant 8) beat 12 at 168 (cfg2: 4.69e9 against 4.53e9; on the cfg5 mesh the two cross between 4 and 6 modes).
+// warp-autonomous kernel wins; from about a dozen modes on the records have to sit in shared memory and the warp kernel
+// with the CTA-shared record table wins; with very many modes a record (336 B per mode) is so large that too few of them
+// fit into shared memory for the triangles of a CTA's markers (15 slots at 26 modes) and the plain warp kernel is used
+// again.  Up to 4 modes the Horner loop is so short that the latency-bound rest of a stage weighs more and 16 warps per SM
+// at 128 registers beat 12 at 168 (measurements: DESIGN.md section 5).
 inline int auto_push_kernel(int n_modes)
 {
-    if (n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES) return 8;
-    return (n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES && n_modes <= TRIMEG_AUTO_FUSED_MAX_MODES) ? 7 : 1;
+    if (n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES) return TRIMEG_PUSH_KERNEL_WARP128;
+    return (n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES && n_modes <= TRIMEG_AUTO_FUSED_MAX_MODES) ? TRIMEG_PUSH_KERNEL_WCACHE
+                                                                                              : TRIMEG_PUSH_KERNEL_WARP;
 }
 
 // launch wrappers implemented in trimeg_push.cu; each returns the cudaError of the launch
@@ -78,16 +79,11 @@ cudaError_t launch_gather(trimeg_ctx *c, size_t n, const double *R, const double
 cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP,
                        double *dV, double *dW, cudaStream_t s);
 cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
-// trimeg_push_warp.cu: warp-autonomous variant (no block barriers; variants 1, 2)
+// trimeg_push_warp.cu: warp-autonomous schedule, records through L1 (TRIMEG_PUSH_KERNEL_WARP, _WARP128)
 cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
                              cudaStream_t s);
 
-// trimeg_push_wcache.cu: warp-autonomous with a CTA-shared record cache in shared memory (variant 7)
-cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
-                               cudaStream_t s);
-
-// trimeg_push_fused.cu: CTA tiles with resident coefficient records, fused evaluate + finish (variants 3..6)
-cudaError_t launch_push_fused(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
-                              cudaStream_t s);
+// trimeg_push_wcache.cu: warp-autonomous with a CTA-shared record table in shared memory (TRIMEG_PUSH_KERNEL_WCACHE)
+cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 
 }  // namespace trimeg

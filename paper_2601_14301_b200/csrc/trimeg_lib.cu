@@ -18,6 +18,26 @@ using namespace trimeg;
         if (e__ != cudaSuccess) return TRIMEG_ERR_CUDA; \
     } while (0)
 
+// Every ABI entry that launches or allocates runs on the context's device, whatever device is current
+// in the calling thread (one context per GPU, several contexts per process allowed).
+struct DeviceGuard {
+    int prev = -1;
+    bool ok = true;
+    explicit DeviceGuard(int dev)
+    {
+        int cur = -1;
+        if (cudaGetDevice(&cur) != cudaSuccess) { ok = false; cudaGetLastError(); return; }
+        if (cur != dev) {
+            if (cudaSetDevice(dev) != cudaSuccess) { ok = false; cudaGetLastError(); return; }
+            prev = cur;
+        }
+    }
+    ~DeviceGuard() { if (prev >= 0) cudaSetDevice(prev); }
+};
+#define ON_CTX_DEVICE(c)                      \
+    DeviceGuard guard__((c)->device);         \
+    if (!guard__.ok) return TRIMEG_ERR_CUDA
+
 // ============================================================================ a0: mesh tables
 __device__ __forceinline__ int vertex_id(int n_theta, int i, int j)
 {   // v(i, j) = 1 + (i-1) n_theta + (j mod n_theta), i >= 1
@@ -316,6 +336,7 @@ static void fill_phys(trimeg_ctx *c)
     d.rho0B0 = p.rho0 * p.B0;
     d.qom = p.qs_over_ms;
     d.invT = 1.0 / p.T; d.kappa_n = p.kappa_n; d.kappa_T = p.kappa_T;
+    d.R0sq = p.R0 * p.R0; d.m2qs = -2.0 * d.qs; d.invT2 = 2.0 / p.T;
     d.eom_variant = p.eom_variant; d.weight_mode = p.weight_mode;
 }
 static int params_ok(const trimeg_params *p)
@@ -395,7 +416,11 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
         c->field.n_first = 0; c->field.n_step = 0; c->field.is_ap = 1;
         c->has_field = 0;
         c->push_kernel = TRIMEG_PUSH_KERNEL_AUTO;
-        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) { const int v = atoi(e); if (v >= TRIMEG_PUSH_KERNEL_AUTO && v <= TRIMEG_PUSH_KERNEL_MAX) c->push_kernel = v; }
+        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) {      // values that do not parse are ignored
+            char *end = nullptr;
+            const long v = strtol(e, &end, 10);
+            if (end != e && *end == '\0' && v >= TRIMEG_PUSH_KERNEL_AUTO && v <= TRIMEG_PUSH_KERNEL_MAX) c->push_kernel = (int)v;
+        }
     } while (0);
     if (d_rin2) cudaFree(d_rin2);
     free(hR); free(hZ);
@@ -407,9 +432,14 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
 int trimeg_mesh_destroy(trimeg_ctx *c)
 {
     if (!c) return TRIMEG_ERR_INVALID_ARG;
+    DeviceGuard guard__(c->device);
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
     cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
-    if (c->hstreams_ready) for (int k = 0; k < 3; ++k) cudaStreamDestroy(c->hstream[k]);
+    if (c->hstreams_ready) {
+        for (int k = 0; k < 3; ++k) cudaStreamDestroy(c->hstream[k]);
+        for (int k = 0; k < 16; ++k) cudaEventDestroy(c->hevent[k]);
+    }
+    if (c->ev_upload) cudaEventDestroy(c->ev_upload);
     cudaGetLastError();
     delete c;
     return TRIMEG_OK;
@@ -448,6 +478,7 @@ int trimeg_set_push_kernel(trimeg_ctx *c, int variant)
 int trimeg_mesh_download_geom(trimeg_ctx *c, double *geom_dev, trimeg_stream stream)
 {
     if (!c || !geom_dev) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     CU_TRY(cudaMemcpyAsync(geom_dev, c->d_geom, sizeof(double) * 6 * (size_t)c->n_tri, cudaMemcpyDeviceToDevice,
                            (cudaStream_t)stream));
     return TRIMEG_OK;
@@ -458,6 +489,7 @@ int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, cons
 {
     if (!c || n_modes < 0 || (kind != 0 && kind != 1)) return TRIMEG_ERR_INVALID_ARG;
     if (n_modes > 0 && (!mode_n_host || !data_dev)) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     cudaStream_t s = (cudaStream_t)stream;
     if (n_modes != c->field.n_modes || !c->d_coef) {
         // tables may still be in use by kernels enqueued earlier
@@ -494,12 +526,16 @@ int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, cons
         }
     }
     c->has_field = 1;
+    // trimeg_push_host runs on the context's own streams: they wait for this upload
+    if (!c->ev_upload) CU_TRY(cudaEventCreateWithFlags(&c->ev_upload, cudaEventDisableTiming));
+    CU_TRY(cudaEventRecord(c->ev_upload, s));
     return TRIMEG_OK;
 }
 
 int trimeg_field_download_coeffs(trimeg_ctx *c, void *coeffs_dev, trimeg_stream stream)
 {
     if (!c || !coeffs_dev) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
     if (c->field.n_modes == 0) return TRIMEG_OK;
     CU_TRY(cudaMemcpyAsync(coeffs_dev, c->d_coef, sizeof(double2) * NCOEF * (size_t)c->n_tri * c->field.n_modes,
@@ -510,6 +546,7 @@ int trimeg_field_download_coeffs(trimeg_ctx *c, void *coeffs_dev, trimeg_stream 
 int trimeg_locate(trimeg_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell, trimeg_stream stream)
 {
     if (!c || (n > 0 && (!R || !Z || !cell))) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     CU_TRY(launch_locate(c, n, R, Z, cell, (cudaStream_t)stream));
     return TRIMEG_OK;
 }
@@ -519,6 +556,7 @@ int trimeg_gather(trimeg_ctx *c, size_t n, const double *R, const double *Z, con
                   trimeg_stream stream)
 {
     if (!c || (n > 0 && (!R || !Z || !phi || !dphi || !dphi_dR || !dphi_dZ))) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
     CU_TRY(launch_gather(c, n, R, Z, phi, cell_hint, dphi, dphi_dR, dphi_dZ, dphi_dphi, (cudaStream_t)stream));
     return TRIMEG_OK;
@@ -528,6 +566,7 @@ int trimeg_rhs(trimeg_ctx *c, const trimeg_markers *m, size_t n, double *dRdt, d
                double *dvpardt, double *dwdt, trimeg_stream stream)
 {
     if (!c || (n > 0 && (!markers_ok(m) || !dRdt || !dZdt || !dphidt || !dvpardt || !dwdt))) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
     if (n == 0) return TRIMEG_OK;
     CU_TRY(launch_rhs(c, *m, n, dRdt, dZdt, dphidt, dvpardt, dwdt, (cudaStream_t)stream));
@@ -537,6 +576,7 @@ int trimeg_rhs(trimeg_ctx *c, const trimeg_markers *m, size_t n, double *dRdt, d
 int trimeg_push(trimeg_ctx *c, trimeg_markers *m, size_t n, double dt, int nsteps, trimeg_stream stream)
 {
     if (!c || nsteps < 0 || (n > 0 && !markers_ok(m)) || !(dt == dt)) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
     if (n == 0) return TRIMEG_OK;
     CU_TRY(launch_push(c, *m, n, dt, nsteps, (cudaStream_t)stream));
@@ -573,6 +613,7 @@ static int sort_into(trimeg_ctx *c, const trimeg_markers &m, size_t n, const Mar
 int trimeg_sort(trimeg_ctx *c, trimeg_markers *m, size_t n, int64_t *perm_dev, trimeg_stream stream)
 {
     if (!c || (n > 0 && !markers_ok(m)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     if (n == 0) return TRIMEG_OK;
     cudaStream_t s = (cudaStream_t)stream;
     MarkerScratch o;
@@ -589,6 +630,7 @@ int trimeg_compact(trimeg_ctx *c, trimeg_markers *m, size_t n, int64_t *perm_dev
                    trimeg_stream stream)
 {
     if (!c || (n > 0 && !markers_ok(m)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     if (n == 0) { if (n_active_host) *n_active_host = 0; return TRIMEG_OK; }
     cudaStream_t s = (cudaStream_t)stream;
     MarkerScratch o;
@@ -612,20 +654,41 @@ int trimeg_compact(trimeg_ctx *c, trimeg_markers *m, size_t n, int64_t *perm_dev
     return TRIMEG_OK;
 }
 
-// Host-buffer path: chunks round-robin over three streams so that the H2D copy of chunk k+1
-// and the D2H copy of chunk k-1 overlap the push of chunk k.
+// Host-buffer path (device buffers are allocated once and kept).  The batch is cut into chunks of
+// consecutive markers; every chunk goes H2D (stream 1) -> locate, cell sort, push with a re-sort every 10 steps, unsort
+// (stream 0) -> D2H (stream 2), so that the copies of chunks k+1 and k-1 run under the push of chunk k.  The push kernels
+// live on markers per triangle, so a chunk keeps at least ~100 markers per triangle: chunks = clamp(n / (100 n_tri), 1, 8).
+// Markers are independent: the result does not depend on the number of chunks.
+static int host_chunks(const trimeg_ctx *c, size_t n)
+{
+    if (const char *e = getenv("TRIMEG_HOST_CHUNKS")) {
+        char *end = nullptr;
+        const long v = strtol(e, &end, 10);
+        if (end != e && *end == '\0' && v >= 1 && v <= 8) return (int)v;
+    }
+    if (n < ((size_t)1 << 20)) return 1;
+    const size_t k = n / (100 * (size_t)c->n_tri);
+    return (int)(k < 1 ? 1 : (k > 8 ? 8 : k));
+}
+
+static MarkerScratch chunk_of(const MarkerScratch &m, size_t off)
+{
+    MarkerScratch o = {m.R + off, m.Z + off, m.phi + off, m.vpar + off, m.mu + off, m.w + off, m.cell + off};
+    return o;
+}
+
 int trimeg_push_host(trimeg_ctx *c, trimeg_markers *mh, size_t n, double dt, int nsteps, int locate_first)
 {
-    if (!c || nsteps < 0 || (n > 0 && !markers_ok(mh)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    if (!c || nsteps < 0 || (n > 0 && !markers_ok(mh)) || n > 0x7fffffffULL || !(dt == dt)) return TRIMEG_ERR_INVALID_ARG;
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
     if (n == 0) return TRIMEG_OK;
+    ON_CTX_DEVICE(c);
     if (!c->hstreams_ready) {
         for (int k = 0; k < 3; ++k) CU_TRY(cudaStreamCreateWithFlags(&c->hstream[k], cudaStreamNonBlocking));
+        for (int k = 0; k < 16; ++k) CU_TRY(cudaEventCreateWithFlags(&c->hevent[k], cudaEventDisableTiming));
         c->hstreams_ready = 1;
     }
-    // The whole batch is made resident and sorted as ONE set: the push kernels live on markers per triangle, and
-    // sorting chunks of the batch separately would divide that density by the number of chunks.  Device buffers
-    // (two marker sets + the permutation) are kept in the context between calls.
+    // device buffers (two marker sets + three permutations, 128 B per marker), kept in the context between calls
     MarkerScratch a, b;
     const size_t rec = carve(nullptr, n, a);
     const size_t permb = align_up(n * sizeof(int64_t), 256);
@@ -638,58 +701,92 @@ int trimeg_push_host(trimeg_ctx *c, trimeg_markers *mh, size_t n, double dt, int
     char *base = (char *)c->d_hbuf;
     carve(base, n, a);
     carve(base + rec, n, b);
-    int64_t *perm = (int64_t *)(base + 2 * rec), *perm2 = (int64_t *)(base + 2 * rec + permb),
-            *perm3 = (int64_t *)(base + 2 * rec + 2 * permb);
-    cudaStream_t s = c->hstream[0];
-    const size_t db = n * sizeof(double);
-    const unsigned grid = (unsigned)((n + 255) / 256);
+    int64_t *const perm_all[3] = {(int64_t *)(base + 2 * rec), (int64_t *)(base + 2 * rec + permb),
+                                  (int64_t *)(base + 2 * rec + 2 * permb)};
+    const int nch = host_chunks(c, n);
+    const size_t per = align_up((n + nch - 1) / nch, 1024);      // chunk starts stay 256-byte aligned in every array
+    cudaStream_t sC = c->hstream[0], sH = c->hstream[1], sD = c->hstream[2];
     int rc = TRIMEG_OK;
-#define H2D(dst, src, bytes) if (rc == TRIMEG_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyHostToDevice, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA
-#define D2H(dst, src, bytes) if (rc == TRIMEG_OK && cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA
-    do {
-        H2D(a.R, mh->R, db); H2D(a.Z, mh->Z, db);
-        if (locate_first) { if (rc == TRIMEG_OK && launch_locate(c, n, a.R, a.Z, a.cell, s) != cudaSuccess) rc = TRIMEG_ERR_CUDA; }
-        else H2D(a.cell, mh->cell, n * sizeof(int32_t));
-        H2D(a.phi, mh->phi, db); H2D(a.vpar, mh->vpar, db); H2D(a.mu, mh->mu, db); H2D(a.w, mh->w, db);
-        if (rc != TRIMEG_OK) break;
-        // markers drift out of their triangles: sort again every HOST_SORT_EVERY steps (set `cur` <-> set `oth`),
-        // `perm` always maps a position in `cur` to the caller's index
-        constexpr int HOST_SORT_EVERY = 10;
-        MarkerScratch cur = a, oth = b;
-        for (int done = 0; done < nsteps || done == 0; done += HOST_SORT_EVERY) {
+#define TRY_CU(expr) if (rc == TRIMEG_OK && (expr) != cudaSuccess) rc = TRIMEG_ERR_CUDA
+    if (c->ev_upload) TRY_CU(cudaStreamWaitEvent(sC, c->ev_upload, 0));
+    // ---- inputs: every chunk's seven arrays on the copy stream
+    for (int k = 0; k < nch && rc == TRIMEG_OK; ++k) {
+        const size_t off = (size_t)k * per;
+        if (off >= n) break;
+        const size_t nk = (n - off < per) ? n - off : per, db = nk * sizeof(double);
+        TRY_CU(cudaMemcpyAsync(a.R + off, mh->R + off, db, cudaMemcpyHostToDevice, sH));
+        TRY_CU(cudaMemcpyAsync(a.Z + off, mh->Z + off, db, cudaMemcpyHostToDevice, sH));
+        if (!locate_first) TRY_CU(cudaMemcpyAsync(a.cell + off, mh->cell + off, nk * sizeof(int32_t), cudaMemcpyHostToDevice, sH));
+        TRY_CU(cudaMemcpyAsync(a.phi + off, mh->phi + off, db, cudaMemcpyHostToDevice, sH));
+        TRY_CU(cudaMemcpyAsync(a.vpar + off, mh->vpar + off, db, cudaMemcpyHostToDevice, sH));
+        TRY_CU(cudaMemcpyAsync(a.mu + off, mh->mu + off, db, cudaMemcpyHostToDevice, sH));
+        TRY_CU(cudaMemcpyAsync(a.w + off, mh->w + off, db, cudaMemcpyHostToDevice, sH));
+        TRY_CU(cudaEventRecord(c->hevent[k], sH));
+    }
+    // ---- per chunk: locate, [sort -> push <= 10 steps] ..., unsort on the compute stream; results out on the third stream
+    constexpr int HOST_SORT_EVERY = 10;
+    for (int k = 0; k < nch && rc == TRIMEG_OK; ++k) {
+        const size_t off = (size_t)k * per;
+        if (off >= n) break;
+        const size_t nk = (n - off < per) ? n - off : per, db = nk * sizeof(double);
+        const unsigned grid = (unsigned)((nk + 255) / 256);
+        MarkerScratch cur = chunk_of(a, off), oth = chunk_of(b, off);
+        int64_t *perm = perm_all[0] + off, *perm2 = perm_all[1] + off, *perm3 = perm_all[2] + off;
+        TRY_CU(cudaStreamWaitEvent(sC, c->hevent[k], 0));
+        if (locate_first) TRY_CU(launch_locate(c, nk, cur.R, cur.Z, cur.cell, sC));
+        // markers drift out of their triangles: sort again every HOST_SORT_EVERY steps (set `cur` <-> set `oth`);
+        // `perm` always maps a position in `cur` to the caller's index (relative to the chunk)
+        for (int done = 0; (done < nsteps || done == 0) && rc == TRIMEG_OK; done += HOST_SORT_EVERY) {
             trimeg_markers mc = {cur.R, cur.Z, cur.phi, cur.vpar, cur.mu, cur.w, cur.cell};
-            rc = sort_into(c, mc, n, oth, (done == 0) ? perm : perm2, c->d_bins, s);     // cur -> oth (sorted by triangle)
+            rc = sort_into(c, mc, nk, oth, (done == 0) ? perm : perm2, c->d_bins, sC);     // cur -> oth (sorted by triangle)
             if (rc != TRIMEG_OK) break;
             if (done > 0) {
-                compose_perm_kernel<<<grid, 256, 0, s>>>(n, perm, perm2, perm3);
+                compose_perm_kernel<<<grid, 256, 0, sC>>>(nk, perm, perm2, perm3);
                 c->n_launches++;
                 int64_t *t = perm; perm = perm3; perm3 = t;
             }
             const MarkerScratch t = cur; cur = oth; oth = t;
-            const int k = (nsteps - done < HOST_SORT_EVERY) ? nsteps - done : HOST_SORT_EVERY;
+            const int steps = (nsteps - done < HOST_SORT_EVERY) ? nsteps - done : HOST_SORT_EVERY;
             trimeg_markers mp = {cur.R, cur.Z, cur.phi, cur.vpar, cur.mu, cur.w, cur.cell};
-            if (k > 0 && launch_push(c, mp, n, dt, k, s) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+            if (steps > 0) TRY_CU(launch_push(c, mp, nk, dt, steps, sC));
             if (nsteps == 0) break;
         }
         if (rc != TRIMEG_OK) break;
         trimeg_markers mo = {oth.R, oth.Z, oth.phi, oth.vpar, oth.mu, oth.w, oth.cell};
-        unpermute_kernel<<<grid, 256, 0, s>>>(n, cur, mo, perm);       // cur -> oth (caller order)
+        unpermute_kernel<<<grid, 256, 0, sC>>>(nk, cur, mo, perm);       // cur -> oth (caller order)
         c->n_launches++;
-        if (cudaGetLastError() != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
-        D2H(mh->R, oth.R, db); D2H(mh->Z, oth.Z, db); D2H(mh->phi, oth.phi, db);
-        D2H(mh->vpar, oth.vpar, db); D2H(mh->w, oth.w, db);
-        D2H(mh->cell, oth.cell, n * sizeof(int32_t));
-    } while (0);
-#undef H2D
-#undef D2H
-    if (cudaStreamSynchronize(s) != cudaSuccess && rc == TRIMEG_OK) rc = TRIMEG_ERR_CUDA;
+        TRY_CU(cudaGetLastError());
+        TRY_CU(cudaEventRecord(c->hevent[8 + k], sC));
+        TRY_CU(cudaStreamWaitEvent(sD, c->hevent[8 + k], 0));
+        TRY_CU(cudaMemcpyAsync(mh->R + off, oth.R, db, cudaMemcpyDeviceToHost, sD));
+        TRY_CU(cudaMemcpyAsync(mh->Z + off, oth.Z, db, cudaMemcpyDeviceToHost, sD));
+        TRY_CU(cudaMemcpyAsync(mh->phi + off, oth.phi, db, cudaMemcpyDeviceToHost, sD));
+        TRY_CU(cudaMemcpyAsync(mh->vpar + off, oth.vpar, db, cudaMemcpyDeviceToHost, sD));
+        TRY_CU(cudaMemcpyAsync(mh->w + off, oth.w, db, cudaMemcpyDeviceToHost, sD));
+        TRY_CU(cudaMemcpyAsync(mh->cell + off, oth.cell, nk * sizeof(int32_t), cudaMemcpyDeviceToHost, sD));
+    }
+#undef TRY_CU
+    for (int k = 0; k < 3; ++k)
+        if (cudaStreamSynchronize(c->hstream[k]) != cudaSuccess && rc == TRIMEG_OK) rc = TRIMEG_ERR_CUDA;
     if (rc != TRIMEG_OK) cudaGetLastError();
     return rc;
+}
+
+int trimeg_release_host_buffers(trimeg_ctx *c)
+{
+    if (!c) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
+    if (c->hstreams_ready)
+        for (int k = 0; k < 3; ++k) CU_TRY(cudaStreamSynchronize(c->hstream[k]));
+    if (c->d_hbuf) { cudaFree(c->d_hbuf); c->d_hbuf = nullptr; c->hbuf_bytes = 0; }
+    if (c->d_scratch) { CU_TRY(cudaDeviceSynchronize()); cudaFree(c->d_scratch); c->d_scratch = nullptr; c->scratch_bytes = 0; }
+    return TRIMEG_OK;
 }
 
 int trimeg_get_stats(trimeg_ctx *c, int64_t *n_lost, int64_t *n_relocated, int64_t *n_launches)
 {
     if (!c) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     Stats h;
     CU_TRY(cudaDeviceSynchronize());
     CU_TRY(cudaMemcpy(&h, c->d_stats, sizeof(Stats), cudaMemcpyDeviceToHost));
@@ -702,6 +799,7 @@ int trimeg_get_stats(trimeg_ctx *c, int64_t *n_lost, int64_t *n_relocated, int64
 int trimeg_get_tile_counters(trimeg_ctx *c, int64_t *out8)
 {
     if (!c || !out8) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     Stats h;
     CU_TRY(cudaDeviceSynchronize());
     CU_TRY(cudaMemcpy(&h, c->d_stats, sizeof(Stats), cudaMemcpyDeviceToHost));
@@ -712,6 +810,7 @@ int trimeg_get_tile_counters(trimeg_ctx *c, int64_t *out8)
 int trimeg_reset_stats(trimeg_ctx *c)
 {
     if (!c) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     CU_TRY(cudaDeviceSynchronize());
     CU_TRY(cudaMemset(c->d_stats, 0, sizeof(Stats)));
     c->n_launches = 0;
@@ -721,6 +820,7 @@ int trimeg_reset_stats(trimeg_ctx *c)
 int trimeg_measure_fp64_peak(trimeg_ctx *c, double *tflops_out)
 {
     if (!c || !tflops_out) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
     int rc = ensure_scratch(c, 256);
     if (rc) return rc;
     cudaEvent_t e0, e1;
@@ -748,7 +848,7 @@ int trimeg_measure_fp64_peak(trimeg_ctx *c, double *tflops_out)
 int trimeg_measure_fp64_peak_operands(trimeg_ctx *c, int n_reg_operands, double *tflops_out)
 {
     if (!c || !tflops_out || n_reg_operands < 1 || n_reg_operands > 3) return TRIMEG_ERR_INVALID_ARG;
-    if (cudaSetDevice(c->device) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_CUDA; }
+    ON_CTX_DEVICE(c);
     int rc = ensure_scratch(c, 1024 * sizeof(double));
     if (rc != TRIMEG_OK) return rc;
     double *buf = (double *)c->d_scratch;

@@ -62,7 +62,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
     const bool has_field = F.n_modes > 0;
     const double hdt = 0.5 * dt, dt6 = dt / 6.0;
     const unsigned lt_mask = (1u << lane) - 1u;
-    long long tph[3] = {0, 0, 0}, tlast = clock64();                // lane 0: grouping, evaluation + equations, fallback
+    TRIMEG_PHASE_CLOCK_INIT                                         // lane 0: grouping, evaluation + equations, fallback
     unsigned n_fallback = 0, n_bins = 0, n_stages = 0, n_regroup = 0;
     int t_last[P], slot[P], n_ev = 0;                               // triangle and evaluation slot of the lane's markers at the last grouping
 #pragma unroll
@@ -154,7 +154,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
                     if (slot[p] >= 0) { ev_own[slot[p]] = lane + 32 * p; ev_tri[slot[p]] = t[p]; }
             }
             __syncwarp();
-            if (lane == 0) { const long long now = clock64(); tph[0] += now - tlast; tlast = now; n_bins += nb; ++n_stages; }
+            if (lane == 0) { TRIMEG_PHASE_CLOCK(0) n_bins += nb; ++n_stages; }
 
             // ------------------------------------------------------------ 2 + 3: batched evaluation, equations (slot role)
             if (lane * P < n_ev) {
@@ -195,7 +195,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
                 }
             }
             __syncwarp();
-            if (lane == 0) { const long long now = clock64(); tph[1] += now - tlast; tlast = now; }
+            if (lane == 0) { TRIMEG_PHASE_CLOCK(1) }
 
             // ------------------------------------------------------------ markers without a slot (home role)
 #pragma unroll 1
@@ -215,7 +215,7 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
                 advance(M, Ph, S, NW, cell, flags, q, stage, fv, dt, hdt, dt6);
             }
             __syncwarp();
-            if (lane == 0) { const long long now = clock64(); tph[2] += now - tlast; tlast = now; }
+            if (lane == 0) { TRIMEG_PHASE_CLOCK(2) }
         }
     }
 
@@ -240,10 +240,8 @@ __global__ void __launch_bounds__(32 * WARPS, MINB) push_warp_kernel(MeshDev M, 
     if (lane == 0) {
         if (lost) atomicAdd(&st->n_lost, (unsigned long long)lost);
         if (moved) atomicAdd(&st->n_moved, (unsigned long long)moved);
-        atomicAdd(&st->tile[0], (unsigned long long)tph[0]);
         atomicAdd(&st->tile[1], (unsigned long long)n_regroup);
-        atomicAdd(&st->tile[3], (unsigned long long)tph[1]);
-        atomicAdd(&st->tile[4], (unsigned long long)tph[2]);
+        TRIMEG_PHASE_CLOCK_FLUSH(st)
         if (n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);
         atomicAdd(&st->tile[6], (unsigned long long)n_bins);
         atomicAdd(&st->tile[7], (unsigned long long)n_stages);
@@ -254,13 +252,10 @@ template <int P, int WARPS, int SLACK, int MINB>
 cudaError_t launch_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     using Cfg = WarpCfg<P, SLACK>;
-    static bool configured = false;
     const size_t shm = Cfg::WARP_BYTES * WARPS;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    // function attributes are per device: set on every launch (cheap), not once per process
+    cudaError_t e = cudaFuncSetAttribute(push_warp_kernel<P, WARPS, SLACK, MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)shm);
+    if (e != cudaSuccess) return e;
     const size_t per_cta = (size_t)Cfg::NW * WARPS;
     const size_t ctas = (n + per_cta - 1) / per_cta;
     push_warp_kernel<P, WARPS, SLACK, MINB><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
@@ -275,9 +270,8 @@ cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     switch (variant) {
-    case 1: return launch_warp<2, 4, 6, 3>(c, m, n, dt, nsteps, s);
-    case 2: return launch_warp<4, 4, 16, 2>(c, m, n, dt, nsteps, s);
-    case 8: return launch_warp<2, 4, 6, 4>(c, m, n, dt, nsteps, s);
+    case TRIMEG_PUSH_KERNEL_WARP: return launch_warp<2, 4, 6, 3>(c, m, n, dt, nsteps, s);
+    case TRIMEG_PUSH_KERNEL_WARP128: return launch_warp<2, 4, 6, 4>(c, m, n, dt, nsteps, s);
     default: return cudaErrorInvalidValue;
     }
 }

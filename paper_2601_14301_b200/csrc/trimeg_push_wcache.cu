@@ -126,7 +126,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
     const bool has_field = F.n_modes > 0;
     const double hdt = 0.5 * dt, dt6 = dt / 6.0;
     const unsigned lt_mask = (1u << lane) - 1u;
-    long long tph[3] = {0, 0, 0}, tlast = clock64();                // lane 0: grouping (+ lookups), evaluation + finish, one-marker path
+    TRIMEG_PHASE_CLOCK_INIT                                         // lane 0: grouping (+ lookups), evaluation + finish, one-marker path
     unsigned n_fallback = 0, n_copied = 0, n_stages = 0;
     int t_last[P], r_last[P];                                       // triangle and record slot of the lane's markers at the last stage
     int slot[P], recp[P], n_ev = 0;                                 // evaluation slot and record of the lane's markers; slots in use
@@ -233,7 +233,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                 }
             }
             __syncwarp();
-            if (lane == 0) { const long long now = clock64(); tph[0] += now - tlast; tlast = now; ++n_stages; }
+            if (lane == 0) { TRIMEG_PHASE_CLOCK(0) ++n_stages; }
 
             // ------------------------------------------------------------ 2 + 3: batched evaluation, equations (slot role)
             if (lane * P < n_ev) {
@@ -274,7 +274,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                 }
             }
             __syncwarp();
-            if (lane == 0) { const long long now = clock64(); tph[1] += now - tlast; tlast = now; }
+            if (lane == 0) { TRIMEG_PHASE_CLOCK(1) }
 
             // ------------------------------------------------------------ markers without a slot (home role)
 #pragma unroll 1
@@ -294,7 +294,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                 advance(M, Ph, S, NW, cell, flags, q, stage, fv, dt, hdt, dt6);
             }
             __syncwarp();
-            if (lane == 0) { const long long now = clock64(); tph[2] += now - tlast; tlast = now; }
+            if (lane == 0) { TRIMEG_PHASE_CLOCK(2) }
         }
         // ---- every WC_SYNC_EVERY steps all warps meet; the table is emptied when it is nearly full of triangles the markers
         // have left (a full table is not an error: triangles without a record go down the one-marker path)
@@ -333,10 +333,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
     if (lane == 0) {
         if (lost) atomicAdd(&st->n_lost, (unsigned long long)lost);
         if (moved) atomicAdd(&st->n_moved, (unsigned long long)moved);
-        atomicAdd(&st->tile[0], (unsigned long long)tph[0]);
         atomicAdd(&st->tile[1], (unsigned long long)n_regroup);
-        atomicAdd(&st->tile[3], (unsigned long long)tph[1]);
-        atomicAdd(&st->tile[4], (unsigned long long)tph[2]);
+        TRIMEG_PHASE_CLOCK_FLUSH(st)
         if (n_fallback) atomicAdd(&st->tile[5], (unsigned long long)n_fallback);
         if (n_copied) atomicAdd(&st->tile[6], (unsigned long long)n_copied);
         atomicAdd(&st->tile[7], (unsigned long long)n_stages);
@@ -347,13 +345,10 @@ template <int P, int WARPS, int SLACK>
 cudaError_t launch_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     using Cfg = WCacheCfg<P, SLACK>;
-    static bool configured = false;
     constexpr size_t SMEM_MAX = 227 * 1024;
-    if (!configured) {
-        cudaError_t e = cudaFuncSetAttribute(push_wcache_kernel<P, WARPS, SLACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
-        if (e != cudaSuccess) return e;
-        configured = true;
-    }
+    // function attributes are per device: set on every launch (cheap), not once per process
+    cudaError_t e = cudaFuncSetAttribute(push_wcache_kernel<P, WARPS, SLACK>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+    if (e != cudaSuccess) return e;
     const size_t fixed = ((size_t)WARPS * Cfg::WARP_BYTES + Cfg::TABLE_BYTES + 15) / 16 * 16;
     const size_t rec_bytes = sizeof(double2) * ((NCOEF * (size_t)c->field.n_modes + 3) | 1);    // as rec_stride in the kernel
     int nslot = c->field.n_modes ? (int)((SMEM_MAX - fixed) / rec_bytes) : 0;
@@ -368,14 +363,10 @@ cudaError_t launch_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, doub
 
 }  // namespace
 
-cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
-                               cudaStream_t s)
+cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
-    switch (variant) {
-    case 7: return launch_wcache<2, 12, 5>(c, m, n, dt, nsteps, s);
-    default: return cudaErrorInvalidValue;
-    }
+    return launch_wcache<2, 12, 5>(c, m, n, dt, nsteps, s);
 }
 
 }  // namespace trimeg

@@ -4,6 +4,21 @@
 #pragma once
 #include "trimeg_device.cuh"
 
+// In-kernel phase timers of the warp kernels (lane 0, clock64): compiled in only with -DTRIMEG_PROFILE
+// (python -m paper_2601_14301_b200.build --profile); the default build carries the cheap event counters alone.
+#ifdef TRIMEG_PROFILE
+#define TRIMEG_PHASE_CLOCK_INIT long long tph[3] = {0, 0, 0}, tlast = clock64();
+#define TRIMEG_PHASE_CLOCK(k) { const long long now__ = clock64(); tph[k] += now__ - tlast; tlast = now__; }
+#define TRIMEG_PHASE_CLOCK_FLUSH(st)                              \
+    atomicAdd(&(st)->tile[0], (unsigned long long)tph[0]);        \
+    atomicAdd(&(st)->tile[3], (unsigned long long)tph[1]);        \
+    atomicAdd(&(st)->tile[4], (unsigned long long)tph[2]);
+#else
+#define TRIMEG_PHASE_CLOCK_INIT
+#define TRIMEG_PHASE_CLOCK(k)
+#define TRIMEG_PHASE_CLOCK_FLUSH(st)
+#endif
+
 namespace trimeg {
 
 constexpr double TWO_PI = 6.283185307179586476925286766559;

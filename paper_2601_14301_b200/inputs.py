@@ -267,6 +267,26 @@ def markers(wl: Workload, n: Optional[int] = None, seed: Optional[int] = None) -
     return {k: np.ascontiguousarray(v, dtype=np.float64) for k, v in out.items()}
 
 
+def positions(wl: Workload, n: Optional[int] = None, seed: Optional[int] = None) -> Dict[str, np.ndarray]:
+    """{R, Z, phi} of markers(wl, n) alone (the first three draws of the same stream: bit-identical to the full
+    sample for the recipes without a final permutation) -- for the gather-only sweep, whose largest sizes (2^28)
+    would otherwise draw three more 2 GB arrays nobody reads."""
+    n = wl.n_markers if n is None else int(n)
+    if wl.marker_recipe == "edge10":
+        m = markers(wl, n, seed)
+        return {k: m[k] for k in ("R", "Z", "phi")}
+    rng = np.random.default_rng([wl.seed if seed is None else seed, 2])
+    u_r = rng.random(n)
+    r = wl.a * (0.1 + 0.8 * u_r) if wl.marker_recipe == "linear_r" else wl.a * np.sqrt(0.01 + 0.80 * u_r)
+    del u_r
+    th = TWO_PI * rng.random(n)
+    R = wl.R0 + r * np.cos(th)
+    Z = r * np.sin(th)
+    del r, th
+    phi = TWO_PI * rng.random(n)
+    return dict(R=R, Z=Z, phi=phi)
+
+
 def subsample(m: Dict[str, np.ndarray], stride: int) -> Dict[str, np.ndarray]:
     """Every stride-th marker (markers are independent: PAPER.md:590)."""
     return {k: np.ascontiguousarray(v[::stride]) for k, v in m.items()}

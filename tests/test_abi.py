@@ -49,13 +49,30 @@ def test_binding_names_match_header():
 
 
 def test_sass_is_sm100a_and_locator_has_no_fma_in_contains():
-    """The cubin embedded in the library targets sm_100a."""
+    """The cubin embedded in the library targets sm_100a, and the SASS of locate_kernel has no DFMA where the
+    contains() test lives (rule L2: every operation individually rounded): the kernel body (hinted walk) and the
+    complete 3x3 rule (the subroutine with the most DMULs) multiply and add separately; fused multiply-adds appear
+    only in the (r, theta) guess (sqrt, atan2), which never decides anything (rule L1)."""
     import subprocess
     from paper_2601_14301_b200 import binding
     out = subprocess.run(["cuobjdump", "-lelf", binding.LIB_PATH], capture_output=True, text=True)
     if out.returncode != 0:
         pytest.skip("cuobjdump unavailable")
     assert "sm_100a" in out.stdout
+    sass = subprocess.run(["cuobjdump", "-sass", binding.LIB_PATH], capture_output=True, text=True).stdout
+    fn = [f for f in re.split(r"\n\s*Function : ", sass) if f.startswith("_ZN6trimeg13locate_kernel")]
+    assert len(fn) == 1
+    ins = [(int(a, 16), op) for a, op in re.findall(r"/\*([0-9a-f]{4,})\*/\s+(?:@!?U?P\d+\s+)?([A-Z][A-Z0-9_.]*)", fn[0])]
+    targets = sorted({int(t, 16) for t in re.findall(r"CALL\.REL\.NOINC\s+(0x[0-9a-f]+)", fn[0])})
+    assert targets, "locate_full / ring_sector_guess are expected as subroutines"
+    bounds = [0] + targets + [max(a for a, _ in ins) + 16]
+    regions = [[op for a, op in ins if lo <= a < hi] for lo, hi in zip(bounds[:-1], bounds[1:])]
+    body = regions[0]
+    full = max(regions[1:], key=lambda r: sum(op.startswith("DMUL") for op in r))
+    for r in (body, full):
+        assert sum(op.startswith("DMUL") for op in r) >= 4 and sum(op.startswith("DADD") for op in r) >= 4
+        assert not any(op.startswith("DFMA") for op in r)
+    assert any(op.startswith("DFMA") for r in regions for op in r)      # the guess does use them: the parse sees DFMAs
 
 
 def test_invalid_arguments_are_rejected_without_a_gpu(lib):
