@@ -34,8 +34,8 @@ import numpy as np
 METRIC = "marker RK4 pushes/sec (incl. field gather)"
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the push kernel, from the committed ncu --set full
 # captures under profiles/: (workload, push kernel, sort_every, markers) -> bytes; null for anything else
-PROFILED_DRAM_BYTES_PER_LAUNCH = {("cfg5", 3, 10, 1 << 24): 1.94e9}
-PUSH_KERNEL_NAMES = {0: "push_kernel", 1: "push_warp_kernel<2,4,6,3>", 2: "push_warp_kernel<2,4,6,4>", 3: "push_wcache_kernel<2,12,5>"}
+PROFILED_DRAM_BYTES_PER_LAUNCH = {("cfg5", 2, 10, 1 << 24): 1.94e9}
+PUSH_KERNEL_NAMES = {0: "push_kernel", 1: "push_lane_kernel<16>", 2: "push_wcache_kernel<2,12,5>"}
 UNIT = "marker-steps/s"
 
 
@@ -451,7 +451,7 @@ def run_gpu(args, wl):
 
     # ---- the other configs, device-timed the same way (N = 1 only): short runs, same live peaks
     sweep = None
-    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers:
+    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes:
         sweep = {}
         for name in ("cfg2", "cfg3"):
             w2 = inputs.WORKLOADS[name]
@@ -524,6 +524,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
+    ap.add_argument("--n-modes", type=int, default=0, help="override the toroidal mode list by n = 0, 2, ..., 2 (K - 1) (schedule selection sweeps)")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
     ap.add_argument("--max-log2", type=int, default=28, help="cfg4 gather sweep: largest marker count 2^k")
@@ -538,6 +539,8 @@ def main():
     wl = inputs.WORKLOADS[args.workload]
     if args.markers:
         wl = dataclasses.replace(wl, n_markers=args.markers)
+    if args.n_modes:
+        wl = dataclasses.replace(wl, modes=tuple(range(0, 2 * args.n_modes, 2)))
     if args.workload == "cfg4":
         return run_gather_sweep(args, wl)
     if args.impl == "reference":

@@ -177,26 +177,25 @@ int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_d
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
 /* Schedule used by trimeg_push / trimeg_push_host (same results, different kernels):
- *  TRIMEG_PUSH_KERNEL_AUTO (the default)  WARP128 for a field of up to 4 toroidal modes, WCACHE for 12 to 26, else WARP;
+ *  TRIMEG_PUSH_KERNEL_AUTO (the default)  LANE for a field of up to 7 toroidal modes, WCACHE above;
  *  TRIMEG_PUSH_KERNEL_THREAD   one thread per marker, state in registers, coefficients through L1 (the plain schedule);
- *  TRIMEG_PUSH_KERNEL_WARP     warp-autonomous: every warp owns 58 markers (state in shared memory), groups them by
- *         triangle with ballots (anew only at a stage where one of them has changed its triangle) and evaluates 2 markers
- *         of one triangle per lane off a single load of each coefficient (through L1), finishes and re-locates them
- *         without any block barrier;
- *  TRIMEG_PUSH_KERNEL_WARP128  the same compiled for 128 registers per thread (16 instead of 12 warps per SM): better
- *         when the Horner loop is short (few modes) and the latency-bound rest of the stage weighs more;
- *  TRIMEG_PUSH_KERNEL_WCACHE   warp-autonomous like WARP (12 warps per CTA, one CTA per SM), with the coefficient records
- *         of the CTA's triangles in a shared, insert-only hash table in shared memory: the first warp that meets a
- *         triangle copies its record in, the others find it there; the warps meet at a barrier every tenth step only.
+ *  TRIMEG_PUSH_KERNEL_LANE     lane-owned markers: every warp owns 64 markers, lane l the markers l and l + 32, for the
+ *         whole call (state in shared memory; no grouping, no evaluation slots); one marker per evaluation in two phases
+ *         (all Horner steps in xi, then those in eta) so that runs of DFMAs share their multiplier (the FP64 pipe reads one
+ *         register operand per cycle); the coefficient records of the CTA's triangles sit in a shared,
+ *         insert-only hash table in shared memory; 16 warps per CTA, one CTA per SM; no block barrier inside a 10-step call;
+ *  TRIMEG_PUSH_KERNEL_WCACHE   every warp owns 59 markers, groups them by triangle with ballots (anew only at a stage where
+ *         one of them has changed its triangle) into evaluation slots, and a lane evaluates 2 markers of one triangle off a
+ *         single load of each coefficient -- from about eight modes on the shared-memory pipe cannot deliver a coefficient
+ *         per marker; same record table; 12 warps per CTA.
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
- * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX.  (The lock-step CTA-tile schedules of round 1 were
- * removed: git history, commit 3003ca4, has them.) */
+ * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX.  (Schedules of earlier rounds that lost everywhere were
+ * removed: lock-step CTA tiles -- commit 3003ca4 --, warp kernels reading the records through L1 -- commit 99b8bd5.) */
 #define TRIMEG_PUSH_KERNEL_AUTO (-1)
 #define TRIMEG_PUSH_KERNEL_THREAD 0
-#define TRIMEG_PUSH_KERNEL_WARP 1
-#define TRIMEG_PUSH_KERNEL_WARP128 2
-#define TRIMEG_PUSH_KERNEL_WCACHE 3
-#define TRIMEG_PUSH_KERNEL_MAX 3
+#define TRIMEG_PUSH_KERNEL_LANE 1
+#define TRIMEG_PUSH_KERNEL_WCACHE 2
+#define TRIMEG_PUSH_KERNEL_MAX 2
 int trimeg_set_push_kernel(trimeg_ctx *ctx, int variant);
 /* The variant trimeg_push will launch (AUTO resolved for the uploaded field; otherwise the TRIMEG_PUSH_KERNEL
  * environment override at context creation -- ignored unless it parses as an integer in range -- or the last

@@ -25,8 +25,8 @@ EXPORTS = (
 
 OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC = 0, -1, -2, -3, -4, -5
 # TRIMEG_PUSH_KERNEL_* of include/trimeg.h
-PUSH_KERNEL_AUTO, PUSH_KERNEL_THREAD, PUSH_KERNEL_WARP, PUSH_KERNEL_WARP128, PUSH_KERNEL_WCACHE = -1, 0, 1, 2, 3
-PUSH_KERNELS = (PUSH_KERNEL_THREAD, PUSH_KERNEL_WARP, PUSH_KERNEL_WARP128, PUSH_KERNEL_WCACHE)
+PUSH_KERNEL_AUTO, PUSH_KERNEL_THREAD, PUSH_KERNEL_LANE, PUSH_KERNEL_WCACHE = -1, 0, 1, 2
+PUSH_KERNELS = (PUSH_KERNEL_THREAD, PUSH_KERNEL_LANE, PUSH_KERNEL_WCACHE)
 
 
 class TrimegError(RuntimeError):

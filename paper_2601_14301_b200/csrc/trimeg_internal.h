@@ -8,13 +8,7 @@
 #include "trimeg_device.cuh"
 
 #ifndef TRIMEG_AUTO_SMALL_MAX_MODES
-#define TRIMEG_AUTO_SMALL_MAX_MODES 4
-#endif
-#ifndef TRIMEG_AUTO_FUSED_MIN_MODES
-#define TRIMEG_AUTO_FUSED_MIN_MODES 12
-#endif
-#ifndef TRIMEG_AUTO_FUSED_MAX_MODES
-#define TRIMEG_AUTO_FUSED_MAX_MODES 26
+#define TRIMEG_AUTO_SMALL_MAX_MODES 7
 #endif
 
 namespace trimeg {
@@ -59,17 +53,15 @@ struct trimeg_ctx {
 
 namespace trimeg {
 
-// TRIMEG_PUSH_KERNEL_AUTO: with few toroidal modes the coefficient records are small, L1 holds them, and the plain
-// warp-autonomous kernel wins; from about a dozen modes on the records have to sit in shared memory and the warp kernel
-// with the CTA-shared record table wins; with very many modes a record (336 B per mode) is so large that too few of them
-// fit into shared memory for the triangles of a CTA's markers (15 slots at 26 modes) and the plain warp kernel is used
-// again.  Up to 4 modes the Horner loop is so short that the latency-bound rest of a stage weighs more and 16 warps per SM
-// at 128 registers beat 12 at 168 (measurements: DESIGN.md section 5).
+// TRIMEG_PUSH_KERNEL_AUTO (measurements: DESIGN.md section 5).  Few toroidal modes: the per-stage work around the mode
+// loop (equations, locate, bookkeeping) weighs as much as the loop, and the kernel with lane-owned markers -- no grouping by
+// triangle, no evaluation slots, 16 warps per SM -- wins although it loads every coefficient once per marker.  From about
+// eight modes on the shared-memory pipe cannot deliver a coefficient per marker any more (a warp-wide 16-byte load is four
+// wavefronts), two markers of one triangle have to share each load, and the warp kernel with evaluation slots and the
+// CTA-shared record table wins (also beyond 26 modes, where only a dozen records fit).
 inline int auto_push_kernel(int n_modes)
 {
-    if (n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES) return TRIMEG_PUSH_KERNEL_WARP128;
-    return (n_modes >= TRIMEG_AUTO_FUSED_MIN_MODES && n_modes <= TRIMEG_AUTO_FUSED_MAX_MODES) ? TRIMEG_PUSH_KERNEL_WCACHE
-                                                                                              : TRIMEG_PUSH_KERNEL_WARP;
+    return (n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES) ? TRIMEG_PUSH_KERNEL_LANE : TRIMEG_PUSH_KERNEL_WCACHE;
 }
 
 // launch wrappers implemented in trimeg_push.cu; each returns the cudaError of the launch
@@ -79,11 +71,11 @@ cudaError_t launch_gather(trimeg_ctx *c, size_t n, const double *R, const double
 cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP,
                        double *dV, double *dW, cudaStream_t s);
 cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
-// trimeg_push_warp.cu: warp-autonomous schedule, records through L1 (TRIMEG_PUSH_KERNEL_WARP, _WARP128)
-cudaError_t launch_push_warp(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, int variant,
-                             cudaStream_t s);
-
 // trimeg_push_wcache.cu: warp-autonomous with a CTA-shared record table in shared memory (TRIMEG_PUSH_KERNEL_WCACHE)
 cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
+
+// trimeg_push_lane.cu: lane-owned markers, one marker per evaluation in two phases, CTA-shared record table
+// (TRIMEG_PUSH_KERNEL_LANE)
+cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 
 }  // namespace trimeg

@@ -164,8 +164,8 @@ cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     const int variant = (c->push_kernel == TRIMEG_PUSH_KERNEL_AUTO) ? auto_push_kernel(c->field.n_modes) : c->push_kernel;
+    if (variant == TRIMEG_PUSH_KERNEL_LANE) return launch_push_lane(c, m, n, dt, nsteps, s);
     if (variant == TRIMEG_PUSH_KERNEL_WCACHE) return launch_push_wcache(c, m, n, dt, nsteps, s);
-    if (variant == TRIMEG_PUSH_KERNEL_WARP || variant == TRIMEG_PUSH_KERNEL_WARP128) return launch_push_warp(c, m, n, dt, nsteps, variant, s);
     push_kernel<<<grid_for(n, PUSH_BLOCK), PUSH_BLOCK, 0, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;
     return cudaGetLastError();

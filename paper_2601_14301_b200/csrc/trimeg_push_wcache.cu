@@ -189,9 +189,27 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                 ++n_regroup;
 #pragma unroll
                 for (int p = 0; p < P; ++p) { slot[p] = -1; recp[p] = -1; rem[p] = __ballot_sync(FULL, t[p] >= 0); }
-                unsigned kn[P];                                    // markers that stayed in their triangle: they know its record
+                // every lane first looks the triangles of its own markers up (plain loads, all lanes at once): the triangle is
+                // usually in the table already.  kr: record slot, -2 = in the table without a slot, -1 = not (yet) there
+                int kr[P];
 #pragma unroll
-                for (int p = 0; p < P; ++p) kn[p] = __ballot_sync(FULL, t[p] >= 0 && t[p] == t_last[p] && r_last[p] >= 0);
+                for (int p = 0; p < P; ++p) {
+                    kr[p] = (t[p] >= 0 && t[p] == t_last[p] && r_last[p] >= 0) ? r_last[p] : -1;
+                    if (t[p] >= 0 && kr[p] < 0) {
+                        unsigned h = wc_hash(t[p]);
+                        const volatile int *vtag = tag;
+#pragma unroll 1
+                        for (int pr = 0; pr < WC_NPROBE; ++pr) {
+                            const int th = vtag[h];
+                            if (th == t[p]) {
+                                if (state[h] == WC_READY) { __threadfence_block(); const int r = rec_of[h]; kr[p] = (r >= 0) ? r : -2; }
+                                break;
+                            }
+                            if (th == WC_EMPTY) break;
+                            h = (h + 1) & (WC_NBIN - 1);
+                        }
+                    }
+                }
 #pragma unroll 1
                 while (nb < WC_NB_MAX && n_ev < NE) {
                     int pl = -1;
@@ -202,13 +220,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                     unsigned rl = 0;
 #pragma unroll
                     for (int p = 0; p < P; ++p)
-                        if (p == pl) {
-                            cand = t[p]; known = (t_last[p] == t[p]) ? r_last[p] : -1;
-                            rl = (rem[p] & kn[p]) ? (rem[p] & kn[p]) : rem[p];      // a marker that knows the record leads, if there is one
-                        }
+                        if (p == pl) { cand = t[p]; known = kr[p]; rl = rem[p]; }
                     const int tl = __shfl_sync(FULL, cand, __ffs(rl) - 1);
-                    int rec = __shfl_sync(FULL, known, __ffs(rl) - 1);      // the marker sat in this triangle at the last stage: same record
-                    if (rec < 0) rec = wc_lookup(tl, lane, tag, state, rec_of, counters, nslot, M, F, REC, rec_len, rec_stride, n_copied);
+                    int rec = __shfl_sync(FULL, known, __ffs(rl) - 1);
+                    if (rec == -1) rec = wc_lookup(tl, lane, tag, state, rec_of, counters, nslot, M, F, REC, rec_len, rec_stride, n_copied);
+                    else if (rec == -2) rec = -1;
                     const int room = (rec >= 0) ? NE - n_ev : 0;   // no record: the triangle's markers keep slot -1
                     int count = 0;
 #pragma unroll
