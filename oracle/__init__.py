@@ -58,6 +58,8 @@ def lib():
         L.orc_rhs_point.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, dp, dp]
         L.orc_push.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, dp, ip,
                                C.c_double, C.c_int, C.c_int]
+        L.orc_scatter.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, ip, dp]
+        L.orc_scatter.restype = C.c_long
         L.orc_max_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -215,6 +217,19 @@ class Oracle:
         self.L.orc_push(self.h, n, _d(out["R"]), _d(out["Z"]), _d(out["phi"]), _d(out["vpar"]),
                         _d(out["mu"]), _d(out["w"]), _i(cell), float(dt), int(nsteps), int(nthreads))
         out["cell"] = cell
+        return out
+
+    def scatter(self, R, Z, phi, w, cell=None) -> np.ndarray:
+        """p2g projection (O8): rhs[n][v][d] = sum_p w_p Lambda_{v,d}(R_p, Z_p) e^{-i n phi_p} for the modes of set_modes /
+        bell_from_dofs / set_coeffs; complex128 [M][n_vert][6].  cell: optional int32 flags, markers with cell < 0 are skipped."""
+        R, Z, phi, w = _f64(R), _f64(Z), _f64(phi), _f64(w)
+        out = np.zeros((self.n_modes, self.n_vert, 6), dtype=np.complex128)
+        cf = None if cell is None else np.ascontiguousarray(cell, dtype=np.int32)
+        rc = self.L.orc_scatter(self.h, R.size, _d(R), _d(Z), _d(phi), _d(w), _i(cf) if cf is not None else None,
+                                _d(out.view(np.float64)))
+        if rc < 0:
+            raise RuntimeError("singular Bell system")
+        self.last_scatter_count = int(rc)
         return out
 
     def max_threads(self) -> int:

@@ -31,6 +31,8 @@
  *   O6 RHS             A.4-A.6, A.10-A.17 (dA = 0), d ln f_M/dt
  *                                                     PAPER.md:1204-1269
  *   O7 RK4             classic 4-stage integrator
+ *   O8 scatter (p2g)   projection of the marker weights onto the same basis: the adjoint of O4
+ *                                                           PAPER.md:232, 249
  */
 #include <math.h>
 #include <stdint.h>
@@ -62,6 +64,7 @@ typedef struct {
     int n_modes;
     int *mode_n;                   /* toroidal mode numbers n (Def. 19) */
     double *coef;                  /* [n_tri][n_modes][21][2] (re, im) */
+    double **basis;                /* O8: per triangle, lazily, [21][18] monomial coefficients of the 18 basis functions */
 } orc_ctx;
 
 /* ------------------------------------------------------------------ O1 mesh */
@@ -129,6 +132,7 @@ void orc_destroy(orc_ctx *c)
 {
     if (!c) return;
     free(c->r_nodes); free(c->Rv); free(c->Zv); free(c->tri); free(c->geom);
+    if (c->basis) { for (int t = 0; t < c->n_tri; ++t) free(c->basis[t]); free(c->basis); }
     free(c->mode_n); free(c->coef); free(c);
 }
 
@@ -587,6 +591,84 @@ void orc_push(const orc_ctx *c, size_t n, double *R, double *Z, double *phi, dou
         }
         R[p] = y[0]; Z[p] = y[1]; phi[p] = y[2]; vpar[p] = y[3]; w[p] = y[4]; cell[p] = cl;
     }
+}
+
+
+/* ------------------------------------------------------------ O8 scatter (p2g) */
+/* "The charge of each particle is projected onto the basis functions"; the P2G projection is the
+ * counterpart of the G2P interpolation.  With the field written as
+ *     dphi(R, phi, Z) = sum_n Re( sum_{v,d} Y_{n,v,d} Lambda_{v,d}(R, Z) e^{i n phi} )
+ * (Lambda_{v,d}: the C1 basis function of degree of freedom d = f, f_R, f_Z, f_RR, f_RZ, f_ZZ at vertex v),
+ * the projection of the marker weights onto the test functions Lambda_{v,d} e^{i n phi} is
+ *     rhs[n][v][d] = sum_p w_p Lambda_{v,d}(R_p, Z_p) e^{-i n phi_p}
+ * (the conjugate toroidal factor, as in any Galerkin projection onto e^{i n phi}), so that for real weights
+ *     sum_p w_p dphi(x_p) = Re sum_{n,v,d} Y_{n,v,d} conj(rhs[n][v][d]):   scatter is the adjoint of gather (O4).
+ * Plain definition, marker by marker: locate -> the 18 basis functions of the triangle at (xi, eta) -> add.
+ * Lambda_j restricted to a triangle is the quintic whose nodal values are the unit vector e_j: its 21 monomial
+ * coefficients are the solution of the same 21 x 21 system as in O2 (bell_factor / bell_solve) with right-hand side e_j. */
+static const double *bell_basis(orc_ctx *c, int t)
+{
+    if (c->basis[t]) return c->basis[t];
+    long double A[21][21], rs[21]; int piv[21];
+    if (bell_factor(c, t, A, rs, piv)) return NULL;
+    double *B = (double *)malloc(sizeof(double) * 21 * 18);
+    for (int j = 0; j < 18; ++j) {
+        long double b[21];
+        for (int r = 0; r < 21; ++r) b[r] = (r == j) ? 1.0L : 0.0L;
+        bell_solve(A, rs, piv, b);
+        for (int k = 0; k < 21; ++k) B[k * 18 + j] = (double)b[k];
+    }
+    c->basis[t] = B;
+    return B;
+}
+
+/* rhs: [n_modes][n_vert][6][2] (re, im), overwritten.  cell_flag may be NULL; markers with cell_flag[p] < 0, and markers
+ * outside the mesh, contribute nothing.  Returns the number of markers that contributed, or -1 (singular element). */
+long orc_scatter(orc_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const double *w,
+                 const int32_t *cell_flag, double *rhs)
+{
+    const size_t per_mode = (size_t)c->n_vert * 6 * 2;
+    memset(rhs, 0, sizeof(double) * per_mode * (c->n_modes > 0 ? c->n_modes : 0));
+    if (!c->basis) c->basis = (double **)calloc((size_t)c->n_tri, sizeof(double *));
+    /* pass 1 (serial): triangles and local coordinates, basis tables of the triangles that hold markers */
+    int32_t *tp = (int32_t *)malloc(sizeof(int32_t) * (n ? n : 1));
+    double *xe = (double *)malloc(sizeof(double) * 2 * (n ? n : 1));
+    long used = 0;
+    for (size_t p = 0; p < n; ++p) {
+        tp[p] = -1;
+        if (cell_flag && cell_flag[p] < 0) continue;
+        double xi, eta;
+        int t = locate_one(c, R[p], Z[p], &xi, &eta);
+        if (t < 0) continue;
+        if (!bell_basis(c, t)) { free(tp); free(xe); return -1; }
+        tp[p] = t; xe[2 * p] = xi; xe[2 * p + 1] = eta;
+        ++used;
+    }
+    /* pass 2: one toroidal mode per thread; inside a mode the markers are added in their order */
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int m = 0; m < c->n_modes; ++m) {
+        double *out = rhs + per_mode * m;
+        const double nn = (double)c->mode_n[m];
+        for (size_t p = 0; p < n; ++p) {
+            const int t = tp[p];
+            if (t < 0) continue;
+            const double *B = c->basis[t];
+            const int *v = c->tri + 3 * t;
+            const double xi = xe[2 * p], eta = xe[2 * p + 1];
+            double mono[21];
+            for (int k = 0; k < 21; ++k) { int i, j; mono_ij(k, &i, &j); mono[k] = ipow(xi, i) * ipow(eta, j); }
+            const double Er = cos(nn * phi[p]), Ei = -sin(nn * phi[p]);        /* e^{-i n phi} */
+            for (int j = 0; j < 18; ++j) {
+                double lam = 0.0;
+                for (int k = 0; k < 21; ++k) lam += B[k * 18 + j] * mono[k];
+                double *o = out + ((size_t)v[j / 6] * 6 + (j % 6)) * 2;
+                o[0] += w[p] * lam * Er;
+                o[1] += w[p] * lam * Ei;
+            }
+        }
+    }
+    free(tp); free(xe);
+    return used;
 }
 
 int orc_max_threads(void)
