@@ -146,6 +146,24 @@ int trimeg_gather(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, c
 int trimeg_rhs(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, double *dRdt, double *dZdt,
                double *dphidt, double *dvpardt, double *dwdt, trimeg_stream stream);
 
+/* ---- particle-to-grid projection / scatter (row f1) -----------------------------------------
+ * "The charge of each particle is projected onto the basis functions" (section 3.1; the P2G
+ * functions of PAPER.md:249; section 6.3: the phase the thesis left on the CPU as "not suitable
+ * for GPU offloading").  The adjoint of trimeg_gather: with Lambda_{v,d} the C1 basis function of degree of
+ * freedom d = (f, f_R, f_Z, f_RR, f_RZ, f_ZZ) at vertex v,
+ *     rhs[n][v][d] = sum_p w_p Lambda_{v,d}(R_p, Z_p) e^{-i n phi_p}
+ * for the toroidal modes n of the uploaded field (trimeg_field_upload supplies the mode list; the field values
+ * are not used), so that for real weights  sum_p w_p dphi(x_p) = Re sum Y_{n,v,d} conj(rhs[n][v][d])  for any
+ * nodal values Y.  rhs_dev: [n_modes][n_vert][6] complex128, device memory, overwritten.
+ * m: the marker arrays (R, Z, phi, w and cell are read; cell is a HINT, cell < 0 = marker skipped; markers
+ * outside the mesh contribute nothing).  Any marker order is correct and costs the same: the markers are
+ * brought into triangle order by an index sort inside (8 B of context scratch per marker, plus 288 B per
+ * triangle and mode for the per-triangle results).  The summation order inside a triangle is unspecified
+ * (results reproduce to rounding).  Multi-GPU: each GPU scatters its markers; one all-reduce (sum) of rhs
+ * is the only collective.  Errors: INVALID_ARG, NO_FIELD (no mode list uploaded), ALLOC, CUDA. */
+int trimeg_scatter(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, void *rhs_dev,
+                   trimeg_stream stream);
+
 /* ---- cell sort (row a1) ---------------------------------------------------------------------
  * Why: the thesis's kernel reads the field tables with 18 % of its accesses coalesced and leaves the
  * on-chip shared memory unused (section 6.4); with the markers ordered by triangle the
@@ -190,7 +208,7 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *         per marker; same record table; 12 warps per CTA.
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX.  (Schedules of earlier rounds that lost everywhere were
- * removed: lock-step CTA tiles -- commit 3003ca4 --, warp kernels reading the records through L1 -- commit 99b8bd5.) */
+ * removed: lock-step CTA tiles -- commit 3003ca4 --, warp kernels reading the records through L1 -- commit a10a1dc.) */
 #define TRIMEG_PUSH_KERNEL_AUTO (-1)
 #define TRIMEG_PUSH_KERNEL_THREAD 0
 #define TRIMEG_PUSH_KERNEL_LANE 1

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libtrimeg.so")
 EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_download_coeffs",
-    "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_sort", "trimeg_compact",
+    "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
     "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
 )
@@ -70,6 +70,7 @@ def load() -> C.CDLL:
     L.trimeg_locate.argtypes = [vp, sz, vp, vp, vp, vp]
     L.trimeg_gather.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.trimeg_rhs.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp, vp, vp, vp, vp]
+    L.trimeg_scatter.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp]
     L.trimeg_sort.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp]
     L.trimeg_compact.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, C.POINTER(sz), vp]
     L.trimeg_push.argtypes = [vp, C.POINTER(trimeg_markers), sz, dbl, i32, vp]
@@ -226,6 +227,17 @@ class Context:
         _check(self.L.trimeg_rhs(self.h, C.byref(ms), n, *[_ptr(out[k], torch.float64) for k in
                                                              ("dRdt", "dZdt", "dphidt", "dvpardt", "dwdt")],
                                  _stream(stream)), "trimeg_rhs")
+        return out
+
+    def scatter(self, m: Dict[str, torch.Tensor], n: Optional[int] = None, out: Optional[torch.Tensor] = None,
+                stream=None) -> torch.Tensor:
+        """rhs[n][v][d] = sum_p w_p Lambda_{v,d}(R_p, Z_p) e^{-i n phi_p}: complex128 [n_modes][n_vert][6]."""
+        n = m["R"].numel() if n is None else int(n)
+        ms = _markers(m, n)
+        if out is None:
+            out = torch.empty((self.n_modes, self.n_vert, 6), dtype=torch.complex128, device=m["R"].device)
+        _check(self.L.trimeg_scatter(self.h, C.byref(ms), n, _ptr(out, torch.complex128) if self.n_modes else C.c_void_p(0),
+                                     _stream(stream)), "trimeg_scatter")
         return out
 
     def sort(self, m: Dict[str, torch.Tensor], want_perm: bool = False, n: Optional[int] = None,

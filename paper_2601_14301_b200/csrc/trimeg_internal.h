@@ -42,6 +42,10 @@ struct trimeg_ctx {
     void *d_scratch;
     size_t scratch_bytes;
     int *d_bins;                    // n_tri + 2 counters
+    // row f1 (scatter): vertex -> (triangle, local vertex) adjacency in CSR form, per-triangle results (grown on demand)
+    int *d_adj_off, *d_adj;
+    void *d_trirhs;
+    size_t trirhs_bytes;
     // host path: two marker sets + permutation of the last trimeg_push_host batch (grown on demand)
     void *d_hbuf;
     size_t hbuf_bytes;
@@ -71,6 +75,12 @@ cudaError_t launch_gather(trimeg_ctx *c, size_t n, const double *R, const double
 cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP,
                        double *dV, double *dW, cudaStream_t s);
 cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
+// trimeg_lib.cu: exclusive scan of nb ints in place, bins[nb] = total
+void launch_scan(int *bins, int nb, cudaStream_t s);
+// trimeg_scatter.cu: row f1, rhs [n_modes][n_vert][6] complex; cell, perm: int32[n] scratch; tri_rhs [n_tri][n_modes][18] complex
+cudaError_t launch_scatter(trimeg_ctx *c, const trimeg_markers &m, size_t n, double2 *rhs, int32_t *cell, int32_t *perm,
+                           double2 *tri_rhs, cudaStream_t s);
+
 // trimeg_push_wcache.cu: warp-autonomous with a CTA-shared record table in shared memory (TRIMEG_PUSH_KERNEL_WCACHE)
 cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 

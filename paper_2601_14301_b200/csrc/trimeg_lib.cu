@@ -8,6 +8,7 @@
 #include <new>
 
 #include "trimeg_internal.h"
+#include "trimeg_mesh.cuh"
 #include "bell_tables.inc"
 
 using namespace trimeg;
@@ -39,20 +40,6 @@ struct DeviceGuard {
     if (!guard__.ok) return TRIMEG_ERR_CUDA
 
 // ============================================================================ a0: mesh tables
-__device__ __forceinline__ int vertex_id(int n_theta, int i, int j)
-{   // v(i, j) = 1 + (i-1) n_theta + (j mod n_theta), i >= 1
-    if (j >= n_theta) j -= n_theta;
-    return 1 + (i - 1) * n_theta + j;
-}
-__device__ __forceinline__ void tri_vertices(int n_theta, int t, int v[3])
-{
-    if (t < n_theta) { v[0] = 0; v[1] = vertex_id(n_theta, 1, t); v[2] = vertex_id(n_theta, 1, t + 1); return; }
-    const int u = t - n_theta, k = u & 1, c = u >> 1, i = c / n_theta + 1, j = c % n_theta;
-    v[0] = vertex_id(n_theta, i, j);
-    if (k == 0) { v[1] = vertex_id(n_theta, i + 1, j); v[2] = vertex_id(n_theta, i + 1, j + 1); }
-    else { v[1] = vertex_id(n_theta, i + 1, j + 1); v[2] = vertex_id(n_theta, i, j + 1); }
-}
-
 // geometry factors with individually rounded operations (they feed the bit-exact locator)
 __global__ void geom_kernel(int n_r, int n_theta, int n_tri, const double *__restrict__ vR,
                             const double *__restrict__ vZ, double *__restrict__ geom, double *__restrict__ rin2)
@@ -187,6 +174,10 @@ __global__ void scan_kernel(int *bins, int nb)
     int run = part[tid] - sum;
     for (int k = lo; k < hi; ++k) { const int c = bins[k]; bins[k] = run; run += c; }
     if (tid == nt - 1) bins[nb] = part[tid];
+}
+
+namespace trimeg {
+void launch_scan(int *bins, int nb, cudaStream_t s) { scan_kernel<<<1, 1024, 0, s>>>(bins, nb); }
 }
 
 struct MarkerScratch { double *R, *Z, *phi, *vpar, *mu, *w; int32_t *cell; };
@@ -409,6 +400,24 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
         double rin2 = 0.0;
         if (cudaGetLastError() != cudaSuccess ||
             cudaMemcpy(&rin2, d_rin2, sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        {   // vertex -> (triangle, local vertex) adjacency for the scatter's assembly, triangles ascending
+            const size_t ne = 3 * (size_t)c->n_tri;
+            int *off = (int *)calloc((size_t)c->n_vert + 1, sizeof(int)), *adj = (int *)malloc(sizeof(int) * ne);
+            int *fill = (int *)calloc((size_t)c->n_vert, sizeof(int));
+            bool ok = off && adj && fill;
+            if (ok) {
+                int v[3];
+                for (int t = 0; t < c->n_tri; ++t) { tri_vertices(n_theta, t, v); for (int k = 0; k < 3; ++k) off[v[k] + 1]++; }
+                for (int q = 0; q < c->n_vert; ++q) off[q + 1] += off[q];
+                for (int t = 0; t < c->n_tri; ++t) { tri_vertices(n_theta, t, v); for (int k = 0; k < 3; ++k) adj[off[v[k]] + fill[v[k]]++] = 3 * t + k; }
+                ok = cudaMalloc(&c->d_adj_off, sizeof(int) * ((size_t)c->n_vert + 1)) == cudaSuccess &&
+                     cudaMalloc(&c->d_adj, sizeof(int) * ne) == cudaSuccess &&
+                     cudaMemcpy(c->d_adj_off, off, sizeof(int) * ((size_t)c->n_vert + 1), cudaMemcpyHostToDevice) == cudaSuccess &&
+                     cudaMemcpy(c->d_adj, adj, sizeof(int) * ne, cudaMemcpyHostToDevice) == cudaSuccess;
+            }
+            free(off); free(adj); free(fill);
+            if (!ok) { rc = TRIMEG_ERR_ALLOC; break; }
+        }
         c->mesh.n_r = n_r; c->mesh.n_theta = n_theta; c->mesh.n_tri = c->n_tri;
         c->mesh.geom = c->d_geom; c->mesh.r_nodes = c->d_r_nodes;
         c->mesh.Rax = hR[0]; c->mesh.Zax = hZ[0]; c->mesh.rin2 = rin2;
@@ -434,6 +443,7 @@ int trimeg_mesh_destroy(trimeg_ctx *c)
     if (!c) return TRIMEG_ERR_INVALID_ARG;
     DeviceGuard guard__(c->device);
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
+    cudaFree(c->d_adj_off); cudaFree(c->d_adj); cudaFree(c->d_trirhs);
     cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
     if (c->hstreams_ready) {
         for (int k = 0; k < 3; ++k) cudaStreamDestroy(c->hstream[k]);
@@ -580,6 +590,28 @@ int trimeg_push(trimeg_ctx *c, trimeg_markers *m, size_t n, double dt, int nstep
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
     if (n == 0) return TRIMEG_OK;
     CU_TRY(launch_push(c, *m, n, dt, nsteps, (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_scatter(trimeg_ctx *c, const trimeg_markers *m, size_t n, void *rhs_dev, trimeg_stream stream)
+{
+    if (!c || (n > 0 && !markers_ok(m)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    const int n_modes = c->field.n_modes;
+    if (n_modes == 0) return TRIMEG_OK;
+    if (!rhs_dev) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
+    int rc = ensure_scratch(c, 2 * align_up((n ? n : 1) * sizeof(int32_t), 256));
+    if (rc) return rc;
+    const size_t need = sizeof(double2) * 18 * (size_t)c->n_tri * n_modes;
+    if (c->trirhs_bytes < need) {
+        if (c->d_trirhs) { CU_TRY(cudaDeviceSynchronize()); cudaFree(c->d_trirhs); c->d_trirhs = nullptr; c->trirhs_bytes = 0; }
+        if (cudaMalloc(&c->d_trirhs, need) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_ALLOC; }
+        c->trirhs_bytes = need;
+    }
+    int32_t *cell = (int32_t *)c->d_scratch, *perm = (int32_t *)((char *)c->d_scratch + align_up((n ? n : 1) * sizeof(int32_t), 256));
+    static const trimeg_markers none = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    CU_TRY(launch_scatter(c, n ? *m : none, n, (double2 *)rhs_dev, cell, perm, (double2 *)c->d_trirhs, (cudaStream_t)stream));
     return TRIMEG_OK;
 }
 
@@ -780,6 +812,7 @@ int trimeg_release_host_buffers(trimeg_ctx *c)
         for (int k = 0; k < 3; ++k) CU_TRY(cudaStreamSynchronize(c->hstream[k]));
     if (c->d_hbuf) { cudaFree(c->d_hbuf); c->d_hbuf = nullptr; c->hbuf_bytes = 0; }
     if (c->d_scratch) { CU_TRY(cudaDeviceSynchronize()); cudaFree(c->d_scratch); c->d_scratch = nullptr; c->scratch_bytes = 0; }
+    if (c->d_trirhs) { CU_TRY(cudaDeviceSynchronize()); cudaFree(c->d_trirhs); c->d_trirhs = nullptr; c->trirhs_bytes = 0; }
     return TRIMEG_OK;
 }
 
