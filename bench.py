@@ -476,6 +476,7 @@ def run_gpu(args, wl):
                          "algorithmic_bytes_per_gather": 52, "algorithmic_flops_per_gather": flops_per_gather(len(w4.modes)),
                          "rows": rows, "clocks": sampler.stop(), "config": workload_config(w4)}
         c4.close()
+        sweep["scatter_cfg5"] = scatter_run(inputs.WORKLOADS["cfg5"], 3, fp64_peak, hbm_peak, with_oracle=not args.no_check)
 
     if rank == 0:
         line = {
@@ -495,6 +496,92 @@ def run_gpu(args, wl):
     return 0
 
 
+def flops_per_scatter(n_modes: int) -> int:
+    """Particle-to-grid projection (row f1), per marker: locator 25 + 20 for the monomials, per mode 21 complex x real
+    multiply-adds (84 flops) + the rotation of the toroidal factor (8)."""
+    return 45 + 92 * n_modes
+
+
+def scatter_run(wl, reps, fp64_peak, hbm_peak, with_oracle=True):
+    """trimeg_scatter on the workload's marker batch (order as drawn), device-timed per call with CUDA events."""
+    import torch
+    from paper_2601_14301_b200 import binding, inputs
+    ctx = binding.context_for(wl, inputs)
+    ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
+    n = wl.n_markers
+    m = inputs.markers(wl, n=n)
+    m["w"] = np.random.default_rng([wl.seed, 7]).standard_normal(n)
+    d = binding.markers_to_device(m, "cuda")
+    ctx.locate(d["R"], d["Z"], cell=d["cell"])
+    out = torch.empty((len(wl.modes), wl.n_vert, 6), dtype=torch.complex128, device="cuda")
+    n_in = int((d["cell"] >= 0).sum())
+    fl = flops_per_scatter(len(wl.modes))
+    rows = []
+    for order in ("as drawn", "cell-sorted"):
+        if order == "cell-sorted":
+            ctx.sort(d)                                   # the order the push leaves the markers in
+        st0 = ctx.get_stats()
+        ts = []
+        for rep in range(3 + reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            ctx.scatter(d, out=out)
+            e1.record()
+            torch.cuda.synchronize()
+            if rep >= 3:
+                ts.append(e0.elapsed_time(e1) * 1e-3)
+        launches = (ctx.get_stats()["n_launches"] - st0["n_launches"]) // (3 + reps)
+        t = sorted(ts)[len(ts) // 2]
+        rows.append({"order": order, "value": n_in / t, "unit": "markers/s", "ms_per_call": t * 1e3, "launches_per_call": int(launches),
+                     "achieved_tflops": fl * n_in / t * 1e-12, "frac": fl * n_in / t * 1e-12 / fp64_peak})
+    best = rows[1]
+    res = {"metric": "markers projected per second (trimeg_scatter, row f1)", "value": best["value"], "unit": "markers/s",
+           "ms_per_call": best["ms_per_call"], "markers": n, "markers_inside": n_in, "order": best["order"], "rows": rows,
+           "roofline": {"bound": "alu", "kernel": "whole call, 6 launches (scatter_moments_kernel dominates)", "achieved": best["achieved_tflops"],
+                        "peak": fp64_peak, "unit": "TFLOP/s", "frac": best["frac"],
+                        "algorithmic_flops_per_marker": fl, "algorithmic_bytes_per_marker": 36,
+                        "hbm_time_frac_of_fp64_time": (36.0 / (hbm_peak * 1e9)) / (fl / (fp64_peak * 1e12))},
+           "config": workload_config(wl)}
+    if with_oracle:
+        import oracle
+        o = oracle.from_workload(wl, inputs)
+        o.set_modes(wl.modes)
+        stride = max(1, n // (1 << 17))
+        sl = slice(0, None, stride)
+        t0 = time.perf_counter()
+        want = o.scatter(m["R"][sl], m["Z"][sl], m["phi"][sl], m["w"][sl])
+        dt_o = time.perf_counter() - t0
+        ds = binding.markers_to_device({k: np.ascontiguousarray(v[sl]) for k, v in m.items()}, "cuda")
+        ctx.locate(ds["R"], ds["Z"], cell=ds["cell"])
+        got = ctx.scatter(ds).cpu().numpy()
+        err = max(float(np.abs(got[k] - want[k]).max() / np.abs(want[k]).max()) for k in range(len(wl.modes)))
+        assert err < 1e-11, f"scatter parity check failed: {err}"
+        res["oracle_check"] = {"sample_markers": int(m["R"][sl].size), "max_rel_err_per_mode": err}
+        res["cpu_baseline"] = {"value": o.last_scatter_count / dt_o, "unit": "markers/s", "kind": "oracle", "cores": o.max_threads(),
+                               "sample": f"every {stride}-th marker ({m['R'][sl].size}), oracle.scatter (one toroidal mode per thread)"}
+    ctx.close()
+    del d, out
+    torch.cuda.empty_cache()
+    return res
+
+
+def run_scatter(args, wl):
+    import torch
+    from paper_2601_14301_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(0)
+    binding.load()
+    ctx = binding.context_for(wl, inputs)
+    fp64_peak = ctx.measure_fp64_peak()
+    ctx.close()
+    hbm_peak, _ = load_peaks()
+    res = scatter_run(wl, max(3, args.steps), fp64_peak, hbm_peak)
+    res.update({"n_gpus": 1, "dtype": "f64", "data": "synthetic", "higher_is_better": True})
+    print(json.dumps(res), flush=True)
+    return 0
+
+
 def run_gather_sweep(args, wl):
     """BASELINE.json configs[3]: gather-only sweep (dphi, d/dR, d/dZ at the markers, no push) on the 64 x 256 mesh with
     modes {0, 5, 10}, marker counts 2^16 .. 2^max in powers of 4, markers as drawn and sorted by triangle.  One JSON line."""
@@ -508,7 +595,7 @@ def run_gather_sweep(args, wl):
     ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
     hbm_peak, _ = load_peaks()
     fp64_peak = ctx.measure_fp64_peak()
-    rows = gather_rows(ctx, wl, range(16, args.max_log2 + 1, 2), args.steps, hbm_peak, fp64_peak)
+    rows = gather_rows(ctx, wl, range(args.min_log2, args.max_log2 + 1, 2), args.steps, hbm_peak, fp64_peak)
     line = {"metric": "field gathers/sec (dphi, d/dR, d/dZ; 3 toroidal modes)", "unit": "gathers/s", "n_gpus": 1,
             "config": workload_config(wl), "dtype": "f64", "data": "synthetic", "hbm_peak_gbs": hbm_peak, "fp64_peak_tflops": fp64_peak,
             "algorithmic_bytes_per_gather": 52, "algorithmic_flops_per_gather": flops_per_gather(len(wl.modes)), "rows": rows}
@@ -522,11 +609,13 @@ def main():
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--op", default="push", choices=["push", "scatter"], help="scatter: time trimeg_scatter (row f1) on the workload's markers")
     ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
     ap.add_argument("--n-modes", type=int, default=0, help="override the toroidal mode list by n = 0, 2, ..., 2 (K - 1) (schedule selection sweeps)")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
+    ap.add_argument("--min-log2", type=int, default=16, help="cfg4 gather sweep: smallest marker count 2^k")
     ap.add_argument("--max-log2", type=int, default=28, help="cfg4 gather sweep: largest marker count 2^k")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -545,6 +634,8 @@ def main():
         return run_gather_sweep(args, wl)
     if args.impl == "reference":
         return run_reference(args, wl)
+    if args.op == "scatter":
+        return run_scatter(args, wl)
     return run_gpu(args, wl)
 
 

@@ -11,8 +11,8 @@
 // (1) is the hot part: a rank-one update of a 21 x 2M matrix per marker.  Markers are brought into triangle order by an
 // index sort (histogram, scan, index scatter -- a few bytes per marker, no marker data is moved), one CTA takes one
 // triangle: it stages the monomials and the weighted toroidal factors of a batch of markers in shared memory and every
-// thread accumulates a 7 x 1 tile of complex moments in registers (7 monomials x one mode), the markers of the batch
-// divided among the lanes that share a mode.  (2) uses the same fixed right inverse and edge bubbles as the library's Bell
+// thread accumulates a 7 x 2 tile of complex moments in registers (7 monomials x 2 modes), the markers of the batch
+// divided among the lanes that share the modes.  (2) uses the same fixed right inverse and edge bubbles as the library's Bell
 // expansion (bell_kernel), transposed -- no linear solve.  (3) runs by vertex over a precomputed vertex -> triangle
 // adjacency: no atomics, and the result does not depend on the order of the triangles.
 #include "trimeg_internal.h"
@@ -26,6 +26,7 @@ namespace {
 constexpr int SC_THREADS = 96;      // 3 warps: warp w accumulates monomials 7 w .. 7 w + 6
 constexpr int SC_BATCH = 64;        // markers staged per round
 constexpr int SC_MBLK = 16;         // toroidal modes per pass over the markers of a triangle
+constexpr int SC_MT = 2;            // toroidal modes per thread
 
 // cell of every marker (hint < 0: lost, skipped), for the index sort
 __global__ void __launch_bounds__(256) scatter_locate_kernel(MeshDev M, size_t n, const double *__restrict__ R,
@@ -93,18 +94,28 @@ __global__ void __launch_bounds__(SC_THREADS) scatter_moments_kernel(MeshDev M, 
 
     for (int m0 = 0; m0 < n_modes; m0 += SC_MBLK) {
         const int mb = min(SC_MBLK, n_modes - m0);       // modes of this block
-        int mp = 1;
-        while (mp < mb) mp <<= 1;                        // lanes of a warp = mp modes x (32 / mp) marker slices
-        const int n_sl = 32 / mp, my_mode = lane & (mp - 1), my_sl = lane / mp;
-        double ar[7], ai[7];
+        int ng = 1;
+        while (SC_MT * ng < mb) ng <<= 1;                // lanes of a warp = ng groups of SC_MT modes x (32 / ng) marker slices
+        const int n_sl = 32 / ng, my_grp = lane & (ng - 1), my_sl = lane / ng, mfill = SC_MT * ng;
+        double ar[7][SC_MT], ai[7][SC_MT];               // 7 monomials x SC_MT modes of complex moments per thread
 #pragma unroll
-        for (int i = 0; i < 7; ++i) ar[i] = ai[i] = 0.0;
+        for (int i = 0; i < 7; ++i)
+#pragma unroll
+            for (int k = 0; k < SC_MT; ++k) ar[i][k] = ai[i][k] = 0.0;
+        // the marker a thread stages in the next batch is fetched (perm -> R, Z, phi, w: two dependent trips to HBM) while
+        // the current batch is being accumulated
+        double nxR = 0.0, nxZ = 0.0, nxP = 0.0, nxW = 0.0;
+        if (tid < SC_BATCH && s0 + tid < s1) { const int p = perm[s0 + tid]; nxR = R[p]; nxZ = Z[p]; nxP = phi[p]; nxW = w[p]; }
         for (int b0 = s0; b0 < s1; b0 += SC_BATCH) {
             const int nb = min(SC_BATCH, s1 - b0);
             __syncthreads();                             // the previous batch has been consumed
+            const double cR = nxR, cZ = nxZ, cP = nxP, cW = nxW;
+            if (tid < SC_BATCH && b0 + SC_BATCH + tid < s1) {
+                const int p = perm[b0 + SC_BATCH + tid];
+                nxR = R[p]; nxZ = Z[p]; nxP = phi[p]; nxW = w[p];
+            }
             if (tid < nb) {                              // ---- stage: monomials, weighted toroidal factors
-                const int p = perm[b0 + tid];
-                const double dx = __dsub_rn(R[p], v0.x), dz = __dsub_rn(Z[p], v0.y);   // local coordinates as the locator's (rule L2)
+                const double dx = __dsub_rn(cR, v0.x), dz = __dsub_rn(cZ, v0.y);   // local coordinates as the locator's (rule L2)
                 const double xi = __dadd_rn(__dmul_rn(gx.x, dx), __dmul_rn(gx.y, dz));
                 const double eta = __dadd_rn(__dmul_rn(ge.x, dx), __dmul_rn(ge.y, dz));
                 double xp[6], ep[6];
@@ -115,7 +126,7 @@ __global__ void __launch_bounds__(SC_THREADS) scatter_moments_kernel(MeshDev M, 
                 for (int d = 0; d < 6; ++d)
 #pragma unroll
                     for (int j = 0; j <= d; ++j) mono[d * (d + 1) / 2 + j][tid] = xp[d - j] * ep[j];
-                const double ph = phi[p], wp = w[p];
+                const double ph = cP, wp = cW;
                 if (F.is_ap) {                           // e^{-i n phi}: rotation from mode to mode
                     double sr, cr, sd, cd;
                     sincos((double)(F.n_first + m0 * F.n_step) * ph, &sr, &cr);
@@ -134,30 +145,39 @@ __global__ void __launch_bounds__(SC_THREADS) scatter_moments_kernel(MeshDev M, 
                         wE[tid][k] = make_double2(wp * cr, -wp * sr);
                     }
                 }
+                for (int k = mb; k < mfill; ++k) wE[tid][k] = make_double2(0.0, 0.0);     // modes past the end of the list
             }
             __syncthreads();
-            if (my_mode < mb) {                          // ---- accumulate: 7 monomials x one mode per thread
-                for (int p = my_sl; p < nb; p += n_sl) {
-                    const double2 e = wE[p][my_mode];
+            // ---- accumulate: a 7 x SC_MT tile of complex moments per thread (15 loaded doubles per 56 multiply-adds: the
+            // shared-memory pipe delivers 16 doubles per cycle and SM, the FP64 pipe takes 64 multiply-adds)
+            for (int p = my_sl; p < nb; p += n_sl) {
+                double2 e[SC_MT];
 #pragma unroll
-                    for (int i = 0; i < 7; ++i) {
-                        const double mk = mono[7 * wrp + i][p];
-                        ar[i] = fma(mk, e.x, ar[i]); ai[i] = fma(mk, e.y, ai[i]);
-                    }
+                for (int k = 0; k < SC_MT; ++k) e[k] = wE[p][SC_MT * my_grp + k];
+#pragma unroll
+                for (int i = 0; i < 7; ++i) {
+                    const double mk = mono[7 * wrp + i][p];
+#pragma unroll
+                    for (int k = 0; k < SC_MT; ++k) { ar[i][k] = fma(mk, e[k].x, ar[i][k]); ai[i][k] = fma(mk, e[k].y, ai[i][k]); }
                 }
             }
         }
         // ---- sum over the marker slices, moments to shared memory
 #pragma unroll
         for (int i = 0; i < 7; ++i)
-            for (int off = mp; off < 32; off <<= 1) {
-                ar[i] += __shfl_xor_sync(0xffffffffu, ar[i], off);
-                ai[i] += __shfl_xor_sync(0xffffffffu, ai[i], off);
-            }
-        __syncthreads();
-        if (my_sl == 0 && my_mode < mb)
 #pragma unroll
-            for (int i = 0; i < 7; ++i) mom[my_mode][7 * wrp + i] = make_double2(ar[i], ai[i]);
+            for (int k = 0; k < SC_MT; ++k)
+                for (int off = ng; off < 32; off <<= 1) {
+                    ar[i][k] += __shfl_xor_sync(0xffffffffu, ar[i][k], off);
+                    ai[i][k] += __shfl_xor_sync(0xffffffffu, ai[i][k], off);
+                }
+        __syncthreads();
+        if (my_sl == 0)
+#pragma unroll
+            for (int k = 0; k < SC_MT; ++k)
+                if (SC_MT * my_grp + k < mb)
+#pragma unroll
+                    for (int i = 0; i < 7; ++i) mom[SC_MT * my_grp + k][7 * wrp + i] = make_double2(ar[i][k], ai[i][k]);
         __syncthreads();
         // ---- (2) transposed Bell expansion, one thread per (mode, real / imaginary part)
         for (int q = tid; q < 2 * mb; q += SC_THREADS) {

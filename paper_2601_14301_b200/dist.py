@@ -63,6 +63,15 @@ def reduce_sum(x: float, device="cpu") -> float:
     return float(t.item())
 
 
+def allreduce_sum_(t: torch.Tensor) -> torch.Tensor:
+    """In-place sum over ranks: the ONE data-path collective of the PIC cycle's particle side -- the right-hand side of
+    trimeg_scatter (row f1: every GPU projects its own markers, the [n_modes][n_vert][6] complex vector is summed; <= 60 MB
+    for the largest config).  complex tensors are reduced through their real view (NCCL has no complex type)."""
+    if dist.is_initialized():
+        dist.all_reduce(torch.view_as_real(t) if t.is_complex() else t, op=dist.ReduceOp.SUM)
+    return t
+
+
 def aggregate(units_local: float, seconds_local: float, counters: Dict[str, int], device="cpu") -> Dict[str, float]:
     """Whole-job numbers: units summed over ranks, time = max over ranks, counters summed."""
     out = dict(units=reduce_sum(units_local, device), seconds=reduce_max(seconds_local, device))

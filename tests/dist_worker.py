@@ -21,7 +21,17 @@ def main():
     D.barrier()
     # rank r "processes" (r + 1) * 100 units in (r + 1) seconds and launches 3 + r kernels
     agg = D.aggregate((rank + 1) * 100.0, float(rank + 1), {"launches": 3 + rank})
-    out = {"rank": rank, "world": world, "lo": lo, "hi": hi, "agg": agg,
+    # row f1 across ranks: every rank projects its shard of the markers (here with the oracle, on the CPU), one all-reduce
+    import oracle
+    import torch
+    o = oracle.from_workload(wl, inputs)
+    o.set_modes(wl.modes)
+    mm = inputs.markers(wl, n=1001, seed=77)
+    part = torch.from_numpy(o.scatter(mm["R"][lo:hi], mm["Z"][lo:hi], mm["phi"][lo:hi], mm["vpar"][lo:hi]))
+    total = D.allreduce_sum_(part.clone()).numpy()
+    whole = o.scatter(mm["R"], mm["Z"], mm["phi"], mm["vpar"])
+    scatter_err = float(np.abs(total - whole).max() / np.abs(whole).max())
+    out = {"rank": rank, "scatter_err": scatter_err, "world": world, "lo": lo, "hi": hi, "agg": agg,
            "checksum": float(np.sum(m["R"])), "max_all": D.reduce_max(float(rank)), "sum_all": D.reduce_sum(float(rank))}
     with open(os.path.join(sys.argv[1], f"rank{rank}.json"), "w") as f:
         json.dump(out, f)

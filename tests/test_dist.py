@@ -32,6 +32,8 @@ def test_two_rank_gloo_aggregation(tmp_path):
         assert o["agg"]["units"] == 300.0 and o["agg"]["seconds"] == 2.0 and o["agg"]["value"] == 150.0
         assert o["agg"]["launches"] == 7.0 and o["max_all"] == 1.0 and o["sum_all"] == 1.0
     assert out[0]["checksum"] != out[1]["checksum"]
+    # row f1: shards projected separately + one all-reduce of the right-hand side = projection of all markers
+    assert all(o["scatter_err"] < 1e-13 for o in out)
 
 
 def test_reference_arm_under_torchrun_prints_one_line():
