@@ -25,7 +25,8 @@ def build(force: bool = False, verbose: bool = False, profile: bool = False) -> 
     profile = profile or os.environ.get("TRIMEG_PROFILE", "") not in ("", "0")
     if not force and not profile and os.path.exists(LIB) and all(os.path.getmtime(LIB) >= os.path.getmtime(d) for d in deps):
         return LIB
-    cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + (["-DTRIMEG_PROFILE"] if profile else []) + \
+    extra = os.environ.get("TRIMEG_NVCC_EXTRA", "").split()          # experiments only (e.g. "-Xptxas -O1")
+    cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + (["-DTRIMEG_PROFILE"] if profile else []) + \
           ["-o", LIB] + [os.path.join(CSRC, s) for s in SOURCES]
     subprocess.check_call(cmd)
     return LIB

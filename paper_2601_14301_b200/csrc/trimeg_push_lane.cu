@@ -153,15 +153,12 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
     for (int step = 0; step < nsteps; ++step) {
 #pragma unroll 1
         for (int stage = 0; stage < 4; ++stage) {
+            const int ps = (stage == 0) ? Y_R : S_R;                 // stage 0 is evaluated at the start-of-step state itself
 #pragma unroll 1
             for (int p = 0; p < 2; ++p) {
                 const int q = lane + 32 * p;
                 const bool act = (flags[q] & FL_ACTIVE) != 0;
                 const int t = act ? cell[q] : -1;
-                if (act && stage == 0) {
-#pragma unroll
-                    for (int k = 0; k < 5; ++k) S[(S_R + k) * NW + q] = S[(Y_R + k) * NW + q];
-                }
                 // ------------------------------------------------ the record of the marker's triangle
                 const int tl_prev = p ? t_last1 : t_last0;
                 int rec = (t == tl_prev) ? (p ? r_last1 : r_last0) : -1;      // still in the triangle of the last stage: same record
@@ -203,17 +200,17 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
                             const double2 *recp = REC + (size_t)rec * rec_stride;
                             tg.t = t; tg.v0 = recp[rec_len]; tg.gx = recp[rec_len + 1]; tg.ge = recp[rec_len + 2];
                             // local coordinates exactly as bary_rn() (rule L2)
-                            const double dx = __dsub_rn(S[S_R * NW + q], tg.v0.x), dz = __dsub_rn(S[S_Z * NW + q], tg.v0.y);
+                            const double dx = __dsub_rn(S[(ps + 0) * NW + q], tg.v0.x), dz = __dsub_rn(S[(ps + 1) * NW + q], tg.v0.y);
                             const double xi = __dadd_rn(__dmul_rn(tg.gx.x, dx), __dmul_rn(tg.gx.y, dz));
                             const double eta = __dadd_rn(__dmul_rn(tg.ge.x, dx), __dmul_rn(tg.ge.y, dz));
                             double f, fx, fe, fp;
-                            gather_lane(F, recp, xi, eta, S[S_P * NW + q], zero, f, fx, fe, fp);
+                            gather_lane(F, recp, xi, eta, S[(ps + 2) * NW + q], zero, f, fx, fe, fp);
                             fv.f = f; fv.fphi = fp;
                             fv.fR = fma(tg.gx.x, fx, tg.ge.x * fe);             // d/dR
                             fv.fZ = fma(tg.gx.y, fx, tg.ge.y * fe);             // d/dZ
                         } else {                                                 // no record slot: coefficients from global memory
-                            const Bary b = bary_rn(M, t, S[S_R * NW + q], S[S_Z * NW + q]);
-                            fv = gather(F, t, b, S[S_P * NW + q]);
+                            const Bary b = bary_rn(M, t, S[(ps + 0) * NW + q], S[(ps + 1) * NW + q]);
+                            fv = gather(F, t, b, S[(ps + 2) * NW + q]);
                             ++n_fallback;
                         }
                     }

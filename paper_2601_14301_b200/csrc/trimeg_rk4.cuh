@@ -37,8 +37,9 @@ __device__ __forceinline__ void advance(const MeshDev &M, const PhysDev &Ph, dou
                                         unsigned char *flags, int q, int stage, const FieldVal &fv, double dt,
                                         double hdt, double dt6, const TriGeom *tg = nullptr)
 {
-    const double R = S[S_R * NW + q], Z = S[S_Z * NW + q];
-    const double v = S[S_V * NW + q], w = S[S_W * NW + q], mu = S[S_MU * NW + q];
+    const int ps = (stage == 0) ? Y_R : S_R;               // stage 0 is evaluated at the start-of-step state itself (no copy Y -> S)
+    const double R = S[(ps + 0) * NW + q], Z = S[(ps + 1) * NW + q];
+    const double v = S[(ps + 3) * NW + q], w = S[(ps + 4) * NW + q], mu = S[S_MU * NW + q];
     const Rates k = rhs_point(Ph, R, Z, v, mu, w, fv);
     const double yR = S[Y_R * NW + q], yZ = S[Y_Z * NW + q], yP = S[Y_P * NW + q];
     const double yV = S[Y_V * NW + q], yW = S[Y_W * NW + q];
