@@ -133,8 +133,11 @@ int trimeg_locate(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, i
  * g2p subroutine of the pullback / density / g2p2g kernels):
  * dphi, d dphi/dR, d dphi/dZ (and d dphi/dphi if dphi_dphi != NULL) at the markers.
  * cell_hint may be NULL.  Markers outside the mesh get 0.  NO_FIELD if no field is loaded.
- * Any marker order is correct; cell-sorted markers (trimeg_sort) with their cells as hint take the
- * warp-grouped kernel (several markers of one triangle share each coefficient load). */
+ * Any marker order is correct.  Batches of 2^18 markers and more that come with hints and a field of up
+ * to 7 modes: cell-sorted markers (hinted cells that never decrease, markers flagged < 0 aside; up to
+ * n / 16 exceptions are tolerated) take a kernel that keeps the coefficient records of its triangles in
+ * shared memory and fetches the next markers while it evaluates the current ones; the device decides
+ * (both kernels are enqueued, the one not chosen returns at once). */
 int trimeg_gather(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, const double *phi,
                   const int32_t *cell_hint, double *dphi, double *dphi_dR, double *dphi_dZ,
                   double *dphi_dphi, trimeg_stream stream);

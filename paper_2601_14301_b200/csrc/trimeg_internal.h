@@ -88,4 +88,9 @@ cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n,
 // (TRIMEG_PUSH_KERNEL_LANE)
 cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 
+// trimeg_push_lane.cu: the gather alone for cell-sorted markers; gate / want: runs iff (*gate * 16 <= n) == want
+cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const int32_t *hint,
+                               double *f, double *fR, double *fZ, double *fP, const int *gate, int want, cudaStream_t s);
+constexpr size_t GATHER_LANE_MIN = 1 << 18;     // below, two more kernel launches cost more than the lane kernel saves
+
 }  // namespace trimeg

@@ -388,7 +388,7 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
             cudaMalloc(&c->d_vZ, sizeof(double) * c->n_vert) != cudaSuccess ||
             cudaMalloc(&c->d_r_nodes, sizeof(double) * (n_r + 1)) != cudaSuccess ||
             cudaMalloc(&c->d_geom, sizeof(double) * 6 * (size_t)c->n_tri) != cudaSuccess ||
-            cudaMalloc(&c->d_bins, sizeof(int) * ((size_t)c->n_tri + 2)) != cudaSuccess ||
+            cudaMalloc(&c->d_bins, sizeof(int) * ((size_t)c->n_tri + 8)) != cudaSuccess ||
             cudaMalloc(&c->d_stats, sizeof(Stats)) != cudaSuccess ||
             cudaMalloc(&d_rin2, sizeof(double)) != cudaSuccess) { rc = TRIMEG_ERR_ALLOC; break; }
         if (cudaMemcpy(c->d_vR, hR, sizeof(double) * c->n_vert, cudaMemcpyHostToDevice) != cudaSuccess ||

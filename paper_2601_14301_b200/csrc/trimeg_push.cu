@@ -10,6 +10,7 @@
 namespace trimeg {
 
 constexpr int PUSH_BLOCK = 128;
+static inline unsigned grid_for(size_t n, int block) { return (unsigned)((n + block - 1) / block); }
 constexpr double TWO_PI = 6.283185307179586476925286766559;
 
 __device__ __forceinline__ void add_stats(Stats *st, int lost, int moved)
@@ -33,23 +34,42 @@ __global__ void __launch_bounds__(256) locate_kernel(MeshDev M, size_t n, const 
     cell[p] = locate(M, R[p], Z[p], -1, b, moved);
 }
 
+// GATED: device-side choice between this kernel and gather_lane_kernel (runs iff (*gate * 16 <= n) == want), grid-stride loop
+// over the markers so that the launch that is not chosen costs nothing; else one thread per marker.
+template <bool GATED>
 __global__ void __launch_bounds__(256) gather_kernel(MeshDev M, FieldDev F, size_t n, const double *__restrict__ R,
                                                      const double *__restrict__ Z, const double *__restrict__ phi,
                                                      const int32_t *__restrict__ hint, double *__restrict__ f,
                                                      double *__restrict__ fR, double *__restrict__ fZ,
-                                                     double *__restrict__ fP)
+                                                     double *__restrict__ fP, const int *gate, int want)
 {
-    const size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-    if (p >= n) return;
-    Bary b;
-    int moved = 0;
-    const double r = R[p], z = Z[p];
-    const int t = locate(M, r, z, hint ? hint[p] : -1, b, moved);
-    FieldVal v;
-    v.f = v.fR = v.fZ = v.fphi = 0.0;
-    if (t >= 0) v = gather(F, t, b, phi[p]);
-    f[p] = v.f; fR[p] = v.fR; fZ[p] = v.fZ;
-    if (fP) fP[p] = v.fphi;
+    if (GATED && (((size_t)*gate * 16 <= n) ? 1 : 0) != want) return;
+    size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (!GATED && p >= n) return;
+    do {
+        if (GATED && p >= n) break;
+        Bary b;
+        int moved = 0;
+        const double r = R[p], z = Z[p];
+        const int t = locate(M, r, z, hint ? hint[p] : -1, b, moved);
+        FieldVal v;
+        v.f = v.fR = v.fZ = v.fphi = 0.0;
+        if (t >= 0) v = gather(F, t, b, phi[p]);
+        f[p] = v.f; fR[p] = v.fR; fZ[p] = v.fZ;
+        if (fP) fP[p] = v.fphi;
+        p += (size_t)gridDim.x * blockDim.x;
+    } while (GATED);
+}
+
+// number of places where the hinted cells decrease (markers flagged < 0 aside): 0 for cell-sorted markers
+__global__ void __launch_bounds__(256) hint_order_kernel(size_t n, const int32_t *__restrict__ hint, int *__restrict__ count)
+{
+    int bad = 0;
+    const size_t stride = (size_t)gridDim.x * blockDim.x, n_up = (n + 31) / 32 * 32;
+    for (size_t p = (size_t)blockIdx.x * blockDim.x + threadIdx.x; p < n_up; p += stride)
+        if (p > 0 && p < n) { const int a = hint[p - 1], c = hint[p]; bad += (a >= 0 && c >= 0 && c < a) ? 1 : 0; }
+    bad = __reduce_add_sync(0xffffffffu, bad);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(count, bad);
 }
 
 // locate -> gather -> equilibrium -> equations at one phase-space point (rows a2-a5)
@@ -132,7 +152,6 @@ __global__ void __launch_bounds__(PUSH_BLOCK) push_kernel(MeshDev M, FieldDev F,
 }
 
 // ------------------------------------------------------------------------------- wrappers
-static inline unsigned grid_for(size_t n, int block) { return (unsigned)((n + block - 1) / block); }
 
 cudaError_t launch_locate(trimeg_ctx *c, size_t n, const double *R, const double *Z, int32_t *cell, cudaStream_t s)
 {
@@ -146,9 +165,32 @@ cudaError_t launch_gather(trimeg_ctx *c, size_t n, const double *R, const double
                           const int32_t *hint, double *f, double *fR, double *fZ, double *fP, cudaStream_t s)
 {
     if (n == 0) return cudaSuccess;
-    gather_kernel<<<grid_for(n, 256), 256, 0, s>>>(c->mesh, c->field, n, R, Z, phi, hint, f, fR, fZ, fP);
+    int *gate = nullptr;
+    const bool two = hint && n >= GATHER_LANE_MIN && c->field.n_modes > 0 && c->field.n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES;
+    if (two) {
+        // Large batches with hints: cell-sorted markers (hinted cells that never decrease; up to n / 16 exceptions are
+        // tolerated) take the lane kernel (records in shared memory, inputs prefetched), anything else the thread-per-marker
+        // kernel.  The device decides: both are enqueued, the one not chosen returns at once.
+        gate = c->d_bins + c->n_tri + 4;
+        cudaError_t e = cudaMemsetAsync(gate, 0, sizeof(int), s);
+        if (e != cudaSuccess) return e;
+        hint_order_kernel<<<(unsigned)min((size_t)grid_for(n, 256), (size_t)c->n_sm * 8), 256, 0, s>>>(n, hint, gate);
+        c->n_launches++;
+    }
+    // the thread-per-marker kernel lives on L1 (every lane fetches its own record): keep the SM's carve-out at maximum L1
+    // whatever kernel ran before
+    if (!two) {
+        gather_kernel<false><<<grid_for(n, 256), 256, 0, s>>>(c->mesh, c->field, n, R, Z, phi, hint, f, fR, fZ, fP, nullptr, 0);
+        c->n_launches++;
+        return cudaGetLastError();
+    }
+    cudaFuncSetAttribute(gather_kernel<true>, cudaFuncAttributePreferredSharedMemoryCarveout, (int)cudaSharedmemCarveoutMaxL1);
+    gather_kernel<true><<<(unsigned)max((size_t)c->n_sm * 64, n / 1024), 256, 0, s>>>(c->mesh, c->field, n, R, Z, phi, hint,
+                                                                                                    f, fR, fZ, fP, gate, 0);
     c->n_launches++;
-    return cudaGetLastError();
+    const cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return launch_gather_lane(c, n, R, Z, phi, hint, f, fR, fZ, fP, gate, 1, s);
 }
 
 cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP,

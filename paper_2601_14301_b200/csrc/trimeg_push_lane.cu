@@ -266,6 +266,129 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
     }
 }
 
+
+// ---------------------------------------------------------------------------------------------- gather alone (configs[3])
+// The gather for cell-sorted markers, with the machinery above and no RK4 state: a CTA of GL_WARPS warps walks over chunks of
+// n_pass x 32 consecutive markers per warp (n_pass <= GL_PASSES_MAX, fewer for small batches so that every SM gets chunks); a lane takes one marker per pass: the inputs of the next pass are fetched
+// while the current one is evaluated (the thread-per-marker kernel waits for its loads at 12-24 warps per SM), the record of
+// the marker's triangle (coefficients + geometry row) comes from the CTA's table in shared memory, the evaluation is the
+// two-phase mode loop.  The warps meet once per chunk; the table is emptied there when it is nearly full.  gate / want:
+// device-side choice between this kernel and gather_kernel (*gate = number of places where the hinted cells decrease).
+constexpr int GL_WARPS = 16;
+constexpr int GL_PASSES_MAX = 16;
+
+__global__ void __launch_bounds__(32 * GL_WARPS, 1) gather_lane_kernel(MeshDev M, FieldDev F, size_t n, const double *__restrict__ R,
+                                                                       const double *__restrict__ Z, const double *__restrict__ phi,
+                                                                       const int32_t *__restrict__ hint, double *__restrict__ f,
+                                                                       double *__restrict__ fR, double *__restrict__ fZ,
+                                                                       double *__restrict__ fP, int nslot, int zero, const int *gate, int want,
+                                                                       int n_pass)
+{
+    if ((((size_t)*gate * 16 <= n) ? 1 : 0) != want) return;
+    constexpr unsigned FULL = 0xffffffffu;
+    extern __shared__ __align__(16) unsigned char smem_g[];
+    const int tid = threadIdx.x, lane = tid & 31, wib = tid >> 5;
+    int *tag = reinterpret_cast<int *>(smem_g);
+    volatile int *state = tag + LN_NBIN;
+    int *rec_of = tag + 2 * LN_NBIN;
+    int *counters = tag + 3 * LN_NBIN;
+    const int rec_len = F.n_modes * NCOEF;
+    const int rec_stride = (rec_len + 3) | 1;
+    double2 *REC = reinterpret_cast<double2 *>(smem_g + (LN_TABLE_BYTES + 15) / 16 * 16);
+    for (int k = tid; k < LN_NBIN; k += 32 * GL_WARPS) { tag[k] = LN_EMPTY; state[k] = 0; rec_of[k] = -1; }
+    if (tid < 4) counters[tid] = 0;
+    __syncthreads();
+    const size_t PER_WARP = 32 * (size_t)n_pass, PER_CTA = PER_WARP * GL_WARPS;
+    const size_t n_chunks = (n + PER_CTA - 1) / PER_CTA;
+    unsigned n_copied = 0;
+    for (size_t chunk = blockIdx.x; chunk < n_chunks; chunk += gridDim.x) {
+        const size_t w0 = chunk * PER_CTA + (size_t)wib * PER_WARP;
+        size_t p = w0 + lane;
+        double nR = 0.0, nZ = 0.0, nP = 0.0;
+        int nH = -1;
+        if (p < n) { nR = R[p]; nZ = Z[p]; nP = phi[p]; nH = hint[p]; }
+#pragma unroll 1
+        for (int pass = 0; pass < n_pass; ++pass, p += 32) {
+            const double r = nR, z = nZ, ph = nP;
+            const int h = nH;
+            const bool in = p < n;
+            if (pass + 1 < n_pass && p + 32 < n) { nR = R[p + 32]; nZ = Z[p + 32]; nP = phi[p + 32]; nH = hint[p + 32]; }
+            // the hinted triangle first, with the geometry row of its record in shared memory (no trip to global memory on the
+            // way): inside by the margin (rule L3) -> done; else the complete locator and a second look-up
+            int t = (in && h >= 0 && h < M.n_tri) ? h : -1;
+            int rec = -1;
+            Bary b;
+            b.xi = b.eta = b.l0 = b.xR = b.xZ = b.eR = b.eZ = 0.0;
+            bool redo = in;
+#pragma unroll 1
+            for (int round = 0; round < 2; ++round) {
+                bool ask = redo && t >= 0;
+                if (ask) {                                   // own probe
+                    unsigned hh = ln_hash(t);
+                    const volatile int *vtag = tag;
+#pragma unroll 1
+                    for (int pr = 0; pr < LN_NPROBE; ++pr) {
+                        const int th = vtag[hh];
+                        if (th == t) {
+                            if (state[hh] == LN_READY) { __threadfence_block(); rec = rec_of[hh]; ask = false; }
+                            break;
+                        }
+                        if (th == LN_EMPTY) break;
+                        hh = (hh + 1) & (LN_NBIN - 1);
+                    }
+                }
+                unsigned need = __ballot_sync(FULL, ask);    // triangles not in the table yet: the warp brings them in
+#pragma unroll 1
+                while (need) {
+                    const int tl = __shfl_sync(FULL, t, __ffs(need) - 1);
+                    const int rr = ln_lookup(tl, lane, tag, state, rec_of, counters, nslot, M, F, REC, rec_len, rec_stride, n_copied);
+                    const bool mine = ask && (t == tl);
+                    if (mine) rec = rr;
+                    need &= ~__ballot_sync(FULL, mine);
+                }
+                if (round == 1) break;
+                if (redo && t >= 0 && rec >= 0) {            // barycentric test exactly as bary_rn() (rule L2)
+                    const double2 *gq = REC + (size_t)rec * rec_stride + rec_len;
+                    const double2 v0 = gq[0], gx = gq[1], ge = gq[2];
+                    const double dx = __dsub_rn(r, v0.x), dz = __dsub_rn(z, v0.y);
+                    b.xi = __dadd_rn(__dmul_rn(gx.x, dx), __dmul_rn(gx.y, dz));
+                    b.eta = __dadd_rn(__dmul_rn(ge.x, dx), __dmul_rn(ge.y, dz));
+                    b.l0 = __dsub_rn(__dsub_rn(1.0, b.xi), b.eta);
+                    b.xR = gx.x; b.xZ = gx.y; b.eR = ge.x; b.eZ = ge.y;
+                    if (fmin(fmin(b.xi, b.eta), b.l0) > LOC_TAU) redo = false;
+                }
+                if (!__any_sync(FULL, redo)) break;
+                if (redo) { int moved = 0; t = locate(M, r, z, h, b, moved); rec = -1; }
+            }
+            if (in) {
+                double v = 0.0, vR = 0.0, vZ = 0.0, vP = 0.0;
+                if (t >= 0) {
+                    if (rec >= 0) {
+                        double fx, fe;
+                        gather_lane(F, REC + (size_t)rec * rec_stride, b.xi, b.eta, ph, zero, v, fx, fe, vP);
+                        vR = fma(b.xR, fx, b.eR * fe);
+                        vZ = fma(b.xZ, fx, b.eZ * fe);
+                    } else {
+                        const FieldVal fv = gather(F, t, b, ph);
+                        v = fv.f; vR = fv.fR; vZ = fv.fZ; vP = fv.fphi;
+                    }
+                }
+                f[p] = v; fR[p] = vR; fZ[p] = vZ;
+                if (fP) fP[p] = vP;
+            }
+        }
+        // ---- all warps meet; the table is emptied when it is nearly full
+        __syncthreads();
+        const int claimed = counters[0];
+        __syncthreads();
+        if (claimed > min(nslot, LN_NBIN * 3 / 4) - 16) {
+            for (int k = tid; k < LN_NBIN; k += 32 * GL_WARPS) { tag[k] = LN_EMPTY; state[k] = 0; rec_of[k] = -1; }
+            if (tid == 0) counters[0] = 0;
+            __syncthreads();
+        }
+    }
+}
+
 template <int WARPS>
 cudaError_t launch_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
@@ -286,6 +409,27 @@ cudaError_t launch_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 }
 
 }  // namespace
+
+cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const int32_t *hint,
+                               double *f, double *fR, double *fZ, double *fP, const int *gate, int want, cudaStream_t s)
+{
+    constexpr size_t SMEM = 160 * 1024;
+    cudaError_t e = cudaFuncSetAttribute(gather_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
+    if (e != cudaSuccess) return e;
+    const size_t fixed = (LN_TABLE_BYTES + 15) / 16 * 16;
+    const size_t rec_bytes = sizeof(double2) * ((NCOEF * (size_t)c->field.n_modes + 3) | 1);
+    int nslot = (int)((SMEM - fixed) / rec_bytes);
+    if (nslot > LN_NBIN * 3 / 4) nslot = LN_NBIN * 3 / 4;
+    size_t n_pass = n / ((size_t)c->n_sm * 4 * 32 * GL_WARPS);                 // at least ~4 chunks per SM
+    n_pass = n_pass < 1 ? 1 : (n_pass > GL_PASSES_MAX ? GL_PASSES_MAX : n_pass);
+    const size_t per_cta = (size_t)32 * n_pass * GL_WARPS;
+    size_t ctas = (n + per_cta - 1) / per_cta;
+    if (ctas > (size_t)c->n_sm * 4) ctas = (size_t)c->n_sm * 4;
+    gather_lane_kernel<<<(unsigned)ctas, 32 * GL_WARPS, fixed + (size_t)nslot * rec_bytes, s>>>(c->mesh, c->field, n, R, Z, phi, hint, f, fR, fZ, fP,
+                                                                                                 nslot, 0, gate, want, (int)n_pass);
+    c->n_launches++;
+    return cudaGetLastError();
+}
 
 cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {

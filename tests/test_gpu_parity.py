@@ -168,6 +168,47 @@ def test_gather_parity(B, inputs, name, n):
             assert e < 1e-12, (k, e)
 
 
+@pytest.mark.parametrize("name,n", [("cfg2", 300007), ("cfg3", 270001)])
+def test_gather_large_batches_sorted_and_unsorted(B, inputs, name, n):
+    """Batches of 2^18 markers and more with hints: cell-sorted markers take the lane kernel (records in shared memory,
+    inputs prefetched), anything else the thread-per-marker kernel; the device decides.  Hints: none, the true cells
+    (unsorted), stale, sorted, sorted with a few markers out of place and flagged ones."""
+    wl, o, ctx, _, coef = _setup(B, inputs, name)
+    m = inputs.markers(wl, n=n)
+    m["R"][::1013] = wl.R0 + 1.5 * wl.a                       # some markers outside the mesh
+    want = o.gather(m["R"], m["Z"], m["phi"])
+    d = _dev(B, m)
+    cells = torch.from_numpy(want["cell"]).cuda()
+    keys = ("dphi", "dphi_dR", "dphi_dZ", "dphi_dphi")
+
+    def check(got, ref):
+        for k in keys:
+            e = rel_err(got[k].cpu().numpy(), ref[k], np.abs(ref[k]).max()).max()
+            assert e < 1e-12, (k, e)
+
+    for hint in (None, cells, torch.zeros(n, dtype=torch.int32, device="cuda")):
+        check(ctx.gather(d["R"], d["Z"], d["phi"], cell_hint=hint), want)
+    key = torch.where(cells < 0, torch.full_like(cells, wl.n_tri), cells)
+    order = torch.argsort(key, stable=True)
+    ds = {k: d[k][order].contiguous() for k in ("R", "Z", "phi")}
+    hs = cells[order].contiguous()
+    on = order.cpu().numpy()
+    ref = {k: want[k][on] for k in keys}
+    lost = want["cell"][on] < 0
+    assert lost.sum() > 100
+    got = ctx.gather(ds["R"], ds["Z"], ds["phi"], cell_hint=hs)           # lost markers (hint -1) at the end
+    check(got, ref)
+    for k in keys:
+        assert np.all(got[k].cpu().numpy()[lost] == 0.0)
+    h2 = hs.clone()
+    h2[::777] = 0                                                          # a few stale hints: still "sorted enough"
+    check(ctx.gather(ds["R"], ds["Z"], ds["phi"], cell_hint=h2), ref)
+    g3 = ctx.gather(ds["R"], ds["Z"], ds["phi"], cell_hint=hs, want_dphi=False)
+    assert "dphi_dphi" not in g3
+    for k in keys[:3]:
+        assert rel_err(g3[k].cpu().numpy(), ref[k], np.abs(ref[k]).max()).max() < 1e-12
+
+
 # ----------------------------------------------------------------------------- a4 + a5
 @pytest.mark.parametrize("name,n,variant,wmode", [("cfg1", 4096, 0, 0), ("cfg1", 1000, 1, 1), ("cfg2", 50021, 0, 0),
                                                   ("cfg3", 20011, 0, 0), ("cfg5", 20011, 0, 0)])
