@@ -330,6 +330,42 @@ class PushRun:
         self.torch.cuda.empty_cache()
 
 
+def e2e_run(ctx, wl, m_np, k_e2e, device_value, D=None, dev=None):
+    """The metric through trimeg_push_host with pinned host SoA buffers: every call starts from the config's initial state
+    (restored untimed), H2D and D2H inside the timed region; one warm-up call (it also allocates)."""
+    import torch
+    n = m_np["R"].size
+    keys = ("R", "Z", "phi", "vpar", "mu", "w")
+    h0 = {k: torch.from_numpy(m_np[k]) for k in keys}
+    h = {k: torch.empty_like(h0[k]).pin_memory() for k in keys}
+    h["cell"] = torch.empty(n, dtype=torch.int32).pin_memory()
+    e2e_s, e2e_units = 0.0, 0
+    for it in range(1 + k_e2e):
+        for k in keys:
+            h[k].copy_(h0[k])
+        h["cell"].fill_(-1)
+        if D is not None:
+            D.barrier()
+        torch.cuda.synchronize()
+        t0 = time.perf_counter()
+        ctx.push_host(h, wl.dt, wl.nsteps, locate_first=True)     # returns when the results are in the host buffers
+        dt_call = time.perf_counter() - t0
+        if it > 0:
+            e2e_s += dt_call
+            e2e_units += int((h["cell"] >= 0).sum()) * wl.nsteps  # markers lost on the way count zero steps
+    if D is not None:
+        ag2 = D.aggregate(e2e_units, e2e_s, {}, device=dev)
+        value = ag2["value"]
+    else:
+        value = e2e_units / e2e_s
+    del h, h0
+    ctx.release_host_buffers()
+    return {"value": value, "unit": UNIT, "h2d_bytes_per_step": n * 6 * 8, "d2h_bytes_per_step": n * (5 * 8 + 4), "steps": k_e2e,
+            "frac_of_device_value": value / device_value,
+            "api": "trimeg_push_host (pinned host SoA in: chunks of the batch go H2D -> locate -> cell sort -> push, re-sort "
+                   "every 10 steps -> unsort -> D2H on three streams, copies under the push of other chunks)"}
+
+
 def gather_rows(ctx, wl, log2s, reps, hbm_peak, fp64_peak):
     """BASELINE.json configs[3]: gather only (dphi, d/dR, d/dZ, no push), markers as drawn and sorted by triangle."""
     import torch
@@ -413,32 +449,7 @@ def run_gpu(args, wl):
     # ---- e2e: host buffers through the C ABI, copies inside the timed region
     e2e = None
     if not args.no_e2e:
-        m_np = run.m_np
-        keys = ("R", "Z", "phi", "vpar", "mu", "w")
-        h0 = {k: torch.from_numpy(m_np[k]) for k in keys}
-        h = {k: torch.empty_like(h0[k]).pin_memory() for k in keys}
-        h["cell"] = torch.empty(n, dtype=torch.int32).pin_memory()
-        k_e2e = max(1, min(args.steps, 3))
-        e2e_s, e2e_units = 0.0, 0
-        for it in range(1 + k_e2e):                       # first call: warm-up (also allocates)
-            for k in keys:
-                h[k].copy_(h0[k])                         # every call starts from the config's initial state (untimed)
-            h["cell"].fill_(-1)
-            D.barrier()
-            torch.cuda.synchronize()
-            t0 = time.perf_counter()
-            ctx.push_host(h, wl.dt, wl.nsteps, locate_first=True)     # returns when the results are in the host buffers
-            dt_call = time.perf_counter() - t0
-            if it > 0:
-                e2e_s += dt_call
-                e2e_units += int((h["cell"] >= 0).sum()) * wl.nsteps  # markers lost on the way count zero steps
-        ag2 = D.aggregate(e2e_units, e2e_s, {}, device=dev)
-        e2e = {"value": ag2["value"], "unit": UNIT, "h2d_bytes_per_step": n * 6 * 8,
-               "d2h_bytes_per_step": n * (5 * 8 + 4), "steps": k_e2e, "frac_of_device_value": ag2["value"] / agg["value"],
-               "api": "trimeg_push_host (pinned host SoA in: chunks of the batch go H2D -> locate -> cell sort -> push, re-sort "
-                      "every 10 steps -> unsort -> D2H on three streams, copies under the push of other chunks)"}
-        del h, h0
-        ctx.release_host_buffers()
+        e2e = e2e_run(ctx, wl, run.m_np, max(1, min(args.steps, 3)), agg["value"], D, dev)
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -459,11 +470,12 @@ def run_gpu(args, wl):
             out = r2.run(2, 3)
             rf = r2.roofline(fp64_peak, out["seconds"])
             chk = None if args.no_check else r2.check_against_oracle(stride=max(1, w2.n_markers // 2048))
+            e2 = None if args.no_e2e else e2e_run(r2.ctx, w2, r2.m_np, 1, out["units"] / out["seconds"])
             sweep[name] = {"value": out["units"] / out["seconds"], "unit": UNIT, "steps": 2, "warmup": 3,
                            "ms_per_step": out["seconds"] / 2 * 1e3, "kernel": rf["kernel"], "frac": rf["frac"],
                            "achieved_tflops": rf["achieved"], "avg_launch_ms": rf["avg_launch_ms"],
                            "push_share_of_step": rf["push_share_of_step"], "clocks": out["clocks"],
-                           "config": workload_config(w2, extra={"sort_every": r2.sort_every}), "oracle_check": chk}
+                           "config": workload_config(w2, extra={"sort_every": r2.sort_every}), "oracle_check": chk, "e2e": e2}
             r2.close()
             del r2
         w4 = inputs.WORKLOADS["cfg4"]

@@ -58,6 +58,10 @@ def lib():
         L.orc_rhs_point.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, dp, dp]
         L.orc_push.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, dp, ip,
                                C.c_double, C.c_int, C.c_int]
+        L.orc_rhs_point_em.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, dp, dp]
+        L.orc_set_aux_coef.argtypes = [C.c_void_p, C.c_int, dp]
+        L.orc_rhs_em.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, dp, ip, dp, dp, dp, dp, dp]
+        L.orc_pullback.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, ip]
         L.orc_scatter.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, ip, dp]
         L.orc_scatter.restype = C.c_long
         L.orc_max_threads.restype = C.c_int
@@ -218,6 +222,43 @@ class Oracle:
                         _d(out["mu"]), _d(out["w"]), _i(cell), float(dt), int(nsteps), int(nthreads))
         out["cell"] = cell
         return out
+
+    # ---- electromagnetic terms (O9, O10): dA^s = aux 0, dA^h = aux 1, on the mode list of the main field
+    # (set_modes / bell_from_dofs / set_coeffs drop the aux tables: set them afterwards)
+    def set_aux_coeffs(self, which: int, coef: Optional[np.ndarray]):
+        if coef is None:
+            self.L.orc_set_aux_coef(self.h, int(which), None)
+            return
+        coef = np.ascontiguousarray(coef, dtype=np.complex128)
+        assert coef.shape == (self.n_tri, self.n_modes, 21), coef.shape
+        self.L.orc_set_aux_coef(self.h, int(which), _d(coef.view(np.float64)))
+
+    def rhs_point_em(self, R, Z, upar, mu, w, fld) -> np.ndarray:
+        """EM right-hand side with the field values handed in: fld [n][3][4] = (value, d/dR, d/dZ, d/dphi) of dPhi, dA^s, dA^h."""
+        a = [_f64(x) for x in (R, Z, upar, mu, w)]
+        fld = np.ascontiguousarray(fld, dtype=np.float64)
+        n = a[0].size
+        assert fld.shape == (n, 3, 4)
+        out = np.empty((n, 5), dtype=np.float64)
+        self.L.orc_rhs_point_em(self.h, n, *[_d(x) for x in a], _d(fld), _d(out))
+        return out
+
+    def rhs_em(self, R, Z, phi, upar, mu, w):
+        a = [_f64(x) for x in (R, Z, phi, upar, mu, w)]
+        n = a[0].size
+        cell = np.empty(n, dtype=np.int32)
+        o = [np.empty(n) for _ in range(5)]
+        self.L.orc_rhs_em(self.h, n, *[_d(x) for x in a], _i(cell), *[_d(x) for x in o])
+        return dict(cell=cell, dRdt=o[0], dZdt=o[1], dphidt=o[2], dudt=o[3], dwdt=o[4])
+
+    def pullback(self, R, Z, phi, upar, w, cell=None):
+        """Returns (u_new, w_new); inputs untouched."""
+        R, Z, phi = _f64(R), _f64(Z), _f64(phi)
+        u = np.array(upar, dtype=np.float64, copy=True, order="C")
+        ww = np.array(w, dtype=np.float64, copy=True, order="C")
+        cf = None if cell is None else np.ascontiguousarray(cell, dtype=np.int32)
+        self.L.orc_pullback(self.h, R.size, _d(R), _d(Z), _d(phi), _d(u), _d(ww), _i(cf) if cf is not None else None)
+        return u, ww
 
     def scatter(self, R, Z, phi, w, cell=None) -> np.ndarray:
         """p2g projection (O8): rhs[n][v][d] = sum_p w_p Lambda_{v,d}(R_p, Z_p) e^{-i n phi_p} for the modes of set_modes /

@@ -33,6 +33,9 @@
  *   O7 RK4             classic 4-stage integrator
  *   O8 scatter (p2g)   projection of the marker weights onto the same basis: the adjoint of O4
  *                                                           PAPER.md:232, 249
+ *   O9 EM RHS          one right-hand side with dA^s, dA^h (mixed variables): A.7-A.9, A.14-A.17 with the
+ *                      ideal Ohm's law substituted
+ *   O10 pullback       u_par, w after the pullback transformation
  */
 #include <math.h>
 #include <stdint.h>
@@ -65,6 +68,7 @@ typedef struct {
     int *mode_n;                   /* toroidal mode numbers n (Def. 19) */
     double *coef;                  /* [n_tri][n_modes][21][2] (re, im) */
     double **basis;                /* O8: per triangle, lazily, [21][18] monomial coefficients of the 18 basis functions */
+    double *coef_aux[2];           /* O9/O10: dA^s (0) and dA^h (1), same layout and mode list as coef; NULL = identically zero */
 } orc_ctx;
 
 /* ------------------------------------------------------------------ O1 mesh */
@@ -133,6 +137,7 @@ void orc_destroy(orc_ctx *c)
     if (!c) return;
     free(c->r_nodes); free(c->Rv); free(c->Zv); free(c->tri); free(c->geom);
     if (c->basis) { for (int t = 0; t < c->n_tri; ++t) free(c->basis[t]); free(c->basis); }
+    free(c->coef_aux[0]); free(c->coef_aux[1]);
     free(c->mode_n); free(c->coef); free(c);
 }
 
@@ -146,6 +151,7 @@ void orc_set_params(orc_ctx *c, const orc_params *p) { c->p = *p; }
 void orc_set_modes(orc_ctx *c, int n_modes, const int *mode_n)
 {
     free(c->mode_n); free(c->coef);
+    free(c->coef_aux[0]); free(c->coef_aux[1]); c->coef_aux[0] = c->coef_aux[1] = NULL;
     c->n_modes = n_modes;
     c->mode_n = (int *)malloc(sizeof(int) * (n_modes > 0 ? n_modes : 1));
     if (n_modes > 0) memcpy(c->mode_n, mode_n, sizeof(int) * n_modes);
@@ -669,6 +675,121 @@ long orc_scatter(orc_ctx *c, size_t n, const double *R, const double *Z, const d
     }
     free(tp); free(xe);
     return used;
+}
+
+/* ------------------------------------------------- O9 electromagnetic right-hand side (mixed variables) */
+/* Fields: dPhi (coef), dA^s (coef_aux[0]), dA^h (coef_aux[1]), dA_par = dA^s + dA^h (A.1), all on the same
+ * basis.  The marker's velocity coordinate is u_par = v_par + (q_s/m_s) <dA^h>; the gyro-average <.> is the
+ * identity (off, as in the thesis's own runs).  Vector form, eps = (m_s/q_s) rho_0 B_0:
+ *   B*_par = B + eps u_par b.curl b;  b0* = b + (eps u_par/B*_par) curl b  [variant 1: (B/B*_par) b + ...]   (A.4-A.6 with u_par)
+ *   b* = b0* + C_E grad(dA^s) x b,  C_E = rho_0 B_0/B*_par                                                (A.7-A.9)
+ *   R0dot, u0dot: A.10-A.13 with u_par (sign of A.11 as reading G1)
+ *   dRdot = C_E b x grad(dG) - (q_s/m_s) dA^h b*,   grad(dG) = grad(dPhi) - u_par grad(dA^s + dA^h)       (A.14-A.16)
+ *   dudot = -(q_s/m_s) [ (b* - b).grad(dPhi) - u_par b*.grad(dA^h) ] - (Rdot_mu d_R + Zdot_mu d_Z + phidot_mu d_phi) dA^s
+ *     = A.17 with the ideal Ohm's law d_t dA^s = -b.grad(dPhi) substituted exactly (reading G26: A.18 as
+ *     printed has b instead of b* in the dA^h term, a second-order difference; the phi term of A.18 lacks its 1/R).
+ *   weight: d ln f_M/dt of PAPER.md:1208 with v_par = u_par - (q_s/m_s) dA^h and d(u_par)/dt perturbed part.
+ * fld[3][4]: (value, d/dR, d/dZ, d/dphi) of dPhi, dA^s, dA^h. */
+static void rhs_point_em(const orc_params *p, double R, double Z, double upar, double mu, double w,
+                         const double fld[3][4], double out[5])
+{
+    orc_eq e; equilibrium(p, R, Z, &e);
+    const double eps = p->rho0 * p->B0 / p->qs_over_ms, qom = p->qs_over_ms;
+    const double *Phi = fld[0], *As = fld[1], *Ah = fld[2];
+    double cR = -e.dbphi_dZ, cZ = e.dbphi_dR + e.bphi / R, cP = e.dbR_dZ - e.dbZ_dR;      /* curl b */
+    double Bsp = e.B + eps * upar * (e.bR * cR + e.bZ * cZ + e.bphi * cP);
+    double lead = (p->eom_variant == 1) ? e.B / Bsp : 1.0;
+    double k = eps * upar / Bsp;
+    double b0R = lead * e.bR + k * cR, b0Z = lead * e.bZ + k * cZ, b0P = lead * e.bphi + k * cP;        /* A.4-A.6 */
+    double CE = p->rho0 * p->B0 / Bsp, Cd = eps * mu / (e.B * Bsp);
+    /* b* (A.7-A.9): b0* + C_E grad(dA^s) x b, with (grad f)_phi = (1/R) d f/d phi */
+    double bsR = b0R + CE * ((e.bZ / R) * As[3] - e.bphi * As[2]);
+    double bsZ = b0Z + CE * (e.bphi * As[1] - (e.bR / R) * As[3]);
+    double bsP = b0P + CE * (e.bR * As[2] - e.bZ * As[1]);
+    /* equilibrium part, A.10-A.13 */
+    double Rmu = Cd * e.Bphi * e.dBdZ, Zmu = -Cd * e.Bphi * e.dBdR, Pmu = (Cd / R) * (e.BZ * e.dBdR - e.BR * e.dBdZ);
+    double R0dot = b0R * upar + Rmu, Z0dot = b0Z * upar + Zmu, P0dot = b0P * upar / R + Pmu;
+    double u0dot = -mu * (b0R * e.dBdR + b0Z * e.dBdZ);
+    /* perturbed part */
+    double GR = Phi[1] - upar * (As[1] + Ah[1]), GZ = Phi[2] - upar * (As[2] + Ah[2]), GP = Phi[3] - upar * (As[3] + Ah[3]);
+    double dRdot = CE * (e.bphi * GZ - (e.bZ / R) * GP) - qom * Ah[0] * bsR;                           /* A.14 */
+    double dZdot = CE * (-e.bphi * GR + (e.bR / R) * GP) - qom * Ah[0] * bsZ;                          /* A.15 */
+    double dPdot = (CE / R) * (e.bZ * GR - e.bR * GZ) - (1.0 / R) * qom * Ah[0] * bsP;                 /* A.16 */
+    double dudot = -qom * ((bsR - e.bR) * Phi[1] + (bsZ - e.bZ) * Phi[2] + ((bsP - e.bphi) / R) * Phi[3]
+                           - upar * (bsR * Ah[1] + bsZ * Ah[2] + (bsP / R) * Ah[3]))
+                   - (Rmu * As[1] + Zmu * As[2] + Pmu * As[3]);                                        /* A.17 + Ohm */
+    /* weight */
+    double vpar = upar - qom * Ah[0];
+    double x = R - p->R0, r = sqrt(x * x + Z * Z);
+    double drdot = (r > 0.0) ? (dRdot * x + dZdot * Z) / r : 0.0;
+    double en = vpar * vpar / p->T + 2.0 * mu * e.B / p->T - 1.5;
+    double L = drdot * (-p->kappa_n - en * p->kappa_T) - (2.0 * mu / p->T) * (dRdot * e.dBdR + dZdot * e.dBdZ)
+             - (2.0 * vpar / p->T) * dudot;
+    out[0] = R0dot + dRdot; out[1] = Z0dot + dZdot; out[2] = P0dot + dPdot; out[3] = u0dot + dudot;
+    out[4] = (p->weight_mode == 0) ? -(1.0 - w) * L : -L;
+}
+void orc_rhs_point_em(const orc_ctx *c, size_t n, const double *R, const double *Z, const double *upar, const double *mu,
+                      const double *w, const double *fld /* [n][3][4] */, double *out /* [n][5] */)
+{
+    for (size_t p = 0; p < n; ++p) {
+        double f3[3][4];
+        memcpy(f3, fld + 12 * p, sizeof(f3));
+        rhs_point_em(&c->p, R[p], Z[p], upar[p], mu[p], w[p], f3, out + 5 * p);
+    }
+}
+void orc_set_aux_coef(orc_ctx *c, int which, const double *coef)
+{
+    const size_t nn = (size_t)c->n_tri * c->n_modes * ORC_NCOEF * 2;
+    free(c->coef_aux[which]); c->coef_aux[which] = NULL;
+    if (coef && nn) { c->coef_aux[which] = (double *)malloc(sizeof(double) * nn); memcpy(c->coef_aux[which], coef, sizeof(double) * nn); }
+}
+/* gather of the three fields at a located point: the same gather_one on each table */
+static void gather_three(const orc_ctx *c, int t, double xi, double eta, double phi, double fld[3][4])
+{
+    memset(fld, 0, sizeof(double) * 12);
+    if (c->n_modes == 0) return;
+    orc_ctx tmp = *c;
+    gather_one(c, t, xi, eta, phi, fld[0]);
+    for (int a = 0; a < 2; ++a)
+        if (c->coef_aux[a]) { tmp.coef = c->coef_aux[a]; gather_one(&tmp, t, xi, eta, phi, fld[1 + a]); }
+}
+/* K1 of the thesis: locate -> gather dPhi, dA^s, dA^h -> equilibrium -> equations; five outputs */
+void orc_rhs_em(const orc_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const double *upar,
+                const double *mu, const double *w, int32_t *cell_out, double *dRdt, double *dZdt, double *dphidt,
+                double *dudt, double *dwdt)
+{
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) {
+        double o[5] = {0, 0, 0, 0, 0}, xi, eta, fld[3][4];
+        int t = locate_one(c, R[p], Z[p], &xi, &eta);
+        if (t >= 0) { gather_three(c, t, xi, eta, phi[p], fld); rhs_point_em(&c->p, R[p], Z[p], upar[p], mu[p], w[p], fld, o); }
+        if (cell_out) cell_out[p] = t;
+        dRdt[p] = o[0]; dZdt[p] = o[1]; dphidt[p] = o[2]; dudt[p] = o[3]; dwdt[p] = o[4];
+    }
+}
+
+/* ------------------------------------------------------------------- O10 pullback (K2 of the thesis) */
+/* PAPER.md:1112-1128 (normalised form): u_new = u_old - (q_s/m_s) <dA^h_old>;
+ * delta f_new = delta f_old - (2 q_s/T) v_par <dA^h_old> f_0  (linearised, Maxwellian f_0; the factor 2 from T_N = m_N v_N^2/2).
+ * In marker weights (w = delta f/f, 1 - w = f_0/f, reading G7): w_new = w_old - (2 q_s/T) v_par dA^h (1 - w_old)
+ * [weight_mode 1: ... x 1]; v_par: the velocity coordinate after the transformation, = u_new (reading G27).
+ * Markers outside the mesh (or flagged cell < 0) are left untouched.  The field side (dA^s += dA^h) is not a marker operation. */
+void orc_pullback(const orc_ctx *c, size_t n, const double *R, const double *Z, const double *phi, double *upar, double *w,
+                  const int32_t *cell_flag)
+{
+#pragma omp parallel for schedule(static)
+    for (size_t p = 0; p < n; ++p) {
+        if (cell_flag && cell_flag[p] < 0) continue;
+        double xi, eta, fld[3][4];
+        int t = locate_one(c, R[p], Z[p], &xi, &eta);
+        if (t < 0) continue;
+        gather_three(c, t, xi, eta, phi[p], fld);
+        const double Ah = fld[2][0];
+        const double unew = upar[p] - c->p.qs_over_ms * Ah;
+        const double fac = (c->p.weight_mode == 0) ? (1.0 - w[p]) : 1.0;
+        w[p] = w[p] - (2.0 * c->p.qs_over_ms / c->p.T) * unew * Ah * fac;
+        upar[p] = unew;
+    }
 }
 
 int orc_max_threads(void)
