@@ -149,6 +149,33 @@ int trimeg_gather(trimeg_ctx *ctx, size_t n, const double *R, const double *Z, c
 int trimeg_rhs(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, double *dRdt, double *dZdt,
                double *dphidt, double *dvpardt, double *dwdt, trimeg_stream stream);
 
+/* ---- electromagnetic terms (row f2) ------------------------------------------------------------
+ * The mixed-variable scheme of the thesis: dA_par = dA^s + dA^h (A.1), the marker's
+ * velocity coordinate is u_par = v_par + (q_s/m_s) <dA^h> (stored in markers.vpar), the gyro-average is the
+ * identity.  dA^s and dA^h live on the basis and mode list of the uploaded field (dPhi):
+ * trimeg_field_upload_aux(which = TRIMEG_FIELD_AS / _AH, data_dev, kind) takes nodal DOFs (kind 0) or
+ * coefficients (kind 1) in the layouts of trimeg_field_upload; data_dev = NULL drops the table (the field is
+ * zero).  A trimeg_field_upload that changes the number of modes drops both.  Ordering as trimeg_field_upload.
+ * Errors: INVALID_ARG, NO_FIELD (upload dPhi first), ALLOC, CUDA. */
+#define TRIMEG_FIELD_AS 1
+#define TRIMEG_FIELD_AH 2
+int trimeg_field_upload_aux(trimeg_ctx *ctx, int which, const void *data_dev, int kind,
+                            trimeg_stream stream);
+/* K1, the thesis's push kernel with the electromagnetic model on: one right-hand side
+ * per marker -- locate, gather dPhi, dA^s, dA^h, analytic equilibrium, b* = b0* + grad(dA^s) x b / B*_par
+ * (A.7-A.9), equilibrium motion A.10-A.13 with u_par, perturbed motion A.14-A.16 with
+ * dG = dPhi - u_par dA_par, parallel acceleration A.17 with the ideal Ohm's law d_t dA^s = -b.grad dPhi
+ * substituted (reading G26 of DESIGN.md), weight rate of PAPER.md:1208 at
+ * v_par = u_par - (q_s/m_s) dA^h.  Five outputs (dRdt, dZdt, dphidt, dudt, dwdt), n doubles each; markers are
+ * not modified; markers outside the mesh get 0. */
+int trimeg_rhs_em(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, double *dRdt, double *dZdt,
+                  double *dphidt, double *dudt, double *dwdt, trimeg_stream stream);
+/* K2, the pullback kernel (section 5.2.1; normalised equations): per marker
+ * u_new = u_old - (q_s/m_s) dA^h, w_new = w_old - (2 q_s/T) u_new dA^h (1 - w_old) (weight_mode 1: x 1), in
+ * place on markers.vpar and markers.w; markers with cell < 0 or outside the mesh are left untouched.  Without
+ * a dA^h table the call does nothing.  (The field side, dA^s += dA^h, is a table operation of the caller.) */
+int trimeg_pullback(trimeg_ctx *ctx, trimeg_markers *m, size_t n, trimeg_stream stream);
+
 /* ---- particle-to-grid projection / scatter (row f1) -----------------------------------------
  * "The charge of each particle is projected onto the basis functions" (section 3.1; the P2G
  * functions of PAPER.md:249; section 6.3: the phase the thesis left on the CPU as "not suitable

@@ -18,13 +18,14 @@ LIB_PATH = os.path.join(_HERE, "libtrimeg.so")
 EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_download_coeffs",
-    "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
+    "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
     "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
 )
 
 OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC = 0, -1, -2, -3, -4, -5
 # TRIMEG_PUSH_KERNEL_* of include/trimeg.h
+FIELD_AS, FIELD_AH = 1, 2      # TRIMEG_FIELD_AS / _AH
 PUSH_KERNEL_AUTO, PUSH_KERNEL_THREAD, PUSH_KERNEL_LANE, PUSH_KERNEL_WCACHE = -1, 0, 1, 2
 PUSH_KERNELS = (PUSH_KERNEL_THREAD, PUSH_KERNEL_LANE, PUSH_KERNEL_WCACHE)
 
@@ -71,6 +72,9 @@ def load() -> C.CDLL:
     L.trimeg_gather.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.trimeg_rhs.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp, vp, vp, vp, vp]
     L.trimeg_scatter.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp]
+    L.trimeg_field_upload_aux.argtypes = [vp, i32, vp, i32, vp]
+    L.trimeg_rhs_em.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp, vp, vp, vp, vp]
+    L.trimeg_pullback.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp]
     L.trimeg_sort.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp]
     L.trimeg_compact.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, C.POINTER(sz), vp]
     L.trimeg_push.argtypes = [vp, C.POINTER(trimeg_markers), sz, dbl, i32, vp]
@@ -228,6 +232,29 @@ class Context:
                                                              ("dRdt", "dZdt", "dphidt", "dvpardt", "dwdt")],
                                  _stream(stream)), "trimeg_rhs")
         return out
+
+    def field_upload_aux(self, which: int, data: Optional[torch.Tensor], kind: int, stream=None):
+        """which: FIELD_AS (dA^s) or FIELD_AH (dA^h); data None drops the table."""
+        if data is not None and self.n_modes > 0:
+            want = (self.n_modes, self.n_vert, 6) if kind == 0 else (self.n_tri, self.n_modes, 21)
+            if tuple(data.shape) != want:
+                raise ValueError(f"field data shape {tuple(data.shape)} != {want}")
+        _check(self.L.trimeg_field_upload_aux(self.h, int(which), _ptr(data, torch.complex128), int(kind), _stream(stream)),
+               "trimeg_field_upload_aux")
+
+    def rhs_em(self, m: Dict[str, torch.Tensor], stream=None) -> Dict[str, torch.Tensor]:
+        n = m["R"].numel()
+        ms = _markers(m, n)
+        out = {k: torch.empty(n, dtype=torch.float64, device=m["R"].device) for k in ("dRdt", "dZdt", "dphidt", "dudt", "dwdt")}
+        _check(self.L.trimeg_rhs_em(self.h, C.byref(ms), n, *[_ptr(out[k], torch.float64) for k in
+                                                                ("dRdt", "dZdt", "dphidt", "dudt", "dwdt")], _stream(stream)),
+               "trimeg_rhs_em")
+        return out
+
+    def pullback(self, m: Dict[str, torch.Tensor], n: Optional[int] = None, stream=None):
+        n = m["R"].numel() if n is None else int(n)
+        ms = _markers(m, n)
+        _check(self.L.trimeg_pullback(self.h, C.byref(ms), n, _stream(stream)), "trimeg_pullback")
 
     def scatter(self, m: Dict[str, torch.Tensor], n: Optional[int] = None, out: Optional[torch.Tensor] = None,
                 stream=None) -> torch.Tensor:

@@ -33,6 +33,7 @@ struct trimeg_ctx {
     // device tables
     double *d_geom, *d_r_nodes, *d_vR, *d_vZ;
     double2 *d_coef;
+    double2 *d_coef_aux[2];         // row f2: dA^s, dA^h on the main field's basis and mode list; NULL = identically zero
     int *d_mode_n;
     int has_field;
     int push_kernel;                // trimeg_set_push_kernel variant
@@ -92,5 +93,10 @@ cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const int32_t *hint,
                                double *f, double *fR, double *fZ, double *fP, const int *gate, int want, cudaStream_t s);
 constexpr size_t GATHER_LANE_MIN = 1 << 18;     // below, two more kernel launches cost more than the lane kernel saves
+
+// trimeg_em.cu: row f2, one EM right-hand side (K1) and the pullback of u_par, w (K2)
+cudaError_t launch_rhs_em(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP, double *dU, double *dW,
+                          cudaStream_t s);
+cudaError_t launch_pullback(trimeg_ctx *c, const trimeg_markers &m, size_t n, cudaStream_t s);
 
 }  // namespace trimeg

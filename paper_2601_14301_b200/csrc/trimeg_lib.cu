@@ -444,6 +444,7 @@ int trimeg_mesh_destroy(trimeg_ctx *c)
     DeviceGuard guard__(c->device);
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
     cudaFree(c->d_adj_off); cudaFree(c->d_adj); cudaFree(c->d_trirhs);
+    cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]);
     cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
     if (c->hstreams_ready) {
         for (int k = 0; k < 3; ++k) cudaStreamDestroy(c->hstream[k]);
@@ -504,8 +505,8 @@ int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, cons
     if (n_modes != c->field.n_modes || !c->d_coef) {
         // tables may still be in use by kernels enqueued earlier
         CU_TRY(cudaDeviceSynchronize());
-        cudaFree(c->d_coef); cudaFree(c->d_mode_n);
-        c->d_coef = nullptr; c->d_mode_n = nullptr; c->has_field = 0; c->field.n_modes = 0;
+        cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]);
+        c->d_coef = nullptr; c->d_mode_n = nullptr; c->d_coef_aux[0] = c->d_coef_aux[1] = nullptr; c->has_field = 0; c->field.n_modes = 0;
         if (n_modes > 0) {
             if (cudaMalloc(&c->d_coef, sizeof(double2) * NCOEF * (size_t)c->n_tri * n_modes) != cudaSuccess ||
                 cudaMalloc(&c->d_mode_n, sizeof(int) * n_modes) != cudaSuccess) {
@@ -539,6 +540,51 @@ int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, cons
     // trimeg_push_host runs on the context's own streams: they wait for this upload
     if (!c->ev_upload) CU_TRY(cudaEventCreateWithFlags(&c->ev_upload, cudaEventDisableTiming));
     CU_TRY(cudaEventRecord(c->ev_upload, s));
+    return TRIMEG_OK;
+}
+
+int trimeg_field_upload_aux(trimeg_ctx *c, int which, const void *data_dev, int kind, trimeg_stream stream)
+{
+    if (!c || (which != TRIMEG_FIELD_AS && which != TRIMEG_FIELD_AH) || (kind != 0 && kind != 1)) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    ON_CTX_DEVICE(c);
+    const int a = which - TRIMEG_FIELD_AS, n_modes = c->field.n_modes;
+    cudaStream_t s = (cudaStream_t)stream;
+    if (!data_dev || n_modes == 0) {                     // drop the table: the field is identically zero
+        if (c->d_coef_aux[a]) { CU_TRY(cudaDeviceSynchronize()); cudaFree(c->d_coef_aux[a]); c->d_coef_aux[a] = nullptr; }
+        return TRIMEG_OK;
+    }
+    const size_t bytes = sizeof(double2) * NCOEF * (size_t)c->n_tri * n_modes;
+    if (!c->d_coef_aux[a] && cudaMalloc(&c->d_coef_aux[a], bytes) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_ALLOC; }
+    if (kind == 1) CU_TRY(cudaMemcpyAsync(c->d_coef_aux[a], data_dev, bytes, cudaMemcpyDeviceToDevice, s));
+    else {
+        const size_t work = (size_t)c->n_tri * n_modes;
+        bell_kernel<<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR, c->d_vZ,
+                                                                   (const double2 *)data_dev, c->d_coef_aux[a]);
+        c->n_launches++;
+        CU_TRY(cudaGetLastError());
+    }
+    return TRIMEG_OK;
+}
+
+int trimeg_rhs_em(trimeg_ctx *c, const trimeg_markers *m, size_t n, double *dRdt, double *dZdt, double *dphidt, double *dudt,
+                  double *dwdt, trimeg_stream stream)
+{
+    if (!c || (n > 0 && (!markers_ok(m) || !dRdt || !dZdt || !dphidt || !dudt || !dwdt))) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (n == 0) return TRIMEG_OK;
+    ON_CTX_DEVICE(c);
+    CU_TRY(launch_rhs_em(c, *m, n, dRdt, dZdt, dphidt, dudt, dwdt, (cudaStream_t)stream));
+    return TRIMEG_OK;
+}
+
+int trimeg_pullback(trimeg_ctx *c, trimeg_markers *m, size_t n, trimeg_stream stream)
+{
+    if (!c || (n > 0 && !markers_ok(m))) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (n == 0) return TRIMEG_OK;
+    ON_CTX_DEVICE(c);
+    CU_TRY(launch_pullback(c, *m, n, (cudaStream_t)stream));
     return TRIMEG_OK;
 }
 
