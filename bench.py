@@ -488,6 +488,7 @@ def run_gpu(args, wl):
                          "algorithmic_bytes_per_gather": 52, "algorithmic_flops_per_gather": flops_per_gather(len(w4.modes)),
                          "rows": rows, "clocks": sampler.stop(), "config": workload_config(w4)}
         c4.close()
+        sweep["em_cfg5"] = em_run(inputs.WORKLOADS["cfg5"], 3, fp64_peak, hbm_peak, with_oracle=not args.no_check)
         sweep["scatter_cfg5"] = scatter_run(inputs.WORKLOADS["cfg5"], 3, fp64_peak, hbm_peak, with_oracle=not args.no_check)
 
     if rank == 0:
@@ -577,6 +578,101 @@ def scatter_run(wl, reps, fp64_peak, hbm_peak, with_oracle=True):
     return res
 
 
+def flops_per_rhs_em(n_modes: int) -> int:
+    """One electromagnetic right-hand side (row f2, the thesis's K1): locator 25, three gathers of 170 per mode + 6, and
+    ~330 for equilibrium, b*, the equations and the weight rate (the electrostatic 155 + the dA^s / dA^h terms)."""
+    return 25 + 3 * (170 * n_modes + 6) + 330
+
+
+def em_run(wl, reps, fp64_peak, hbm_peak, with_oracle=True):
+    """trimeg_rhs_em (K1) and trimeg_pullback (K2) on the workload's marker batch, as drawn and cell-sorted; the three fields
+    are seeded like the workload's own (amplitudes 1e-3, 1e-3, 3e-4)."""
+    import torch
+    from paper_2601_14301_b200 import binding, inputs
+    ctx = binding.context_for(wl, inputs)
+    dofs = [inputs.field_dofs(wl, seed=wl.seed + 100 * a, sigma=sg) for a, sg in enumerate((1e-3, 1e-3, 3e-4))]
+    ctx.field_upload(wl.modes, torch.from_numpy(dofs[0]).cuda(), kind=0)
+    ctx.field_upload_aux(binding.FIELD_AS, torch.from_numpy(dofs[1]).cuda(), kind=0)
+    ctx.field_upload_aux(binding.FIELD_AH, torch.from_numpy(dofs[2]).cuda(), kind=0)
+    n = wl.n_markers
+    m = inputs.markers(wl, n=n)
+    d = binding.markers_to_device(m, "cuda")
+    ctx.locate(d["R"], d["Z"], cell=d["cell"])
+    n_in = int((d["cell"] >= 0).sum())
+    fl = flops_per_rhs_em(len(wl.modes))
+    rows = []
+    for order in ("as drawn", "cell-sorted"):
+        if order == "cell-sorted":
+            ctx.sort(d)
+        for op in ("rhs_em", "pullback"):
+            ts = []
+            u0, w0 = d["vpar"].clone(), d["w"].clone()
+            for rep in range(3 + reps):
+                if op == "pullback":
+                    d["vpar"].copy_(u0); d["w"].copy_(w0)
+                e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                e0.record()
+                out = ctx.rhs_em(d) if op == "rhs_em" else ctx.pullback(d)
+                e1.record()
+                torch.cuda.synchronize()
+                if rep >= 3:
+                    ts.append(e0.elapsed_time(e1) * 1e-3)
+            d["vpar"].copy_(u0); d["w"].copy_(w0)
+            t = sorted(ts)[len(ts) // 2]
+            row = {"op": op, "order": order, "value": n_in / t, "unit": "markers/s", "ms_per_call": t * 1e3}
+            if op == "rhs_em":
+                row.update({"achieved_tflops": fl * n_in / t * 1e-12, "frac": fl * n_in / t * 1e-12 / fp64_peak})
+            else:
+                row.update({"algorithmic_GBps": 60.0 * n_in / t * 1e-9, "frac_hbm": 60.0 * n_in / t * 1e-9 / hbm_peak})
+            rows.append(row)
+    best = [r for r in rows if r["op"] == "rhs_em" and r["order"] == "cell-sorted"][0]
+    res = {"metric": "marker right-hand sides per second, electromagnetic model (trimeg_rhs_em, the thesis's K1); pullbacks per second (K2)",
+           "value": best["value"], "unit": "marker-RHS/s", "markers": n, "markers_inside": n_in, "rows": rows,
+           "roofline": {"bound": "alu", "kernel": "rhs_em_kernel", "achieved": best["achieved_tflops"], "peak": fp64_peak, "unit": "TFLOP/s",
+                        "frac": best["frac"], "algorithmic_flops_per_marker": fl, "algorithmic_bytes_per_marker": 92},
+           "paper_context": "thesis K1, 32e6 electrons on 1 H100: 0.21 s = 1.5e8 marker-RHS/s; K2 + density + g2p2g 0.10-0.13 s "
+                            "(PAPER.md:911-917; EQDSK equilibrium, cubic splines in phi: other hardware, not like-for-like)",
+           "config": workload_config(wl)}
+    if with_oracle:
+        import oracle
+        o = oracle.from_workload(wl, inputs)
+        coefs = [o.bell_from_dofs(wl.modes, x) for x in dofs]
+        o.set_coeffs(wl.modes, coefs[0]); o.set_aux_coeffs(0, coefs[1]); o.set_aux_coeffs(1, coefs[2])
+        stride = max(1, n // (1 << 17))
+        ms = {k: np.ascontiguousarray(v[::stride]) for k, v in m.items()}
+        t0 = time.perf_counter()
+        want = o.rhs_em(ms["R"], ms["Z"], ms["phi"], ms["vpar"], ms["mu"], ms["w"])
+        dt_o = time.perf_counter() - t0
+        ds = binding.markers_to_device(ms, "cuda")
+        got = ctx.rhs_em(ds)
+        err = max(float(np.abs(got[k].cpu().numpy() - want[k]).max() / np.abs(want[k]).max()) for k in ("dRdt", "dZdt", "dphidt", "dudt", "dwdt"))
+        assert err < 1e-10, f"rhs_em parity check failed: {err}"      # library Bell expansion vs the oracle's: 1e-11 per coefficient
+        res["oracle_check"] = {"sample_markers": int(ms["R"].size), "max_rel_err": err}
+        res["cpu_baseline"] = {"value": ms["R"].size / dt_o, "unit": "marker-RHS/s", "kind": "oracle", "cores": o.max_threads(),
+                               "sample": f"every {stride}-th marker ({ms['R'].size}), oracle.rhs_em with OpenMP over markers"}
+    ctx.close()
+    del d
+    torch.cuda.empty_cache()
+    return res
+
+
+def run_em(args, wl):
+    import torch
+    from paper_2601_14301_b200 import binding, inputs
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(0)
+    binding.load()
+    ctx = binding.context_for(wl, inputs)
+    fp64_peak = ctx.measure_fp64_peak()
+    ctx.close()
+    hbm_peak, _ = load_peaks()
+    res = em_run(wl, max(3, args.steps), fp64_peak, hbm_peak)
+    res.update({"n_gpus": 1, "dtype": "f64", "data": "synthetic", "higher_is_better": True})
+    print(json.dumps(res), flush=True)
+    return 0
+
+
 def run_scatter(args, wl):
     import torch
     from paper_2601_14301_b200 import binding, inputs
@@ -621,7 +717,8 @@ def main():
     ap.add_argument("--steps", type=int, default=4)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--op", default="push", choices=["push", "scatter"], help="scatter: time trimeg_scatter (row f1) on the workload's markers")
+    ap.add_argument("--op", default="push", choices=["push", "scatter", "em"],
+                    help="scatter: time trimeg_scatter (row f1); em: trimeg_rhs_em and trimeg_pullback (row f2) on the workload's markers")
     ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
     ap.add_argument("--n-modes", type=int, default=0, help="override the toroidal mode list by n = 0, 2, ..., 2 (K - 1) (schedule selection sweeps)")
@@ -648,6 +745,8 @@ def main():
         return run_reference(args, wl)
     if args.op == "scatter":
         return run_scatter(args, wl)
+    if args.op == "em":
+        return run_em(args, wl)
     return run_gpu(args, wl)
 
 
