@@ -62,6 +62,10 @@ def lib():
         L.orc_set_aux_coef.argtypes = [C.c_void_p, C.c_int, dp]
         L.orc_rhs_em.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, dp, ip, dp, dp, dp, dp, dp]
         L.orc_pullback.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, dp, ip]
+        L.orc_set_spline.argtypes = [C.c_void_p, C.c_int, dp]
+        L.orc_get_spline.argtypes = [C.c_void_p, dp]
+        L.orc_bell_spline_from_dofs.argtypes = [C.c_void_p, C.c_int, dp]
+        L.orc_bell_spline_from_dofs.restype = C.c_int
         L.orc_scatter.argtypes = [C.c_void_p, C.c_size_t, dp, dp, dp, dp, ip, dp]
         L.orc_scatter.restype = C.c_long
         L.orc_max_threads.restype = C.c_int
@@ -221,6 +225,29 @@ class Oracle:
         self.L.orc_push(self.h, n, _d(out["R"]), _d(out["Z"]), _d(out["phi"]), _d(out["vpar"]),
                         _d(out["mu"]), _d(out["w"]), _i(cell), float(dt), int(nsteps), int(nthreads))
         out["cell"] = cell
+        return out
+
+    # ---- cubic B-spline toroidal basis (O11): the field of gather / rhs / push becomes sum_j N_j(phi) P_j(xi, eta)
+    def set_spline_coeffs(self, n_phi: int, coef: Optional[np.ndarray]):
+        """coef real [n_tri][n_phi][21] (None: zeros); n_phi = 0 returns to the harmonic field."""
+        self.n_phi = int(n_phi)
+        if n_phi > 0 and coef is not None:
+            coef = np.ascontiguousarray(coef, dtype=np.float64)
+            assert coef.shape == (self.n_tri, n_phi, 21), coef.shape
+            self.L.orc_set_spline(self.h, int(n_phi), _d(coef))
+        else:
+            self.L.orc_set_spline(self.h, int(n_phi), None)
+
+    def bell_spline_from_dofs(self, dofs: np.ndarray) -> np.ndarray:
+        """dofs real [n_phi][n_vert][6] -> coefficients real [n_tri][n_phi][21]; the field becomes the spline field."""
+        dofs = np.ascontiguousarray(dofs, dtype=np.float64)
+        n_phi = dofs.shape[0]
+        assert dofs.shape == (n_phi, self.n_vert, 6), dofs.shape
+        if self.L.orc_bell_spline_from_dofs(self.h, n_phi, _d(dofs)) != 0:
+            raise RuntimeError("singular Bell system")
+        self.n_phi = n_phi
+        out = np.empty((self.n_tri, n_phi, 21), dtype=np.float64)
+        self.L.orc_get_spline(self.h, _d(out))
         return out
 
     # ---- electromagnetic terms (O9, O10): dA^s = aux 0, dA^h = aux 1, on the mode list of the main field

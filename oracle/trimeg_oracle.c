@@ -36,6 +36,8 @@
  *   O9 EM RHS          one right-hand side with dA^s, dA^h (mixed variables): A.7-A.9, A.14-A.17 with the
  *                      ideal Ohm's law substituted
  *   O10 pullback       u_par, w after the pullback transformation
+ *   O11 spline basis   the thesis's own toroidal discretisation: cubic B-splines in phi instead of harmonics
+ *                                                           PAPER.md:223, 365-368
  */
 #include <math.h>
 #include <stdint.h>
@@ -69,6 +71,8 @@ typedef struct {
     double *coef;                  /* [n_tri][n_modes][21][2] (re, im) */
     double **basis;                /* O8: per triangle, lazily, [21][18] monomial coefficients of the 18 basis functions */
     double *coef_aux[2];           /* O9/O10: dA^s (0) and dA^h (1), same layout and mode list as coef; NULL = identically zero */
+    int n_phi;                     /* O11: > 0 = the field is Y = sum_j N_j(phi) P_j(xi, eta) on n_phi toroidal planes */
+    double *coef_spl;              /* [n_tri][n_phi][21] real monomial coefficients, one quintic per triangle and plane */
 } orc_ctx;
 
 /* ------------------------------------------------------------------ O1 mesh */
@@ -137,7 +141,7 @@ void orc_destroy(orc_ctx *c)
     if (!c) return;
     free(c->r_nodes); free(c->Rv); free(c->Zv); free(c->tri); free(c->geom);
     if (c->basis) { for (int t = 0; t < c->n_tri; ++t) free(c->basis[t]); free(c->basis); }
-    free(c->coef_aux[0]); free(c->coef_aux[1]);
+    free(c->coef_aux[0]); free(c->coef_aux[1]); free(c->coef_spl);
     free(c->mode_n); free(c->coef); free(c);
 }
 
@@ -392,8 +396,10 @@ void orc_bary(const orc_ctx *c, size_t n, const int32_t *t, const double *R, con
  *   d/dR, d/dZ  = sum_n Re((xi_X dP/dxi + eta_X dP/deta) E_n)
  *   d/dphi      = sum_n Re(i n P_n E_n)
  * No factor 2 for n > 0; Im of the n = 0 mode is ignored (reading G15). */
+static void gather_one_spline(const orc_ctx *c, int t, double xi, double eta, double phi, double out[4]);
 static void gather_one(const orc_ctx *c, int t, double xi, double eta, double phi, double out[4])
 {
+    if (c->n_phi > 0) { gather_one_spline(c, t, xi, eta, phi, out); return; }
     const double *g = c->geom + 6 * t;
     double f = 0.0, fR = 0.0, fZ = 0.0, fp = 0.0;
     for (int m = 0; m < c->n_modes; ++m) {
@@ -527,7 +533,7 @@ static int rhs_full(const orc_ctx *c, double R, double Z, double phi, double vpa
     double xi, eta, fld[4] = {0, 0, 0, 0};
     int t = locate_one(c, R, Z, &xi, &eta);
     if (t < 0) return -1;
-    if (c->n_modes > 0) gather_one(c, t, xi, eta, phi, fld);
+    if (c->n_modes > 0 || c->n_phi > 0) gather_one(c, t, xi, eta, phi, fld);
     rhs_point(&c->p, R, Z, vpar, mu, w, fld, out);
     return t;
 }
@@ -790,6 +796,83 @@ void orc_pullback(const orc_ctx *c, size_t n, const double *R, const double *Z, 
         w[p] = w[p] - (2.0 * c->p.qs_over_ms / c->p.T) * unew * Ah * fac;
         upar[p] = unew;
     }
+}
+
+/* ------------------------------------------------- O11 cubic B-spline toroidal basis (the thesis's own) */
+/* Y(R, Phi, Z) = sum_i sum_j Lambda_i(xi, eta) N_j(Phi) Y_ij: C1 triangles in (R, Z), cubic splines in
+ * Phi on a uniform periodic grid.  Reading G28: N_j(phi) = beta((phi - phi_j)/h), phi_j = j h,
+ * h = 2 pi/N_phi, wrapped periodically, beta the uniform cubic B-spline
+ *     beta(x) = 2/3 - x^2 + |x|^3/2  (|x| < 1),  (2 - |x|)^3/6  (1 <= |x| < 2),  0 else.
+ * Per triangle and plane j the (R, Z) part is the quintic P_j of the plane's nodal DOFs (O2).  Plain definition: the sum
+ * runs over ALL planes.  Outputs as O4: value, d/dR, d/dZ, d/dphi. */
+static double bspl(double x) { double a = fabs(x); if (a < 1.0) return 2.0 / 3.0 - a * a + 0.5 * a * a * a; if (a < 2.0) { double u = 2.0 - a; return u * u * u / 6.0; } return 0.0; }
+static double bspl_d(double x)
+{
+    double a = fabs(x), sgn = (x < 0.0) ? -1.0 : 1.0, d;
+    if (a < 1.0) d = -2.0 * a + 1.5 * a * a;
+    else if (a < 2.0) { double u = 2.0 - a; d = -0.5 * u * u; }
+    else d = 0.0;
+    return sgn * d;
+}
+static void gather_one_spline(const orc_ctx *c, int t, double xi, double eta, double phi, double out[4])
+{
+    const double *g = c->geom + 6 * t;
+    const int np = c->n_phi;
+    const double h = ORC_TWO_PI / np;
+    double f = 0.0, fR = 0.0, fZ = 0.0, fp = 0.0;
+    double mono[21], mx[21], me[21];
+    for (int k = 0; k < 21; ++k) {
+        int i, j; mono_ij(k, &i, &j);
+        mono[k] = ipow(xi, i) * ipow(eta, j);
+        mx[k] = (i >= 1) ? i * ipow(xi, i - 1) * ipow(eta, j) : 0.0;
+        me[k] = (j >= 1) ? j * ipow(xi, i) * ipow(eta, j - 1) : 0.0;
+    }
+    for (int j = 0; j < np; ++j) {
+        double x = (phi - j * h) / h;
+        x -= np * floor(x / np + 0.5);                   /* nearest periodic image: x in [-np/2, np/2) */
+        const double N = bspl(x), Nd = bspl_d(x) / h;
+        if (N == 0.0 && Nd == 0.0) continue;
+        const double *cf = c->coef_spl + ((size_t)t * np + j) * ORC_NCOEF;
+        double P = 0.0, Px = 0.0, Pe = 0.0;
+        for (int k = 0; k < 21; ++k) { P += cf[k] * mono[k]; Px += cf[k] * mx[k]; Pe += cf[k] * me[k]; }
+        f += N * P;
+        fR += N * (g[2] * Px + g[4] * Pe);
+        fZ += N * (g[3] * Px + g[5] * Pe);
+        fp += Nd * P;
+    }
+    out[0] = f; out[1] = fR; out[2] = fZ; out[3] = fp;
+}
+/* n_phi = 0 returns to the harmonic field of orc_set_modes / orc_set_coef.  coef: [n_tri][n_phi][21] real, or NULL (zeros). */
+void orc_set_spline(orc_ctx *c, int n_phi, const double *coef)
+{
+    free(c->coef_spl); c->coef_spl = NULL; c->n_phi = n_phi > 0 ? n_phi : 0;
+    if (c->n_phi == 0) return;
+    const size_t nn = (size_t)c->n_tri * c->n_phi * ORC_NCOEF;
+    c->coef_spl = (double *)calloc(nn, sizeof(double));
+    if (coef) memcpy(c->coef_spl, coef, sizeof(double) * nn);
+}
+void orc_get_spline(const orc_ctx *c, double *coef) { memcpy(coef, c->coef_spl, sizeof(double) * (size_t)c->n_tri * c->n_phi * ORC_NCOEF); }
+/* dofs: [n_phi][n_vert][6] real nodal values per plane; the Bell expansion of O2 plane by plane */
+int orc_bell_spline_from_dofs(orc_ctx *c, int n_phi, const double *dofs)
+{
+    orc_set_spline(c, n_phi, NULL);
+    int bad = 0;
+#pragma omp parallel for schedule(static) reduction(+ : bad)
+    for (int t = 0; t < c->n_tri; ++t) {
+        long double A[21][21], rs[21]; int piv[21];
+        if (bell_factor(c, t, A, rs, piv)) { bad += 1; continue; }
+        const int *v = c->tri + 3 * t;
+        for (int j = 0; j < n_phi; ++j) {
+            long double b[21];
+            for (int pnt = 0; pnt < 3; ++pnt)
+                for (int d = 0; d < 6; ++d) b[6 * pnt + d] = dofs[((size_t)j * c->n_vert + v[pnt]) * 6 + d];
+            b[18] = b[19] = b[20] = 0.0L;
+            bell_solve(A, rs, piv, b);
+            double *o = c->coef_spl + ((size_t)t * n_phi + j) * ORC_NCOEF;
+            for (int k = 0; k < 21; ++k) o[k] = (double)b[k];
+        }
+    }
+    return bad ? -1 : 0;
 }
 
 int orc_max_threads(void)
