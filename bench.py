@@ -45,6 +45,12 @@ def flops_per_marker_step(n_modes: int) -> int:
     return 4 * (200 + 170 * n_modes)
 
 
+def flops_per_marker_step_spline() -> int:
+    """Row f3, field on the cubic B-spline toroidal basis: per stage 200 as above, four REAL quintics with both
+    derivatives (85 each, half of a complex mode), 28 for the eight spline weights, 32 for the four weighted sums."""
+    return 4 * (200 + 4 * 85 + 28 + 32)
+
+
 def flops_per_gather(n_modes: int) -> int:
     """Gather only (configs[3]): locator 25 + 170 per mode + 6 for the chain rule."""
     return 25 + 170 * n_modes + 6
@@ -126,7 +132,7 @@ def _strided(m, n_s):
     return {k: np.ascontiguousarray(v[::stride][:n_s]) for k, v in m.items()}, stride
 
 
-def time_oracle(wl, m_np, target_seconds: float, steps: int = 1, warmup: int = 0, one_core_seconds: float = 0.0):
+def time_oracle(wl, m_np, target_seconds: float, steps: int = 1, warmup: int = 0, one_core_seconds: float = 0.0, n_phi: int = 0):
     """Time oracle.push (as it stands, never tuned) the way BASELINE.md §4 / SURVEY.md §8(d) plan it: a STRIDED
     subsample of the workload's seeded marker draw, pushed for the workload's full number of RK4 steps, with OpenMP
     over markers on all host cores -- and, if one_core_seconds > 0, once more on one core with a smaller strided
@@ -135,7 +141,10 @@ def time_oracle(wl, m_np, target_seconds: float, steps: int = 1, warmup: int = 0
     import oracle
     from paper_2601_14301_b200 import inputs
     o = oracle.from_workload(wl, inputs)
-    o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
+    if n_phi:
+        o.bell_spline_from_dofs(inputs.spline_dofs(wl, n_phi))
+    else:
+        o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
     cores = o.max_threads()
     nsteps = max(1, wl.nsteps)
     probe, _ = _strided(m_np, 2048)
@@ -176,7 +185,7 @@ def run_reference(args, wl):
         return 0
     m_np = inputs.markers(wl, n=wl.n_markers)
     budget = 150.0 / max(1, args.steps + args.warmup)
-    r = time_oracle(wl, m_np, min(20.0, budget), steps=args.steps, warmup=args.warmup)
+    r = time_oracle(wl, m_np, min(20.0, budget), steps=args.steps, warmup=args.warmup, n_phi=args.n_phi)
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3, "higher_is_better": True,
@@ -193,11 +202,13 @@ def run_reference(args, wl):
     return 0
 
 
-def workload_config(wl, extra=None):
+def workload_config(wl, extra=None, n_phi=0):
     c = {"workload": f"{wl.name} (BASELINE.json configs[{int(wl.name[3:]) - 1}])",
          "mesh": f"{wl.n_r}x{wl.n_theta} rings x sectors, {wl.n_tri} triangles",
          "toroidal_modes": list(wl.modes), "markers_per_gpu": wl.n_markers, "dt": wl.dt,
          "rk4_steps_per_step": wl.nsteps, "l2": "inputs larger than L2 (no flush needed)"}
+    if n_phi:
+        c["toroidal_basis"] = f"cubic B-splines on {n_phi} planes (row f3), the mode list's perturbation sampled on the planes"
     if extra:
         c.update(extra)
     return c
@@ -209,14 +220,18 @@ class PushRun:
     working copy).  A bench step = restore the batch to the workload's initial state (device copy), compact, then
     [cell sort -> fused push of `sort_every` RK4 steps] until the workload's nsteps are done."""
 
-    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True):
+    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True, n_phi=0):
         import torch
         from paper_2601_14301_b200 import binding, inputs
         self.torch, self.wl = torch, wl
         self.n = wl.n_markers
         self.sort_every = max(1, min(sort_every, wl.nsteps))
         self.ctx = binding.context_for(wl, inputs)
-        self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
+        self.n_phi = n_phi
+        if n_phi:                                          # row f3: the same perturbation on n_phi B-spline planes
+            self.ctx.field_upload_spline(torch.from_numpy(inputs.spline_dofs(wl, n_phi)).cuda(), kind=0)
+        else:
+            self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
         if push_kernel >= 0:
             self.ctx.set_push_kernel(push_kernel)
         m_np = inputs.markers(wl, n=self.n, seed=seed)
@@ -272,13 +287,22 @@ class PushRun:
         return {"units": units, "seconds": t0.elapsed_time(t1) * 1e-3, "clocks": clocks, "launches": st1["n_launches"] - st0["n_launches"],
                 "lost_per_step": lost / max(1, steps), "n_start": self.n_start}
 
+    def kernel_name(self):
+        k = self.ctx.get_push_kernel()
+        if self.n_phi and k == 1:
+            return "push_lane_kernel<16> (B-spline plane records)"
+        return PUSH_KERNEL_NAMES.get(k, "push kernel")
+
+    def flops_unit(self):
+        return flops_per_marker_step_spline() if self.n_phi else flops_per_marker_step(len(self.wl.modes))
+
     def roofline(self, fp64_peak, seconds):
         wl = self.wl
         push_s = sum(a.elapsed_time(b) for a, b, _ in self.push_events) * 1e-3
         push_units = sum(u for _, _, u in self.push_events)
         n_push = len(self.push_events)
-        flops = flops_per_marker_step(len(wl.modes)) * push_units
-        return {"bound": "alu", "kernel": PUSH_KERNEL_NAMES.get(self.ctx.get_push_kernel(), "push kernel"),
+        flops = self.flops_unit() * push_units
+        return {"bound": "alu", "kernel": self.kernel_name(),
                 "achieved": flops / push_s * 1e-12, "peak": fp64_peak, "unit": "TFLOP/s",
                 "frac": (flops / push_s * 1e-12) / fp64_peak, "launches": n_push, "avg_launch_ms": push_s / max(1, n_push) * 1e3,
                 "push_share_of_step": push_s / seconds, "units_per_launch": push_units / max(1, n_push)}
@@ -309,7 +333,10 @@ class PushRun:
         for k, v in ds.items():
             got[k][idx] = v.cpu().numpy()
         o = oracle.from_workload(wl, inputs)
-        o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
+        if self.n_phi:
+            o.bell_spline_from_dofs(inputs.spline_dofs(wl, self.n_phi))
+        else:
+            o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
         want = o.push(sample, wl.dt, wl.nsteps)
         assert np.array_equal(got["cell"] < 0, want["cell"] < 0), "lost-marker sets differ"
         worst = 0.0
@@ -417,7 +444,7 @@ def run_gpu(args, wl):
     binding.load()
 
     n = wl.n_markers
-    run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank))
+    run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank), n_phi=args.n_phi)
     ctx = run.ctx
     fp64_peak = ctx.measure_fp64_peak()
     fp64_peak3 = ctx.measure_fp64_peak_operands(3)     # DFMA stream with three fresh register operands
@@ -428,7 +455,7 @@ def run_gpu(args, wl):
     tile_counters = ctx.get_tile_counters()
 
     roof = run.roofline(fp64_peak, res["seconds"])
-    flops_unit = flops_per_marker_step(len(wl.modes))
+    flops_unit = run.flops_unit()
     t_fp64 = flops_unit * roof["units_per_launch"] / (fp64_peak * 1e12)
     t_hbm = bytes_per_marker_call(run.sort_every) * res["n_start"] / (hbm_peak * 1e9)
     roof.update({
@@ -453,7 +480,7 @@ def run_gpu(args, wl):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        r = time_oracle(wl, run.m_np, 15.0, one_core_seconds=6.0)
+        r = time_oracle(wl, run.m_np, 15.0, one_core_seconds=6.0, n_phi=args.n_phi)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "nproc": r["nproc"], "kind": "oracle", "sample": r["sample"],
                "value_one_core": r.get("value_one_core"), "sample_one_core": r.get("sample_one_core"),
                "note": "the oracle is the unoptimised correctness checker (plain monomial sums, gcc -O2): a baseline, not a "
@@ -462,7 +489,7 @@ def run_gpu(args, wl):
 
     # ---- the other configs, device-timed the same way (N = 1 only): short runs, same live peaks
     sweep = None
-    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes:
+    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes and not args.n_phi:
         sweep = {}
         for name in ("cfg2", "cfg3"):
             w2 = inputs.WORKLOADS[name]
@@ -496,7 +523,7 @@ def run_gpu(args, wl):
             "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": agg["seconds"] / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(wl, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
+            "config": workload_config(wl, n_phi=args.n_phi, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
                                                  "lost_markers_per_step": res["lost_per_step"],
                                                  "unit_count": "every bench step restarts from the config's initial state; a marker "
                                                                "that leaves the mesh during a step counts zero steps for it"}),
@@ -722,6 +749,7 @@ def main():
     ap.add_argument("--workload", default="cfg5", choices=["cfg1", "cfg2", "cfg3", "cfg4", "cfg5"])
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
     ap.add_argument("--n-modes", type=int, default=0, help="override the toroidal mode list by n = 0, 2, ..., 2 (K - 1) (schedule selection sweeps)")
+    ap.add_argument("--n-phi", type=int, default=0, help="row f3: the field on N cubic B-spline toroidal planes instead of the harmonic mode list")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
     ap.add_argument("--min-log2", type=int, default=16, help="cfg4 gather sweep: smallest marker count 2^k")

@@ -46,6 +46,7 @@ extern "C" {
 #define TRIMEG_ERR_NO_FIELD    (-3)  /* a gather/rhs/push was asked before trimeg_field_upload   */
 #define TRIMEG_ERR_CUDA        (-4)  /* a CUDA runtime call or kernel launch failed              */
 #define TRIMEG_ERR_ALLOC       (-5)  /* device or host allocation failed                         */
+#define TRIMEG_ERR_UNSUPPORTED (-6)  /* the call is not defined for the loaded field's toroidal basis */
 
 #define TRIMEG_NCOEF 21              /* monomials xi^i eta^j, 0 <= i+j <= 5        */
 
@@ -118,6 +119,22 @@ int trimeg_field_upload(trimeg_ctx *ctx, int n_modes, const int *mode_n_host,
                         const void *data_dev, int kind, trimeg_stream stream);
 /* test hook: coefficient table in the kind-1 layout to device memory */
 int trimeg_field_download_coeffs(trimeg_ctx *ctx, void *coeffs_dev, trimeg_stream stream);
+
+/* ---- field on the cubic B-spline toroidal basis (row f3) ---------------------------------------
+ * The thesis's own toroidal discretisation ("the cubic B-spline in the toroidal direction";
+ * PAPER.md:365-368 Y = sum_i sum_j Lambda_i(xi, eta) N_j(Phi) Y_ij; PAPER.md:320-326 uniform periodic grid in phi):
+ *   dphi(R, phi, Z) = sum_{j=0}^{n_phi-1} N_j(phi) P_j(xi, eta),   N_j(phi) = beta(phi/h - j),  h = 2 pi/n_phi,
+ * periodic in j, beta the uniform cubic B-spline (reading G28 of DESIGN.md), P_j the real C1 quintic of plane j.
+ * Four planes are non-zero at any phi.
+ *   kind 0: data_dev = nodal DOFs [n_phi][n_vert][6] float64, the six per vertex as in trimeg_field_upload;
+ *   kind 1: data_dev = coefficients [n_tri][n_phi][21] float64, monomial order as in trimeg_field_upload.
+ * n_phi >= 4.  Replaces whatever field was loaded (harmonic table, mode list and the dA^s / dA^h tables are dropped);
+ * a later trimeg_field_upload returns to harmonics.  trimeg_locate / gather / rhs / push / push_host / sort / compact
+ * work on either basis; trimeg_scatter, trimeg_field_upload_aux, trimeg_rhs_em and trimeg_pullback return
+ * UNSUPPORTED while a B-spline field is loaded.  trimeg_field_download_coeffs writes [n_tri][n_phi][21] float64.
+ * Ordering as trimeg_field_upload.  Errors: INVALID_ARG (n_phi < 4, NULL), ALLOC, CUDA. */
+int trimeg_field_upload_spline(trimeg_ctx *ctx, int n_phi, const double *data_dev, int kind,
+                               trimeg_stream stream);
 
 /* ---- locator (row a2) ----------------------------------------------
  * cell[p] = lowest triangle index t whose contains() test passes for (R[p], Z[p]), the test

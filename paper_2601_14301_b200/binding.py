@@ -17,13 +17,13 @@ LIB_PATH = os.path.join(_HERE, "libtrimeg.so")
 
 EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
-    "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_download_coeffs",
+    "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_upload_spline", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
     "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
 )
 
-OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC = 0, -1, -2, -3, -4, -5
+OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
 # TRIMEG_PUSH_KERNEL_* of include/trimeg.h
 FIELD_AS, FIELD_AH = 1, 2      # TRIMEG_FIELD_AS / _AH
 PUSH_KERNEL_AUTO, PUSH_KERNEL_THREAD, PUSH_KERNEL_LANE, PUSH_KERNEL_WCACHE = -1, 0, 1, 2
@@ -67,6 +67,7 @@ def load() -> C.CDLL:
     L.trimeg_set_params.argtypes = [vp, C.POINTER(trimeg_params)]
     L.trimeg_mesh_download_geom.argtypes = [vp, vp, vp]
     L.trimeg_field_upload.argtypes = [vp, i32, C.POINTER(i32), vp, i32, vp]
+    L.trimeg_field_upload_spline.argtypes = [vp, i32, vp, i32, vp]
     L.trimeg_field_download_coeffs.argtypes = [vp, vp, vp]
     L.trimeg_locate.argtypes = [vp, sz, vp, vp, vp, vp]
     L.trimeg_gather.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, vp, vp]
@@ -156,6 +157,7 @@ class Context:
         _check(self.L.trimeg_mesh_info(self.h, C.byref(nv), C.byref(nt)), "trimeg_mesh_info")
         self.n_r, self.n_theta, self.n_vert, self.n_tri = int(n_r), int(n_theta), nv.value, nt.value
         self.n_modes = 0
+        self.n_phi = 0
 
     def close(self):
         if getattr(self, "h", None) and self.h.value:
@@ -189,8 +191,25 @@ class Context:
         ptr = _ptr(data, torch.complex128) if M > 0 else C.c_void_p(0)
         _check(self.L.trimeg_field_upload(self.h, M, modes, ptr, int(kind), _stream(stream)), "trimeg_field_upload")
         self.n_modes = M
+        self.n_phi = 0
+
+    def field_upload_spline(self, data: torch.Tensor, kind: int, stream=None):
+        """Row f3: real nodal DOFs [n_phi][n_vert][6] (kind 0) or coefficients [n_tri][n_phi][21] (kind 1)."""
+        n_phi = int(data.shape[0] if kind == 0 else data.shape[1])
+        want = (n_phi, self.n_vert, 6) if kind == 0 else (self.n_tri, n_phi, 21)
+        if tuple(data.shape) != want:
+            raise ValueError(f"field data shape {tuple(data.shape)} != {want}")
+        _check(self.L.trimeg_field_upload_spline(self.h, n_phi, _ptr(data, torch.float64), int(kind), _stream(stream)),
+               "trimeg_field_upload_spline")
+        self.n_modes = 0
+        self.n_phi = n_phi
 
     def field_download_coeffs(self, stream=None) -> torch.Tensor:
+        if getattr(self, "n_phi", 0):
+            out = torch.empty((self.n_tri, self.n_phi, 21), dtype=torch.float64, device="cuda")
+            _check(self.L.trimeg_field_download_coeffs(self.h, _ptr(out, torch.float64), _stream(stream)),
+                   "trimeg_field_download_coeffs")
+            return out
         out = torch.empty((self.n_tri, self.n_modes, 21), dtype=torch.complex128, device="cuda")
         if self.n_modes:
             _check(self.L.trimeg_field_download_coeffs(self.h, _ptr(out, torch.complex128), _stream(stream)),

@@ -30,6 +30,11 @@ struct FieldDev {
     const int *mode_n;      // [n_modes] (device)
     int n_first, n_step;    // arithmetic progression n_k = n_first + k n_step if is_ap
     int is_ap;
+    // row f3: cubic B-spline toroidal basis.  n_phi > 0: the field is
+    // sum_j N_j(phi) P_j(xi, eta) on n_phi uniform periodic planes (then n_modes == 0)
+    int n_phi;
+    const double *spl;      // [n_tri][n_phi][21] real
+    double inv_h;           // n_phi / (2 pi)
 };
 
 struct PhysDev {
@@ -205,18 +210,19 @@ __device__ __forceinline__ void eval_quintic(const double2 *__restrict__ c, doub
     P.re = pr; P.im = pi; Px.re = pxr; Px.im = pxi; Pe.re = per; Pe.im = pei;
 }
 
-// A mode with n = 0: only Re(P) reaches the result (reading G15) -- the real chains of eval_quintic alone.
-__device__ __forceinline__ void eval_quintic_real(const double2 *__restrict__ c, double xi, double eta,
-                                                  double &P, double &Px, double &Pe)
+// A real quintic (the real chains of eval_quintic alone), coefficient k at c[k * STRIDE].
+template <int STRIDE>
+__device__ __forceinline__ void eval_quintic_real_s(const double *__restrict__ c, double xi, double eta,
+                                                    double &P, double &Px, double &Pe)
 {
     double pr = 0.0, pxr = 0.0, per = 0.0;
 #pragma unroll
     for (int j = 5; j >= 0; --j) {
         const int n = 5 - j;
-        double ar = __ldg(&c[kidx(n, j)].x), dr = 0.0;
+        double ar = __ldg(c + STRIDE * kidx(n, j)), dr = 0.0;
 #pragma unroll
         for (int i = n - 1; i >= 0; --i) {
-            const double cx = __ldg(&c[kidx(i, j)].x);
+            const double cx = __ldg(c + STRIDE * kidx(i, j));
             if (i == n - 1) dr = ar;
             else dr = fma(dr, xi, ar);
             ar = fma(ar, xi, cx);
@@ -230,6 +236,38 @@ __device__ __forceinline__ void eval_quintic_real(const double2 *__restrict__ c,
     }
     P = pr; Px = pxr; Pe = per;
 }
+// A mode with n = 0: only Re(P) reaches the result (reading G15).
+__device__ __forceinline__ void eval_quintic_real(const double2 *__restrict__ c, double xi, double eta,
+                                                  double &P, double &Px, double &Pe)
+{
+    eval_quintic_real_s<2>(reinterpret_cast<const double *>(c), xi, eta, P, Px, Pe);
+}
+
+// Row f3: the four cubic B-splines that are non-zero at phi (reading G28: N_j(phi) = beta(phi/h - j), h = 2 pi/n_phi,
+// periodic in j) and their phi-derivatives.  With x = phi/h, j0 = floor(x), t = x - j0 in [0, 1):
+//   planes j0-1, j0, j0+1, j0+2 carry beta(t+1), beta(t), beta(t-1), beta(t-2).
+struct SplineW { int j0; double N[4], D[4]; };
+__device__ __forceinline__ SplineW spline_weights(int n_phi, double inv_h, double phi)
+{
+    SplineW s;
+    const double x = phi * inv_h;
+    const double fl = floor(x);
+    const double t = x - fl, u = 1.0 - t;
+    const double np = (double)n_phi;
+    s.j0 = (int)(fl - np * floor(fl / np));
+    if (s.j0 >= n_phi) s.j0 -= n_phi;                      // fl / np rounded up to an integer
+    if (s.j0 < 0) s.j0 += n_phi;
+    const double t2 = t * t, u2 = u * u;
+    s.N[0] = u2 * u * (1.0 / 6.0);
+    s.N[1] = fma(t2, fma(0.5, t, -1.0), 2.0 / 3.0);
+    s.N[2] = fma(u2, fma(0.5, u, -1.0), 2.0 / 3.0);
+    s.N[3] = t2 * t * (1.0 / 6.0);
+    s.D[0] = -0.5 * u2 * inv_h;
+    s.D[1] = t * fma(1.5, t, -2.0) * inv_h;
+    s.D[2] = -u * fma(1.5, u, -2.0) * inv_h;
+    s.D[3] = 0.5 * t2 * inv_h;
+    return s;
+}
 
 struct FieldVal { double f, fR, fZ, fphi; };   // dphi, d/dR, d/dZ, d/dphi
 
@@ -237,7 +275,18 @@ struct FieldVal { double f, fR, fZ, fphi; };   // dphi, d/dR, d/dZ, d/dphi
 __device__ __forceinline__ FieldVal gather(const FieldDev &F, int t, const Bary &b, double phi)
 {
     double f = 0.0, fx = 0.0, fe = 0.0, fp = 0.0;
-    if (F.n_modes > 0) {
+    if (F.n_phi > 0) {
+        const SplineW s = spline_weights(F.n_phi, F.inv_h, phi);
+        const double *base = F.spl + (size_t)t * F.n_phi * NCOEF;
+        int j = (s.j0 == 0) ? F.n_phi - 1 : s.j0 - 1;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            double P, Px, Pe;
+            eval_quintic_real_s<1>(base + j * NCOEF, b.xi, b.eta, P, Px, Pe);
+            f = fma(s.N[k], P, f); fx = fma(s.N[k], Px, fx); fe = fma(s.N[k], Pe, fe); fp = fma(s.D[k], P, fp);
+            j = (j + 1 == F.n_phi) ? 0 : j + 1;
+        }
+    } else if (F.n_modes > 0) {
         const double2 *c = F.coef + (size_t)t * F.n_modes * NCOEF;
         double Er, Ei, Dr = 1.0, Di = 0.0;
         if (F.is_ap) {

@@ -34,6 +34,7 @@ struct trimeg_ctx {
     double *d_geom, *d_r_nodes, *d_vR, *d_vZ;
     double2 *d_coef;
     double2 *d_coef_aux[2];         // row f2: dA^s, dA^h on the main field's basis and mode list; NULL = identically zero
+    double *d_coef_spl;             // row f3: [n_tri][n_phi][21] real, the field on the cubic B-spline toroidal basis (then d_coef == NULL)
     int *d_mode_n;
     int has_field;
     int push_kernel;                // trimeg_set_push_kernel variant
@@ -67,6 +68,19 @@ namespace trimeg {
 inline int auto_push_kernel(int n_modes)
 {
     return (n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES) ? TRIMEG_PUSH_KERNEL_LANE : TRIMEG_PUSH_KERNEL_WCACHE;
+}
+
+// The schedule a push call runs.  Row f3 (field on cubic B-spline planes): the lane kernel holds plane records as it holds
+// mode records (two planes take the place of a complex mode) when the record is a whole number of 16-byte units (n_phi even)
+// and a useful number of records fits into shared memory; else, or when the thread schedule is asked for, thread per marker.
+constexpr int TRIMEG_SPLINE_LANE_MAX_PLANES = 48;
+inline int effective_push_kernel(const trimeg_ctx *c)
+{
+    if (c->field.n_phi > 0) {
+        const bool lane_ok = (c->field.n_phi % 2 == 0) && c->field.n_phi <= TRIMEG_SPLINE_LANE_MAX_PLANES;
+        return (c->push_kernel == TRIMEG_PUSH_KERNEL_THREAD || !lane_ok) ? TRIMEG_PUSH_KERNEL_THREAD : TRIMEG_PUSH_KERNEL_LANE;
+    }
+    return (c->push_kernel == TRIMEG_PUSH_KERNEL_AUTO) ? auto_push_kernel(c->field.n_modes) : c->push_kernel;
 }
 
 // launch wrappers implemented in trimeg_push.cu; each returns the cudaError of the launch

@@ -137,9 +137,78 @@ __device__ __forceinline__ void gather_lane_impl(const FieldDev &F, const double
     }
 }
 
+// ---- row f3: the field on cubic B-spline toroidal planes.  Two planes take the places of the real and the imaginary part
+// of a complex mode: one two-phase evaluation per pair of planes, (j0-1, j0) and (j0+1, j0+2), each plane a real record
+// of 21 doubles (8-byte shared-memory loads: planes are 21 doubles apart, markers of one triangle on different planes
+// read different banks).  Per-plane chains and the order of the four weighted sums are those of gather().
+__device__ __forceinline__ void eval_quintic_2ph_pair(const double *__restrict__ c0, const double *__restrict__ c1, double xi,
+                                                      double eta, int opaque, double &pr, double &pi, double &pxr, double &pxi,
+                                                      double &per, double &pei)
+{
+    double Ar[6], Ai[6], Dr[6], Di[6];
+#pragma unroll
+    for (int j = 5; j >= 0; --j) {
+        const int n = 5 - j;
+        double ar = 0.0, ai = 0.0, dr = 0.0, di = 0.0;
+#pragma unroll
+        for (int i = n; i >= 0; --i) {
+            const double cx = c0[kidx(i, j)], cy = c1[kidx(i, j)];
+            if (i == n) { ar = cx; ai = cy; }
+            else {
+                if (i == n - 1) { dr = ar; di = ai; }
+                else { dr = fma(dr, xi, ar); di = fma(di, xi, ai); }
+                ar = fma(ar, xi, cx); ai = fma(ai, xi, cy);
+            }
+        }
+        Ar[j] = ar; Ai[j] = ai; Dr[j] = dr; Di[j] = di;
+    }
+    if (opaque >= 0) {
+        double qr = Ar[5], qi = Ai[5], er = 0.0, ei = 0.0, xr = Dr[4], xm = Di[4];
+#pragma unroll
+        for (int j = 4; j >= 0; --j) {
+            if (j == 4) { er = qr; ei = qi; }
+            else {
+                er = fma(er, eta, qr); ei = fma(ei, eta, qi);
+                xr = fma(xr, eta, Dr[j]); xm = fma(xm, eta, Di[j]);
+            }
+            qr = fma(qr, eta, Ar[j]); qi = fma(qi, eta, Ai[j]);
+        }
+        pr = qr; pi = qi; pxr = xr; pxi = xm; per = er; pei = ei;
+    } else {
+        double s = 0.0;
+#pragma unroll
+        for (int j = 0; j < 6; ++j) s += (Ar[j] + Ai[j]) + (Dr[j] + Di[j]);
+        pr = pi = pxr = pxi = per = pei = s;
+    }
+}
+
+__device__ __forceinline__ void gather_lane_spline(const FieldDev &F, const double *rec, double xi, double eta, double phi,
+                                                   int zero, double &f, double &fx, double &fe, double &fp)
+{
+    const SplineW s = spline_weights(F.n_phi, F.inv_h, phi);
+    const int ja = (s.j0 == 0) ? F.n_phi - 1 : s.j0 - 1;
+    const int jc = (s.j0 + 1 == F.n_phi) ? 0 : s.j0 + 1;
+    const int jd = (jc + 1 == F.n_phi) ? 0 : jc + 1;
+    double pr, pi, pxr, pxi, per, pei;
+    eval_quintic_2ph_pair(rec + ja * NCOEF, rec + s.j0 * NCOEF, xi, eta, s.j0 + zero, pr, pi, pxr, pxi, per, pei);
+    f = s.N[0] * pr; fx = s.N[0] * pxr; fe = s.N[0] * per; fp = s.D[0] * pr;
+    f = fma(s.N[1], pi, f); fx = fma(s.N[1], pxi, fx); fe = fma(s.N[1], pei, fe); fp = fma(s.D[1], pi, fp);
+    eval_quintic_2ph_pair(rec + jc * NCOEF, rec + jd * NCOEF, xi, eta, jd + zero, pr, pi, pxr, pxi, per, pei);
+    f = fma(s.N[2], pr, f); fx = fma(s.N[2], pxr, fx); fe = fma(s.N[2], per, fe); fp = fma(s.D[2], pr, fp);
+    f = fma(s.N[3], pi, f); fx = fma(s.N[3], pxi, fx); fe = fma(s.N[3], pei, fe); fp = fma(s.D[3], pi, fp);
+}
+
+// length of a triangle's record in 16-byte units, and where it starts in the global table (harmonic or B-spline field)
+__device__ __host__ __forceinline__ int lane_rec_len(const FieldDev &F) { return F.n_phi > 0 ? F.n_phi * NCOEF / 2 : F.n_modes * NCOEF; }
+__device__ __forceinline__ const double2 *lane_rec_src(const FieldDev &F, int t)
+{
+    return F.n_phi > 0 ? reinterpret_cast<const double2 *>(F.spl + (size_t)t * F.n_phi * NCOEF) : F.coef + (size_t)t * F.n_modes * NCOEF;
+}
+
 __device__ __forceinline__ void gather_lane(const FieldDev &F, const double2 *c, double xi, double eta, double phi, int zero,
                                             double &f, double &fx, double &fe, double &fp)
 {
+    if (F.n_phi > 0) { gather_lane_spline(F, reinterpret_cast<const double *>(c), xi, eta, phi, zero, f, fx, fe, fp); return; }
     if (F.is_ap) gather_lane_impl<true>(F, c, xi, eta, phi, zero, f, fx, fe, fp);
     else gather_lane_impl<false>(F, c, xi, eta, phi, zero, f, fx, fe, fp);
 }

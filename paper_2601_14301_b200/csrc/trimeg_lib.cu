@@ -71,8 +71,10 @@ __global__ void geom_kernel(int n_r, int n_theta, int n_tri, const double *__res
 // No linear solve: DOFs are mapped to reference coordinates with the edge vectors, multiplied
 // by the fixed right inverse P18 of the vertex conditions, and the three edge bubbles are
 // scaled so that the normal derivative is cubic on every edge (see gen_bell_tables.py).
+// REAL: dofs and coefficients are real (row f3: one "mode" per toroidal plane of the cubic B-spline basis).
+template <bool REAL>
 __global__ void bell_kernel(int n_theta, int n_tri, int n_vert, int n_modes, const double *__restrict__ vR,
-                            const double *__restrict__ vZ, const double2 *__restrict__ dofs, double2 *__restrict__ coef)
+                            const double *__restrict__ vZ, const void *__restrict__ dofs_v, void *__restrict__ coef_v)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (size_t)n_tri * n_modes) return;
@@ -84,8 +86,16 @@ __global__ void bell_kernel(int n_theta, int n_tri, int n_vert, int n_modes, con
     double dr[18], di[18];
 #pragma unroll
     for (int p = 0; p < 3; ++p) {
-        const double2 *d = dofs + ((size_t)m * n_vert + v[p]) * 6;
-        const double2 f = d[0], fR = d[1], fZ = d[2], fRR = d[3], fRZ = d[4], fZZ = d[5];
+        const size_t at = ((size_t)m * n_vert + v[p]) * 6;
+        double2 f, fR, fZ, fRR, fRZ, fZZ;
+        if (REAL) {
+            const double *d = (const double *)dofs_v + at;
+            f = make_double2(d[0], 0.0); fR = make_double2(d[1], 0.0); fZ = make_double2(d[2], 0.0);
+            fRR = make_double2(d[3], 0.0); fRZ = make_double2(d[4], 0.0); fZZ = make_double2(d[5], 0.0);
+        } else {
+            const double2 *d = (const double2 *)dofs_v + at;
+            f = d[0]; fR = d[1]; fZ = d[2]; fRR = d[3]; fRZ = d[4]; fZZ = d[5];
+        }
 #define TR(dst, X)                                                                                           \
         dst[6 * p + 0] = f.X;                                                                                \
         dst[6 * p + 1] = e1R * fR.X + e1Z * fZ.X;                                                            \
@@ -129,13 +139,14 @@ __global__ void bell_kernel(int n_theta, int n_tri, int n_vert, int n_modes, con
         z[1][part] = -G1 / e22;
         z[2][part] = G2 / ett;
     }
-    double2 *out = coef + ((size_t)t * n_modes + m) * NCOEF;
+    const size_t to = ((size_t)t * n_modes + m) * NCOEF;
 #pragma unroll
     for (int k = 0; k < 21; ++k) {
         double2 o;
         o.x = cr[k] + z[0][0] * c_bubble[0][k] + z[1][0] * c_bubble[1][k] + z[2][0] * c_bubble[2][k];
         o.y = ci[k] + z[0][1] * c_bubble[0][k] + z[1][1] * c_bubble[1][k] + z[2][1] * c_bubble[2][k];
-        out[k] = o;
+        if (REAL) ((double *)coef_v)[to + k] = o.x;
+        else ((double2 *)coef_v)[to + k] = o;
     }
 }
 
@@ -444,7 +455,7 @@ int trimeg_mesh_destroy(trimeg_ctx *c)
     DeviceGuard guard__(c->device);
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
     cudaFree(c->d_adj_off); cudaFree(c->d_adj); cudaFree(c->d_trirhs);
-    cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]);
+    cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]); cudaFree(c->d_coef_spl);
     cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
     if (c->hstreams_ready) {
         for (int k = 0; k < 3; ++k) cudaStreamDestroy(c->hstream[k]);
@@ -475,8 +486,7 @@ int trimeg_set_params(trimeg_ctx *c, const trimeg_params *p)
 int trimeg_get_push_kernel(const trimeg_ctx *c)
 {
     if (!c) return -2;
-    if (c->push_kernel != TRIMEG_PUSH_KERNEL_AUTO) return c->push_kernel;
-    return trimeg::auto_push_kernel(c->field.n_modes);
+    return trimeg::effective_push_kernel(c);
 }
 
 int trimeg_set_push_kernel(trimeg_ctx *c, int variant)
@@ -502,6 +512,10 @@ int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, cons
     if (n_modes > 0 && (!mode_n_host || !data_dev)) return TRIMEG_ERR_INVALID_ARG;
     ON_CTX_DEVICE(c);
     cudaStream_t s = (cudaStream_t)stream;
+    if (c->d_coef_spl) {                                 // back from the B-spline basis (row f3) to harmonics
+        CU_TRY(cudaDeviceSynchronize());
+        cudaFree(c->d_coef_spl); c->d_coef_spl = nullptr; c->field.n_phi = 0; c->field.spl = nullptr;
+    }
     if (n_modes != c->field.n_modes || !c->d_coef) {
         // tables may still be in use by kernels enqueued earlier
         CU_TRY(cudaDeviceSynchronize());
@@ -530,8 +544,8 @@ int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, cons
                                    cudaMemcpyDeviceToDevice, s));
         } else {
             const size_t work = (size_t)c->n_tri * n_modes;
-            bell_kernel<<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR,
-                                                                       c->d_vZ, (const double2 *)data_dev, c->d_coef);
+            bell_kernel<false><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR,
+                                                                       c->d_vZ, data_dev, c->d_coef);
             c->n_launches++;
             CU_TRY(cudaGetLastError());
         }
@@ -547,6 +561,7 @@ int trimeg_field_upload_aux(trimeg_ctx *c, int which, const void *data_dev, int 
 {
     if (!c || (which != TRIMEG_FIELD_AS && which != TRIMEG_FIELD_AH) || (kind != 0 && kind != 1)) return TRIMEG_ERR_INVALID_ARG;
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (c->field.n_phi > 0) return TRIMEG_ERR_UNSUPPORTED;
     ON_CTX_DEVICE(c);
     const int a = which - TRIMEG_FIELD_AS, n_modes = c->field.n_modes;
     cudaStream_t s = (cudaStream_t)stream;
@@ -559,11 +574,41 @@ int trimeg_field_upload_aux(trimeg_ctx *c, int which, const void *data_dev, int 
     if (kind == 1) CU_TRY(cudaMemcpyAsync(c->d_coef_aux[a], data_dev, bytes, cudaMemcpyDeviceToDevice, s));
     else {
         const size_t work = (size_t)c->n_tri * n_modes;
-        bell_kernel<<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR, c->d_vZ,
-                                                                   (const double2 *)data_dev, c->d_coef_aux[a]);
+        bell_kernel<false><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR, c->d_vZ,
+                                                                   data_dev, c->d_coef_aux[a]);
         c->n_launches++;
         CU_TRY(cudaGetLastError());
     }
+    return TRIMEG_OK;
+}
+
+// Row f3: the field on the cubic B-spline toroidal basis.  The harmonic table, its mode list and the aux tables go.
+int trimeg_field_upload_spline(trimeg_ctx *c, int n_phi, const double *data_dev, int kind, trimeg_stream stream)
+{
+    if (!c || n_phi < 4 || !data_dev || (kind != 0 && kind != 1)) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
+    cudaStream_t s = (cudaStream_t)stream;
+    const size_t bytes = sizeof(double) * NCOEF * (size_t)c->n_tri * n_phi;
+    if (n_phi != c->field.n_phi || !c->d_coef_spl || c->d_coef) {
+        CU_TRY(cudaDeviceSynchronize());                 // tables may still be in use by kernels enqueued earlier
+        cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]); cudaFree(c->d_coef_spl);
+        c->d_coef = nullptr; c->d_mode_n = nullptr; c->d_coef_aux[0] = c->d_coef_aux[1] = nullptr; c->d_coef_spl = nullptr;
+        c->has_field = 0; c->field.n_modes = 0; c->field.n_phi = 0; c->field.coef = nullptr; c->field.mode_n = nullptr; c->field.spl = nullptr;
+        if (cudaMalloc(&c->d_coef_spl, bytes) != cudaSuccess) { cudaGetLastError(); c->d_coef_spl = nullptr; return TRIMEG_ERR_ALLOC; }
+    }
+    c->field.is_ap = 1; c->field.n_first = 0; c->field.n_step = 0;
+    c->field.n_phi = n_phi; c->field.spl = c->d_coef_spl; c->field.inv_h = (double)n_phi / 6.283185307179586476925286766559;
+    if (kind == 1) CU_TRY(cudaMemcpyAsync(c->d_coef_spl, data_dev, bytes, cudaMemcpyDeviceToDevice, s));
+    else {
+        const size_t work = (size_t)c->n_tri * n_phi;
+        bell_kernel<true><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_phi, c->d_vR, c->d_vZ,
+                                                                         data_dev, c->d_coef_spl);
+        c->n_launches++;
+        CU_TRY(cudaGetLastError());
+    }
+    c->has_field = 1;
+    if (!c->ev_upload) CU_TRY(cudaEventCreateWithFlags(&c->ev_upload, cudaEventDisableTiming));
+    CU_TRY(cudaEventRecord(c->ev_upload, s));
     return TRIMEG_OK;
 }
 
@@ -572,6 +617,7 @@ int trimeg_rhs_em(trimeg_ctx *c, const trimeg_markers *m, size_t n, double *dRdt
 {
     if (!c || (n > 0 && (!markers_ok(m) || !dRdt || !dZdt || !dphidt || !dudt || !dwdt))) return TRIMEG_ERR_INVALID_ARG;
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (c->field.n_phi > 0) return TRIMEG_ERR_UNSUPPORTED;
     if (n == 0) return TRIMEG_OK;
     ON_CTX_DEVICE(c);
     CU_TRY(launch_rhs_em(c, *m, n, dRdt, dZdt, dphidt, dudt, dwdt, (cudaStream_t)stream));
@@ -582,6 +628,7 @@ int trimeg_pullback(trimeg_ctx *c, trimeg_markers *m, size_t n, trimeg_stream st
 {
     if (!c || (n > 0 && !markers_ok(m))) return TRIMEG_ERR_INVALID_ARG;
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (c->field.n_phi > 0) return TRIMEG_ERR_UNSUPPORTED;
     if (n == 0) return TRIMEG_OK;
     ON_CTX_DEVICE(c);
     CU_TRY(launch_pullback(c, *m, n, (cudaStream_t)stream));
@@ -593,6 +640,11 @@ int trimeg_field_download_coeffs(trimeg_ctx *c, void *coeffs_dev, trimeg_stream 
     if (!c || !coeffs_dev) return TRIMEG_ERR_INVALID_ARG;
     ON_CTX_DEVICE(c);
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (c->field.n_phi > 0) {                            // row f3: real [n_tri][n_phi][21]
+        CU_TRY(cudaMemcpyAsync(coeffs_dev, c->d_coef_spl, sizeof(double) * NCOEF * (size_t)c->n_tri * c->field.n_phi,
+                               cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+        return TRIMEG_OK;
+    }
     if (c->field.n_modes == 0) return TRIMEG_OK;
     CU_TRY(cudaMemcpyAsync(coeffs_dev, c->d_coef, sizeof(double2) * NCOEF * (size_t)c->n_tri * c->field.n_modes,
                            cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
@@ -643,6 +695,7 @@ int trimeg_scatter(trimeg_ctx *c, const trimeg_markers *m, size_t n, void *rhs_d
 {
     if (!c || (n > 0 && !markers_ok(m)) || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
     if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (c->field.n_phi > 0) return TRIMEG_ERR_UNSUPPORTED;
     const int n_modes = c->field.n_modes;
     if (n_modes == 0) return TRIMEG_OK;
     if (!rhs_dev) return TRIMEG_ERR_INVALID_ARG;
@@ -963,6 +1016,7 @@ const char *trimeg_strerror(int code)
     case TRIMEG_ERR_NO_FIELD: return "no field uploaded";
     case TRIMEG_ERR_CUDA: return "CUDA error";
     case TRIMEG_ERR_ALLOC: return "allocation failed";
+    case TRIMEG_ERR_UNSUPPORTED: return "not defined for the loaded field's toroidal basis";
     default: return "unknown error";
     }
 }

@@ -205,7 +205,7 @@ cudaError_t launch_rhs(trimeg_ctx *c, const trimeg_markers &m, size_t n, double 
 cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
-    const int variant = (c->push_kernel == TRIMEG_PUSH_KERNEL_AUTO) ? auto_push_kernel(c->field.n_modes) : c->push_kernel;
+    const int variant = effective_push_kernel(c);
     if (variant == TRIMEG_PUSH_KERNEL_LANE) return launch_push_lane(c, m, n, dt, nsteps, s);
     if (variant == TRIMEG_PUSH_KERNEL_WCACHE) return launch_push_wcache(c, m, n, dt, nsteps, s);
     push_kernel<<<grid_for(n, PUSH_BLOCK), PUSH_BLOCK, 0, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);

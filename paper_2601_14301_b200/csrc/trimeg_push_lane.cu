@@ -32,7 +32,7 @@ constexpr int LN_SYNC_EVERY = 10;   // RK4 steps between two meetings of the CTA
 constexpr int LN_MAXSPIN = 400;     // polls of a record another warp is copying (64 ns apart) before giving up
 enum { LN_LOADING = 1, LN_READY = 2 };
 
-constexpr size_t LN_WARP_BYTES = (sizeof(double) * (size_t)N_STATE * LN_NW + sizeof(int) * (size_t)LN_NW + LN_NW + 15) / 16 * 16;
+constexpr size_t LN_WARP_BYTES = (sizeof(double) * (size_t)N_STATE * LN_NW + sizeof(int) * (size_t)LN_NW + 2 * LN_NW + 15) / 16 * 16;
 constexpr size_t LN_TABLE_BYTES = sizeof(int) * (3 * LN_NBIN + 4);     // tag, state, rec_of, counters
 
 __device__ __forceinline__ unsigned ln_hash(int t) { return ((unsigned)t * 0x9E3779B1u) >> 25; }   // 7 bits
@@ -70,7 +70,7 @@ __device__ __forceinline__ int ln_lookup(int tl, int lane, int *tag, volatile in
     if ((code & 3) == 2) {                               // this warp copies the record: coefficients, then the geometry row
         rec = rec_of[h];
         rec = __shfl_sync(FULL, rec, 0);
-        const double2 *src = F.coef + (size_t)tl * rec_len;
+        const double2 *src = lane_rec_src(F, tl);
         const double2 *geo = reinterpret_cast<const double2 *>(M.geom + 6 * (size_t)tl);
         double2 *dst = REC + (size_t)rec * rec_stride;
 #pragma unroll 4
@@ -105,17 +105,18 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
     double *S = reinterpret_cast<double *>(wbase);                  // [N_STATE][NW]
     int *cell = reinterpret_cast<int *>(S + (size_t)N_STATE * NW);   // [NW] current triangle
     unsigned char *flags = reinterpret_cast<unsigned char *>(cell + NW);     // [NW]
+    unsigned char *orig = flags + NW;                                // [NW] marker (offset in the warp's 64) that sits in a slot
     int *tag = reinterpret_cast<int *>(smem_l + (size_t)WARPS * LN_WARP_BYTES);      // [LN_NBIN] triangle of a bin
     volatile int *state = tag + LN_NBIN;                             // [LN_NBIN] 0 / LN_LOADING / LN_READY
     int *rec_of = tag + 2 * LN_NBIN;                                 // [LN_NBIN] record slot, -1 = none
     int *counters = tag + 3 * LN_NBIN;                               // [0] bins claimed since the table was emptied
-    const int rec_len = F.n_modes * NCOEF;
+    const int rec_len = lane_rec_len(F);
     const int rec_stride = (rec_len + 3) | 1;                        // odd number of 16-byte units: records start in different banks
     double2 *REC = reinterpret_cast<double2 *>(smem_l + ((size_t)WARPS * LN_WARP_BYTES + LN_TABLE_BYTES + 15) / 16 * 16);
 
     const size_t base = ((size_t)blockIdx.x * WARPS + wib) * NW;
     const int nt = (base >= n) ? 0 : (int)((n - base < (size_t)NW) ? (n - base) : (size_t)NW);   // empty warps stay for the barriers
-    const bool has_field = F.n_modes > 0;
+    const bool has_field = F.n_modes > 0 || F.n_phi > 0;
     const double hdt = 0.5 * dt, dt6 = dt / 6.0;
     TRIMEG_PHASE_CLOCK_INIT                                          // lane 0: record lookups, evaluation + finish, (unused)
     unsigned n_fallback = 0, n_copied = 0, n_stages = 0, n_regroup = 0;
@@ -123,29 +124,66 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
 
     for (int k = tid; k < LN_NBIN; k += 32 * WARPS) { tag[k] = LN_EMPTY; state[k] = 0; rec_of[k] = -1; }
     if (tid < 4) counters[tid] = 0;
-    // ---- load the warp's markers, locate the start positions
+    // ---- load the warp's markers, locate the start positions.  B-spline field: the warp's markers take their slots in the
+    // order of (triangle, toroidal plane), so that the lanes of a pass read neighbouring planes of a record -- different
+    // shared-memory banks (planes are 21 doubles apart) -- instead of planes at random (bank conflicts); the order holds for
+    // the call (a marker crosses a small fraction of a plane spacing per step).  orig[] takes every marker home at the end.
+    unsigned *skey = reinterpret_cast<unsigned *>(S + (size_t)A_R * NW);      // scratch: the accumulators are written at stage 0
+    double ldR[2], ldZ[2], ldP[2], ldV[2], ldW[2], ldM[2];
+    int ldc[2];
+    unsigned char ldf[2];
 #pragma unroll
     for (int p = 0; p < 2; ++p) {
         const int q = lane + 32 * p;
         unsigned char fl = 0;
         int c = -1;
+        ldR[p] = ldZ[p] = ldP[p] = ldV[p] = ldW[p] = ldM[p] = 0.0;
         if (q < nt) {
             const size_t g = base + q;
             c = m.cell[g];
             if (c >= 0) {
-                const double R = m.R[g], Z = m.Z[g];
-                S[Y_R * NW + q] = R; S[Y_Z * NW + q] = Z; S[Y_P * NW + q] = m.phi[g];
-                S[Y_V * NW + q] = m.vpar[g]; S[Y_W * NW + q] = m.w[g]; S[S_MU * NW + q] = m.mu[g];
+                ldR[p] = m.R[g]; ldZ[p] = m.Z[g]; ldP[p] = m.phi[g]; ldV[p] = m.vpar[g]; ldW[p] = m.w[g]; ldM[p] = m.mu[g];
                 fl = FL_ACTIVE | FL_WASACTIVE;
                 Bary b;
                 int moved = 0;
-                const int t = locate(M, R, Z, c, b, moved);
+                const int t = locate(M, ldR[p], ldZ[p], c, b, moved);
                 if (moved) fl |= FL_MOVED;
                 if (t < 0) fl = (fl | FL_LOST) & ~FL_ACTIVE;
                 else c = t;
             }
         }
-        cell[q] = c; flags[q] = fl;
+        ldc[p] = c; ldf[p] = fl;
+        if (F.n_phi > 0) {
+            unsigned key = 0xffffffffu;
+            if (fl & FL_ACTIVE) key = (((unsigned)c << 6) | (unsigned)spline_weights(F.n_phi, F.inv_h, ldP[p]).j0) & 0x7fffffffu;
+            skey[q] = key;
+        }
+    }
+    int slot[2] = {lane, lane + 32};
+    if (F.n_phi > 0) {
+        __syncwarp();
+#pragma unroll
+        for (int p = 0; p < 2; ++p) {
+            const int q = lane + 32 * p;
+            const unsigned key = skey[q];
+            int r = 0;
+#pragma unroll 8
+            for (int o = 0; o < NW; ++o) {
+                const unsigned ko = skey[o];
+                r += (ko < key || (ko == key && o < q)) ? 1 : 0;
+            }
+            slot[p] = r;
+        }
+        __syncwarp();
+    }
+#pragma unroll
+    for (int p = 0; p < 2; ++p) {
+        const int q = slot[p];
+        if (ldf[p] & FL_WASACTIVE) {
+            S[Y_R * NW + q] = ldR[p]; S[Y_Z * NW + q] = ldZ[p]; S[Y_P * NW + q] = ldP[p];
+            S[Y_V * NW + q] = ldV[p]; S[Y_W * NW + q] = ldW[p]; S[S_MU * NW + q] = ldM[p];
+        }
+        cell[q] = ldc[p]; flags[q] = ldf[p]; orig[q] = (unsigned char)(lane + 32 * p);
     }
     __syncthreads();
 
@@ -242,10 +280,9 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
 #pragma unroll
     for (int p = 0; p < 2; ++p) {
         const int q = lane + 32 * p;
-        if (q >= nt) continue;
         const unsigned char fl = flags[q];
-        if (!(fl & FL_WASACTIVE)) continue;
-        const size_t g = base + q;
+        if (!(fl & FL_WASACTIVE)) continue;              // empty slots of a ragged last warp, markers flagged on entry
+        const size_t g = base + orig[q];
         m.R[g] = S[Y_R * NW + q]; m.Z[g] = S[Y_Z * NW + q]; m.phi[g] = S[Y_P * NW + q];
         m.vpar[g] = S[Y_V * NW + q]; m.w[g] = S[Y_W * NW + q];
         m.cell[g] = (fl & FL_LOST) ? -1 : cell[q];
@@ -292,7 +329,7 @@ __global__ void __launch_bounds__(32 * GL_WARPS, 1) gather_lane_kernel(MeshDev M
     volatile int *state = tag + LN_NBIN;
     int *rec_of = tag + 2 * LN_NBIN;
     int *counters = tag + 3 * LN_NBIN;
-    const int rec_len = F.n_modes * NCOEF;
+    const int rec_len = lane_rec_len(F);
     const int rec_stride = (rec_len + 3) | 1;
     double2 *REC = reinterpret_cast<double2 *>(smem_g + (LN_TABLE_BYTES + 15) / 16 * 16);
     for (int k = tid; k < LN_NBIN; k += 32 * GL_WARPS) { tag[k] = LN_EMPTY; state[k] = 0; rec_of[k] = -1; }
@@ -397,8 +434,8 @@ cudaError_t launch_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
     cudaError_t e = cudaFuncSetAttribute(push_lane_kernel<WARPS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
     if (e != cudaSuccess) return e;
     const size_t fixed = ((size_t)WARPS * LN_WARP_BYTES + LN_TABLE_BYTES + 15) / 16 * 16;
-    const size_t rec_bytes = sizeof(double2) * ((NCOEF * (size_t)c->field.n_modes + 3) | 1);    // as rec_stride in the kernel
-    int nslot = c->field.n_modes ? (int)((SMEM_MAX - fixed) / rec_bytes) : 0;
+    const size_t rec_bytes = sizeof(double2) * (((size_t)lane_rec_len(c->field) + 3) | 1);    // as rec_stride in the kernel
+    int nslot = lane_rec_len(c->field) ? (int)((SMEM_MAX - fixed) / rec_bytes) : 0;
     if (nslot > LN_NBIN * 3 / 4) nslot = LN_NBIN * 3 / 4;
     const size_t shm = fixed + (size_t)nslot * rec_bytes;
     const size_t per_cta = (size_t)LN_NW * WARPS;
@@ -417,7 +454,7 @@ cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const d
     cudaError_t e = cudaFuncSetAttribute(gather_lane_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM);
     if (e != cudaSuccess) return e;
     const size_t fixed = (LN_TABLE_BYTES + 15) / 16 * 16;
-    const size_t rec_bytes = sizeof(double2) * ((NCOEF * (size_t)c->field.n_modes + 3) | 1);
+    const size_t rec_bytes = sizeof(double2) * (((size_t)lane_rec_len(c->field) + 3) | 1);
     int nslot = (int)((SMEM - fixed) / rec_bytes);
     if (nslot > LN_NBIN * 3 / 4) nslot = LN_NBIN * 3 / 4;
     size_t n_pass = n / ((size_t)c->n_sm * 4 * 32 * GL_WARPS);                 // at least ~4 chunks per SM
@@ -434,6 +471,11 @@ cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const d
 cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
+#ifndef TRIMEG_SPLINE_LANE_WARPS
+#define TRIMEG_SPLINE_LANE_WARPS 16
+#endif
+    // B-spline plane records are long (n_phi x 168 bytes): fewer warps leave room for more of them per marker
+    if (c->field.n_phi > 0) return launch_lane<TRIMEG_SPLINE_LANE_WARPS>(c, m, n, dt, nsteps, s);
     return launch_lane<16>(c, m, n, dt, nsteps, s);      // 16 warps at 128 registers (12 at 168 lose 8 % with 3 modes, 1 % with 16)
 }
 

@@ -218,6 +218,19 @@ def field_dofs(wl: Workload, seed: Optional[int] = None, sigma: float = 1e-3) ->
     return np.ascontiguousarray(dofs)
 
 
+def spline_dofs(wl: Workload, n_phi: int, seed: Optional[int] = None, sigma: float = 1e-3) -> np.ndarray:
+    """Row f3: real nodal DOFs [n_phi][n_vert][6] for the cubic B-spline toroidal basis -- the workload's perturbation
+    sum_n Re(Y_n e^{i n phi}) sampled on the n_phi planes phi_j = 2 pi j/n_phi (same radial envelopes, helicity and
+    amplitudes as field_dofs; the samples are used as spline coefficients as they are)."""
+    Y = field_dofs(wl, seed, sigma)
+    phi_j = 2.0 * np.pi * np.arange(n_phi) / n_phi
+    out = np.zeros((n_phi, wl.n_vert, 6))
+    for k, n in enumerate(wl.modes):
+        e = np.exp(1j * n * phi_j)
+        out += (Y[k][None, :, :] * e[:, None, None]).real
+    return np.ascontiguousarray(out)
+
+
 # --------------------------------------------------------------------------
 # markers
 # --------------------------------------------------------------------------
