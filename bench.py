@@ -515,6 +515,19 @@ def run_gpu(args, wl):
                          "algorithmic_bytes_per_gather": 52, "algorithmic_flops_per_gather": flops_per_gather(len(w4.modes)),
                          "rows": rows, "clocks": sampler.stop(), "config": workload_config(w4)}
         c4.close()
+        # row f3: cfg5's mesh, markers and perturbation with the field on 32 cubic B-spline planes
+        r3 = PushRun(inputs.WORKLOADS["cfg5"], args.sort_every, -1, keep_host=True, n_phi=32)
+        out = r3.run(2, 3)
+        rf = r3.roofline(fp64_peak, out["seconds"])
+        chk = None if args.no_check else r3.check_against_oracle(stride=max(1, r3.wl.n_markers // 2048))
+        sweep["spline_cfg5"] = {"value": out["units"] / out["seconds"], "unit": UNIT, "steps": 2, "warmup": 3,
+                                "ms_per_step": out["seconds"] / 2 * 1e3, "kernel": rf["kernel"], "frac": rf["frac"],
+                                "achieved_tflops": rf["achieved"], "avg_launch_ms": rf["avg_launch_ms"],
+                                "algorithmic_flops_per_marker_step": r3.flops_unit(),
+                                "push_share_of_step": rf["push_share_of_step"], "clocks": out["clocks"],
+                                "config": workload_config(r3.wl, n_phi=32, extra={"sort_every": r3.sort_every}), "oracle_check": chk}
+        r3.close()
+        del r3
         sweep["em_cfg5"] = em_run(inputs.WORKLOADS["cfg5"], 3, fp64_peak, hbm_peak, with_oracle=not args.no_check)
         sweep["scatter_cfg5"] = scatter_run(inputs.WORKLOADS["cfg5"], 3, fp64_peak, hbm_peak, with_oracle=not args.no_check)
 
