@@ -38,6 +38,7 @@
  *   O10 pullback       u_par, w after the pullback transformation
  *   O11 spline basis   the thesis's own toroidal discretisation: cubic B-splines in phi instead of harmonics
  *                                                           PAPER.md:223, 365-368
+ *   O12 reduced model  eom_variant 2: the "dominant terms" equations A.19-A.29 (b* -> b)
  */
 #include <math.h>
 #include <stdint.h>
@@ -54,7 +55,7 @@ typedef struct {
     double R0, a, B0, q0, q2;      /* circular equilibrium, q(r) = q0 + q2 (r/a)^2 */
     double rho0, qs_over_ms;       /* rho_0, q_s/m_s               */
     double T, kappa_n, kappa_T;    /* Tbar, log-gradients (1/length) */
-    int eom_variant;               /* 0 = b0* as printed (A.4-A.6); 1 = (B/B*par) b + ... (reading G2) */
+    int eom_variant;               /* 0 = b0* as printed (A.4-A.6); 1 = (B/B*par) b + ... (reading G2); 2 = reduced model A.19-A.29 (O12) */
     int weight_mode;               /* 0: wdot = -(1-w) L ; 1: wdot = -L (reading G7) */
 } orc_params;
 
@@ -485,9 +486,18 @@ void orc_equilibrium(const orc_ctx *c, size_t n, const double *R, const double *
 /* ------------------------------------------------------------------- O6 RHS */
 /* Electrostatic subset (dA^s = dA^h = 0  =>  u_par = v_par, b* = b0*, dG = dPhi).
  * eps = (m_s/q_s) rho_0 B_0 (reading G23). */
+static void rhs_point_em_reduced(const orc_params *p, double R, double Z, double upar, double mu, double w,
+                                 const double fld[3][4], int ohm, double out[5]);
 static void rhs_point(const orc_params *p, double R, double Z, double vpar, double mu, double w,
                       const double fld[4] /* dphi, d/dR, d/dZ, d/dphi */, double out[5])
 {
+    if (p->eom_variant == 2) {                        /* O12: the reduced model with dA^s = dA^h = 0 and NO Ohm's-law substitution */
+        double f3[3][4];
+        memset(f3, 0, sizeof(f3));
+        memcpy(f3[0], fld, sizeof(double) * 4);
+        rhs_point_em_reduced(p, R, Z, vpar, mu, w, f3, 0, out);
+        return;
+    }
     orc_eq e; equilibrium(p, R, Z, &e);
     double eps = p->rho0 * p->B0 / p->qs_over_ms;
     double cR = -e.dbphi_dZ;                          /* (curl b)_R   , bracket of A.4 */
@@ -699,6 +709,7 @@ long orc_scatter(orc_ctx *c, size_t n, const double *R, const double *Z, const d
 static void rhs_point_em(const orc_params *p, double R, double Z, double upar, double mu, double w,
                          const double fld[3][4], double out[5])
 {
+    if (p->eom_variant == 2) { rhs_point_em_reduced(p, R, Z, upar, mu, w, fld, 1, out); return; }   /* O12, A.29 */
     orc_eq e; equilibrium(p, R, Z, &e);
     const double eps = p->rho0 * p->B0 / p->qs_over_ms, qom = p->qs_over_ms;
     const double *Phi = fld[0], *As = fld[1], *Ah = fld[2];
@@ -731,6 +742,53 @@ static void rhs_point_em(const orc_params *p, double R, double Z, double upar, d
     double en = vpar * vpar / p->T + 2.0 * mu * e.B / p->T - 1.5;
     double L = drdot * (-p->kappa_n - en * p->kappa_T) - (2.0 * mu / p->T) * (dRdot * e.dBdR + dZdot * e.dBdZ)
              - (2.0 * vpar / p->T) * dudot;
+    out[0] = R0dot + dRdot; out[1] = Z0dot + dZdot; out[2] = P0dot + dPdot; out[3] = u0dot + dudot;
+    out[4] = (p->weight_mode == 0) ? -(1.0 - w) * L : -L;
+}
+/* ------------------------------------------------- O12 reduced equations of motion (eom_variant 2) */
+/* "Only the dominant terms ... obtained by replacing b* with b" (A.19-A.29):
+ *   R0dot = u_par b + C_d B x grad B,        C_d = (m_s/q_s) rho_0 (u_par^2 + mu B) B_0/B^3                 (A.19-A.21)
+ *   u0dot = -mu b.grad B                      (A.22; reading G29: b, as the sentence above says -- A.22 prints b0*, a copy of A.13;
+ *                                              with b the unperturbed motion conserves u^2/2 + mu B exactly, and for F = const, as
+ *                                              here, (b0* - b).grad B = 0 anyway: R b_phi = F/B, curl b's poloidal part is perpendicular to grad B)
+ *   dRdot = C_E b x grad(dG) - (q_s/m_s) dA^h b,   C_E = rho_0 B_0/B,  dG = dPhi - u_par (dA^s + dA^h)    (A.24-A.26)
+ *   dudot = -(q_s/m_s) [ b.grad(dPhi) - u_par b.grad(dA^h) ] - v_mu.grad(dA^s),   v_mu = C_mu B x grad B,
+ *           C_mu = (m_s/q_s) rho_0 mu B B_0/B^3                                                              (A.28 without d_t dA^s)
+ *   reading G30: the velocity in C_d and in the dA^h term of A.28 / A.29 is printed v_par; the coordinate u_par is taken, as in
+ *   A.17 from which A.28 follows by b* -> b (the difference is second order in the fields).
+ *   weight: d ln f_M/dt of PAPER.md:1208 along the perturbed velocity, v_par = u_par - (q_s/m_s) dA^h in the Maxwellian.
+ * ohm = 0: the electrostatic push (orc_rhs / orc_push with eom_variant 2, dA = 0, d_t dA^s = 0); ohm = 1: orc_rhs_em, A.29. */
+static void rhs_point_em_reduced(const orc_params *p, double R, double Z, double upar, double mu, double w,
+                                 const double fld[3][4], int ohm, double out[5])
+{
+    orc_eq e; equilibrium(p, R, Z, &e);
+    const double eps = p->rho0 * p->B0 / p->qs_over_ms, qom = p->qs_over_ms;
+    const double *Phi = fld[0], *As = fld[1], *Ah = fld[2];
+    const double B3 = e.B * e.B * e.B;
+    const double Cd = eps * (upar * upar + mu * e.B) / B3;
+    const double Cmu = eps * mu * e.B / B3;
+    const double CE = p->rho0 * p->B0 / e.B;
+    /* (B x grad B) in (R, phi, Z): (B_phi d_Z B, B_Z d_R B - B_R d_Z B, -B_phi d_R B) */
+    const double xR = e.Bphi * e.dBdZ, xZ = -e.Bphi * e.dBdR, xP = e.BZ * e.dBdR - e.BR * e.dBdZ;
+    const double R0dot = e.bR * upar + Cd * xR;                                                   /* A.19 */
+    const double Z0dot = e.bZ * upar + Cd * xZ;                                                   /* A.20 */
+    const double P0dot = e.bphi * upar / R + Cd * xP / R;                                         /* A.21 */
+    const double u0dot = -mu * (e.bR * e.dBdR + e.bZ * e.dBdZ);                                   /* A.22 (G29) */
+    const double GR = Phi[1] - upar * (As[1] + Ah[1]), GZ = Phi[2] - upar * (As[2] + Ah[2]), GP = Phi[3] - upar * (As[3] + Ah[3]);
+    const double dRdot = CE * (e.bphi * GZ - (e.bZ / R) * GP) - qom * Ah[0] * e.bR;               /* A.24 */
+    const double dZdot = CE * (-e.bphi * GR + (e.bR / R) * GP) - qom * Ah[0] * e.bZ;              /* A.25 */
+    const double dPdot = (CE / R) * (e.bZ * GR - e.bR * GZ) - (1.0 / R) * qom * Ah[0] * e.bphi;   /* A.26 */
+    /* A.28; ohm: d_t dA^s = -b.grad(dPhi) cancels the parallel electric field, which leaves A.29 */
+    const double keepE = ohm ? 0.0 : 1.0;
+    const double dudot = -qom * (e.bR * (keepE * Phi[1] - upar * Ah[1]) + e.bZ * (keepE * Phi[2] - upar * Ah[2])
+                                 + (e.bphi / R) * (keepE * Phi[3] - upar * Ah[3]))
+                         - Cmu * (xR * As[1] + xZ * As[2] + (xP / R) * As[3]);
+    const double vpar = upar - qom * Ah[0];
+    const double x = R - p->R0, r = sqrt(x * x + Z * Z);
+    const double drdot = (r > 0.0) ? (dRdot * x + dZdot * Z) / r : 0.0;
+    const double en = vpar * vpar / p->T + 2.0 * mu * e.B / p->T - 1.5;
+    const double L = drdot * (-p->kappa_n - en * p->kappa_T) - (2.0 * mu / p->T) * (dRdot * e.dBdR + dZdot * e.dBdZ)
+                   - (2.0 * vpar / p->T) * dudot;
     out[0] = R0dot + dRdot; out[1] = Z0dot + dZdot; out[2] = P0dot + dPdot; out[3] = u0dot + dudot;
     out[4] = (p->weight_mode == 0) ? -(1.0 - w) * L : -L;
 }
