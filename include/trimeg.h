@@ -62,7 +62,10 @@ typedef struct {
     double qs_over_ms;       /* q_s / m_s                                                         */
     double T;                /* Tbar of the Maxwellian; sigma_vpar = sqrt(T/2)    */
     double kappa_n, kappa_T; /* -d ln n0/dr, -d ln T/dr (inverse length)           */
-    int eom_variant;         /* 0: b0* as printed in A.4-A.6; 1: (B/B*par) b + ... (reading G2)   */
+    int eom_variant;         /* 0: b0* as printed in A.4-A.6; 1: (B/B*par) b + ... (reading G2);
+                              * 2: the reduced model A.19-A.29, b* -> b, C_d = (m/q) rho_0 (u^2 + mu B) B_0/B^3
+                              *    (row f4): in trimeg_rhs / trimeg_push A.28 with dA = 0, in
+                              *    trimeg_rhs_em A.24-A.26 and A.29 (ideal Ohm's law); the pullback is unchanged */
     int weight_mode;         /* 0: dw/dt = -(1-w) d ln f_M/dt; 1: dw/dt = -d ln f_M/dt (G7)       */
 } trimeg_params;
 

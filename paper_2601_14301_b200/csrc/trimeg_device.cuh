@@ -352,9 +352,83 @@ __device__ __forceinline__ double rsqrt_fast(double x)
 // d ln f_M/dt (kappa_X along -rhat, G6/G10).
 struct Rates { double R, Z, phi, vpar, w; };
 
+// Row f4, eom_variant 2: the reduced equations A.19-A.29 ("only the dominant terms ... replacing b* with b",
+// PAPER.md:1276-1307; readings G29, G30): R0dot = u b + C_d B x grad B with C_d = eps (u^2 + mu B)/B^3, u0dot = -mu b.grad B,
+// dRdot = C_E b x grad(dG) - (q/m) dA^h b with C_E = rho_0 B_0/B, dudot = -(q/m)[b.grad dPhi - u b.grad dA^h] - v_mu.grad dA^s
+// (A.28); EM = true: dA^s, dA^h present and the parallel electric field cancelled by the ideal Ohm's law (A.29).
+template <bool EM>
+__device__ __forceinline__ Rates rhs_point_reduced(const PhysDev &p, double R, double Z, double upar, double mu, double w,
+                                                   const FieldVal &Phi, const FieldVal &As, const FieldVal &Ah)
+{
+    const double x = R - p.R0;
+    const double s = fma(x, x, Z * Z);
+    const double qb = fma(p.qs, s, p.q0);
+    const double iq = rcp_fast(qb);
+    const double iq2 = iq * iq;
+    const double g = fma(s, iq2, p.R0sq);
+    const double gs = iq2 * fma(s * p.m2qs, iq, 1.0);
+    const double isg = rsqrt_fast(g);
+    const double sg = g * isg;
+    const double h = iq * isg;
+    const double iR = rcp_fast(R);
+    const double u = p.B0 * iR;
+    const double B = u * sg;
+    const double iB = (R * p.invB0) * isg;
+    const double uq = u * iq;                            // B_Z = uq x, B_R = -uq Z
+    const double bR = -Z * h, bZ = x * h, bphi = p.R0 * isg;
+    const double ug = u * (gs * isg);
+    const double dBdZ = ug * Z;
+    const double dBdR = fma(ug, x, -(B * iR));
+    const double iB2 = iB * iB;
+    const double eB3 = p.eps * (iB2 * iB);               // (m/q) rho_0 B_0 / B^3
+    const double Cd = eB3 * fma(upar, upar, mu * B);
+    const double CE = p.rho0B0 * iB;
+    const double Bphi = u * p.R0;
+    const double xR = Bphi * dBdZ, xZ = -Bphi * dBdR;    // (B x grad B)_R, _Z
+    const double xP = uq * fma(x, dBdR, Z * dBdZ);       // (B x grad B)_phi = B_Z dB/dR - B_R dB/dZ
+    const double R0dot = fma(bR, upar, Cd * xR);         // A.19
+    const double Z0dot = fma(bZ, upar, Cd * xZ);         // A.20
+    const double P0 = fma(bphi, upar, Cd * xP);          // A.21 (times R)
+    const double u0dot = -mu * fma(bR, dBdR, bZ * dBdZ); // A.22 (G29)
+    const double PhP = Phi.fphi * iR;
+    double dRdot, dZdot, dP, dudot, vpar;
+    if (EM) {
+        const double AsP = As.fphi * iR, AhP = Ah.fphi * iR;
+        const double GR = fma(-upar, As.fR + Ah.fR, Phi.fR), GZ = fma(-upar, As.fZ + Ah.fZ, Phi.fZ);
+        const double GP = fma(-upar, AsP + AhP, PhP);
+        const double qA = p.qom * Ah.f;
+        dRdot = fma(CE, fma(bphi, GZ, -bZ * GP), -qA * bR);          // A.24
+        dZdot = fma(CE, fma(-bphi, GR, bR * GP), -qA * bZ);          // A.25
+        dP = fma(CE, fma(bZ, GR, -bR * GZ), -qA * bphi);             // A.26 (times R)
+        const double Cmu = eB3 * (mu * B);
+        const double t2 = fma(bR, Ah.fR, fma(bZ, Ah.fZ, bphi * AhP));
+        dudot = fma(p.qom * upar, t2, -Cmu * fma(xR, As.fR, fma(xZ, As.fZ, xP * AsP)));   // A.29
+        vpar = upar - qA;
+    } else {
+        dRdot = CE * fma(bphi, Phi.fZ, -bZ * PhP);
+        dZdot = CE * fma(-bphi, Phi.fR, bR * PhP);
+        dP = CE * fma(bZ, Phi.fR, -bR * Phi.fZ);
+        dudot = -p.qom * fma(bR, Phi.fR, fma(bZ, Phi.fZ, bphi * PhP));                    // A.28, dA = 0
+        vpar = upar;
+    }
+    const double ir = (s > 1e-300) ? rsqrt_fast(s) : 0.0;
+    const double drdot = fma(dRdot, x, dZdot * Z) * ir;
+    const double en = fma(vpar * vpar, p.invT, fma(mu * B, p.invT2, -1.5));
+    const double L = fma(drdot, -fma(en, p.kappa_T, p.kappa_n),
+                         fma(-(mu * p.invT2), fma(dRdot, dBdR, dZdot * dBdZ), -(vpar * p.invT2) * dudot));
+    Rates o;
+    o.R = R0dot + dRdot;
+    o.Z = Z0dot + dZdot;
+    o.phi = iR * (P0 + dP);
+    o.vpar = u0dot + dudot;
+    o.w = (p.weight_mode == 0) ? (w - 1.0) * L : -L;
+    return o;
+}
+
 __device__ __forceinline__ Rates rhs_point(const PhysDev &p, double R, double Z, double vpar, double mu,
                                            double w, const FieldVal &fld)
 {
+    if (p.eom_variant == 2) return rhs_point_reduced<false>(p, R, Z, vpar, mu, w, fld, fld, fld);
     const double x = R - p.R0;
     const double s = fma(x, x, Z * Z);
     const double qb = fma(p.qs, s, p.q0);

@@ -344,7 +344,7 @@ static void fill_phys(trimeg_ctx *c)
 static int params_ok(const trimeg_params *p)
 {
     return p && p->R0 > 0 && p->a > 0 && p->a < p->R0 && p->B0 != 0 && p->q0 > 0 && p->qs_over_ms != 0 && p->T > 0 &&
-           (p->eom_variant == 0 || p->eom_variant == 1) && (p->weight_mode == 0 || p->weight_mode == 1);
+           (p->eom_variant >= 0 && p->eom_variant <= 2) && (p->weight_mode == 0 || p->weight_mode == 1);
 }
 static int markers_ok(const trimeg_markers *m)
 { return m && m->R && m->Z && m->phi && m->vpar && m->mu && m->w && m->cell; }
