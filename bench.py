@@ -132,7 +132,8 @@ def _strided(m, n_s):
     return {k: np.ascontiguousarray(v[::stride][:n_s]) for k, v in m.items()}, stride
 
 
-def time_oracle(wl, m_np, target_seconds: float, steps: int = 1, warmup: int = 0, one_core_seconds: float = 0.0, n_phi: int = 0):
+def time_oracle(wl, m_np, target_seconds: float, steps: int = 1, warmup: int = 0, one_core_seconds: float = 0.0, n_phi: int = 0,
+                eom_variant: int = 0):
     """Time oracle.push (as it stands, never tuned) the way BASELINE.md §4 / SURVEY.md §8(d) plan it: a STRIDED
     subsample of the workload's seeded marker draw, pushed for the workload's full number of RK4 steps, with OpenMP
     over markers on all host cores -- and, if one_core_seconds > 0, once more on one core with a smaller strided
@@ -140,7 +141,7 @@ def time_oracle(wl, m_np, target_seconds: float, steps: int = 1, warmup: int = 0
     independent, so the rate scales linearly to the full batch.  Returns a dict."""
     import oracle
     from paper_2601_14301_b200 import inputs
-    o = oracle.from_workload(wl, inputs)
+    o = oracle.from_workload(wl, inputs, eom_variant=eom_variant)
     if n_phi:
         o.bell_spline_from_dofs(inputs.spline_dofs(wl, n_phi))
     else:
@@ -185,7 +186,7 @@ def run_reference(args, wl):
         return 0
     m_np = inputs.markers(wl, n=wl.n_markers)
     budget = 150.0 / max(1, args.steps + args.warmup)
-    r = time_oracle(wl, m_np, min(20.0, budget), steps=args.steps, warmup=args.warmup, n_phi=args.n_phi)
+    r = time_oracle(wl, m_np, min(20.0, budget), steps=args.steps, warmup=args.warmup, n_phi=args.n_phi, eom_variant=args.eom_variant)
     line = {
         "impl": "reference", "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": r["seconds_per_step"] * 1e3, "higher_is_better": True,
@@ -202,11 +203,13 @@ def run_reference(args, wl):
     return 0
 
 
-def workload_config(wl, extra=None, n_phi=0):
+def workload_config(wl, extra=None, n_phi=0, eom_variant=0):
     c = {"workload": f"{wl.name} (BASELINE.json configs[{int(wl.name[3:]) - 1}])",
          "mesh": f"{wl.n_r}x{wl.n_theta} rings x sectors, {wl.n_tri} triangles",
          "toroidal_modes": list(wl.modes), "markers_per_gpu": wl.n_markers, "dt": wl.dt,
          "rk4_steps_per_step": wl.nsteps, "l2": "inputs larger than L2 (no flush needed)"}
+    if eom_variant:
+        c["eom_variant"] = {1: "1 (b0* normalised by B/B*par, reading G2)", 2: "2 (reduced equations A.19-A.29, row f4)"}[eom_variant]
     if n_phi:
         c["toroidal_basis"] = f"cubic B-splines on {n_phi} planes (row f3), the mode list's perturbation sampled on the planes"
     if extra:
@@ -220,14 +223,14 @@ class PushRun:
     working copy).  A bench step = restore the batch to the workload's initial state (device copy), compact, then
     [cell sort -> fused push of `sort_every` RK4 steps] until the workload's nsteps are done."""
 
-    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True, n_phi=0):
+    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True, n_phi=0, eom_variant=0):
         import torch
         from paper_2601_14301_b200 import binding, inputs
         self.torch, self.wl = torch, wl
         self.n = wl.n_markers
         self.sort_every = max(1, min(sort_every, wl.nsteps))
-        self.ctx = binding.context_for(wl, inputs)
-        self.n_phi = n_phi
+        self.ctx = binding.context_for(wl, inputs, eom_variant=eom_variant)
+        self.n_phi, self.eom_variant = n_phi, eom_variant
         if n_phi:                                          # row f3: the same perturbation on n_phi B-spline planes
             self.ctx.field_upload_spline(torch.from_numpy(inputs.spline_dofs(wl, n_phi)).cuda(), kind=0)
         else:
@@ -294,7 +297,9 @@ class PushRun:
         return PUSH_KERNEL_NAMES.get(k, "push kernel")
 
     def flops_unit(self):
-        return flops_per_marker_step_spline() if self.n_phi else flops_per_marker_step(len(self.wl.modes))
+        f = flops_per_marker_step_spline() if self.n_phi else flops_per_marker_step(len(self.wl.modes))
+        # reduced equations (row f4): no curl b, no B*_par -- 140 instead of 200 flops per stage outside the gather
+        return f - 4 * 60 if self.eom_variant == 2 else f
 
     def roofline(self, fp64_peak, seconds):
         wl = self.wl
@@ -332,7 +337,7 @@ class PushRun:
         idx = ident.cpu().numpy()
         for k, v in ds.items():
             got[k][idx] = v.cpu().numpy()
-        o = oracle.from_workload(wl, inputs)
+        o = oracle.from_workload(wl, inputs, eom_variant=self.eom_variant)
         if self.n_phi:
             o.bell_spline_from_dofs(inputs.spline_dofs(wl, self.n_phi))
         else:
@@ -444,7 +449,7 @@ def run_gpu(args, wl):
     binding.load()
 
     n = wl.n_markers
-    run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank), n_phi=args.n_phi)
+    run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank), n_phi=args.n_phi, eom_variant=args.eom_variant)
     ctx = run.ctx
     fp64_peak = ctx.measure_fp64_peak()
     fp64_peak3 = ctx.measure_fp64_peak_operands(3)     # DFMA stream with three fresh register operands
@@ -480,7 +485,7 @@ def run_gpu(args, wl):
 
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        r = time_oracle(wl, run.m_np, 15.0, one_core_seconds=6.0, n_phi=args.n_phi)
+        r = time_oracle(wl, run.m_np, 15.0, one_core_seconds=6.0, n_phi=args.n_phi, eom_variant=args.eom_variant)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "nproc": r["nproc"], "kind": "oracle", "sample": r["sample"],
                "value_one_core": r.get("value_one_core"), "sample_one_core": r.get("sample_one_core"),
                "note": "the oracle is the unoptimised correctness checker (plain monomial sums, gcc -O2): a baseline, not a "
@@ -489,7 +494,7 @@ def run_gpu(args, wl):
 
     # ---- the other configs, device-timed the same way (N = 1 only): short runs, same live peaks
     sweep = None
-    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes and not args.n_phi:
+    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes and not args.n_phi and not args.eom_variant:
         sweep = {}
         for name in ("cfg2", "cfg3"):
             w2 = inputs.WORKLOADS[name]
@@ -536,7 +541,7 @@ def run_gpu(args, wl):
             "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": agg["seconds"] / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(wl, n_phi=args.n_phi, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
+            "config": workload_config(wl, n_phi=args.n_phi, eom_variant=args.eom_variant, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
                                                  "lost_markers_per_step": res["lost_per_step"],
                                                  "unit_count": "every bench step restarts from the config's initial state; a marker "
                                                                "that leaves the mesh during a step counts zero steps for it"}),
@@ -763,6 +768,7 @@ def main():
     ap.add_argument("--markers", type=int, default=0, help="override markers per GPU (testing)")
     ap.add_argument("--n-modes", type=int, default=0, help="override the toroidal mode list by n = 0, 2, ..., 2 (K - 1) (schedule selection sweeps)")
     ap.add_argument("--n-phi", type=int, default=0, help="row f3: the field on N cubic B-spline toroidal planes instead of the harmonic mode list")
+    ap.add_argument("--eom-variant", type=int, default=0, choices=[0, 1, 2], help="trimeg_params.eom_variant (2: the reduced equations A.19-A.29, row f4)")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
     ap.add_argument("--min-log2", type=int, default=16, help="cfg4 gather sweep: smallest marker count 2^k")
