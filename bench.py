@@ -399,10 +399,15 @@ def e2e_run(ctx, wl, m_np, k_e2e, device_value, D=None, dev=None):
 
 
 def gather_rows(ctx, wl, log2s, reps, hbm_peak, fp64_peak):
-    """BASELINE.json configs[3]: gather only (dphi, d/dR, d/dZ, no push), markers as drawn and sorted by triangle."""
+    """BASELINE.json configs[3]: gather only (dphi, d/dR, d/dZ, no push), markers as drawn and sorted by triangle.
+    Markers as drawn: every marker reads the coefficient record of a random triangle; the row's `frac_record_gather` is the
+    record bytes per second against the same access pattern without arithmetic (trimeg_measure_gather_peak on a table of
+    the field's size)."""
     import torch
     from paper_2601_14301_b200 import inputs
     flops = flops_per_gather(len(wl.modes))
+    rec_bytes = 16 * 21 * len(wl.modes)
+    gather_peak = ctx.measure_gather_peak(rec_bytes * wl.n_tri, rec_bytes) if rec_bytes else None
     rows = []
     for lg in log2s:
         n = 1 << lg
@@ -430,6 +435,9 @@ def gather_rows(ctx, wl, log2s, reps, hbm_peak, fp64_peak):
             rows.append({"markers": n, "order": name, "gathers_per_s": n / t, "ms": t * 1e3,
                          "algorithmic_GBps": 52.0 * n / t * 1e-9, "frac_hbm": 52.0 * n / t * 1e-9 / hbm_peak,
                          "algorithmic_TFLOPs": flops * n / t * 1e-12, "frac_fp64": flops * n / t * 1e-12 / fp64_peak})
+            if name == "as drawn" and gather_peak:
+                rows[-1].update({"record_GBps": rec_bytes * n / t * 1e-9, "record_gather_peak_GBps": gather_peak,
+                                 "frac_record_gather": rec_bytes * n / t * 1e-9 / gather_peak})
         del R, Z, phi, cell, out
         torch.cuda.empty_cache()
     return rows

@@ -314,6 +314,13 @@ int trimeg_measure_fp64_peak(trimeg_ctx *ctx, double *tflops_out);
  * markers -- runs at 2/3 of trimeg_measure_fp64_peak.  INVALID_ARG outside 1..3. */
 int trimeg_measure_fp64_peak_operands(trimeg_ctx *ctx, int n_reg_operands, double *tflops_out);
 
+/* Denominator for the gather of markers in random order (configs[3] "as drawn"): GB/s of record bytes when every
+ * thread reads a whole record of `record_bytes` (a multiple of 16; e.g. 1008 = 3 modes x 21 complex coefficients), 16
+ * bytes at a time, from a record chosen at random in a zero-filled table of `table_bytes` (33 MB: resident in the 126 MB
+ * L2; 1.4 GB: from HBM), and nothing else -- the access pattern of gather_kernel without its arithmetic.  Best of 4
+ * launches.  Not part of the path.  Allocates and frees the table; synchronises.  Errors: INVALID_ARG, ALLOC, CUDA. */
+int trimeg_measure_gather_peak(trimeg_ctx *ctx, size_t table_bytes, int record_bytes, double *gbs_out);
+
 const char *trimeg_strerror(int code);
 const char *trimeg_version(void);
 

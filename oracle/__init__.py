@@ -36,6 +36,9 @@ def lib():
         ip = C.POINTER(C.c_int32)
         L.orc_create.restype = C.c_void_p
         L.orc_create.argtypes = [C.c_int, C.c_int, dp, dp, dp, C.POINTER(_Params)]
+        L.orc_create_unstructured.restype = C.c_void_p
+        L.orc_create_unstructured.argtypes = [C.c_int, dp, dp, C.c_int, ip, C.c_int, C.c_int, C.POINTER(_Params)]
+        L.orc_box_count.argtypes = [C.c_void_p]
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_n_tri.argtypes = [C.c_void_p]
         L.orc_n_vert.argtypes = [C.c_void_p]
@@ -106,6 +109,31 @@ class Oracle:
         self.n_vert = self.L.orc_n_vert(self.h)
         self.n_modes = 0
         self.mode_n = np.zeros(0, dtype=np.int32)
+
+    @classmethod
+    def unstructured(cls, Rv, Zv, tri, params: Dict, nbx: int = 0, nby: int = 0) -> "Oracle":
+        """O13: any conforming triangulation (vertex coordinates, int32 [n_tri][3]); nbx x nby boxes (default: about one
+        triangle's area per box)."""
+        self = cls.__new__(cls)
+        self.L = lib()
+        self.n_r = self.n_theta = 0
+        self._Rv, self._Zv = _f64(Rv), _f64(Zv)
+        tri = np.ascontiguousarray(tri, dtype=np.int32)
+        if nbx <= 0 or nby <= 0:
+            nbx = nby = max(1, int(np.sqrt(tri.shape[0] / 2.0)))
+        self._p = _Params(**params)
+        self.h = self.L.orc_create_unstructured(self._Rv.size, _d(self._Rv), _d(self._Zv), tri.shape[0], _i(tri), int(nbx), int(nby),
+                                                C.byref(self._p))
+        if not self.h:
+            raise ValueError("orc_create_unstructured failed (degenerate triangle or bad index)")
+        self.n_tri = self.L.orc_n_tri(self.h)
+        self.n_vert = self.L.orc_n_vert(self.h)
+        self.n_modes = 0
+        self.mode_n = np.zeros(0, dtype=np.int32)
+        return self
+
+    def box_entries(self) -> int:
+        return int(self.L.orc_box_count(self.h))
 
     def __del__(self):
         try:

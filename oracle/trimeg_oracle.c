@@ -38,6 +38,7 @@
  *   O10 pullback       u_par, w after the pullback transformation
  *   O11 spline basis   the thesis's own toroidal discretisation: cubic B-splines in phi instead of harmonics
  *                                                           PAPER.md:223, 365-368
+ *   O13 general mesh   unstructured triangulation with the thesis's box-grid locator
  *   O12 reduced model  eom_variant 2: the "dominant terms" equations A.19-A.29 (b* -> b)
  */
 #include <math.h>
@@ -72,6 +73,10 @@ typedef struct {
     double *coef;                  /* [n_tri][n_modes][21][2] (re, im) */
     double **basis;                /* O8: per triangle, lazily, [21][18] monomial coefficients of the 18 basis functions */
     double *coef_aux[2];           /* O9/O10: dA^s (0) and dA^h (1), same layout and mode list as coef; NULL = identically zero */
+    /* O13: unstructured mesh (n_r == 0): box grid of PAPER.md:261-291, 602 in CSR form */
+    int nbx, nby;                  /* boxes in R and Z */
+    double bx0, bz0, bdx, bdz;     /* lower-left corner of the grid, box sizes */
+    int *box_off, *box_tri;        /* [nbx*nby + 1], triangle lists (ascending) */
     int n_phi;                     /* O11: > 0 = the field is Y = sum_j N_j(phi) P_j(xi, eta) on n_phi toroidal planes */
     double *coef_spl;              /* [n_tri][n_phi][21] real monomial coefficients, one quintic per triangle and plane */
 } orc_ctx;
@@ -137,9 +142,117 @@ orc_ctx *orc_create(int n_r, int n_theta, const double *r_nodes,
     return c;
 }
 
+void orc_destroy(orc_ctx *c);
+static int inside(const orc_ctx *c, int t, double R, double Z, double *xi, double *eta, double *lam0);
+static double min3(double a, double b, double c);
+/* ------------------------------------------------- O13 unstructured mesh + box-grid locator */
+/* "An intermediate grid ... of bounding boxes, where each element is itself a vector storing all the triangular elements that
+ * overlap with the corresponding box"; the search discretises the particle position to a box "in O(1) time" and loops over
+ * the box's triangles calling the inside-triangle test until one contains the particle.
+ * Triangles: any conforming triangulation, vertices counter-clockwise (a clockwise triple is turned).  Lists are ascending in
+ * t, so the first hit is the lowest index (reading O3 as on the structured mesh).  A triangle is entered in every box its
+ * bounding box, inflated by 1e-6 of the box size, overlaps.  Reading G31 (no passage fixes what happens on an edge where
+ * rounding fails both neighbours' tests): if no triangle of the box passes, the one with the largest smallest barycentric
+ * coordinate is taken when that coordinate is >= -1e-12, else the marker is outside (-1).  The definition the grid is pinned
+ * against is the same rule over ALL triangles (orc_locate_brute). */
+#define ORC_GAP_TOL 1e-12
+orc_ctx *orc_create_unstructured(int n_vert, const double *Rv, const double *Zv, int n_tri, const int *tri, int nbx, int nby,
+                                 const orc_params *p)
+{
+    if (n_vert < 3 || n_tri < 1 || nbx < 1 || nby < 1) return NULL;
+    orc_ctx *c = (orc_ctx *)calloc(1, sizeof(orc_ctx));
+    c->n_r = 0; c->n_theta = 0; c->n_vert = n_vert; c->n_tri = n_tri; c->p = *p;
+    c->Rv = (double *)malloc(sizeof(double) * n_vert); c->Zv = (double *)malloc(sizeof(double) * n_vert);
+    memcpy(c->Rv, Rv, sizeof(double) * n_vert); memcpy(c->Zv, Zv, sizeof(double) * n_vert);
+    c->tri = (int *)malloc(sizeof(int) * 3 * n_tri);
+    memcpy(c->tri, tri, sizeof(int) * 3 * n_tri);
+    c->geom = (double *)malloc(sizeof(double) * 6 * n_tri);
+    double lo[2] = {INFINITY, INFINITY}, hi[2] = {-INFINITY, -INFINITY};
+    for (int v = 0; v < n_vert; ++v) {
+        if (Rv[v] < lo[0]) lo[0] = Rv[v];
+        if (Rv[v] > hi[0]) hi[0] = Rv[v];
+        if (Zv[v] < lo[1]) lo[1] = Zv[v];
+        if (Zv[v] > hi[1]) hi[1] = Zv[v];
+    }
+    for (int t = 0; t < n_tri; ++t) {
+        int *v = c->tri + 3 * t;
+        for (int q = 0; q < 3; ++q) if (v[q] < 0 || v[q] >= n_vert) { orc_destroy(c); return NULL; }
+        double e1R = Rv[v[1]] - Rv[v[0]], e1Z = Zv[v[1]] - Zv[v[0]], e2R = Rv[v[2]] - Rv[v[0]], e2Z = Zv[v[2]] - Zv[v[0]];
+        double D = e1R * e2Z - e2R * e1Z;
+        if (D == 0.0) { orc_destroy(c); return NULL; }
+        if (D < 0.0) { int tmp = v[1]; v[1] = v[2]; v[2] = tmp; double a = e1R, b = e1Z; e1R = e2R; e1Z = e2Z; e2R = a; e2Z = b; D = -D; }
+        double *g = c->geom + 6 * t;
+        g[0] = Rv[v[0]]; g[1] = Zv[v[0]];
+        g[2] = e2Z / D; g[3] = -e2R / D; g[4] = -e1Z / D; g[5] = e1R / D;
+    }
+    c->nbx = nbx; c->nby = nby;
+    c->bx0 = lo[0]; c->bz0 = lo[1];
+    c->bdx = (hi[0] - lo[0]) / nbx; c->bdz = (hi[1] - lo[1]) / nby;
+    const int nb = nbx * nby;
+    c->box_off = (int *)calloc((size_t)nb + 1, sizeof(int));
+    for (int pass = 0; pass < 2; ++pass) {              /* count, then fill; t ascending keeps every list sorted */
+        int *fill = (pass == 1) ? (int *)calloc((size_t)nb, sizeof(int)) : NULL;
+        for (int t = 0; t < n_tri; ++t) {
+            const int *v = c->tri + 3 * t;
+            double tl[2] = {INFINITY, INFINITY}, th[2] = {-INFINITY, -INFINITY};
+            for (int q = 0; q < 3; ++q) {
+                if (Rv[v[q]] < tl[0]) tl[0] = Rv[v[q]];
+                if (Rv[v[q]] > th[0]) th[0] = Rv[v[q]];
+                if (Zv[v[q]] < tl[1]) tl[1] = Zv[v[q]];
+                if (Zv[v[q]] > th[1]) th[1] = Zv[v[q]];
+            }
+            int i0 = (int)floor((tl[0] - c->bx0) / c->bdx - 1e-6), i1 = (int)floor((th[0] - c->bx0) / c->bdx + 1e-6);
+            int j0 = (int)floor((tl[1] - c->bz0) / c->bdz - 1e-6), j1 = (int)floor((th[1] - c->bz0) / c->bdz + 1e-6);
+            if (i0 < 0) i0 = 0;
+            if (j0 < 0) j0 = 0;
+            if (i1 > nbx - 1) i1 = nbx - 1;
+            if (j1 > nby - 1) j1 = nby - 1;
+            for (int i = i0; i <= i1; ++i)
+                for (int j = j0; j <= j1; ++j) {
+                    const int b = j * nbx + i;
+                    if (pass == 0) c->box_off[b + 1]++;
+                    else c->box_tri[c->box_off[b] + fill[b]++] = t;
+                }
+        }
+        if (pass == 0) {
+            for (int b = 0; b < nb; ++b) c->box_off[b + 1] += c->box_off[b];
+            c->box_tri = (int *)malloc(sizeof(int) * (size_t)(c->box_off[nb] > 0 ? c->box_off[nb] : 1));
+        } else free(fill);
+    }
+    return c;
+}
+/* the rule over an index list (all triangles when list == NULL) */
+static int locate_list(const orc_ctx *c, const int *list, int n, double R, double Z, double *xi_out, double *eta_out)
+{
+    double xi, eta, l0, bm = -INFINITY, bxi = 0.0, bet = 0.0;
+    int best = -1;
+    for (int q = 0; q < n; ++q) {
+        const int t = list ? list[q] : q;
+        if (inside(c, t, R, Z, &xi, &eta, &l0)) { if (xi_out) { *xi_out = xi; *eta_out = eta; } return t; }
+        const double m = min3(xi, eta, l0);
+        if (m > bm) { bm = m; best = t; bxi = xi; bet = eta; }       /* first (lowest t) of equal margins */
+    }
+    if (best >= 0 && bm >= -ORC_GAP_TOL) { if (xi_out) { *xi_out = bxi; *eta_out = bet; } return best; }
+    return -1;
+}
+static int locate_box(const orc_ctx *c, double R, double Z, double *xi_out, double *eta_out)
+{
+    const double fx = floor((R - c->bx0) / c->bdx), fz = floor((Z - c->bz0) / c->bdz);
+    if (!(fx >= -1.0 && fx <= (double)c->nbx && fz >= -1.0 && fz <= (double)c->nby)) return -1;       /* also NaN */
+    int i = (int)fx, j = (int)fz;
+    if (i < 0) i = 0;                                   /* points on (or a rounding beyond) the outer frame */
+    if (i > c->nbx - 1) i = c->nbx - 1;
+    if (j < 0) j = 0;
+    if (j > c->nby - 1) j = c->nby - 1;
+    const int b = j * c->nbx + i;
+    return locate_list(c, c->box_tri + c->box_off[b], c->box_off[b + 1] - c->box_off[b], R, Z, xi_out, eta_out);
+}
+int orc_box_count(const orc_ctx *c) { return c->box_off ? c->box_off[c->nbx * c->nby] : 0; }
+
 void orc_destroy(orc_ctx *c)
 {
     if (!c) return;
+    free(c->box_off); free(c->box_tri);
     free(c->r_nodes); free(c->Rv); free(c->Zv); free(c->tri); free(c->geom);
     if (c->basis) { for (int t = 0; t < c->n_tri; ++t) free(c->basis[t]); free(c->basis); }
     free(c->coef_aux[0]); free(c->coef_aux[1]); free(c->coef_spl);
@@ -308,6 +421,7 @@ static double min3(double a, double b, double c) { double m = a < b ? a : b; ret
 static int locate_brute_one(const orc_ctx *c, double R, double Z)
 {
     double xi, eta, l0;
+    if (c->n_r == 0) return locate_list(c, NULL, c->n_tri, R, Z, NULL, NULL);      /* O13: the rule over all triangles */
     for (int t = 0; t < c->n_tri; ++t)
         if (inside(c, t, R, Z, &xi, &eta, &l0)) return t;
     double x = R - c->Rv[0], z = Z - c->Zv[0];
@@ -353,6 +467,7 @@ static int candidates(const orc_ctx *c, double R, double Z, int *cand)
 }
 static int locate_one(const orc_ctx *c, double R, double Z, double *xi_out, double *eta_out)
 {
+    if (c->n_r == 0) return locate_box(c, R, Z, xi_out, eta_out);                  /* O13 */
     int cand[18];
     int n = candidates(c, R, Z, cand);
     double xi, eta, l0;

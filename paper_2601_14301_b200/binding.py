@@ -20,7 +20,7 @@ EXPORTS = (
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_upload_spline", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
-    "trimeg_measure_fp64_peak", "trimeg_strerror", "trimeg_version",
+    "trimeg_measure_fp64_peak", "trimeg_measure_gather_peak", "trimeg_strerror", "trimeg_version",
 )
 
 OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
@@ -88,6 +88,7 @@ def load() -> C.CDLL:
     L.trimeg_get_push_kernel.argtypes = [vp]
     L.trimeg_measure_fp64_peak.argtypes = [vp, dp]
     L.trimeg_measure_fp64_peak_operands.argtypes = [vp, i32, dp]
+    L.trimeg_measure_gather_peak.argtypes = [vp, sz, i32, dp]
     L.trimeg_strerror.argtypes = [i32]
     L.trimeg_strerror.restype = C.c_char_p
     L.trimeg_version.restype = C.c_char_p
@@ -331,6 +332,12 @@ class Context:
     def measure_fp64_peak(self) -> float:
         v = C.c_double(0.0)
         _check(self.L.trimeg_measure_fp64_peak(self.h, C.byref(v)), "trimeg_measure_fp64_peak")
+        return float(v.value)
+
+    def measure_gather_peak(self, table_bytes: int, record_bytes: int) -> float:
+        v = C.c_double(0.0)
+        _check(self.L.trimeg_measure_gather_peak(self.h, int(table_bytes), int(record_bytes), C.byref(v)),
+               "trimeg_measure_gather_peak")
         return float(v.value)
 
     def measure_fp64_peak_operands(self, n_reg_operands: int) -> float:

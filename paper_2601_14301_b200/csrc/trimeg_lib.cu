@@ -1007,6 +1007,61 @@ int trimeg_measure_fp64_peak_operands(trimeg_ctx *c, int n_reg_operands, double 
     return rc;
 }
 
+// Denominator for the gather of markers as drawn: every thread reads `rec16` consecutive 16-byte words of a record chosen at
+// random in a table of `n_rec` records (what gather_kernel does with one coefficient record per marker), nothing else.
+__global__ void __launch_bounds__(256) gather_peak_kernel(const double2 *__restrict__ table, unsigned n_rec, int rec16, int iters,
+                                                          double *__restrict__ sink)
+{
+    unsigned x = (blockIdx.x * 256u + threadIdx.x) * 2654435761u + 12345u;
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+#pragma unroll 1
+    for (int it = 0; it < iters; ++it) {
+        x ^= x << 13; x ^= x >> 17; x ^= x << 5;         // xorshift32: a fresh record per iteration
+        const double2 *r = table + (size_t)(x % n_rec) * rec16;
+        int k = 0;
+#pragma unroll 1
+        for (; k + 4 <= rec16; k += 4) {
+            const double2 v0 = __ldg(r + k), v1 = __ldg(r + k + 1), v2 = __ldg(r + k + 2), v3 = __ldg(r + k + 3);
+            a0 += v0.x + v0.y; a1 += v1.x + v1.y; a2 += v2.x + v2.y; a3 += v3.x + v3.y;
+        }
+        for (; k < rec16; ++k) { const double2 v = __ldg(r + k); a0 += v.x + v.y; }
+    }
+    if (a0 + a1 + a2 + a3 == 1.2345e-300) sink[0] = a0;
+}
+
+int trimeg_measure_gather_peak(trimeg_ctx *c, size_t table_bytes, int record_bytes, double *gbs_out)
+{
+    if (!c || !gbs_out || record_bytes < 16 || record_bytes % 16 != 0 || table_bytes < (size_t)record_bytes) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
+    const int rec16 = record_bytes / 16;
+    const size_t n_rec = table_bytes / record_bytes;
+    if (n_rec > 0xffffffffull) return TRIMEG_ERR_INVALID_ARG;
+    double2 *table = nullptr;
+    if (cudaMalloc(&table, n_rec * record_bytes + 256) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_ALLOC; }
+    cudaMemset(table, 0, n_rec * record_bytes);
+    double *sink = (double *)(table + n_rec * rec16);
+    const int blocks = c->n_sm * 16, iters = 64;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    double best = 0.0;
+    int rc = TRIMEG_OK;
+    for (int rep = 0; rep < 5; ++rep) {
+        cudaEventRecord(e0, 0);
+        gather_peak_kernel<<<blocks, 256>>>(table, (unsigned)n_rec, rec16, iters, sink);
+        cudaEventRecord(e1, 0);
+        if (cudaEventSynchronize(e1) != cudaSuccess) { cudaGetLastError(); rc = TRIMEG_ERR_CUDA; break; }
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        const double gbs = (double)blocks * 256.0 * iters * record_bytes / (ms * 1e-3) * 1e-9;
+        if (rep > 0 && gbs > best) best = gbs;
+        c->n_launches++;
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(table);
+    *gbs_out = best;
+    return rc;
+}
+
 const char *trimeg_strerror(int code)
 {
     switch (code) {

@@ -218,6 +218,51 @@ def field_dofs(wl: Workload, seed: Optional[int] = None, sigma: float = 1e-3) ->
     return np.ascontiguousarray(dofs)
 
 
+def unstructured_mesh(wl: Workload, seed: Optional[int] = None, jitter: float = 0.25):
+    """Row f4 (general geometry): an unstructured triangulation of the workload's cross-section -- the ring x sector vertices,
+    interior ones displaced at random by up to `jitter` of the local spacing, Delaunay-triangulated (scipy), then vertex
+    numbers, triangle order and the starting vertex of every triangle shuffled, so that nothing of the ring x sector
+    structure is left in the numbering.  The outer ring stays on the circle r = a (the boundary polygon is the structured
+    mesh's).  Returns (Rv, Zv, tri int32 [n_tri][3], counter-clockwise)."""
+    from scipy.spatial import Delaunay
+    rng = np.random.default_rng([wl.seed if seed is None else seed, 7])
+    r_nodes, Rv, Zv = mesh_nodes(wl)
+    Rv, Zv = Rv.copy(), Zv.copy()
+    nth = wl.n_theta
+    for i in range(1, wl.n_r):                                   # interior rings (the axis vertex and the last ring stay)
+        dr = min(r_nodes[i] - r_nodes[i - 1], r_nodes[i + 1] - r_nodes[i])
+        h = jitter * min(dr, 2.0 * np.pi * r_nodes[i] / nth)
+        sl = slice(1 + (i - 1) * nth, 1 + i * nth)
+        Rv[sl] += h * (2.0 * rng.random(nth) - 1.0)
+        Zv[sl] += h * (2.0 * rng.random(nth) - 1.0)
+    tri = Delaunay(np.stack([Rv, Zv], axis=1)).simplices.astype(np.int64)
+    e1R, e1Z = Rv[tri[:, 1]] - Rv[tri[:, 0]], Zv[tri[:, 1]] - Zv[tri[:, 0]]
+    e2R, e2Z = Rv[tri[:, 2]] - Rv[tri[:, 0]], Zv[tri[:, 2]] - Zv[tri[:, 0]]
+    area2 = e1R * e2Z - e2R * e1Z
+    tri = tri[np.abs(area2) > 1e-12 * np.abs(area2).max()]         # slivers between collinear hull points, if any
+    cw = (Rv[tri[:, 1]] - Rv[tri[:, 0]]) * (Zv[tri[:, 2]] - Zv[tri[:, 0]]) - (Rv[tri[:, 2]] - Rv[tri[:, 0]]) * (Zv[tri[:, 1]] - Zv[tri[:, 0]]) < 0
+    tri[cw] = tri[cw][:, [0, 2, 1]]
+    perm_v = rng.permutation(Rv.size)                              # new number of old vertex v is inv[v]
+    inv = np.empty_like(perm_v); inv[perm_v] = np.arange(Rv.size)
+    Rv, Zv = Rv[perm_v], Zv[perm_v]
+    tri = inv[tri]
+    tri = tri[rng.permutation(tri.shape[0])]
+    rot = rng.integers(0, 3, tri.shape[0])
+    tri = np.stack([tri[np.arange(tri.shape[0]), (rot + k) % 3] for k in range(3)], axis=1)
+    return np.ascontiguousarray(Rv), np.ascontiguousarray(Zv), np.ascontiguousarray(tri, dtype=np.int32)
+
+
+def field_dofs_at(wl: Workload, Rv, Zv, seed: Optional[int] = None, sigma: float = 1e-3) -> np.ndarray:
+    """Nodal DOFs [M][n_vert][6] complex128 of the workload's analytic perturbation at arbitrary vertices (row f4)."""
+    amps = mode_amplitudes(wl, seed, sigma)
+    dofs = np.empty((len(wl.modes), Rv.size, 6), dtype=np.complex128)
+    for k, n in enumerate(wl.modes):
+        dofs[k] = analytic_field(wl, amps, n, Rv, Zv)
+    ax = np.hypot(Rv - wl.R0, Zv) < 1e-12
+    dofs[:, ax, :] = 0.0                                           # axis vertex (reading G14)
+    return np.ascontiguousarray(dofs)
+
+
 def spline_dofs(wl: Workload, n_phi: int, seed: Optional[int] = None, sigma: float = 1e-3) -> np.ndarray:
     """Row f3: real nodal DOFs [n_phi][n_vert][6] for the cubic B-spline toroidal basis -- the workload's perturbation
     sum_n Re(Y_n e^{i n phi}) sampled on the n_phi planes phi_j = 2 pi j/n_phi (same radial envelopes, helicity and
