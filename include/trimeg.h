@@ -97,6 +97,20 @@ typedef struct {
 int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_nodes_host,
                        const double *vert_R_host, const double *vert_Z_host,
                        const trimeg_params *params);
+/* Row f4, general geometry: any conforming triangulation of the poloidal cross-section with the thesis's own locator
+ * (section 3.3: an intermediate grid of boxes, each with the list of the triangles that
+ * overlap it; the marker's box is found in O(1), its triangles are tested one by one with the inside-triangle test).
+ *   vert_R_host, vert_Z_host: n_vert vertex coordinates; tri_host: int32 [n_tri][3] vertex numbers (a clockwise triple is
+ *   turned by swapping its second and third vertex); nbx x nby boxes over the bounding rectangle of the vertices (0: about
+ *   one triangle's area per box).  The library builds the geometry table, the neighbour table across the three edges, the
+ *   box lists (ascending triangle numbers, bounding boxes inflated by 1e-6 of a box) and the vertex adjacency.
+ * Locating rule: the lowest-numbered triangle of the box whose test passes (= of all triangles); if none passes, the one
+ * with the largest smallest barycentric coordinate when that is >= -1e-12, else outside (reading G31 of DESIGN.md).
+ * Every other call works as on the ring x sector mesh (the equilibrium stays the analytic one of trimeg_params; markers
+ * outside the triangulation are lost).  Errors: INVALID_ARG, MESH (vertex number out of range, degenerate triangle, an
+ * edge with three owners, non-finite coordinates), CUDA, ALLOC. */
+int trimeg_mesh_create_unstructured(trimeg_ctx **out, int n_vert, const double *vert_R_host, const double *vert_Z_host,
+                                    int n_tri, const int32_t *tri_host, int nbx, int nby, const trimeg_params *params);
 int trimeg_mesh_destroy(trimeg_ctx *ctx);
 int trimeg_mesh_info(const trimeg_ctx *ctx, int *n_vert, int *n_tri);
 int trimeg_set_params(trimeg_ctx *ctx, const trimeg_params *params);

@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtrimeg.so")
 
 EXPORTS = (
-    "trimeg_mesh_create", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
+    "trimeg_mesh_create", "trimeg_mesh_create_unstructured", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_upload_spline", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
@@ -62,6 +62,7 @@ def load() -> C.CDLL:
     vp, sz, dbl, i32 = C.c_void_p, C.c_size_t, C.c_double, C.c_int
     dp = C.POINTER(C.c_double)
     L.trimeg_mesh_create.argtypes = [C.POINTER(vp), i32, i32, dp, dp, dp, C.POINTER(trimeg_params)]
+    L.trimeg_mesh_create_unstructured.argtypes = [C.POINTER(vp), i32, dp, dp, i32, C.POINTER(C.c_int32), i32, i32, C.POINTER(trimeg_params)]
     L.trimeg_mesh_destroy.argtypes = [vp]
     L.trimeg_mesh_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     L.trimeg_set_params.argtypes = [vp, C.POINTER(trimeg_params)]
@@ -159,6 +160,31 @@ class Context:
         self.n_r, self.n_theta, self.n_vert, self.n_tri = int(n_r), int(n_theta), nv.value, nt.value
         self.n_modes = 0
         self.n_phi = 0
+
+    @classmethod
+    def unstructured(cls, vert_R, vert_Z, tri, params: Dict, nbx: int = 0, nby: int = 0) -> "Context":
+        """Row f4: any conforming triangulation (trimeg_mesh_create_unstructured)."""
+        import numpy as np
+        self = cls.__new__(cls)
+        self.L = load()
+        self.h = C.c_void_p(0)
+        vR = np.ascontiguousarray(vert_R, dtype=np.float64)
+        vZ = np.ascontiguousarray(vert_Z, dtype=np.float64)
+        tr = np.ascontiguousarray(tri, dtype=np.int32)
+        if tr.ndim != 2 or tr.shape[1] != 3 or vR.shape != vZ.shape:
+            raise ValueError("tri must be [n_tri][3], vert_R and vert_Z of one length")
+        dp = C.POINTER(C.c_double)
+        p = trimeg_params(**params)
+        rc = self.L.trimeg_mesh_create_unstructured(C.byref(self.h), int(vR.size), vR.ctypes.data_as(dp), vZ.ctypes.data_as(dp),
+                                                    int(tr.shape[0]), tr.ctypes.data_as(C.POINTER(C.c_int32)), int(nbx), int(nby),
+                                                    C.byref(p))
+        _check(rc, "trimeg_mesh_create_unstructured")
+        nv, nt = C.c_int(0), C.c_int(0)
+        _check(self.L.trimeg_mesh_info(self.h, C.byref(nv), C.byref(nt)), "trimeg_mesh_info")
+        self.n_r, self.n_theta, self.n_vert, self.n_tri = 0, 0, nv.value, nt.value
+        self.n_modes = 0
+        self.n_phi = 0
+        return self
 
     def close(self):
         if getattr(self, "h", None) and self.h.value:

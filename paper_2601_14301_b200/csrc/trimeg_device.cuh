@@ -22,7 +22,14 @@ struct MeshDev {
     const double *r_nodes;  // [n_r + 1]
     double Rax, Zax;        // axis vertex
     double rin2;            // squared inscribed radius of the outer polygon (gap rule, O3)
+    // row f4, unstructured triangulation (n_r == 0): neighbour table and the thesis's box grid
+    const int *nbr;         // [n_tri][3] triangle across the edge where barycentric coordinate 0 / 1 / 2 vanishes, -1 = boundary
+    const int *box_off;     // [nbx * nby + 1]
+    const int *box_tri;     // triangles whose (inflated) bounding box overlaps the box, ascending
+    int nbx, nby;
+    double bx0, bz0, inv_bdx, inv_bdz;
 };
+constexpr double LOC_GAP_TOL = 1e-12;   // reading G31
 
 struct FieldDev {
     int n_modes;
@@ -73,6 +80,7 @@ __device__ __forceinline__ Bary bary_rn(const MeshDev &M, int t, double R, doubl
 // ring x sector numbering (O1).
 __device__ __forceinline__ int neighbour(const MeshDev &M, int t, int which)
 {
+    if (M.n_r == 0) return __ldg(M.nbr + 3 * (size_t)t + which);
     const int nth = M.n_theta;
     if (t < nth) {                                   // axis fan, sector j = t
         if (which == 0) return nth + 2 * t + 1;      // outer chord -> ring 1, k = 1
@@ -108,10 +116,39 @@ static __device__ __noinline__ void ring_sector_guess(const MeshDev &M, double R
     j0 = (int)jf;
 }
 
+// Unstructured mesh: the box of the point, its triangles in ascending order, first one whose test passes; if none passes
+// the one with the largest smallest barycentric coordinate when that is >= -LOC_GAP_TOL (reading G31).  Same decisions as
+// the rule over all triangles: every triangle that can pass (or come within the gap tolerance) at a point of the box is
+// in the box's list (bounding boxes inflated by 1e-6 of the box size).
+static __device__ __noinline__ int locate_box(const MeshDev &M, double R, double Z, Bary &out)
+{
+    const double fx = floor((R - M.bx0) * M.inv_bdx), fz = floor((Z - M.bz0) * M.inv_bdz);
+    if (!(fx >= -1.0 && fx <= (double)M.nbx && fz >= -1.0 && fz <= (double)M.nby)) return -1;      // also NaN
+    int i = (int)fx, j = (int)fz;
+    i = max(0, min(M.nbx - 1, i)); j = max(0, min(M.nby - 1, j));
+    const int b = j * M.nbx + i;
+    const int q0 = __ldg(M.box_off + b), q1 = __ldg(M.box_off + b + 1);
+    int gap_best = -1;
+    double gap_m = -INFINITY;
+    Bary gb;
+    gb.xi = gb.eta = gb.l0 = gb.xR = gb.xZ = gb.eR = gb.eZ = 0.0;
+#pragma unroll 1
+    for (int q = q0; q < q1; ++q) {
+        const int t = __ldg(M.box_tri + q);
+        const Bary bb = bary_rn(M, t, R, Z);
+        if (bb.xi >= 0.0 && bb.eta >= 0.0 && bb.l0 >= 0.0) { out = bb; return t; }
+        const double m = fmin(fmin(bb.xi, bb.eta), bb.l0);
+        if (m > gap_m) { gap_m = m; gap_best = t; gb = bb; }
+    }
+    if (gap_best >= 0 && gap_m >= -LOC_GAP_TOL) { out = gb; return gap_best; }
+    return -1;
+}
+
 // The complete rule of reading O3 on the 3x3 cell neighbourhood of the guess: lowest t whose
 // test passes; if none passes, the gap rule.  Same decisions as a brute-force search.
 static __device__ __noinline__ int locate_full(const MeshDev &M, double R, double Z, Bary &out)
 {
+    if (M.n_r == 0) return locate_box(M, R, Z, out);
     int i0, j0;
     ring_sector_guess(M, R, Z, i0, j0);
     int best = -1, gap_best = -1;
@@ -152,6 +189,7 @@ __device__ __forceinline__ int locate(const MeshDev &M, double R, double Z, int 
 {
     int t = hint;
     if (t < 0 || t >= M.n_tri) {
+        if (M.n_r == 0) { moved = 1; return locate_box(M, R, Z, out); }
         int i0, j0;
         ring_sector_guess(M, R, Z, i0, j0);
         if (i0 > M.n_r - 1) i0 = M.n_r - 1;

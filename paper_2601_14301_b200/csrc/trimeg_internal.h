@@ -32,6 +32,7 @@ struct trimeg_ctx {
     trimeg::PhysDev phys;
     // device tables
     double *d_geom, *d_r_nodes, *d_vR, *d_vZ;
+    int *d_tri, *d_nbr, *d_box_off, *d_box_tri;   // row f4, unstructured mesh: vertex triples, neighbours, box grid (NULL on the ring x sector mesh)
     double2 *d_coef;
     double2 *d_coef_aux[2];         // row f2: dA^s, dA^h on the main field's basis and mode list; NULL = identically zero
     double *d_coef_spl;             // row f3: [n_tri][n_phi][21] real, the field on the cubic B-spline toroidal basis (then d_coef == NULL)

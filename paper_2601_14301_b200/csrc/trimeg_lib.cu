@@ -8,6 +8,9 @@
 #include <new>
 
 #include "trimeg_internal.h"
+#include <algorithm>
+#include <unordered_map>
+#include <vector>
 #include "trimeg_mesh.cuh"
 #include "bell_tables.inc"
 
@@ -41,11 +44,11 @@ struct DeviceGuard {
 
 // ============================================================================ a0: mesh tables
 // geometry factors with individually rounded operations (they feed the bit-exact locator)
-__global__ void geom_kernel(int n_r, int n_theta, int n_tri, const double *__restrict__ vR,
+__global__ void geom_kernel(int n_r, int n_theta, const int *__restrict__ tri, int n_tri, const double *__restrict__ vR,
                             const double *__restrict__ vZ, double *__restrict__ geom, double *__restrict__ rin2)
 {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
-    if (t == 0) {
+    if (t == 0 && n_r > 0) {
         const int va = vertex_id(n_theta, n_r, 0), vb = vertex_id(n_theta, n_r, 1);
         const double mx = __dsub_rn(__dmul_rn(0.5, __dadd_rn(vR[va], vR[vb])), vR[0]);
         const double mz = __dsub_rn(__dmul_rn(0.5, __dadd_rn(vZ[va], vZ[vb])), vZ[0]);
@@ -53,7 +56,7 @@ __global__ void geom_kernel(int n_r, int n_theta, int n_tri, const double *__res
     }
     if (t >= n_tri) return;
     int v[3];
-    tri_vertices(n_theta, t, v);
+    tri_vertices(n_theta, tri, t, v);
     const double R0 = vR[v[0]], Z0 = vZ[v[0]];
     const double e1R = __dsub_rn(vR[v[1]], R0), e1Z = __dsub_rn(vZ[v[1]], Z0);
     const double e2R = __dsub_rn(vR[v[2]], R0), e2Z = __dsub_rn(vZ[v[2]], Z0);
@@ -73,14 +76,14 @@ __global__ void geom_kernel(int n_r, int n_theta, int n_tri, const double *__res
 // scaled so that the normal derivative is cubic on every edge (see gen_bell_tables.py).
 // REAL: dofs and coefficients are real (row f3: one "mode" per toroidal plane of the cubic B-spline basis).
 template <bool REAL>
-__global__ void bell_kernel(int n_theta, int n_tri, int n_vert, int n_modes, const double *__restrict__ vR,
+__global__ void bell_kernel(int n_theta, const int *__restrict__ tri, int n_tri, int n_vert, int n_modes, const double *__restrict__ vR,
                             const double *__restrict__ vZ, const void *__restrict__ dofs_v, void *__restrict__ coef_v)
 {
     const size_t idx = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (idx >= (size_t)n_tri * n_modes) return;
     const int t = (int)(idx / n_modes), m = (int)(idx % n_modes);
     int v[3];
-    tri_vertices(n_theta, t, v);
+    tri_vertices(n_theta, tri, t, v);
     const double e1R = vR[v[1]] - vR[v[0]], e1Z = vZ[v[1]] - vZ[v[0]];
     const double e2R = vR[v[2]] - vR[v[0]], e2Z = vZ[v[2]] - vZ[v[0]];
     double dr[18], di[18];
@@ -406,7 +409,7 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
             cudaMemcpy(c->d_vZ, hZ, sizeof(double) * c->n_vert, cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemcpy(c->d_r_nodes, r_nodes_host, sizeof(double) * (n_r + 1), cudaMemcpyHostToDevice) != cudaSuccess ||
             cudaMemset(c->d_stats, 0, sizeof(Stats)) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
-        geom_kernel<<<(c->n_tri + 255) / 256, 256>>>(n_r, n_theta, c->n_tri, c->d_vR, c->d_vZ, c->d_geom, d_rin2);
+        geom_kernel<<<(c->n_tri + 255) / 256, 256>>>(n_r, n_theta, nullptr, c->n_tri, c->d_vR, c->d_vZ, c->d_geom, d_rin2);
         c->n_launches++;
         double rin2 = 0.0;
         if (cudaGetLastError() != cudaSuccess ||
@@ -418,9 +421,9 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
             bool ok = off && adj && fill;
             if (ok) {
                 int v[3];
-                for (int t = 0; t < c->n_tri; ++t) { tri_vertices(n_theta, t, v); for (int k = 0; k < 3; ++k) off[v[k] + 1]++; }
+                for (int t = 0; t < c->n_tri; ++t) { tri_vertices(n_theta, nullptr, t, v); for (int k = 0; k < 3; ++k) off[v[k] + 1]++; }
                 for (int q = 0; q < c->n_vert; ++q) off[q + 1] += off[q];
-                for (int t = 0; t < c->n_tri; ++t) { tri_vertices(n_theta, t, v); for (int k = 0; k < 3; ++k) adj[off[v[k]] + fill[v[k]]++] = 3 * t + k; }
+                for (int t = 0; t < c->n_tri; ++t) { tri_vertices(n_theta, nullptr, t, v); for (int k = 0; k < 3; ++k) adj[off[v[k]] + fill[v[k]]++] = 3 * t + k; }
                 ok = cudaMalloc(&c->d_adj_off, sizeof(int) * ((size_t)c->n_vert + 1)) == cudaSuccess &&
                      cudaMalloc(&c->d_adj, sizeof(int) * ne) == cudaSuccess &&
                      cudaMemcpy(c->d_adj_off, off, sizeof(int) * ((size_t)c->n_vert + 1), cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -449,12 +452,146 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
     return TRIMEG_OK;
 }
 
+int trimeg_mesh_create_unstructured(trimeg_ctx **out, int n_vert, const double *vert_R_host, const double *vert_Z_host, int n_tri,
+                                    const int32_t *tri_host, int nbx, int nby, const trimeg_params *params)
+try {
+    if (!out) return TRIMEG_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (!vert_R_host || !vert_Z_host || !tri_host || n_vert < 3 || n_tri < 1 || n_tri > 0x3fffffff || nbx < 0 || nby < 0 ||
+        (long long)nbx * nby > 0x3fffffffLL || !params_ok(params)) return TRIMEG_ERR_INVALID_ARG;
+    if (nbx == 0 || nby == 0) { nbx = nby = (int)fmax(1.0, floor(sqrt(0.5 * n_tri))); }   // about one triangle's area per box
+    // ---- host tables: triangles turned counter-clockwise, neighbours across the three edges, box grid in CSR form
+    std::vector<int> tri(3 * (size_t)n_tri), nbr(3 * (size_t)n_tri, -1);
+    double lo[2] = {INFINITY, INFINITY}, hi[2] = {-INFINITY, -INFINITY};
+    for (int v = 0; v < n_vert; ++v) {
+        if (!(fabs(vert_R_host[v]) < INFINITY) || !(fabs(vert_Z_host[v]) < INFINITY)) return TRIMEG_ERR_MESH;
+        lo[0] = fmin(lo[0], vert_R_host[v]); hi[0] = fmax(hi[0], vert_R_host[v]);
+        lo[1] = fmin(lo[1], vert_Z_host[v]); hi[1] = fmax(hi[1], vert_Z_host[v]);
+    }
+    if (!(hi[0] > lo[0]) || !(hi[1] > lo[1])) return TRIMEG_ERR_MESH;
+    for (int t = 0; t < n_tri; ++t) {
+        int a = tri_host[3 * (size_t)t], b = tri_host[3 * (size_t)t + 1], d = tri_host[3 * (size_t)t + 2];
+        if (a < 0 || b < 0 || d < 0 || a >= n_vert || b >= n_vert || d >= n_vert) return TRIMEG_ERR_MESH;
+        const double D = (vert_R_host[b] - vert_R_host[a]) * (vert_Z_host[d] - vert_Z_host[a]) -
+                         (vert_R_host[d] - vert_R_host[a]) * (vert_Z_host[b] - vert_Z_host[a]);
+        if (D == 0.0 || D != D) return TRIMEG_ERR_MESH;
+        if (D < 0.0) { const int x = b; b = d; d = x; }
+        tri[3 * (size_t)t] = a; tri[3 * (size_t)t + 1] = b; tri[3 * (size_t)t + 2] = d;
+    }
+    {   // neighbour across the edge opposite to local vertex k (the edge on which barycentric coordinate k vanishes)
+        std::unordered_map<unsigned long long, int> edge;      // (min vertex, max vertex) -> 3 t + k of the first owner
+        edge.reserve(3 * (size_t)n_tri);
+        for (int t = 0; t < n_tri; ++t)
+            for (int k = 0; k < 3; ++k) {
+                const int a = tri[3 * (size_t)t + (k + 1) % 3], b = tri[3 * (size_t)t + (k + 2) % 3];
+                const unsigned long long key = ((unsigned long long)(unsigned)std::min(a, b) << 32) | (unsigned)std::max(a, b);
+                auto it = edge.find(key);
+                if (it == edge.end()) edge.emplace(key, 3 * t + k);
+                else {
+                    if (it->second < 0) return TRIMEG_ERR_MESH;    // an edge with three owners: not a conforming triangulation
+                    nbr[3 * (size_t)t + k] = it->second / 3;
+                    nbr[(size_t)it->second] = t;
+                    it->second = -1;
+                }
+            }
+    }
+    const double bdx = (hi[0] - lo[0]) / nbx, bdz = (hi[1] - lo[1]) / nby;
+    const size_t nb = (size_t)nbx * nby;
+    std::vector<int> box_off(nb + 1, 0), box_tri;
+    for (int pass = 0; pass < 2; ++pass) {
+        std::vector<int> fill(pass ? nb : 0, 0);
+        for (int t = 0; t < n_tri; ++t) {
+            double tl[2] = {INFINITY, INFINITY}, th[2] = {-INFINITY, -INFINITY};
+            for (int k = 0; k < 3; ++k) {
+                const int v = tri[3 * (size_t)t + k];
+                tl[0] = fmin(tl[0], vert_R_host[v]); th[0] = fmax(th[0], vert_R_host[v]);
+                tl[1] = fmin(tl[1], vert_Z_host[v]); th[1] = fmax(th[1], vert_Z_host[v]);
+            }
+            const int i0 = std::max(0, (int)floor((tl[0] - lo[0]) / bdx - 1e-6)), i1 = std::min(nbx - 1, (int)floor((th[0] - lo[0]) / bdx + 1e-6));
+            const int j0 = std::max(0, (int)floor((tl[1] - lo[1]) / bdz - 1e-6)), j1 = std::min(nby - 1, (int)floor((th[1] - lo[1]) / bdz + 1e-6));
+            for (int j = j0; j <= j1; ++j)
+                for (int i = i0; i <= i1; ++i) {
+                    const size_t b = (size_t)j * nbx + i;
+                    if (pass == 0) box_off[b + 1]++;
+                    else box_tri[(size_t)box_off[b] + fill[b]++] = t;
+                }
+        }
+        if (pass == 0) {
+            for (size_t b = 0; b < nb; ++b) {
+                if ((long long)box_off[b + 1] + box_off[b] > 0x7fffffffLL) return TRIMEG_ERR_INVALID_ARG;
+                box_off[b + 1] += box_off[b];
+            }
+            box_tri.resize(std::max<size_t>(1, (size_t)box_off[nb]));
+        }
+    }
+    std::vector<int> adj_off((size_t)n_vert + 1, 0), adj(3 * (size_t)n_tri);
+    {
+        std::vector<int> fill((size_t)n_vert, 0);
+        for (size_t e = 0; e < 3 * (size_t)n_tri; ++e) adj_off[(size_t)tri[e] + 1]++;
+        for (int q = 0; q < n_vert; ++q) adj_off[q + 1] += adj_off[q];
+        for (size_t e = 0; e < 3 * (size_t)n_tri; ++e) adj[(size_t)adj_off[tri[e]] + fill[tri[e]]++] = (int)e;
+    }
+
+    trimeg_ctx *c = new (std::nothrow) trimeg_ctx;
+    if (!c) return TRIMEG_ERR_ALLOC;
+    memset(c, 0, sizeof(*c));
+    if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
+    cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device);
+    c->n_r = 0; c->n_theta = 0; c->n_vert = n_vert; c->n_tri = n_tri;
+    c->params = *params;
+    fill_phys(c);
+    int rc = TRIMEG_OK;
+    do {
+        if (cudaMalloc(&c->d_vR, sizeof(double) * n_vert) != cudaSuccess || cudaMalloc(&c->d_vZ, sizeof(double) * n_vert) != cudaSuccess ||
+            cudaMalloc(&c->d_geom, sizeof(double) * 6 * (size_t)n_tri) != cudaSuccess ||
+            cudaMalloc(&c->d_bins, sizeof(int) * ((size_t)n_tri + 8)) != cudaSuccess ||
+            cudaMalloc(&c->d_stats, sizeof(Stats)) != cudaSuccess ||
+            cudaMalloc(&c->d_tri, sizeof(int) * 3 * (size_t)n_tri) != cudaSuccess ||
+            cudaMalloc(&c->d_nbr, sizeof(int) * 3 * (size_t)n_tri) != cudaSuccess ||
+            cudaMalloc(&c->d_box_off, sizeof(int) * (nb + 1)) != cudaSuccess ||
+            cudaMalloc(&c->d_box_tri, sizeof(int) * box_tri.size()) != cudaSuccess ||
+            cudaMalloc(&c->d_adj_off, sizeof(int) * ((size_t)n_vert + 1)) != cudaSuccess ||
+            cudaMalloc(&c->d_adj, sizeof(int) * 3 * (size_t)n_tri) != cudaSuccess) { rc = TRIMEG_ERR_ALLOC; break; }
+        if (cudaMemcpy(c->d_vR, vert_R_host, sizeof(double) * n_vert, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_vZ, vert_Z_host, sizeof(double) * n_vert, cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_tri, tri.data(), sizeof(int) * tri.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_nbr, nbr.data(), sizeof(int) * nbr.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_box_off, box_off.data(), sizeof(int) * box_off.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_box_tri, box_tri.data(), sizeof(int) * box_tri.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_adj_off, adj_off.data(), sizeof(int) * adj_off.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemcpy(c->d_adj, adj.data(), sizeof(int) * adj.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
+            cudaMemset(c->d_stats, 0, sizeof(Stats)) != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        geom_kernel<<<(n_tri + 255) / 256, 256>>>(0, 0, c->d_tri, n_tri, c->d_vR, c->d_vZ, c->d_geom, nullptr);
+        c->n_launches++;
+        if (cudaGetLastError() != cudaSuccess || cudaDeviceSynchronize() != cudaSuccess) { rc = TRIMEG_ERR_CUDA; break; }
+        c->mesh.n_r = 0; c->mesh.n_theta = 0; c->mesh.n_tri = n_tri;
+        c->mesh.geom = c->d_geom; c->mesh.r_nodes = nullptr;
+        c->mesh.Rax = 0.0; c->mesh.Zax = 0.0; c->mesh.rin2 = 0.0;
+        c->mesh.nbr = c->d_nbr; c->mesh.box_off = c->d_box_off; c->mesh.box_tri = c->d_box_tri;
+        c->mesh.nbx = nbx; c->mesh.nby = nby; c->mesh.bx0 = lo[0]; c->mesh.bz0 = lo[1];
+        c->mesh.inv_bdx = 1.0 / bdx; c->mesh.inv_bdz = 1.0 / bdz;
+        c->field.is_ap = 1;
+        c->push_kernel = TRIMEG_PUSH_KERNEL_AUTO;
+        if (const char *e = getenv("TRIMEG_PUSH_KERNEL")) {
+            char *end = nullptr;
+            const long v = strtol(e, &end, 10);
+            if (end != e && *end == '\0' && v >= TRIMEG_PUSH_KERNEL_AUTO && v <= TRIMEG_PUSH_KERNEL_MAX) c->push_kernel = (int)v;
+        }
+    } while (0);
+    if (rc != TRIMEG_OK) { cudaGetLastError(); trimeg_mesh_destroy(c); return rc; }
+    *out = c;
+    return TRIMEG_OK;
+} catch (...) {                                           // host tables (std::vector) could not be allocated: nothing crosses the C boundary
+    return TRIMEG_ERR_ALLOC;
+}
+
 int trimeg_mesh_destroy(trimeg_ctx *c)
 {
     if (!c) return TRIMEG_ERR_INVALID_ARG;
     DeviceGuard guard__(c->device);
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
     cudaFree(c->d_adj_off); cudaFree(c->d_adj); cudaFree(c->d_trirhs);
+    cudaFree(c->d_tri); cudaFree(c->d_nbr); cudaFree(c->d_box_off); cudaFree(c->d_box_tri);
     cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]); cudaFree(c->d_coef_spl);
     cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
     if (c->hstreams_ready) {
@@ -544,7 +681,7 @@ int trimeg_field_upload(trimeg_ctx *c, int n_modes, const int *mode_n_host, cons
                                    cudaMemcpyDeviceToDevice, s));
         } else {
             const size_t work = (size_t)c->n_tri * n_modes;
-            bell_kernel<false><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR,
+            bell_kernel<false><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->d_tri, c->n_tri, c->n_vert, n_modes, c->d_vR,
                                                                        c->d_vZ, data_dev, c->d_coef);
             c->n_launches++;
             CU_TRY(cudaGetLastError());
@@ -574,7 +711,7 @@ int trimeg_field_upload_aux(trimeg_ctx *c, int which, const void *data_dev, int 
     if (kind == 1) CU_TRY(cudaMemcpyAsync(c->d_coef_aux[a], data_dev, bytes, cudaMemcpyDeviceToDevice, s));
     else {
         const size_t work = (size_t)c->n_tri * n_modes;
-        bell_kernel<false><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_modes, c->d_vR, c->d_vZ,
+        bell_kernel<false><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->d_tri, c->n_tri, c->n_vert, n_modes, c->d_vR, c->d_vZ,
                                                                    data_dev, c->d_coef_aux[a]);
         c->n_launches++;
         CU_TRY(cudaGetLastError());
@@ -601,7 +738,7 @@ int trimeg_field_upload_spline(trimeg_ctx *c, int n_phi, const double *data_dev,
     if (kind == 1) CU_TRY(cudaMemcpyAsync(c->d_coef_spl, data_dev, bytes, cudaMemcpyDeviceToDevice, s));
     else {
         const size_t work = (size_t)c->n_tri * n_phi;
-        bell_kernel<true><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->n_tri, c->n_vert, n_phi, c->d_vR, c->d_vZ,
+        bell_kernel<true><<<(unsigned)((work + 127) / 128), 128, 0, s>>>(c->n_theta, c->d_tri, c->n_tri, c->n_vert, n_phi, c->d_vR, c->d_vZ,
                                                                          data_dev, c->d_coef_spl);
         c->n_launches++;
         CU_TRY(cudaGetLastError());

@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(256) scatter_index_kernel(size_t n, const int3
 }
 
 // (1) + (2): one CTA per triangle.  tri_rhs [n_tri][n_modes][18] complex.
-__global__ void __launch_bounds__(SC_THREADS) scatter_moments_kernel(MeshDev M, FieldDev F, int n_theta, const double *__restrict__ vR,
+__global__ void __launch_bounds__(SC_THREADS) scatter_moments_kernel(MeshDev M, FieldDev F, int n_theta, const int *__restrict__ tri, const double *__restrict__ vR,
                                                                      const double *__restrict__ vZ, const double *__restrict__ R,
                                                                      const double *__restrict__ Z, const double *__restrict__ phi,
                                                                      const double *__restrict__ w, const int32_t *__restrict__ perm,
@@ -88,7 +88,7 @@ __global__ void __launch_bounds__(SC_THREADS) scatter_moments_kernel(MeshDev M, 
     const double2 v0 = __ldg(g), gx = __ldg(g + 1), ge = __ldg(g + 2);
     // edge vectors of the triangle (for the transposed map from reference derivatives to (R, Z) derivatives)
     int vtx[3];
-    tri_vertices(n_theta, t, vtx);
+    tri_vertices(n_theta, tri, t, vtx);
     const double e1R = vR[vtx[1]] - vR[vtx[0]], e1Z = vZ[vtx[1]] - vZ[vtx[0]];
     const double e2R = vR[vtx[2]] - vR[vtx[0]], e2Z = vZ[vtx[2]] - vZ[vtx[0]];
 
@@ -265,7 +265,7 @@ cudaError_t launch_scatter(trimeg_ctx *c, const trimeg_markers &m, size_t n, dou
         scatter_index_kernel<<<grid, 256, 0, s>>>(n, cell, c->n_tri, c->d_bins, perm);
         c->n_launches += 4;
     }
-    scatter_moments_kernel<<<c->n_tri, SC_THREADS, 0, s>>>(c->mesh, c->field, c->n_theta, c->d_vR, c->d_vZ, m.R, m.Z, m.phi, m.w,
+    scatter_moments_kernel<<<c->n_tri, SC_THREADS, 0, s>>>(c->mesh, c->field, c->n_theta, c->d_tri, c->d_vR, c->d_vZ, m.R, m.Z, m.phi, m.w,
                                                           perm, c->d_bins, tri_rhs);
     const size_t work = (size_t)n_modes * c->n_vert * 6;
     scatter_assemble_kernel<<<(unsigned)((work + 255) / 256), 256, 0, s>>>(c->n_vert, n_modes, c->d_adj_off, c->d_adj, tri_rhs, rhs);
