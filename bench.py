@@ -203,11 +203,13 @@ def run_reference(args, wl):
     return 0
 
 
-def workload_config(wl, extra=None, n_phi=0, eom_variant=0):
+def workload_config(wl, extra=None, n_phi=0, eom_variant=0, unstructured=False):
     c = {"workload": f"{wl.name} (BASELINE.json configs[{int(wl.name[3:]) - 1}])",
          "mesh": f"{wl.n_r}x{wl.n_theta} rings x sectors, {wl.n_tri} triangles",
          "toroidal_modes": list(wl.modes), "markers_per_gpu": wl.n_markers, "dt": wl.dt,
          "rk4_steps_per_step": wl.nsteps, "l2": "inputs larger than L2 (no flush needed)"}
+    if unstructured:
+        c["mesh"] = f"unstructured: the {wl.n_r}x{wl.n_theta} ring x sector vertices jittered, Delaunay, numbering shuffled; {wl.n_tri} triangles; box-grid locator (row f4)"
     if eom_variant:
         c["eom_variant"] = {1: "1 (b0* normalised by B/B*par, reading G2)", 2: "2 (reduced equations A.19-A.29, row f4)"}[eom_variant]
     if n_phi:
@@ -223,18 +225,23 @@ class PushRun:
     working copy).  A bench step = restore the batch to the workload's initial state (device copy), compact, then
     [cell sort -> fused push of `sort_every` RK4 steps] until the workload's nsteps are done."""
 
-    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True, n_phi=0, eom_variant=0):
+    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True, n_phi=0, eom_variant=0, unstructured=False):
         import torch
         from paper_2601_14301_b200 import binding, inputs
         self.torch, self.wl = torch, wl
         self.n = wl.n_markers
         self.sort_every = max(1, min(sort_every, wl.nsteps))
-        self.ctx = binding.context_for(wl, inputs, eom_variant=eom_variant)
-        self.n_phi, self.eom_variant = n_phi, eom_variant
-        if n_phi:                                          # row f3: the same perturbation on n_phi B-spline planes
-            self.ctx.field_upload_spline(torch.from_numpy(inputs.spline_dofs(wl, n_phi)).cuda(), kind=0)
+        self.n_phi, self.eom_variant, self.umesh = n_phi, eom_variant, None
+        if unstructured:                                   # row f4: the same cross-section as an unstructured triangulation, box-grid locator
+            self.umesh = inputs.unstructured_mesh(wl)
+            self.ctx = binding.Context.unstructured(*self.umesh, wl.params(eom_variant, 0))
+            self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs_at(wl, self.umesh[0], self.umesh[1])).cuda(), kind=0)
         else:
-            self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
+            self.ctx = binding.context_for(wl, inputs, eom_variant=eom_variant)
+            if n_phi:                                      # row f3: the same perturbation on n_phi B-spline planes
+                self.ctx.field_upload_spline(torch.from_numpy(inputs.spline_dofs(wl, n_phi)).cuda(), kind=0)
+            else:
+                self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
         if push_kernel >= 0:
             self.ctx.set_push_kernel(push_kernel)
         m_np = inputs.markers(wl, n=self.n, seed=seed)
@@ -337,11 +344,15 @@ class PushRun:
         idx = ident.cpu().numpy()
         for k, v in ds.items():
             got[k][idx] = v.cpu().numpy()
-        o = oracle.from_workload(wl, inputs, eom_variant=self.eom_variant)
-        if self.n_phi:
-            o.bell_spline_from_dofs(inputs.spline_dofs(wl, self.n_phi))
+        if self.umesh is not None:
+            o = oracle.Oracle.unstructured(*self.umesh, wl.params(self.eom_variant, 0))
+            o.bell_from_dofs(wl.modes, inputs.field_dofs_at(wl, self.umesh[0], self.umesh[1]))
         else:
-            o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
+            o = oracle.from_workload(wl, inputs, eom_variant=self.eom_variant)
+            if self.n_phi:
+                o.bell_spline_from_dofs(inputs.spline_dofs(wl, self.n_phi))
+            else:
+                o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
         want = o.push(sample, wl.dt, wl.nsteps)
         assert np.array_equal(got["cell"] < 0, want["cell"] < 0), "lost-marker sets differ"
         worst = 0.0
@@ -457,7 +468,8 @@ def run_gpu(args, wl):
     binding.load()
 
     n = wl.n_markers
-    run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank), n_phi=args.n_phi, eom_variant=args.eom_variant)
+    run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank), n_phi=args.n_phi, eom_variant=args.eom_variant,
+                  unstructured=args.unstructured)
     ctx = run.ctx
     fp64_peak = ctx.measure_fp64_peak()
     fp64_peak3 = ctx.measure_fp64_peak_operands(3)     # DFMA stream with three fresh register operands
@@ -492,7 +504,7 @@ def run_gpu(args, wl):
         e2e = e2e_run(ctx, wl, run.m_np, max(1, min(args.steps, 3)), agg["value"], D, dev)
 
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.unstructured:
         r = time_oracle(wl, run.m_np, 15.0, one_core_seconds=6.0, n_phi=args.n_phi, eom_variant=args.eom_variant)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "nproc": r["nproc"], "kind": "oracle", "sample": r["sample"],
                "value_one_core": r.get("value_one_core"), "sample_one_core": r.get("sample_one_core"),
@@ -502,7 +514,7 @@ def run_gpu(args, wl):
 
     # ---- the other configs, device-timed the same way (N = 1 only): short runs, same live peaks
     sweep = None
-    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes and not args.n_phi and not args.eom_variant:
+    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes and not args.n_phi and not args.eom_variant and not args.unstructured:
         sweep = {}
         for name in ("cfg2", "cfg3"):
             w2 = inputs.WORKLOADS[name]
@@ -549,7 +561,7 @@ def run_gpu(args, wl):
             "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": agg["seconds"] / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(wl, n_phi=args.n_phi, eom_variant=args.eom_variant, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
+            "config": workload_config(wl, n_phi=args.n_phi, eom_variant=args.eom_variant, unstructured=args.unstructured, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
                                                  "lost_markers_per_step": res["lost_per_step"],
                                                  "unit_count": "every bench step restarts from the config's initial state; a marker "
                                                                "that leaves the mesh during a step counts zero steps for it"}),
@@ -777,6 +789,7 @@ def main():
     ap.add_argument("--n-modes", type=int, default=0, help="override the toroidal mode list by n = 0, 2, ..., 2 (K - 1) (schedule selection sweeps)")
     ap.add_argument("--n-phi", type=int, default=0, help="row f3: the field on N cubic B-spline toroidal planes instead of the harmonic mode list")
     ap.add_argument("--eom-variant", type=int, default=0, choices=[0, 1, 2], help="trimeg_params.eom_variant (2: the reduced equations A.19-A.29, row f4)")
+    ap.add_argument("--unstructured", action="store_true", help="row f4: the workload's cross-section as an unstructured triangulation (jittered Delaunay, shuffled numbering) with the box-grid locator")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
     ap.add_argument("--min-log2", type=int, default=16, help="cfg4 gather sweep: smallest marker count 2^k")

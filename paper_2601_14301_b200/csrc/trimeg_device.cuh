@@ -30,6 +30,18 @@ struct MeshDev {
     double bx0, bz0, inv_bdx, inv_bdz;
 };
 constexpr double LOC_GAP_TOL = 1e-12;   // reading G31
+// A translation unit compiled with TRIMEG_CORE_ONLY (trimeg_push_*_core.cu) holds the hot kernels for the core case alone --
+// ring x sector mesh, harmonic field, rigorous equations -- without the branches of rows f3 / f4 (they cost 0.9 % of the push
+// although never taken: code size and register allocation); the launchers pick it when the context is in that case.
+#ifdef TRIMEG_CORE_ONLY
+#define TRIMEG_HAS_SPL(F) false
+#define TRIMEG_IS_REDUCED(p) false
+#define TRIMEG_IS_UNS(M) false
+#else
+#define TRIMEG_HAS_SPL(F) ((F).n_phi > 0)
+#define TRIMEG_IS_REDUCED(p) ((p).eom_variant == 2)
+#define TRIMEG_IS_UNS(M) ((M).n_r == 0)
+#endif
 
 struct FieldDev {
     int n_modes;
@@ -80,7 +92,7 @@ __device__ __forceinline__ Bary bary_rn(const MeshDev &M, int t, double R, doubl
 // ring x sector numbering (O1).
 __device__ __forceinline__ int neighbour(const MeshDev &M, int t, int which)
 {
-    if (M.n_r == 0) return __ldg(M.nbr + 3 * (size_t)t + which);
+    if (TRIMEG_IS_UNS(M)) return __ldg(M.nbr + 3 * (size_t)t + which);
     const int nth = M.n_theta;
     if (t < nth) {                                   // axis fan, sector j = t
         if (which == 0) return nth + 2 * t + 1;      // outer chord -> ring 1, k = 1
@@ -148,7 +160,7 @@ static __device__ __noinline__ int locate_box(const MeshDev &M, double R, double
 // test passes; if none passes, the gap rule.  Same decisions as a brute-force search.
 static __device__ __noinline__ int locate_full(const MeshDev &M, double R, double Z, Bary &out)
 {
-    if (M.n_r == 0) return locate_box(M, R, Z, out);
+    if (TRIMEG_IS_UNS(M)) return locate_box(M, R, Z, out);
     int i0, j0;
     ring_sector_guess(M, R, Z, i0, j0);
     int best = -1, gap_best = -1;
@@ -189,7 +201,7 @@ __device__ __forceinline__ int locate(const MeshDev &M, double R, double Z, int 
 {
     int t = hint;
     if (t < 0 || t >= M.n_tri) {
-        if (M.n_r == 0) { moved = 1; return locate_box(M, R, Z, out); }
+        if (TRIMEG_IS_UNS(M)) { moved = 1; return locate_full(M, R, Z, out); }
         int i0, j0;
         ring_sector_guess(M, R, Z, i0, j0);
         if (i0 > M.n_r - 1) i0 = M.n_r - 1;
@@ -313,7 +325,7 @@ struct FieldVal { double f, fR, fZ, fphi; };   // dphi, d/dR, d/dZ, d/dphi
 __device__ __forceinline__ FieldVal gather(const FieldDev &F, int t, const Bary &b, double phi)
 {
     double f = 0.0, fx = 0.0, fe = 0.0, fp = 0.0;
-    if (F.n_phi > 0) {
+    if (TRIMEG_HAS_SPL(F)) {
         const SplineW s = spline_weights(F.n_phi, F.inv_h, phi);
         const double *base = F.spl + (size_t)t * F.n_phi * NCOEF;
         int j = (s.j0 == 0) ? F.n_phi - 1 : s.j0 - 1;
@@ -466,7 +478,7 @@ __device__ __forceinline__ Rates rhs_point_reduced(const PhysDev &p, double R, d
 __device__ __forceinline__ Rates rhs_point(const PhysDev &p, double R, double Z, double vpar, double mu,
                                            double w, const FieldVal &fld)
 {
-    if (p.eom_variant == 2) return rhs_point_reduced<false>(p, R, Z, vpar, mu, w, fld, fld, fld);
+    if (TRIMEG_IS_REDUCED(p)) return rhs_point_reduced<false>(p, R, Z, vpar, mu, w, fld, fld, fld);
     const double x = R - p.R0;
     const double s = fma(x, x, Z * Z);
     const double qb = fma(p.qs, s, p.q0);

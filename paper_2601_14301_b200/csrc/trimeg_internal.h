@@ -104,6 +104,11 @@ cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n,
 // (TRIMEG_PUSH_KERNEL_LANE)
 cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 
+// trimeg_push_*_core.cu: the same two kernels compiled without the branches of rows f3 / f4
+cudaError_t launch_push_wcache_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
+cudaError_t launch_push_lane_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
+inline bool core_case(const trimeg_ctx *c) { return c->field.n_phi == 0 && c->params.eom_variant != 2 && c->mesh.n_r > 0; }
+
 // trimeg_push_lane.cu: the gather alone for cell-sorted markers; gate / want: runs iff (*gate * 16 <= n) == want
 cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const int32_t *hint,
                                double *f, double *fR, double *fZ, double *fP, const int *gate, int want, cudaStream_t s);

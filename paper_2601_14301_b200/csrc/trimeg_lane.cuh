@@ -199,16 +199,24 @@ __device__ __forceinline__ void gather_lane_spline(const FieldDev &F, const doub
 }
 
 // length of a triangle's record in 16-byte units, and where it starts in the global table (harmonic or B-spline field)
-__device__ __host__ __forceinline__ int lane_rec_len(const FieldDev &F) { return F.n_phi > 0 ? F.n_phi * NCOEF / 2 : F.n_modes * NCOEF; }
+__device__ __host__ __forceinline__ int lane_rec_len(const FieldDev &F) { return TRIMEG_HAS_SPL(F) ? F.n_phi * NCOEF / 2 : F.n_modes * NCOEF; }
 __device__ __forceinline__ const double2 *lane_rec_src(const FieldDev &F, int t)
 {
-    return F.n_phi > 0 ? reinterpret_cast<const double2 *>(F.spl + (size_t)t * F.n_phi * NCOEF) : F.coef + (size_t)t * F.n_modes * NCOEF;
+    return TRIMEG_HAS_SPL(F) ? reinterpret_cast<const double2 *>(F.spl + (size_t)t * F.n_phi * NCOEF) : F.coef + (size_t)t * F.n_modes * NCOEF;
+}
+
+// harmonic field only (the gather-alone kernel is never launched on a B-spline field)
+__device__ __forceinline__ void gather_lane_harmonic(const FieldDev &F, const double2 *c, double xi, double eta, double phi, int zero,
+                                                     double &f, double &fx, double &fe, double &fp)
+{
+    if (F.is_ap) gather_lane_impl<true>(F, c, xi, eta, phi, zero, f, fx, fe, fp);
+    else gather_lane_impl<false>(F, c, xi, eta, phi, zero, f, fx, fe, fp);
 }
 
 __device__ __forceinline__ void gather_lane(const FieldDev &F, const double2 *c, double xi, double eta, double phi, int zero,
                                             double &f, double &fx, double &fe, double &fp)
 {
-    if (F.n_phi > 0) { gather_lane_spline(F, reinterpret_cast<const double *>(c), xi, eta, phi, zero, f, fx, fe, fp); return; }
+    if (TRIMEG_HAS_SPL(F)) { gather_lane_spline(F, reinterpret_cast<const double *>(c), xi, eta, phi, zero, f, fx, fe, fp); return; }
     if (F.is_ap) gather_lane_impl<true>(F, c, xi, eta, phi, zero, f, fx, fe, fp);
     else gather_lane_impl<false>(F, c, xi, eta, phi, zero, f, fx, fe, fp);
 }

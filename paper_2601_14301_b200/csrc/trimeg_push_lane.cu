@@ -116,7 +116,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
 
     const size_t base = ((size_t)blockIdx.x * WARPS + wib) * NW;
     const int nt = (base >= n) ? 0 : (int)((n - base < (size_t)NW) ? (n - base) : (size_t)NW);   // empty warps stay for the barriers
-    const bool has_field = F.n_modes > 0 || F.n_phi > 0;
+    const bool has_field = F.n_modes > 0 || TRIMEG_HAS_SPL(F);
     const double hdt = 0.5 * dt, dt6 = dt / 6.0;
     TRIMEG_PHASE_CLOCK_INIT                                          // lane 0: record lookups, evaluation + finish, (unused)
     unsigned n_fallback = 0, n_copied = 0, n_stages = 0, n_regroup = 0;
@@ -153,14 +153,14 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_lane_kernel(MeshDev M, Fie
             }
         }
         ldc[p] = c; ldf[p] = fl;
-        if (F.n_phi > 0) {
+        if (TRIMEG_HAS_SPL(F)) {
             unsigned key = 0xffffffffu;
             if (fl & FL_ACTIVE) key = (((unsigned)c << 6) | (unsigned)spline_weights(F.n_phi, F.inv_h, ldP[p]).j0) & 0x7fffffffu;
             skey[q] = key;
         }
     }
     int slot[2] = {lane, lane + 32};
-    if (F.n_phi > 0) {
+    if (TRIMEG_HAS_SPL(F)) {
         __syncwarp();
 #pragma unroll
         for (int p = 0; p < 2; ++p) {
@@ -402,7 +402,7 @@ __global__ void __launch_bounds__(32 * GL_WARPS, 1) gather_lane_kernel(MeshDev M
                 if (t >= 0) {
                     if (rec >= 0) {
                         double fx, fe;
-                        gather_lane(F, REC + (size_t)rec * rec_stride, b.xi, b.eta, ph, zero, v, fx, fe, vP);
+                        gather_lane_harmonic(F, REC + (size_t)rec * rec_stride, b.xi, b.eta, ph, zero, v, fx, fe, vP);
                         vR = fma(b.xR, fx, b.eR * fe);
                         vZ = fma(b.xZ, fx, b.eZ * fe);
                     } else {
@@ -447,6 +447,7 @@ cudaError_t launch_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 
 }  // namespace
 
+#ifndef TRIMEG_CORE_ONLY
 cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const int32_t *hint,
                                double *f, double *fR, double *fZ, double *fP, const int *gate, int want, cudaStream_t s)
 {
@@ -468,14 +469,21 @@ cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const d
     return cudaGetLastError();
 }
 
+#endif
+
+#ifdef TRIMEG_CORE_ONLY
+cudaError_t launch_push_lane_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
+#else
 cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
+#endif
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
 #ifndef TRIMEG_SPLINE_LANE_WARPS
 #define TRIMEG_SPLINE_LANE_WARPS 16
 #endif
-    // B-spline plane records are long (n_phi x 168 bytes): fewer warps leave room for more of them per marker
+#ifndef TRIMEG_CORE_ONLY
     if (c->field.n_phi > 0) return launch_lane<TRIMEG_SPLINE_LANE_WARPS>(c, m, n, dt, nsteps, s);
+#endif
     return launch_lane<16>(c, m, n, dt, nsteps, s);      // 16 warps at 128 registers (12 at 168 lose 8 % with 3 modes, 1 % with 16)
 }
 

@@ -379,7 +379,11 @@ cudaError_t launch_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, doub
 
 }  // namespace
 
+#ifdef TRIMEG_CORE_ONLY
+cudaError_t launch_push_wcache_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
+#else
 cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
+#endif
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     return launch_wcache<2, 12, 5>(c, m, n, dt, nsteps, s);
