@@ -209,7 +209,9 @@ def workload_config(wl, extra=None, n_phi=0, eom_variant=0, unstructured=False):
          "toroidal_modes": list(wl.modes), "markers_per_gpu": wl.n_markers, "dt": wl.dt,
          "rk4_steps_per_step": wl.nsteps, "l2": "inputs larger than L2 (no flush needed)"}
     if unstructured:
-        c["mesh"] = f"unstructured: the {wl.n_r}x{wl.n_theta} ring x sector vertices jittered, Delaunay, numbering shuffled; {wl.n_tri} triangles; box-grid locator (row f4)"
+        c["mesh"] = (f"unstructured: the {wl.n_r}x{wl.n_theta} ring x sector vertices jittered, Delaunay, numbering shuffled"
+                     + ("" if unstructured == "shuffled" else ", triangles renumbered along a Hilbert curve (trimeg_mesh_locality_order)")
+                     + f"; {wl.n_tri} triangles; box-grid locator (row f4)")
     if eom_variant:
         c["eom_variant"] = {1: "1 (b0* normalised by B/B*par, reading G2)", 2: "2 (reduced equations A.19-A.29, row f4)"}[eom_variant]
     if n_phi:
@@ -233,7 +235,10 @@ class PushRun:
         self.sort_every = max(1, min(sort_every, wl.nsteps))
         self.n_phi, self.eom_variant, self.umesh = n_phi, eom_variant, None
         if unstructured:                                   # row f4: the same cross-section as an unstructured triangulation, box-grid locator
-            self.umesh = inputs.unstructured_mesh(wl)
+            Rv, Zv, tri = inputs.unstructured_mesh(wl)
+            if unstructured != "shuffled":                 # the caller's one-off renumbering along a Hilbert curve (include/trimeg.h)
+                tri = np.ascontiguousarray(tri[binding.mesh_locality_order(Rv, Zv, tri)])
+            self.umesh = (Rv, Zv, tri)
             self.ctx = binding.Context.unstructured(*self.umesh, wl.params(eom_variant, 0))
             self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs_at(wl, self.umesh[0], self.umesh[1])).cuda(), kind=0)
         else:
@@ -553,6 +558,19 @@ def run_gpu(args, wl):
                                 "config": workload_config(r3.wl, n_phi=32, extra={"sort_every": r3.sort_every}), "oracle_check": chk}
         r3.close()
         del r3
+        # row f4: cfg5's cross-section as an unstructured triangulation (Hilbert-renumbered), box-grid locator
+        r4 = PushRun(inputs.WORKLOADS["cfg5"], args.sort_every, -1, keep_host=True, unstructured="hilbert")
+        out = r4.run(2, 3)
+        rf = r4.roofline(fp64_peak, out["seconds"])
+        chk = None if args.no_check else r4.check_against_oracle(stride=max(1, r4.wl.n_markers // 2048))
+        sweep["unstructured_cfg5"] = {"value": out["units"] / out["seconds"], "unit": UNIT, "steps": 2, "warmup": 3,
+                                      "ms_per_step": out["seconds"] / 2 * 1e3, "kernel": rf["kernel"], "frac": rf["frac"],
+                                      "achieved_tflops": rf["achieved"], "avg_launch_ms": rf["avg_launch_ms"],
+                                      "push_share_of_step": rf["push_share_of_step"], "clocks": out["clocks"],
+                                      "config": workload_config(r4.wl, unstructured="hilbert", extra={"sort_every": r4.sort_every}),
+                                      "oracle_check": chk}
+        r4.close()
+        del r4
         sweep["em_cfg5"] = em_run(inputs.WORKLOADS["cfg5"], 3, fp64_peak, hbm_peak, with_oracle=not args.no_check)
         sweep["scatter_cfg5"] = scatter_run(inputs.WORKLOADS["cfg5"], 3, fp64_peak, hbm_peak, with_oracle=not args.no_check)
 
@@ -789,7 +807,9 @@ def main():
     ap.add_argument("--n-modes", type=int, default=0, help="override the toroidal mode list by n = 0, 2, ..., 2 (K - 1) (schedule selection sweeps)")
     ap.add_argument("--n-phi", type=int, default=0, help="row f3: the field on N cubic B-spline toroidal planes instead of the harmonic mode list")
     ap.add_argument("--eom-variant", type=int, default=0, choices=[0, 1, 2], help="trimeg_params.eom_variant (2: the reduced equations A.19-A.29, row f4)")
-    ap.add_argument("--unstructured", action="store_true", help="row f4: the workload's cross-section as an unstructured triangulation (jittered Delaunay, shuffled numbering) with the box-grid locator")
+    ap.add_argument("--unstructured", nargs="?", const="hilbert", default=None, choices=["hilbert", "shuffled"],
+                    help="row f4: the workload's cross-section as an unstructured triangulation (jittered Delaunay, shuffled numbering) with "
+                         "the box-grid locator; 'hilbert' (default): triangles renumbered by trimeg_mesh_locality_order first, 'shuffled': as generated")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
     ap.add_argument("--min-log2", type=int, default=16, help="cfg4 gather sweep: smallest marker count 2^k")

@@ -111,6 +111,15 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
  * edge with three owners, non-finite coordinates), CUDA, ALLOC. */
 int trimeg_mesh_create_unstructured(trimeg_ctx **out, int n_vert, const double *vert_R_host, const double *vert_Z_host,
                                     int n_tri, const int32_t *tri_host, int nbx, int nby, const trimeg_params *params);
+/* Host utility for unstructured meshes (no device work): order_host[q] = the triangle that should get number q so that
+ * triangles close in space are close in number -- Hilbert curve over the bounding rectangle, by centroid.  The push keeps the
+ * coefficient records of the triangles a CTA's cell-sorted markers sit in in shared memory; when the neighbours of consecutive
+ * triangles are unrelated (a shuffled or advancing-front numbering) the CTA meets far more records than it can hold.  Apply
+ * the order to the triangle list (tri_new[q] = tri[order[q]]) BEFORE trimeg_mesh_create_unstructured and use the new numbers
+ * everywhere; the library never renumbers behind the caller's back (cell numbers are the caller's).
+ * Errors: INVALID_ARG, MESH (vertex number out of range, degenerate bounding rectangle), ALLOC. */
+int trimeg_mesh_locality_order(int n_vert, const double *vert_R_host, const double *vert_Z_host, int n_tri,
+                               const int32_t *tri_host, int32_t *order_host);
 int trimeg_mesh_destroy(trimeg_ctx *ctx);
 int trimeg_mesh_info(const trimeg_ctx *ctx, int *n_vert, int *n_tri);
 int trimeg_set_params(trimeg_ctx *ctx, const trimeg_params *params);

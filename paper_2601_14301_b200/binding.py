@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libtrimeg.so")
 
 EXPORTS = (
-    "trimeg_mesh_create", "trimeg_mesh_create_unstructured", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
+    "trimeg_mesh_create", "trimeg_mesh_create_unstructured", "trimeg_mesh_locality_order", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_upload_spline", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
@@ -63,6 +63,7 @@ def load() -> C.CDLL:
     dp = C.POINTER(C.c_double)
     L.trimeg_mesh_create.argtypes = [C.POINTER(vp), i32, i32, dp, dp, dp, C.POINTER(trimeg_params)]
     L.trimeg_mesh_create_unstructured.argtypes = [C.POINTER(vp), i32, dp, dp, i32, C.POINTER(C.c_int32), i32, i32, C.POINTER(trimeg_params)]
+    L.trimeg_mesh_locality_order.argtypes = [i32, dp, dp, i32, C.POINTER(C.c_int32), C.POINTER(C.c_int32)]
     L.trimeg_mesh_destroy.argtypes = [vp]
     L.trimeg_mesh_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     L.trimeg_set_params.argtypes = [vp, C.POINTER(trimeg_params)]
@@ -389,6 +390,21 @@ def context_for(wl, inputs_module=None, eom_variant: int = 0, weight_mode: int =
         from . import inputs as inputs_module
     r, Rv, Zv = inputs_module.mesh_nodes(wl)
     return Context(wl.n_r, wl.n_theta, r, wl.params(eom_variant, weight_mode), Rv, Zv)
+
+
+def mesh_locality_order(vert_R, vert_Z, tri):
+    """trimeg_mesh_locality_order: int32 permutation `order`; use tri[order] as the triangle list (host only, no GPU needed)."""
+    import numpy as np
+    L = load()
+    vR = np.ascontiguousarray(vert_R, dtype=np.float64)
+    vZ = np.ascontiguousarray(vert_Z, dtype=np.float64)
+    tr = np.ascontiguousarray(tri, dtype=np.int32)
+    order = np.empty(tr.shape[0], dtype=np.int32)
+    dp = C.POINTER(C.c_double)
+    ip = C.POINTER(C.c_int32)
+    _check(L.trimeg_mesh_locality_order(int(vR.size), vR.ctypes.data_as(dp), vZ.ctypes.data_as(dp), int(tr.shape[0]),
+                                        tr.ctypes.data_as(ip), order.ctypes.data_as(ip)), "trimeg_mesh_locality_order")
+    return order
 
 
 def markers_to_device(m, device="cuda") -> Dict[str, torch.Tensor]:

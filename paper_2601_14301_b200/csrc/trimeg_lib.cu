@@ -10,6 +10,7 @@
 #include "trimeg_internal.h"
 #include <algorithm>
 #include <unordered_map>
+#include <utility>
 #include <vector>
 #include "trimeg_mesh.cuh"
 #include "bell_tables.inc"
@@ -582,6 +583,46 @@ try {
     *out = c;
     return TRIMEG_OK;
 } catch (...) {                                           // host tables (std::vector) could not be allocated: nothing crosses the C boundary
+    return TRIMEG_ERR_ALLOC;
+}
+
+// Host utility: a numbering of the triangles along a space-filling curve (Hilbert curve over a 2^16 x 2^16 grid on the
+// bounding rectangle, by centroid).  No device work.
+int trimeg_mesh_locality_order(int n_vert, const double *vert_R_host, const double *vert_Z_host, int n_tri, const int32_t *tri_host,
+                               int32_t *order_host)
+try {
+    if (!vert_R_host || !vert_Z_host || !tri_host || !order_host || n_vert < 3 || n_tri < 1) return TRIMEG_ERR_INVALID_ARG;
+    double lo[2] = {INFINITY, INFINITY}, hi[2] = {-INFINITY, -INFINITY};
+    for (int v = 0; v < n_vert; ++v) {
+        lo[0] = fmin(lo[0], vert_R_host[v]); hi[0] = fmax(hi[0], vert_R_host[v]);
+        lo[1] = fmin(lo[1], vert_Z_host[v]); hi[1] = fmax(hi[1], vert_Z_host[v]);
+    }
+    if (!(hi[0] > lo[0]) || !(hi[1] > lo[1])) return TRIMEG_ERR_MESH;
+    std::vector<std::pair<unsigned long long, int>> key((size_t)n_tri);
+    for (int t = 0; t < n_tri; ++t) {
+        double cR = 0.0, cZ = 0.0;
+        for (int k = 0; k < 3; ++k) {
+            const int v = tri_host[3 * (size_t)t + k];
+            if (v < 0 || v >= n_vert) return TRIMEG_ERR_MESH;
+            cR += vert_R_host[v]; cZ += vert_Z_host[v];
+        }
+        unsigned x = (unsigned)fmin(65535.0, fmax(0.0, (cR / 3.0 - lo[0]) / (hi[0] - lo[0]) * 65536.0));
+        unsigned y = (unsigned)fmin(65535.0, fmax(0.0, (cZ / 3.0 - lo[1]) / (hi[1] - lo[1]) * 65536.0));
+        unsigned long long d = 0;                        // Hilbert index of (x, y), 16 levels
+        for (unsigned sft = 1u << 15; sft > 0; sft >>= 1) {
+            const unsigned rx = (x & sft) ? 1u : 0u, ry = (y & sft) ? 1u : 0u;
+            d += (unsigned long long)sft * sft * ((3u * rx) ^ ry);
+            if (ry == 0) {
+                if (rx == 1) { x = 65535u - x; y = 65535u - y; }
+                const unsigned tmp = x; x = y; y = tmp;
+            }
+        }
+        key[(size_t)t] = std::make_pair(d, t);
+    }
+    std::sort(key.begin(), key.end());
+    for (int q = 0; q < n_tri; ++q) order_host[q] = key[(size_t)q].second;
+    return TRIMEG_OK;
+} catch (...) {
     return TRIMEG_ERR_ALLOC;
 }
 

@@ -195,6 +195,33 @@ def test_scatter_em_and_spline_field_on_the_unstructured_mesh(B, inputs):
     _assert_state_close(got, wp, 1e-10)
 
 
+def test_locality_order_is_a_renumbering_with_the_same_physics(B, inputs):
+    """tri[order] is the same mesh: cells map through the order, states agree to rounding (the same triangles, the same
+    arithmetic: bit for bit unless a marker sits within the locator's margin of an edge)."""
+    wl = inputs.WORKLOADS["cfg2"]
+    Rv, Zv, tri = inputs.unstructured_mesh(wl)
+    order = B.mesh_locality_order(Rv, Zv, tri)
+    assert np.array_equal(np.sort(order), np.arange(tri.shape[0]))
+    cen = np.stack([Rv[tri[order]].mean(axis=1), Zv[tri[order]].mean(axis=1)], axis=1)
+    assert np.hypot(*(cen[1:] - cen[:-1]).T).mean() < 0.05                # neighbours in number are neighbours in space
+    inv = np.empty_like(order); inv[order] = np.arange(order.size, dtype=order.dtype)
+    n = 40009
+    m = inputs.markers(wl, n=n)
+    out = []
+    for t in (tri, np.ascontiguousarray(tri[order])):
+        ctx = B.Context.unstructured(Rv, Zv, t, wl.params())
+        ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs_at(wl, Rv, Zv)).cuda(), kind=0)
+        d = B.markers_to_device(m)
+        ctx.locate(d["R"], d["Z"], cell=d["cell"])
+        ctx.push(d, wl.dt, 5)
+        out.append({k: v.cpu().numpy() for k, v in d.items()})
+    a, b = out
+    lost = a["cell"] < 0
+    assert np.array_equal(lost, b["cell"] < 0)
+    assert np.array_equal(inv[a["cell"][~lost]], b["cell"][~lost])
+    _assert_state_close(a, b, 1e-13)
+
+
 def test_mesh_errors(B, inputs):
     wl = inputs.WORKLOADS["cfg1"]
     Rv, Zv, tri = inputs.unstructured_mesh(wl)
