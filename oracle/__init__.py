@@ -39,6 +39,8 @@ def lib():
         L.orc_create_unstructured.restype = C.c_void_p
         L.orc_create_unstructured.argtypes = [C.c_int, dp, dp, C.c_int, ip, C.c_int, C.c_int, C.POINTER(_Params)]
         L.orc_box_count.argtypes = [C.c_void_p]
+        L.orc_set_equilibrium_table.argtypes = [C.c_void_p, C.c_int, C.c_int, C.c_double, C.c_double, C.c_double, C.c_double, dp,
+                                                C.c_int, C.c_double, C.c_double, dp]
         L.orc_destroy.argtypes = [C.c_void_p]
         L.orc_n_tri.argtypes = [C.c_void_p]
         L.orc_n_vert.argtypes = [C.c_void_p]
@@ -131,6 +133,15 @@ class Oracle:
         self.n_modes = 0
         self.mode_n = np.zeros(0, dtype=np.int32)
         return self
+
+    def set_equilibrium_table(self, tab: Optional[Dict]):
+        """O14: tab = dict(C [nR][nZ], Ra, Za, hR, hZ, D [nF], pa, hp) (inputs.equilibrium_table); None: analytic equilibrium."""
+        if tab is None:
+            self.L.orc_set_equilibrium_table(self.h, 0, 0, 0.0, 0.0, 0.0, 0.0, None, 0, 0.0, 0.0, None)
+            return
+        Cc, D = _f64(tab["C"]), _f64(tab["D"])
+        self.L.orc_set_equilibrium_table(self.h, Cc.shape[0], Cc.shape[1], float(tab["Ra"]), float(tab["Za"]), float(tab["hR"]),
+                                         float(tab["hZ"]), _d(Cc), D.size, float(tab["pa"]), float(tab["hp"]), _d(D))
 
     def box_entries(self) -> int:
         return int(self.L.orc_box_count(self.h))

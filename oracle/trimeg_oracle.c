@@ -39,6 +39,7 @@
  *   O11 spline basis   the thesis's own toroidal discretisation: cubic B-splines in phi instead of harmonics
  *                                                           PAPER.md:223, 365-368
  *   O13 general mesh   unstructured triangulation with the thesis's box-grid locator
+ *   O14 tabulated eq.  equilibrium from cubic-B-spline tables of psi(R, Z) and F(psi)
  *   O12 reduced model  eom_variant 2: the "dominant terms" equations A.19-A.29 (b* -> b)
  */
 #include <math.h>
@@ -60,6 +61,7 @@ typedef struct {
     int weight_mode;               /* 0: wdot = -(1-w) L ; 1: wdot = -L (reading G7) */
 } orc_params;
 
+struct orc_eqtab;
 typedef struct {
     int n_r, n_theta, n_vert, n_tri;
     double *r_nodes;               /* n_r + 1 */
@@ -77,6 +79,7 @@ typedef struct {
     int nbx, nby;                  /* boxes in R and Z */
     double bx0, bz0, bdx, bdz;     /* lower-left corner of the grid, box sizes */
     int *box_off, *box_tri;        /* [nbx*nby + 1], triangle lists (ascending) */
+    struct orc_eqtab *eq;          /* O14: tabulated (psi, F) equilibrium, NULL = the analytic circular one */
     int n_phi;                     /* O11: > 0 = the field is Y = sum_j N_j(phi) P_j(xi, eta) on n_phi toroidal planes */
     double *coef_spl;              /* [n_tri][n_phi][21] real monomial coefficients, one quintic per triangle and plane */
 } orc_ctx;
@@ -143,6 +146,8 @@ orc_ctx *orc_create(int n_r, int n_theta, const double *r_nodes,
 }
 
 void orc_destroy(orc_ctx *c);
+void orc_set_equilibrium_table(orc_ctx *c, int nR, int nZ, double Ra, double Za, double hR, double hZ, const double *C,
+                               int nF, double pa, double hp, const double *D);
 static int inside(const orc_ctx *c, int t, double R, double Z, double *xi, double *eta, double *lam0);
 static double min3(double a, double b, double c);
 /* ------------------------------------------------- O13 unstructured mesh + box-grid locator */
@@ -253,6 +258,7 @@ void orc_destroy(orc_ctx *c)
 {
     if (!c) return;
     free(c->box_off); free(c->box_tri);
+    orc_set_equilibrium_table(c, 0, 0, 0, 0, 0, 0, NULL, 0, 0, 0, NULL);
     free(c->r_nodes); free(c->Rv); free(c->Zv); free(c->tri); free(c->geom);
     if (c->basis) { for (int t = 0; t < c->n_tri; ++t) free(c->basis[t]); free(c->basis); }
     free(c->coef_aux[0]); free(c->coef_aux[1]); free(c->coef_spl);
@@ -560,11 +566,12 @@ void orc_gather(const orc_ctx *c, size_t n, const double *R, const double *Z, co
 typedef struct {
     double B, BR, BZ, Bphi, bR, bZ, bphi, dBdR, dBdZ;
     double dbR_dZ, dbZ_dR, dbphi_dR, dbphi_dZ, psi;
+    double psiR, psiZ;             /* O14: grad psi (tabulated equilibrium only; the analytic one uses rhat) */
 } orc_eq;
 
 /* B = grad psi x grad phi + F grad phi; B_R = -psi_Z/R, B_Z = psi_R/R,
  * B_phi = F/R with psi'(r) = B0 r/q(r) (reading G11), F = B0 R0. */
-static void equilibrium(const orc_params *p, double R, double Z, orc_eq *e)
+static void equilibrium_analytic(const orc_params *p, double R, double Z, orc_eq *e)
 {
     double x = R - p->R0;
     double s = x * x + Z * Z;
@@ -590,10 +597,95 @@ static void equilibrium(const orc_params *p, double R, double Z, orc_eq *e)
     e->psi = (p->q2 != 0.0) ? p->B0 * a2 / (2.0 * p->q2) * log(1.0 + p->q2 * s / (p->q0 * a2))
                             : p->B0 * s / (2.0 * p->q0);
 }
+/* ----------------------------------------------------------- O14 tabulated equilibrium */
+/* "The equilibrium configuration is computed as functions of (R, Z) ... starting from the magnetic equilibrium constructed from
+ * the EQDSK output file ... B_phi = F/R by means of b-spline interpolation of the poloidal current function F";
+ * B_R = -psi_Z/R, B_Z = psi_R/R, B_phi = F/R.  Reading G32 (the thesis names the interpolation, not its form):
+ *   psi(R, Z) = sum_ij C[i][j] beta((R - Ra)/hR - i) beta((Z - Za)/hZ - j),   F(psi) = sum_k D[k] beta((psi - pa)/hp - k),
+ * beta the uniform cubic B-spline of O11, the caller hands in COEFFICIENTS (a prefiltered EQDSK grid).  All sixteen (four)
+ * non-zero terms are summed; the F index is clamped to the table (the end pieces extend as cubics).  First and second
+ * derivatives of psi and F' give B, grad B, b and the derivatives of b that curl b needs, by the quotient rule.
+ * The profile gradients of the weight equation point along grad psi/|grad psi| (= rhat in the circular case). */
+typedef struct orc_eqtab {
+    int nR, nZ, nF;
+    double Ra, Za, hR, hZ, pa, hp;
+    double *C, *D;
+} orc_eqtab;
+static double bspl(double x);
+static double bspl_d(double x);
+static double bspl_dd(double x) { double a = fabs(x); if (a < 1.0) return -2.0 + 3.0 * a; if (a < 2.0) return 2.0 - a; return 0.0; }
+static void equilibrium_table(const orc_eqtab *q, double R, double Z, orc_eq *e)
+{
+    const double xr = (R - q->Ra) / q->hR, xz = (Z - q->Za) / q->hZ;
+    int i0 = (int)floor(xr), j0 = (int)floor(xz);
+    double psi = 0, pR = 0, pZ = 0, pRR = 0, pRZ = 0, pZZ = 0;
+    for (int i = i0 - 1; i <= i0 + 2; ++i)
+        for (int j = j0 - 1; j <= j0 + 2; ++j) {
+            if (i < 0 || i >= q->nR || j < 0 || j >= q->nZ) continue;         /* outside the table: no contribution */
+            const double c = q->C[(size_t)i * q->nZ + j], a = xr - i, b = xz - j;
+            psi += c * bspl(a) * bspl(b);
+            pR += c * bspl_d(a) * bspl(b) / q->hR;       pZ += c * bspl(a) * bspl_d(b) / q->hZ;
+            pRR += c * bspl_dd(a) * bspl(b) / (q->hR * q->hR);
+            pRZ += c * bspl_d(a) * bspl_d(b) / (q->hR * q->hZ);
+            pZZ += c * bspl(a) * bspl_dd(b) / (q->hZ * q->hZ);
+        }
+    const double xp = (psi - q->pa) / q->hp;
+    int k0 = (int)floor(xp);
+    if (k0 < 1) k0 = 1;
+    if (k0 > q->nF - 3) k0 = q->nF - 3;
+    double F = 0, Fp = 0;
+    {   /* the cubic piece of interval k0, written with the piece's own four polynomials so that it extends beyond the table */
+        const double t = xp - k0, u = 1.0 - t;
+        const double N[4] = {u * u * u / 6.0, 2.0 / 3.0 - t * t + 0.5 * t * t * t, 2.0 / 3.0 - u * u + 0.5 * u * u * u, t * t * t / 6.0};
+        const double M[4] = {-0.5 * u * u, -2.0 * t + 1.5 * t * t, 2.0 * u - 1.5 * u * u, 0.5 * t * t};
+        for (int k = 0; k < 4; ++k) { F += q->D[k0 - 1 + k] * N[k]; Fp += q->D[k0 - 1 + k] * M[k] / q->hp; }
+    }
+    const double BR = -pZ / R, BZ = pR / R, BP = F / R;
+    const double BR_R = -pRZ / R + pZ / (R * R), BR_Z = -pZZ / R;
+    const double BZ_R = pRR / R - pR / (R * R), BZ_Z = pRZ / R;
+    const double BP_R = Fp * pR / R - F / (R * R), BP_Z = Fp * pZ / R;
+    const double B = sqrt(BR * BR + BZ * BZ + BP * BP);
+    const double B_R = (BR * BR_R + BZ * BZ_R + BP * BP_R) / B, B_Z = (BR * BR_Z + BZ * BZ_Z + BP * BP_Z) / B;
+    e->B = B; e->BR = BR; e->BZ = BZ; e->Bphi = BP;
+    e->bR = BR / B; e->bZ = BZ / B; e->bphi = BP / B;
+    e->dBdR = B_R; e->dBdZ = B_Z;
+    e->dbR_dZ = (BR_Z - e->bR * B_Z) / B;
+    e->dbZ_dR = (BZ_R - e->bZ * B_R) / B;
+    e->dbphi_dR = (BP_R - e->bphi * B_R) / B;
+    e->dbphi_dZ = (BP_Z - e->bphi * B_Z) / B;
+    e->psi = psi; e->psiR = pR; e->psiZ = pZ;
+}
+static void equilibrium(const orc_ctx *c, double R, double Z, orc_eq *e)
+{
+    if (c->eq) equilibrium_table(c->eq, R, Z, e);
+    else { equilibrium_analytic(&c->p, R, Z, e); e->psiR = e->psiZ = 0.0; }
+}
+/* rate of change of the radial label along a velocity: along rhat (analytic equilibrium), along grad psi/|grad psi| (table) */
+static double radial_rate(const orc_ctx *c, const orc_eq *e, double R, double Z, double dRdot, double dZdot)
+{
+    if (c->eq) {
+        const double g = sqrt(e->psiR * e->psiR + e->psiZ * e->psiZ);
+        return (g > 0.0) ? (dRdot * e->psiR + dZdot * e->psiZ) / g : 0.0;
+    }
+    const double x = R - c->p.R0, r = sqrt(x * x + Z * Z);
+    return (r > 0.0) ? (dRdot * x + dZdot * Z) / r : 0.0;
+}
+/* C: [nR][nZ] coefficients of psi; D: [nF] coefficients of F; NULL C returns to the analytic equilibrium */
+void orc_set_equilibrium_table(orc_ctx *c, int nR, int nZ, double Ra, double Za, double hR, double hZ, const double *C,
+                               int nF, double pa, double hp, const double *D)
+{
+    if (c->eq) { free(c->eq->C); free(c->eq->D); free(c->eq); c->eq = NULL; }
+    if (!C) return;
+    orc_eqtab *q = (orc_eqtab *)calloc(1, sizeof(orc_eqtab));
+    q->nR = nR; q->nZ = nZ; q->nF = nF; q->Ra = Ra; q->Za = Za; q->hR = hR; q->hZ = hZ; q->pa = pa; q->hp = hp;
+    q->C = (double *)malloc(sizeof(double) * (size_t)nR * nZ); memcpy(q->C, C, sizeof(double) * (size_t)nR * nZ);
+    q->D = (double *)malloc(sizeof(double) * (size_t)nF); memcpy(q->D, D, sizeof(double) * (size_t)nF);
+    c->eq = q;
+}
 void orc_equilibrium(const orc_ctx *c, size_t n, const double *R, const double *Z, double *out /* [n][14] */)
 {
     for (size_t p = 0; p < n; ++p) {
-        orc_eq e; equilibrium(&c->p, R[p], Z[p], &e);
+        orc_eq e; equilibrium(c, R[p], Z[p], &e);
         memcpy(out + 14 * p, &e, sizeof(double) * 14);
     }
 }
@@ -601,19 +693,20 @@ void orc_equilibrium(const orc_ctx *c, size_t n, const double *R, const double *
 /* ------------------------------------------------------------------- O6 RHS */
 /* Electrostatic subset (dA^s = dA^h = 0  =>  u_par = v_par, b* = b0*, dG = dPhi).
  * eps = (m_s/q_s) rho_0 B_0 (reading G23). */
-static void rhs_point_em_reduced(const orc_params *p, double R, double Z, double upar, double mu, double w,
+static void rhs_point_em_reduced(const orc_ctx *c, double R, double Z, double upar, double mu, double w,
                                  const double fld[3][4], int ohm, double out[5]);
-static void rhs_point(const orc_params *p, double R, double Z, double vpar, double mu, double w,
+static void rhs_point(const orc_ctx *c, double R, double Z, double vpar, double mu, double w,
                       const double fld[4] /* dphi, d/dR, d/dZ, d/dphi */, double out[5])
 {
+    const orc_params *p = &c->p;
     if (p->eom_variant == 2) {                        /* O12: the reduced model with dA^s = dA^h = 0 and NO Ohm's-law substitution */
         double f3[3][4];
         memset(f3, 0, sizeof(f3));
         memcpy(f3[0], fld, sizeof(double) * 4);
-        rhs_point_em_reduced(p, R, Z, vpar, mu, w, f3, 0, out);
+        rhs_point_em_reduced(c, R, Z, vpar, mu, w, f3, 0, out);
         return;
     }
-    orc_eq e; equilibrium(p, R, Z, &e);
+    orc_eq e; equilibrium(c, R, Z, &e);
     double eps = p->rho0 * p->B0 / p->qs_over_ms;
     double cR = -e.dbphi_dZ;                          /* (curl b)_R   , bracket of A.4 */
     double cZ = e.dbphi_dR + e.bphi / R;              /* (curl b)_Z   , bracket of A.5 */
@@ -637,9 +730,7 @@ static void rhs_point(const orc_params *p, double R, double Z, double vpar, doub
     double dPdot = (CE / R) * (e.bZ * fR - e.bR * fZ);                           /* A.16 */
     double dvdot = -p->qs_over_ms * (b0R * fR + b0Z * fZ + (b0P / R) * fP);      /* A.17, dA = 0 (G3) */
     /* d ln f_M / dt, mbar = 1, kappa_X = -kappa_X rhat (G6, G10) */
-    double x = R - p->R0;
-    double r = sqrt(x * x + Z * Z);
-    double drdot = (r > 0.0) ? (dRdot * x + dZdot * Z) / r : 0.0;     /* dRvec . rhat */
+    double drdot = radial_rate(c, &e, R, Z, dRdot, dZdot);            /* dRvec . rhat */
     double en = vpar * vpar / p->T + 2.0 * mu * e.B / p->T - 1.5;
     double L = drdot * (-p->kappa_n - en * p->kappa_T)
              - (2.0 * mu / p->T) * (dRdot * e.dBdR + dZdot * e.dBdZ)
@@ -659,7 +750,7 @@ static int rhs_full(const orc_ctx *c, double R, double Z, double phi, double vpa
     int t = locate_one(c, R, Z, &xi, &eta);
     if (t < 0) return -1;
     if (c->n_modes > 0 || c->n_phi > 0) gather_one(c, t, xi, eta, phi, fld);
-    rhs_point(&c->p, R, Z, vpar, mu, w, fld, out);
+    rhs_point(c, R, Z, vpar, mu, w, fld, out);
     return t;
 }
 
@@ -679,7 +770,7 @@ void orc_rhs(const orc_ctx *c, size_t n, const double *R, const double *Z, const
 void orc_rhs_point(const orc_ctx *c, size_t n, const double *R, const double *Z, const double *vpar,
                    const double *mu, const double *w, const double *fld /* [n][4] */, double *out /* [n][5] */)
 {
-    for (size_t p = 0; p < n; ++p) rhs_point(&c->p, R[p], Z[p], vpar[p], mu[p], w[p], fld + 4 * p, out + 5 * p);
+    for (size_t p = 0; p < n; ++p) rhs_point(c, R[p], Z[p], vpar[p], mu[p], w[p], fld + 4 * p, out + 5 * p);
 }
 
 /* ------------------------------------------------------------------- O7 RK4 */
@@ -821,11 +912,12 @@ long orc_scatter(orc_ctx *c, size_t n, const double *R, const double *Z, const d
  *     printed has b instead of b* in the dA^h term, a second-order difference; the phi term of A.18 lacks its 1/R).
  *   weight: d ln f_M/dt of PAPER.md:1208 with v_par = u_par - (q_s/m_s) dA^h and d(u_par)/dt perturbed part.
  * fld[3][4]: (value, d/dR, d/dZ, d/dphi) of dPhi, dA^s, dA^h. */
-static void rhs_point_em(const orc_params *p, double R, double Z, double upar, double mu, double w,
+static void rhs_point_em(const orc_ctx *c, double R, double Z, double upar, double mu, double w,
                          const double fld[3][4], double out[5])
 {
-    if (p->eom_variant == 2) { rhs_point_em_reduced(p, R, Z, upar, mu, w, fld, 1, out); return; }   /* O12, A.29 */
-    orc_eq e; equilibrium(p, R, Z, &e);
+    const orc_params *p = &c->p;
+    if (p->eom_variant == 2) { rhs_point_em_reduced(c, R, Z, upar, mu, w, fld, 1, out); return; }   /* O12, A.29 */
+    orc_eq e; equilibrium(c, R, Z, &e);
     const double eps = p->rho0 * p->B0 / p->qs_over_ms, qom = p->qs_over_ms;
     const double *Phi = fld[0], *As = fld[1], *Ah = fld[2];
     double cR = -e.dbphi_dZ, cZ = e.dbphi_dR + e.bphi / R, cP = e.dbR_dZ - e.dbZ_dR;      /* curl b */
@@ -852,8 +944,7 @@ static void rhs_point_em(const orc_params *p, double R, double Z, double upar, d
                    - (Rmu * As[1] + Zmu * As[2] + Pmu * As[3]);                                        /* A.17 + Ohm */
     /* weight */
     double vpar = upar - qom * Ah[0];
-    double x = R - p->R0, r = sqrt(x * x + Z * Z);
-    double drdot = (r > 0.0) ? (dRdot * x + dZdot * Z) / r : 0.0;
+    double drdot = radial_rate(c, &e, R, Z, dRdot, dZdot);
     double en = vpar * vpar / p->T + 2.0 * mu * e.B / p->T - 1.5;
     double L = drdot * (-p->kappa_n - en * p->kappa_T) - (2.0 * mu / p->T) * (dRdot * e.dBdR + dZdot * e.dBdZ)
              - (2.0 * vpar / p->T) * dudot;
@@ -873,10 +964,11 @@ static void rhs_point_em(const orc_params *p, double R, double Z, double upar, d
  *   A.17 from which A.28 follows by b* -> b (the difference is second order in the fields).
  *   weight: d ln f_M/dt of PAPER.md:1208 along the perturbed velocity, v_par = u_par - (q_s/m_s) dA^h in the Maxwellian.
  * ohm = 0: the electrostatic push (orc_rhs / orc_push with eom_variant 2, dA = 0, d_t dA^s = 0); ohm = 1: orc_rhs_em, A.29. */
-static void rhs_point_em_reduced(const orc_params *p, double R, double Z, double upar, double mu, double w,
+static void rhs_point_em_reduced(const orc_ctx *c, double R, double Z, double upar, double mu, double w,
                                  const double fld[3][4], int ohm, double out[5])
 {
-    orc_eq e; equilibrium(p, R, Z, &e);
+    const orc_params *p = &c->p;
+    orc_eq e; equilibrium(c, R, Z, &e);
     const double eps = p->rho0 * p->B0 / p->qs_over_ms, qom = p->qs_over_ms;
     const double *Phi = fld[0], *As = fld[1], *Ah = fld[2];
     const double B3 = e.B * e.B * e.B;
@@ -899,8 +991,7 @@ static void rhs_point_em_reduced(const orc_params *p, double R, double Z, double
                                  + (e.bphi / R) * (keepE * Phi[3] - upar * Ah[3]))
                          - Cmu * (xR * As[1] + xZ * As[2] + (xP / R) * As[3]);
     const double vpar = upar - qom * Ah[0];
-    const double x = R - p->R0, r = sqrt(x * x + Z * Z);
-    const double drdot = (r > 0.0) ? (dRdot * x + dZdot * Z) / r : 0.0;
+    const double drdot = radial_rate(c, &e, R, Z, dRdot, dZdot);
     const double en = vpar * vpar / p->T + 2.0 * mu * e.B / p->T - 1.5;
     const double L = drdot * (-p->kappa_n - en * p->kappa_T) - (2.0 * mu / p->T) * (dRdot * e.dBdR + dZdot * e.dBdZ)
                    - (2.0 * vpar / p->T) * dudot;
@@ -913,7 +1004,7 @@ void orc_rhs_point_em(const orc_ctx *c, size_t n, const double *R, const double 
     for (size_t p = 0; p < n; ++p) {
         double f3[3][4];
         memcpy(f3, fld + 12 * p, sizeof(f3));
-        rhs_point_em(&c->p, R[p], Z[p], upar[p], mu[p], w[p], f3, out + 5 * p);
+        rhs_point_em(c, R[p], Z[p], upar[p], mu[p], w[p], f3, out + 5 * p);
     }
 }
 void orc_set_aux_coef(orc_ctx *c, int which, const double *coef)
@@ -941,7 +1032,7 @@ void orc_rhs_em(const orc_ctx *c, size_t n, const double *R, const double *Z, co
     for (size_t p = 0; p < n; ++p) {
         double o[5] = {0, 0, 0, 0, 0}, xi, eta, fld[3][4];
         int t = locate_one(c, R[p], Z[p], &xi, &eta);
-        if (t >= 0) { gather_three(c, t, xi, eta, phi[p], fld); rhs_point_em(&c->p, R[p], Z[p], upar[p], mu[p], w[p], fld, o); }
+        if (t >= 0) { gather_three(c, t, xi, eta, phi[p], fld); rhs_point_em(c, R[p], Z[p], upar[p], mu[p], w[p], fld, o); }
         if (cell_out) cell_out[p] = t;
         dRdt[p] = o[0]; dZdt[p] = o[1]; dphidt[p] = o[2]; dudt[p] = o[3]; dwdt[p] = o[4];
     }

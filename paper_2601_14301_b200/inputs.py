@@ -252,6 +252,43 @@ def unstructured_mesh(wl: Workload, seed: Optional[int] = None, jitter: float = 
     return np.ascontiguousarray(Rv), np.ascontiguousarray(Zv), np.ascontiguousarray(tri, dtype=np.int32)
 
 
+def _bspline_prefilter(y: np.ndarray, axis: int) -> np.ndarray:
+    """Coefficients c[-1..n] (returned with index shift +1, length n + 2) of the uniform cubic B-spline that interpolates the
+    n samples y along `axis` with zero second derivative at both ends: (c[i-1] + 4 c[i] + c[i+1])/6 = y[i]."""
+    y = np.moveaxis(np.asarray(y, dtype=np.float64), axis, 0)
+    n = y.shape[0]
+    A = np.zeros((n + 2, n + 2))
+    rhs = np.zeros((n + 2,) + y.shape[1:])
+    A[0, 0:3] = (1.0, -2.0, 1.0)
+    A[n + 1, n - 1:n + 2] = (1.0, -2.0, 1.0)
+    for i in range(n):
+        A[i + 1, i:i + 3] = (1.0 / 6.0, 4.0 / 6.0, 1.0 / 6.0)
+        rhs[i + 1] = y[i]
+    c = np.linalg.solve(A, rhs.reshape(n + 2, -1)).reshape((n + 2,) + y.shape[1:])
+    return np.moveaxis(c, 0, axis)
+
+
+def equilibrium_table(wl: Workload, nR: int = 65, nZ: int = 65, nF: int = 17, kappa: float = 1.0, f1: float = 0.0) -> Dict:
+    """Row f4 (tabulated equilibrium): stands in for an EQDSK file.  psi(R, Z) = psi_c(x^2 + (Z/kappa)^2), psi_c the poloidal
+    flux of the configs' circular equilibrium (psi' = B0 r/q, q = q0 + q2 r^2/a^2; kappa = 1 is that equilibrium itself,
+    kappa > 1 an elongated one), sampled on nR x nZ points over [R0 -+ 1.25 a] x [-+ 1.25 kappa a] and turned into uniform
+    cubic-B-spline coefficients (interpolating, natural ends); F(psi) = B0 R0 (1 + f1 psi), exactly representable.  Returns
+    dict(C [nR+2][nZ+2], Ra, Za, hR, hZ, D [nF], pa, hp): psi = sum C[i][j] beta((R-Ra)/hR - i) beta((Z-Za)/hZ - j)."""
+    Rg = np.linspace(wl.R0 - 1.25 * wl.a, wl.R0 + 1.25 * wl.a, nR)
+    Zg = np.linspace(-1.25 * kappa * wl.a, 1.25 * kappa * wl.a, nZ)
+    s = (Rg[:, None] - wl.R0) ** 2 + (Zg[None, :] / kappa) ** 2
+    a2 = wl.a * wl.a
+    psi = wl.B0 * a2 / (2.0 * wl.q2) * np.log1p(wl.q2 * s / (wl.q0 * a2)) if wl.q2 != 0.0 else wl.B0 * s / (2.0 * wl.q0)
+    C = _bspline_prefilter(_bspline_prefilter(psi, 0), 1)
+    hR, hZ = Rg[1] - Rg[0], Zg[1] - Zg[0]
+    pmax = float(psi.max())
+    hp = pmax / (nF - 3)
+    pk = -hp + hp * np.arange(nF)                                  # knot k of F sits at psi = pa + k hp, pa = -hp
+    D = wl.B0 * wl.R0 * (1.0 + f1 * pk)
+    return dict(C=np.ascontiguousarray(C), Ra=float(Rg[0] - hR), Za=float(Zg[0] - hZ), hR=float(hR), hZ=float(hZ),
+                D=np.ascontiguousarray(D), pa=float(-hp), hp=float(hp), kappa=float(kappa), f1=float(f1))
+
+
 def field_dofs_at(wl: Workload, Rv, Zv, seed: Optional[int] = None, sigma: float = 1e-3) -> np.ndarray:
     """Nodal DOFs [M][n_vert][6] complex128 of the workload's analytic perturbation at arbitrary vertices (row f4)."""
     amps = mode_amplitudes(wl, seed, sigma)
