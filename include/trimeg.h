@@ -123,6 +123,20 @@ int trimeg_mesh_locality_order(int n_vert, const double *vert_R_host, const doub
 int trimeg_mesh_destroy(trimeg_ctx *ctx);
 int trimeg_mesh_info(const trimeg_ctx *ctx, int *n_vert, int *n_tri);
 int trimeg_set_params(trimeg_ctx *ctx, const trimeg_params *params);
+/* Row f4, equilibrium from tables ("the magnetic equilibrium constructed from the EQDSK output file ... B_phi = F/R by means
+ * of b-spline interpolation of the poloidal current function F"; B = grad psi x grad phi + F grad phi,
+ * B_R = -psi_Z/R, B_Z = psi_R/R).  Reading G32 of DESIGN.md:
+ *   psi(R, Z) = sum_ij C[i][j] beta((R - Ra)/hR - i) beta((Z - Za)/hZ - j),   F(psi) = sum_k D[k] beta((psi - pa)/hp - k),
+ * beta the uniform cubic B-spline; C_host [nR][nZ] and D_host [nF] are COEFFICIENTS (a prefiltered EQDSK grid), host memory,
+ * copied.  |B|, grad B, b, curl b follow from the first and second derivatives of psi and from F'.  The F index is clamped to
+ * the table (the end pieces extend as cubics).  While a table is loaded every right-hand side (trimeg_rhs, trimeg_push,
+ * trimeg_push_host, trimeg_rhs_em; all eom_variants) uses it in place of the analytic circular equilibrium of trimeg_params
+ * (whose R0, a, q0, q2, B0 are then unused), and the profile gradients kappa_n, kappa_T act along grad psi/|grad psi|.
+ * C_host = NULL returns to the analytic equilibrium.  Synchronises the device.
+ * Errors: INVALID_ARG (sizes < 4, spacings <= 0, or a mesh vertex whose 4 x 4 stencil is not inside the table:
+ * every vertex needs Ra + hR <= R <= Ra + (nR - 2) hR and the same in Z), ALLOC, CUDA. */
+int trimeg_equilibrium_upload(trimeg_ctx *ctx, int nR, int nZ, double Ra, double Za, double hR, double hZ,
+                              const double *C_host, int nF, double pa, double hp, const double *D_host);
 /* test hook: geometry table [n_tri][6] = (R_v0, Z_v0, xi_R, xi_Z, eta_R, eta_Z) to device memory */
 int trimeg_mesh_download_geom(trimeg_ctx *ctx, double *geom_dev, trimeg_stream stream);
 

@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libtrimeg.so")
 
 EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_create_unstructured", "trimeg_mesh_locality_order", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
-    "trimeg_mesh_download_geom", "trimeg_field_upload", "trimeg_field_upload_spline", "trimeg_field_download_coeffs",
+    "trimeg_mesh_download_geom", "trimeg_equilibrium_upload", "trimeg_field_upload", "trimeg_field_upload_spline", "trimeg_field_download_coeffs",
     "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
     "trimeg_measure_fp64_peak", "trimeg_measure_gather_peak", "trimeg_strerror", "trimeg_version",
@@ -68,6 +68,7 @@ def load() -> C.CDLL:
     L.trimeg_mesh_info.argtypes = [vp, C.POINTER(i32), C.POINTER(i32)]
     L.trimeg_set_params.argtypes = [vp, C.POINTER(trimeg_params)]
     L.trimeg_mesh_download_geom.argtypes = [vp, vp, vp]
+    L.trimeg_equilibrium_upload.argtypes = [vp, i32, i32, dbl, dbl, dbl, dbl, dp, i32, dbl, dbl, dp]
     L.trimeg_field_upload.argtypes = [vp, i32, C.POINTER(i32), vp, i32, vp]
     L.trimeg_field_upload_spline.argtypes = [vp, i32, vp, i32, vp]
     L.trimeg_field_download_coeffs.argtypes = [vp, vp, vp]
@@ -202,6 +203,19 @@ class Context:
     def set_params(self, params: Dict):
         p = trimeg_params(**params)
         _check(self.L.trimeg_set_params(self.h, C.byref(p)), "trimeg_set_params")
+
+    def equilibrium_upload(self, tab: Optional[Dict]):
+        """Row f4: tab = dict(C [nR][nZ], Ra, Za, hR, hZ, D [nF], pa, hp) of B-spline coefficients; None: analytic equilibrium."""
+        import numpy as np
+        dp = C.POINTER(C.c_double)
+        if tab is None:
+            _check(self.L.trimeg_equilibrium_upload(self.h, 0, 0, 0.0, 0.0, 0.0, 0.0, None, 0, 0.0, 0.0, None), "trimeg_equilibrium_upload")
+            return
+        Cc = np.ascontiguousarray(tab["C"], dtype=np.float64)
+        D = np.ascontiguousarray(tab["D"], dtype=np.float64)
+        _check(self.L.trimeg_equilibrium_upload(self.h, Cc.shape[0], Cc.shape[1], float(tab["Ra"]), float(tab["Za"]), float(tab["hR"]),
+                                                float(tab["hZ"]), Cc.ctypes.data_as(dp), D.size, float(tab["pa"]), float(tab["hp"]),
+                                                D.ctypes.data_as(dp)), "trimeg_equilibrium_upload")
 
     def mesh_download_geom(self, stream=None) -> torch.Tensor:
         out = torch.empty((self.n_tri, 6), dtype=torch.float64, device="cuda")

@@ -37,7 +37,9 @@ constexpr double LOC_GAP_TOL = 1e-12;   // reading G31
 #define TRIMEG_HAS_SPL(F) false
 #define TRIMEG_IS_REDUCED(p) false
 #define TRIMEG_IS_UNS(M) false
+#define TRIMEG_HAS_EQTAB(p) false
 #else
+#define TRIMEG_HAS_EQTAB(p) ((p).eq_C != nullptr)
 #define TRIMEG_HAS_SPL(F) ((F).n_phi > 0)
 #define TRIMEG_IS_REDUCED(p) ((p).eom_variant == 2)
 #define TRIMEG_IS_UNS(M) ((M).n_r == 0)
@@ -64,6 +66,11 @@ struct PhysDev {
     double invT, kappa_n, kappa_T;
     double R0sq, m2qs, invT2;       // R0^2, -2 qs, 2 / T
     int eom_variant, weight_mode;
+    // row f4: equilibrium from cubic-B-spline tables of psi(R, Z) and F(psi) (reading G32); C == NULL:
+    // the analytic circular equilibrium above
+    int eq_nR, eq_nZ, eq_nF;
+    double eq_Ra, eq_Za, eq_ihR, eq_ihZ, eq_pa, eq_ihp;   // first knot positions, reciprocal spacings
+    const double *eq_C, *eq_D;      // [nR][nZ], [nF] coefficients
 };
 
 // --------------------------------------------------------------------------- a2 locator
@@ -402,6 +409,130 @@ __device__ __forceinline__ double rsqrt_fast(double x)
 // d ln f_M/dt (kappa_X along -rhat, G6/G10).
 struct Rates { double R, Z, phi, vpar, w; };
 
+// ---- row f4: tabulated equilibrium.  psi(R, Z) = sum C[i][j] beta((R - Ra)/hR - i) beta((Z - Za)/hZ - j), F(psi) likewise in one
+// dimension; B_R = -psi_Z/R, B_Z = psi_R/R, B_phi = F/R; |B|, grad B, b and curl b from the first and second
+// derivatives by the quotient rule.  The sixteen (four) non-zero terms; the caller guarantees that the mesh lies where the
+// 4 x 4 stencil is inside the table (checked at upload); the F index is clamped (the end pieces extend as cubics).
+struct EqVal { double B, BR, BZ, BP, bR, bZ, bphi, dBdR, dBdZ, curlR, curlZ, curlP, psiR, psiZ; };
+
+__device__ __forceinline__ void bspl4(double t, double ih, double N[4], double D1[4], double D2[4])
+{
+    const double u = 1.0 - t, t2 = t * t, u2 = u * u;
+    N[0] = u2 * u * (1.0 / 6.0); N[1] = fma(t2, fma(0.5, t, -1.0), 2.0 / 3.0); N[2] = fma(u2, fma(0.5, u, -1.0), 2.0 / 3.0); N[3] = t2 * t * (1.0 / 6.0);
+    D1[0] = -0.5 * u2 * ih; D1[1] = t * fma(1.5, t, -2.0) * ih; D1[2] = -u * fma(1.5, u, -2.0) * ih; D1[3] = 0.5 * t2 * ih;
+    const double ih2 = ih * ih;
+    D2[0] = u * ih2; D2[1] = fma(3.0, t, -2.0) * ih2; D2[2] = fma(3.0, u, -2.0) * ih2; D2[3] = t * ih2;
+}
+
+static __device__ __noinline__ EqVal eq_table(const PhysDev &p, double R, double Z)
+{
+    const double xr = (R - p.eq_Ra) * p.eq_ihR, xz = (Z - p.eq_Za) * p.eq_ihZ;
+    const double fr = floor(xr), fz = floor(xz);
+    int i0 = (int)fr, j0 = (int)fz;
+    i0 = max(1, min(p.eq_nR - 3, i0)); j0 = max(1, min(p.eq_nZ - 3, j0));
+    double NR[4], DR[4], ER[4], NZ[4], DZ[4], EZ[4];
+    bspl4(xr - (double)i0, p.eq_ihR, NR, DR, ER);
+    bspl4(xz - (double)j0, p.eq_ihZ, NZ, DZ, EZ);
+    double psi = 0.0, pR = 0.0, pZ = 0.0, pRR = 0.0, pRZ = 0.0, pZZ = 0.0;
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+        const double *row = p.eq_C + (size_t)(i0 - 1 + a) * p.eq_nZ + (j0 - 1);
+        double s0 = 0.0, s1 = 0.0, s2 = 0.0;             // sum over Z of the row with beta, beta', beta''
+#pragma unroll
+        for (int b = 0; b < 4; ++b) {
+            const double c = __ldg(row + b);
+            s0 = fma(c, NZ[b], s0); s1 = fma(c, DZ[b], s1); s2 = fma(c, EZ[b], s2);
+        }
+        psi = fma(NR[a], s0, psi); pR = fma(DR[a], s0, pR); pRR = fma(ER[a], s0, pRR);
+        pZ = fma(NR[a], s1, pZ); pRZ = fma(DR[a], s1, pRZ); pZZ = fma(NR[a], s2, pZZ);
+    }
+    const double xp = (psi - p.eq_pa) * p.eq_ihp;
+    int k0 = (int)floor(xp);
+    k0 = max(1, min(p.eq_nF - 3, k0));
+    double NF[4], DF[4], EF[4];
+    bspl4(xp - (double)k0, p.eq_ihp, NF, DF, EF);
+    double F = 0.0, Fp = 0.0;
+#pragma unroll
+    for (int k = 0; k < 4; ++k) { const double d = __ldg(p.eq_D + k0 - 1 + k); F = fma(d, NF[k], F); Fp = fma(d, DF[k], Fp); }
+    const double iR = 1.0 / R, iR2 = iR * iR;
+    EqVal e;
+    e.BR = -pZ * iR; e.BZ = pR * iR; e.BP = F * iR;
+    const double BR_R = fma(-pRZ, iR, pZ * iR2), BR_Z = -pZZ * iR;
+    const double BZ_R = fma(pRR, iR, -pR * iR2), BZ_Z = pRZ * iR;
+    const double BP_R = fma(Fp * pR, iR, -F * iR2), BP_Z = Fp * pZ * iR;
+    e.B = sqrt(fma(e.BR, e.BR, fma(e.BZ, e.BZ, e.BP * e.BP)));
+    const double iB = 1.0 / e.B;
+    e.dBdR = fma(e.BR, BR_R, fma(e.BZ, BZ_R, e.BP * BP_R)) * iB;
+    e.dBdZ = fma(e.BR, BR_Z, fma(e.BZ, BZ_Z, e.BP * BP_Z)) * iB;
+    e.bR = e.BR * iB; e.bZ = e.BZ * iB; e.bphi = e.BP * iB;
+    const double dbR_dZ = fma(-e.bR, e.dBdZ, BR_Z) * iB, dbZ_dR = fma(-e.bZ, e.dBdR, BZ_R) * iB;
+    const double dbP_dR = fma(-e.bphi, e.dBdR, BP_R) * iB, dbP_dZ = fma(-e.bphi, e.dBdZ, BP_Z) * iB;
+    e.curlR = -dbP_dZ;                                   // brackets of A.4-A.6
+    e.curlZ = fma(e.bphi, iR, dbP_dR);
+    e.curlP = dbR_dZ - dbZ_dR;
+    e.psiR = pR; e.psiZ = pZ;
+    return e;
+}
+
+// The equations of every variant on a general equilibrium value, as the oracle states them (O6, O9, O12): rigorous (0, 1) and
+// reduced (2), electrostatic (EM = false: A.17 / A.28 with dA = 0) and electromagnetic under the ideal Ohm's law.  The
+// profile gradients act along grad psi (reading G32).
+template <bool EM>
+__device__ __forceinline__ Rates rhs_from_eq(const PhysDev &p, const EqVal &e, double R, double upar, double mu, double w,
+                                             const FieldVal &Phi, const FieldVal &As, const FieldVal &Ah)
+{
+    const double iR = 1.0 / R;
+    const bool reduced = p.eom_variant == 2;
+    const double iB = 1.0 / e.B;
+    const double ev = p.eps * upar;
+    const double Bsp = reduced ? e.B : fma(ev, fma(e.bR, e.curlR, fma(e.bZ, e.curlZ, e.bphi * e.curlP)), e.B);
+    const double iBsp = 1.0 / Bsp;
+    const double k = reduced ? 0.0 : ev * iBsp;
+    const double lead = (p.eom_variant == 1) ? e.B * iBsp : 1.0;
+    const double b0R = fma(lead, e.bR, k * e.curlR), b0Z = fma(lead, e.bZ, k * e.curlZ), b0P = fma(lead, e.bphi, k * e.curlP);
+    const double CE = p.rho0B0 * iBsp;
+    // drift coefficient: rigorous eps mu/(B B*par), reduced eps (u^2 + mu B)/B^3
+    const double Cmu = reduced ? p.eps * mu * iB * iB : p.eps * mu * iB * iBsp;
+    const double Cd = reduced ? p.eps * fma(upar, upar, mu * e.B) * iB * iB * iB : Cmu;
+    const double xR = e.BP * e.dBdZ, xZ = -e.BP * e.dBdR, xP = fma(e.BZ, e.dBdR, -e.BR * e.dBdZ);   // B x grad B
+    const double R0dot = fma(b0R, upar, Cd * xR), Z0dot = fma(b0Z, upar, Cd * xZ), P0 = fma(b0P, upar, Cd * xP);
+    const double u0dot = -mu * fma(b0R, e.dBdR, b0Z * e.dBdZ);
+    const double PhP = Phi.fphi * iR;
+    double dRdot, dZdot, dP, dudot, vpar = upar;
+    if (EM) {
+        const double AsP = As.fphi * iR, AhP = Ah.fphi * iR;
+        const double bsR = reduced ? e.bR : fma(CE, fma(e.bZ, AsP, -e.bphi * As.fZ), b0R);      // b* (A.7-A.9); reduced: b
+        const double bsZ = reduced ? e.bZ : fma(CE, fma(e.bphi, As.fR, -e.bR * AsP), b0Z);
+        const double bsP = reduced ? e.bphi : fma(CE, fma(e.bR, As.fZ, -e.bZ * As.fR), b0P);
+        const double GR = fma(-upar, As.fR + Ah.fR, Phi.fR), GZ = fma(-upar, As.fZ + Ah.fZ, Phi.fZ), GP = fma(-upar, AsP + AhP, PhP);
+        const double qA = p.qom * Ah.f;
+        dRdot = fma(CE, fma(e.bphi, GZ, -e.bZ * GP), -qA * bsR);
+        dZdot = fma(CE, fma(-e.bphi, GR, e.bR * GP), -qA * bsZ);
+        dP = fma(CE, fma(e.bZ, GR, -e.bR * GZ), -qA * bsP);
+        const double t1 = reduced ? 0.0 : fma(bsR - e.bR, Phi.fR, fma(bsZ - e.bZ, Phi.fZ, (bsP - e.bphi) * PhP));
+        const double t2 = fma(bsR, Ah.fR, fma(bsZ, Ah.fZ, bsP * AhP));
+        dudot = fma(-p.qom, fma(-upar, t2, t1), -Cmu * fma(xR, As.fR, fma(xZ, As.fZ, xP * AsP)));
+        vpar = upar - qA;
+    } else {
+        dRdot = CE * fma(e.bphi, Phi.fZ, -e.bZ * PhP);
+        dZdot = CE * fma(-e.bphi, Phi.fR, e.bR * PhP);
+        dP = CE * fma(e.bZ, Phi.fR, -e.bR * Phi.fZ);
+        dudot = -p.qom * fma(b0R, Phi.fR, fma(b0Z, Phi.fZ, b0P * PhP));
+    }
+    const double g2 = fma(e.psiR, e.psiR, e.psiZ * e.psiZ);
+    const double drdot = (g2 > 0.0) ? fma(dRdot, e.psiR, dZdot * e.psiZ) * rsqrt(g2) : 0.0;
+    const double en = fma(vpar * vpar, p.invT, fma(mu * e.B, p.invT2, -1.5));
+    const double L = fma(drdot, -fma(en, p.kappa_T, p.kappa_n),
+                         fma(-(mu * p.invT2), fma(dRdot, e.dBdR, dZdot * e.dBdZ), -(vpar * p.invT2) * dudot));
+    Rates o;
+    o.R = R0dot + dRdot;
+    o.Z = Z0dot + dZdot;
+    o.phi = iR * (P0 + dP);
+    o.vpar = u0dot + dudot;
+    o.w = (p.weight_mode == 0) ? (w - 1.0) * L : -L;
+    return o;
+}
+
 // Row f4, eom_variant 2: the reduced equations A.19-A.29 ("only the dominant terms ... replacing b* with b",
 // PAPER.md:1276-1307; readings G29, G30): R0dot = u b + C_d B x grad B with C_d = eps (u^2 + mu B)/B^3, u0dot = -mu b.grad B,
 // dRdot = C_E b x grad(dG) - (q/m) dA^h b with C_E = rho_0 B_0/B, dudot = -(q/m)[b.grad dPhi - u b.grad dA^h] - v_mu.grad dA^s
@@ -478,6 +609,7 @@ __device__ __forceinline__ Rates rhs_point_reduced(const PhysDev &p, double R, d
 __device__ __forceinline__ Rates rhs_point(const PhysDev &p, double R, double Z, double vpar, double mu,
                                            double w, const FieldVal &fld)
 {
+    if (TRIMEG_HAS_EQTAB(p)) return rhs_from_eq<false>(p, eq_table(p, R, Z), R, vpar, mu, w, fld, fld, fld);
     if (TRIMEG_IS_REDUCED(p)) return rhs_point_reduced<false>(p, R, Z, vpar, mu, w, fld, fld, fld);
     const double x = R - p.R0;
     const double s = fma(x, x, Z * Z);

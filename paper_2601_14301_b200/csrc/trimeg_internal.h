@@ -32,6 +32,8 @@ struct trimeg_ctx {
     trimeg::PhysDev phys;
     // device tables
     double *d_geom, *d_r_nodes, *d_vR, *d_vZ;
+    double *d_eqC, *d_eqD;          // row f4: tabulated equilibrium (NULL: analytic)
+    double bbox[4];                 // R min, R max, Z min, Z max of the vertices
     int *d_tri, *d_nbr, *d_box_off, *d_box_tri;   // row f4, unstructured mesh: vertex triples, neighbours, box grid (NULL on the ring x sector mesh)
     double2 *d_coef;
     double2 *d_coef_aux[2];         // row f2: dA^s, dA^h on the main field's basis and mode list; NULL = identically zero
@@ -107,7 +109,10 @@ cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 // trimeg_push_*_core.cu: the same two kernels compiled without the branches of rows f3 / f4
 cudaError_t launch_push_wcache_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 cudaError_t launch_push_lane_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
-inline bool core_case(const trimeg_ctx *c) { return c->field.n_phi == 0 && c->params.eom_variant != 2 && c->mesh.n_r > 0; }
+inline bool core_case(const trimeg_ctx *c)
+{
+    return c->field.n_phi == 0 && c->params.eom_variant != 2 && c->mesh.n_r > 0 && c->phys.eq_C == nullptr;
+}
 
 // trimeg_push_lane.cu: the gather alone for cell-sorted markers; gate / want: runs iff (*gate * 16 <= n) == want
 cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const int32_t *hint,

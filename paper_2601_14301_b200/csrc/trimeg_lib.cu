@@ -396,6 +396,11 @@ int trimeg_mesh_create(trimeg_ctx **out, int n_r, int n_theta, const double *r_n
                 hZ[1 + (i - 1) * n_theta + j] = r_nodes_host[i] * sin(th);
             }
     }
+    c->bbox[0] = c->bbox[2] = INFINITY; c->bbox[1] = c->bbox[3] = -INFINITY;
+    for (int v = 0; v < c->n_vert; ++v) {
+        c->bbox[0] = fmin(c->bbox[0], hR[v]); c->bbox[1] = fmax(c->bbox[1], hR[v]);
+        c->bbox[2] = fmin(c->bbox[2], hZ[v]); c->bbox[3] = fmax(c->bbox[3], hZ[v]);
+    }
     int rc = TRIMEG_OK;
     double *d_rin2 = nullptr;
     do {
@@ -539,6 +544,7 @@ try {
     if (cudaGetDevice(&c->device) != cudaSuccess) { delete c; return TRIMEG_ERR_CUDA; }
     cudaDeviceGetAttribute(&c->n_sm, cudaDevAttrMultiProcessorCount, c->device);
     c->n_r = 0; c->n_theta = 0; c->n_vert = n_vert; c->n_tri = n_tri;
+    c->bbox[0] = lo[0]; c->bbox[1] = hi[0]; c->bbox[2] = lo[1]; c->bbox[3] = hi[1];
     c->params = *params;
     fill_phys(c);
     int rc = TRIMEG_OK;
@@ -632,6 +638,7 @@ int trimeg_mesh_destroy(trimeg_ctx *c)
     DeviceGuard guard__(c->device);
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
     cudaFree(c->d_adj_off); cudaFree(c->d_adj); cudaFree(c->d_trirhs);
+    cudaFree(c->d_eqC); cudaFree(c->d_eqD);
     cudaFree(c->d_tri); cudaFree(c->d_nbr); cudaFree(c->d_box_off); cudaFree(c->d_box_tri);
     cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]); cudaFree(c->d_coef_spl);
     cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
@@ -642,6 +649,32 @@ int trimeg_mesh_destroy(trimeg_ctx *c)
     if (c->ev_upload) cudaEventDestroy(c->ev_upload);
     cudaGetLastError();
     delete c;
+    return TRIMEG_OK;
+}
+
+int trimeg_equilibrium_upload(trimeg_ctx *c, int nR, int nZ, double Ra, double Za, double hR, double hZ, const double *C_host,
+                              int nF, double pa, double hp, const double *D_host)
+{
+    if (!c) return TRIMEG_ERR_INVALID_ARG;
+    ON_CTX_DEVICE(c);
+    CU_TRY(cudaDeviceSynchronize());                     // the tables may be in use by kernels enqueued earlier
+    cudaFree(c->d_eqC); cudaFree(c->d_eqD);
+    c->d_eqC = c->d_eqD = nullptr; c->phys.eq_C = c->phys.eq_D = nullptr;
+    if (!C_host) return TRIMEG_OK;                       // back to the analytic equilibrium
+    if (!D_host || nR < 4 || nZ < 4 || nF < 4 || !(hR > 0.0) || !(hZ > 0.0) || !(hp > 0.0) || (long long)nR * nZ > 0x3fffffffLL)
+        return TRIMEG_ERR_INVALID_ARG;
+    // every point of the mesh needs its 4 x 4 stencil inside the table: (x - a)/h in [1, n - 2]
+    const double tol = 1e-9;
+    if (c->bbox[0] < Ra + hR * (1.0 - tol) || c->bbox[1] > Ra + hR * (nR - 2 + tol) || c->bbox[2] < Za + hZ * (1.0 - tol) ||
+        c->bbox[3] > Za + hZ * (nZ - 2 + tol)) return TRIMEG_ERR_INVALID_ARG;
+    if (cudaMalloc(&c->d_eqC, sizeof(double) * (size_t)nR * nZ) != cudaSuccess || cudaMalloc(&c->d_eqD, sizeof(double) * nF) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(c->d_eqC); c->d_eqC = nullptr; return TRIMEG_ERR_ALLOC;
+    }
+    CU_TRY(cudaMemcpy(c->d_eqC, C_host, sizeof(double) * (size_t)nR * nZ, cudaMemcpyHostToDevice));
+    CU_TRY(cudaMemcpy(c->d_eqD, D_host, sizeof(double) * nF, cudaMemcpyHostToDevice));
+    PhysDev &d = c->phys;
+    d.eq_nR = nR; d.eq_nZ = nZ; d.eq_nF = nF; d.eq_Ra = Ra; d.eq_Za = Za; d.eq_ihR = 1.0 / hR; d.eq_ihZ = 1.0 / hZ;
+    d.eq_pa = pa; d.eq_ihp = 1.0 / hp; d.eq_C = c->d_eqC; d.eq_D = c->d_eqD;
     return TRIMEG_OK;
 }
 
