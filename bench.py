@@ -203,7 +203,7 @@ def run_reference(args, wl):
     return 0
 
 
-def workload_config(wl, extra=None, n_phi=0, eom_variant=0, unstructured=False):
+def workload_config(wl, extra=None, n_phi=0, eom_variant=0, unstructured=False, eq_table=0):
     c = {"workload": f"{wl.name} (BASELINE.json configs[{int(wl.name[3:]) - 1}])",
          "mesh": f"{wl.n_r}x{wl.n_theta} rings x sectors, {wl.n_tri} triangles",
          "toroidal_modes": list(wl.modes), "markers_per_gpu": wl.n_markers, "dt": wl.dt,
@@ -212,6 +212,8 @@ def workload_config(wl, extra=None, n_phi=0, eom_variant=0, unstructured=False):
         c["mesh"] = (f"unstructured: the {wl.n_r}x{wl.n_theta} ring x sector vertices jittered, Delaunay, numbering shuffled"
                      + ("" if unstructured == "shuffled" else ", triangles renumbered along a Hilbert curve (trimeg_mesh_locality_order)")
                      + f"; {wl.n_tri} triangles; box-grid locator (row f4)")
+    if eq_table:
+        c["equilibrium"] = f"cubic-B-spline tables {eq_table}x{eq_table} of psi (the configs' flux function, elongation 1.2) and F(psi) = B0 R0 (1 + 0.1 psi) (row f4)"
     if eom_variant:
         c["eom_variant"] = {1: "1 (b0* normalised by B/B*par, reading G2)", 2: "2 (reduced equations A.19-A.29, row f4)"}[eom_variant]
     if n_phi:
@@ -227,7 +229,7 @@ class PushRun:
     working copy).  A bench step = restore the batch to the workload's initial state (device copy), compact, then
     [cell sort -> fused push of `sort_every` RK4 steps] until the workload's nsteps are done."""
 
-    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True, n_phi=0, eom_variant=0, unstructured=False):
+    def __init__(self, wl, sort_every, push_kernel=-1, seed=None, keep_host=True, n_phi=0, eom_variant=0, unstructured=False, eq_table=0):
         import torch
         from paper_2601_14301_b200 import binding, inputs
         self.torch, self.wl = torch, wl
@@ -247,6 +249,10 @@ class PushRun:
                 self.ctx.field_upload_spline(torch.from_numpy(inputs.spline_dofs(wl, n_phi)).cuda(), kind=0)
             else:
                 self.ctx.field_upload(wl.modes, torch.from_numpy(inputs.field_dofs(wl)).cuda(), kind=0)
+        self.eq_tab = None
+        if eq_table:                                       # row f4: the configs' circular flux function, elongated by 1.2, as B-spline tables
+            self.eq_tab = inputs.equilibrium_table(wl, eq_table, eq_table, 33, kappa=1.2, f1=0.1)
+            self.ctx.equilibrium_upload(self.eq_tab)
         if push_kernel >= 0:
             self.ctx.set_push_kernel(push_kernel)
         m_np = inputs.markers(wl, n=self.n, seed=seed)
@@ -358,6 +364,8 @@ class PushRun:
                 o.bell_spline_from_dofs(inputs.spline_dofs(wl, self.n_phi))
             else:
                 o.bell_from_dofs(wl.modes, inputs.field_dofs(wl))
+        if self.eq_tab is not None:
+            o.set_equilibrium_table(self.eq_tab)
         want = o.push(sample, wl.dt, wl.nsteps)
         assert np.array_equal(got["cell"] < 0, want["cell"] < 0), "lost-marker sets differ"
         worst = 0.0
@@ -474,7 +482,7 @@ def run_gpu(args, wl):
 
     n = wl.n_markers
     run = PushRun(wl, args.sort_every, args.push_kernel, seed=D.rank_seed(wl.seed, rank), n_phi=args.n_phi, eom_variant=args.eom_variant,
-                  unstructured=args.unstructured)
+                  unstructured=args.unstructured, eq_table=args.eq_table)
     ctx = run.ctx
     fp64_peak = ctx.measure_fp64_peak()
     fp64_peak3 = ctx.measure_fp64_peak_operands(3)     # DFMA stream with three fresh register operands
@@ -509,7 +517,7 @@ def run_gpu(args, wl):
         e2e = e2e_run(ctx, wl, run.m_np, max(1, min(args.steps, 3)), agg["value"], D, dev)
 
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.unstructured:
+    if rank == 0 and world == 1 and not args.no_cpu_baseline and not args.unstructured and not args.eq_table:
         r = time_oracle(wl, run.m_np, 15.0, one_core_seconds=6.0, n_phi=args.n_phi, eom_variant=args.eom_variant)
         cpu = {"value": r["value"], "unit": UNIT, "cores": r["cores"], "nproc": r["nproc"], "kind": "oracle", "sample": r["sample"],
                "value_one_core": r.get("value_one_core"), "sample_one_core": r.get("sample_one_core"),
@@ -519,7 +527,7 @@ def run_gpu(args, wl):
 
     # ---- the other configs, device-timed the same way (N = 1 only): short runs, same live peaks
     sweep = None
-    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes and not args.n_phi and not args.eom_variant and not args.unstructured:
+    if rank == 0 and world == 1 and not args.no_sweep and wl.name == "cfg5" and not args.markers and not args.n_modes and not args.n_phi and not args.eom_variant and not args.unstructured and not args.eq_table:
         sweep = {}
         for name in ("cfg2", "cfg3"):
             w2 = inputs.WORKLOADS[name]
@@ -579,7 +587,7 @@ def run_gpu(args, wl):
             "metric": METRIC, "value": agg["value"], "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": agg["seconds"] / args.steps * 1e3, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": workload_config(wl, n_phi=args.n_phi, eom_variant=args.eom_variant, unstructured=args.unstructured, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
+            "config": workload_config(wl, n_phi=args.n_phi, eom_variant=args.eom_variant, unstructured=args.unstructured, eq_table=args.eq_table, extra={"sort_every": run.sort_every, "parallelism": f"marker-shard x{world}",
                                                  "lost_markers_per_step": res["lost_per_step"],
                                                  "unit_count": "every bench step restarts from the config's initial state; a marker "
                                                                "that leaves the mesh during a step counts zero steps for it"}),
@@ -810,6 +818,7 @@ def main():
     ap.add_argument("--unstructured", nargs="?", const="hilbert", default=None, choices=["hilbert", "shuffled"],
                     help="row f4: the workload's cross-section as an unstructured triangulation (jittered Delaunay, shuffled numbering) with "
                          "the box-grid locator; 'hilbert' (default): triangles renumbered by trimeg_mesh_locality_order first, 'shuffled': as generated")
+    ap.add_argument("--eq-table", type=int, default=0, help="row f4: equilibrium from N x N cubic-B-spline tables (the configs' flux function elongated by 1.2, F' != 0) instead of the analytic one")
     ap.add_argument("--sort-every", type=int, default=10, help="RK4 steps fused per sort + push call")
     ap.add_argument("--push-kernel", type=int, default=-1, help="trimeg_set_push_kernel variant (-1 = library default)")
     ap.add_argument("--min-log2", type=int, default=16, help="cfg4 gather sweep: smallest marker count 2^k")

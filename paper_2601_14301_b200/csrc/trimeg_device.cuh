@@ -39,7 +39,7 @@ constexpr double LOC_GAP_TOL = 1e-12;   // reading G31
 #define TRIMEG_IS_UNS(M) false
 #define TRIMEG_HAS_EQTAB(p) false
 #else
-#define TRIMEG_HAS_EQTAB(p) ((p).eq_C != nullptr)
+#define TRIMEG_HAS_EQTAB(p) ((p).eq != nullptr)
 #define TRIMEG_HAS_SPL(F) ((F).n_phi > 0)
 #define TRIMEG_IS_REDUCED(p) ((p).eom_variant == 2)
 #define TRIMEG_IS_UNS(M) ((M).n_r == 0)
@@ -66,8 +66,12 @@ struct PhysDev {
     double invT, kappa_n, kappa_T;
     double R0sq, m2qs, invT2;       // R0^2, -2 qs, 2 / T
     int eom_variant, weight_mode;
-    // row f4: equilibrium from cubic-B-spline tables of psi(R, Z) and F(psi) (reading G32); C == NULL:
-    // the analytic circular equilibrium above
+    // row f4: equilibrium from cubic-B-spline tables of psi(R, Z) and F(psi) (reading G32), a
+    // descriptor in device memory (kept out of the kernel parameters: the hot kernels' code does not change with it);
+    // NULL: the analytic circular equilibrium above
+    const struct EqTabDev *eq;
+};
+struct EqTabDev {
     int eq_nR, eq_nZ, eq_nF;
     double eq_Ra, eq_Za, eq_ihR, eq_ihZ, eq_pa, eq_ihp;   // first knot positions, reciprocal spacings
     const double *eq_C, *eq_D;      // [nR][nZ], [nF] coefficients
@@ -424,8 +428,9 @@ __device__ __forceinline__ void bspl4(double t, double ih, double N[4], double D
     D2[0] = u * ih2; D2[1] = fma(3.0, t, -2.0) * ih2; D2[2] = fma(3.0, u, -2.0) * ih2; D2[3] = t * ih2;
 }
 
-static __device__ __noinline__ EqVal eq_table(const PhysDev &p, double R, double Z)
+static __device__ __noinline__ EqVal eq_table(const EqTabDev *__restrict__ q, double R, double Z)
 {
+    const EqTabDev p = *q;
     const double xr = (R - p.eq_Ra) * p.eq_ihR, xz = (Z - p.eq_Za) * p.eq_ihZ;
     const double fr = floor(xr), fz = floor(xz);
     int i0 = (int)fr, j0 = (int)fz;
@@ -609,7 +614,7 @@ __device__ __forceinline__ Rates rhs_point_reduced(const PhysDev &p, double R, d
 __device__ __forceinline__ Rates rhs_point(const PhysDev &p, double R, double Z, double vpar, double mu,
                                            double w, const FieldVal &fld)
 {
-    if (TRIMEG_HAS_EQTAB(p)) return rhs_from_eq<false>(p, eq_table(p, R, Z), R, vpar, mu, w, fld, fld, fld);
+    if (TRIMEG_HAS_EQTAB(p)) return rhs_from_eq<false>(p, eq_table(p.eq, R, Z), R, vpar, mu, w, fld, fld, fld);
     if (TRIMEG_IS_REDUCED(p)) return rhs_point_reduced<false>(p, R, Z, vpar, mu, w, fld, fld, fld);
     const double x = R - p.R0;
     const double s = fma(x, x, Z * Z);

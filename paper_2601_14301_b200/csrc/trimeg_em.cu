@@ -18,7 +18,7 @@ struct Fld3 { FieldVal phi, as, ah; };
 // O9 of the oracle, operation for operation up to the table-seeded reciprocals of trimeg_device.cuh
 __device__ __forceinline__ Rates rhs_point_em(const PhysDev &p, double R, double Z, double upar, double mu, double w, const Fld3 &F)
 {
-    if (TRIMEG_HAS_EQTAB(p)) return rhs_from_eq<true>(p, eq_table(p, R, Z), R, upar, mu, w, F.phi, F.as, F.ah);
+    if (TRIMEG_HAS_EQTAB(p)) return rhs_from_eq<true>(p, eq_table(p.eq, R, Z), R, upar, mu, w, F.phi, F.as, F.ah);
     if (p.eom_variant == 2) return rhs_point_reduced<true>(p, R, Z, upar, mu, w, F.phi, F.as, F.ah);   // row f4, A.19-A.29
     const double x = R - p.R0;
     const double s = fma(x, x, Z * Z);

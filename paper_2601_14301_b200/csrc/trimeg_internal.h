@@ -33,6 +33,7 @@ struct trimeg_ctx {
     // device tables
     double *d_geom, *d_r_nodes, *d_vR, *d_vZ;
     double *d_eqC, *d_eqD;          // row f4: tabulated equilibrium (NULL: analytic)
+    trimeg::EqTabDev *d_eqdesc;     // its descriptor in device memory
     double bbox[4];                 // R min, R max, Z min, Z max of the vertices
     int *d_tri, *d_nbr, *d_box_off, *d_box_tri;   // row f4, unstructured mesh: vertex triples, neighbours, box grid (NULL on the ring x sector mesh)
     double2 *d_coef;
@@ -111,7 +112,7 @@ cudaError_t launch_push_wcache_core(trimeg_ctx *c, const trimeg_markers &m, size
 cudaError_t launch_push_lane_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 inline bool core_case(const trimeg_ctx *c)
 {
-    return c->field.n_phi == 0 && c->params.eom_variant != 2 && c->mesh.n_r > 0 && c->phys.eq_C == nullptr;
+    return c->field.n_phi == 0 && c->params.eom_variant != 2 && c->mesh.n_r > 0 && c->phys.eq == nullptr;
 }
 
 // trimeg_push_lane.cu: the gather alone for cell-sorted markers; gate / want: runs iff (*gate * 16 <= n) == want

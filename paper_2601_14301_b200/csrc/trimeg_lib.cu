@@ -638,7 +638,7 @@ int trimeg_mesh_destroy(trimeg_ctx *c)
     DeviceGuard guard__(c->device);
     cudaFree(c->d_vR); cudaFree(c->d_vZ); cudaFree(c->d_r_nodes); cudaFree(c->d_geom); cudaFree(c->d_bins);
     cudaFree(c->d_adj_off); cudaFree(c->d_adj); cudaFree(c->d_trirhs);
-    cudaFree(c->d_eqC); cudaFree(c->d_eqD);
+    cudaFree(c->d_eqC); cudaFree(c->d_eqD); cudaFree(c->d_eqdesc);
     cudaFree(c->d_tri); cudaFree(c->d_nbr); cudaFree(c->d_box_off); cudaFree(c->d_box_tri);
     cudaFree(c->d_coef_aux[0]); cudaFree(c->d_coef_aux[1]); cudaFree(c->d_coef_spl);
     cudaFree(c->d_stats); cudaFree(c->d_coef); cudaFree(c->d_mode_n); cudaFree(c->d_scratch); cudaFree(c->d_hbuf);
@@ -658,8 +658,8 @@ int trimeg_equilibrium_upload(trimeg_ctx *c, int nR, int nZ, double Ra, double Z
     if (!c) return TRIMEG_ERR_INVALID_ARG;
     ON_CTX_DEVICE(c);
     CU_TRY(cudaDeviceSynchronize());                     // the tables may be in use by kernels enqueued earlier
-    cudaFree(c->d_eqC); cudaFree(c->d_eqD);
-    c->d_eqC = c->d_eqD = nullptr; c->phys.eq_C = c->phys.eq_D = nullptr;
+    cudaFree(c->d_eqC); cudaFree(c->d_eqD); cudaFree(c->d_eqdesc);
+    c->d_eqC = c->d_eqD = nullptr; c->d_eqdesc = nullptr; c->phys.eq = nullptr;
     if (!C_host) return TRIMEG_OK;                       // back to the analytic equilibrium
     if (!D_host || nR < 4 || nZ < 4 || nF < 4 || !(hR > 0.0) || !(hZ > 0.0) || !(hp > 0.0) || (long long)nR * nZ > 0x3fffffffLL)
         return TRIMEG_ERR_INVALID_ARG;
@@ -667,14 +667,17 @@ int trimeg_equilibrium_upload(trimeg_ctx *c, int nR, int nZ, double Ra, double Z
     const double tol = 1e-9;
     if (c->bbox[0] < Ra + hR * (1.0 - tol) || c->bbox[1] > Ra + hR * (nR - 2 + tol) || c->bbox[2] < Za + hZ * (1.0 - tol) ||
         c->bbox[3] > Za + hZ * (nZ - 2 + tol)) return TRIMEG_ERR_INVALID_ARG;
-    if (cudaMalloc(&c->d_eqC, sizeof(double) * (size_t)nR * nZ) != cudaSuccess || cudaMalloc(&c->d_eqD, sizeof(double) * nF) != cudaSuccess) {
-        cudaGetLastError(); cudaFree(c->d_eqC); c->d_eqC = nullptr; return TRIMEG_ERR_ALLOC;
+    if (cudaMalloc(&c->d_eqC, sizeof(double) * (size_t)nR * nZ) != cudaSuccess || cudaMalloc(&c->d_eqD, sizeof(double) * nF) != cudaSuccess ||
+        cudaMalloc(&c->d_eqdesc, sizeof(EqTabDev)) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(c->d_eqC); cudaFree(c->d_eqD); c->d_eqC = c->d_eqD = nullptr; return TRIMEG_ERR_ALLOC;
     }
     CU_TRY(cudaMemcpy(c->d_eqC, C_host, sizeof(double) * (size_t)nR * nZ, cudaMemcpyHostToDevice));
     CU_TRY(cudaMemcpy(c->d_eqD, D_host, sizeof(double) * nF, cudaMemcpyHostToDevice));
-    PhysDev &d = c->phys;
+    EqTabDev d;
     d.eq_nR = nR; d.eq_nZ = nZ; d.eq_nF = nF; d.eq_Ra = Ra; d.eq_Za = Za; d.eq_ihR = 1.0 / hR; d.eq_ihZ = 1.0 / hZ;
     d.eq_pa = pa; d.eq_ihp = 1.0 / hp; d.eq_C = c->d_eqC; d.eq_D = c->d_eqD;
+    CU_TRY(cudaMemcpy(c->d_eqdesc, &d, sizeof(d), cudaMemcpyHostToDevice));
+    c->phys.eq = c->d_eqdesc;
     return TRIMEG_OK;
 }
 
