@@ -47,6 +47,7 @@ extern "C" {
 #define TRIMEG_ERR_CUDA        (-4)  /* a CUDA runtime call or kernel launch failed              */
 #define TRIMEG_ERR_ALLOC       (-5)  /* device or host allocation failed                         */
 #define TRIMEG_ERR_UNSUPPORTED (-6)  /* the call is not defined for the loaded field's toroidal basis */
+#define TRIMEG_ERR_CAPACITY    (-7)  /* trimeg_scatter_static: the problem needs more than the fixed static scratch */
 
 #define TRIMEG_NCOEF 21              /* monomials xi^i eta^j, 0 <= i+j <= 5        */
 
@@ -250,6 +251,22 @@ int trimeg_pullback(trimeg_ctx *ctx, trimeg_markers *m, size_t n, trimeg_stream 
  * is the only collective.  Errors: INVALID_ARG, NO_FIELD (no mode list uploaded), ALLOC, CUDA. */
 int trimeg_scatter(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, void *rhs_dev,
                    trimeg_stream stream);
+
+/* The same projection for callers that cannot allocate device memory (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc): trimeg_scatter_static calls no cudaMalloc, cudaFree or any allocating routine.
+ * All its scratch -- histogram bins, the two int32 index arrays of the sort, the per-triangle results -- lives in ONE
+ * array of TRIMEG_SCATTER_STATIC_BYTES (16 MiB) in the library's device image, which every GPU that loads the library
+ * holds until the process exits.  Same arguments, same kernels, same result (to the rounding of the unspecified summation
+ * order inside a triangle) as trimeg_scatter.  Capacity: with the scratch laid out as
+ *     256-aligned 4 (n_tri + 8)  +  2 x 256-aligned 4 n  +  288 n_tri n_modes   bytes  <=  TRIMEG_SCATTER_STATIC_BYTES
+ * (e.g. 480 triangles x 2 modes with up to 2.0e6 markers; 32 512 triangles x 3 modes does not fit), else the call
+ * returns TRIMEG_ERR_CAPACITY and does nothing: use trimeg_scatter.  The array is shared by every context of a device and
+ * keeps the last call's contents (the call clears what must start at zero): two calls that overlap on the GPU -- on two
+ * streams, or from two contexts of one device -- race; calls on one stream are ordered and safe.  The array's device
+ * address is looked up once per device (cudaGetSymbolAddress) on the first call.
+ * Errors: INVALID_ARG, NO_FIELD, UNSUPPORTED (B-spline field), CAPACITY, CUDA. */
+#define TRIMEG_SCATTER_STATIC_BYTES (16 * 1024 * 1024)
+int trimeg_scatter_static(trimeg_ctx *ctx, const trimeg_markers *m, size_t n, void *rhs_dev, trimeg_stream stream);
 
 /* ---- cell sort (row a1) ---------------------------------------------------------------------
  * Why: the thesis's kernel reads the field tables with 18 % of its accesses coalesced and leaves the

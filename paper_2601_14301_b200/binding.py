@@ -18,12 +18,13 @@ LIB_PATH = os.path.join(_HERE, "libtrimeg.so")
 EXPORTS = (
     "trimeg_mesh_create", "trimeg_mesh_create_unstructured", "trimeg_mesh_locality_order", "trimeg_mesh_destroy", "trimeg_mesh_info", "trimeg_set_params",
     "trimeg_mesh_download_geom", "trimeg_equilibrium_upload", "trimeg_field_upload", "trimeg_field_upload_spline", "trimeg_field_download_coeffs",
-    "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_sort", "trimeg_compact",
+    "trimeg_locate", "trimeg_gather", "trimeg_rhs", "trimeg_field_upload_aux", "trimeg_rhs_em", "trimeg_pullback", "trimeg_scatter", "trimeg_scatter_static", "trimeg_sort", "trimeg_compact",
     "trimeg_push", "trimeg_set_push_kernel", "trimeg_get_push_kernel", "trimeg_push_host", "trimeg_release_host_buffers", "trimeg_get_stats", "trimeg_reset_stats", "trimeg_get_tile_counters", "trimeg_measure_fp64_peak_operands",
     "trimeg_measure_fp64_peak", "trimeg_measure_gather_peak", "trimeg_strerror", "trimeg_version",
 )
 
-OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC, ERR_UNSUPPORTED = 0, -1, -2, -3, -4, -5, -6
+OK, ERR_INVALID_ARG, ERR_MESH, ERR_NO_FIELD, ERR_CUDA, ERR_ALLOC, ERR_UNSUPPORTED, ERR_CAPACITY = 0, -1, -2, -3, -4, -5, -6, -7
+SCATTER_STATIC_BYTES = 16 * 1024 * 1024      # TRIMEG_SCATTER_STATIC_BYTES
 # TRIMEG_PUSH_KERNEL_* of include/trimeg.h
 FIELD_AS, FIELD_AH = 1, 2      # TRIMEG_FIELD_AS / _AH
 PUSH_KERNEL_AUTO, PUSH_KERNEL_THREAD, PUSH_KERNEL_LANE, PUSH_KERNEL_WCACHE = -1, 0, 1, 2
@@ -76,6 +77,7 @@ def load() -> C.CDLL:
     L.trimeg_gather.argtypes = [vp, sz, vp, vp, vp, vp, vp, vp, vp, vp, vp]
     L.trimeg_rhs.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp, vp, vp, vp, vp]
     L.trimeg_scatter.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp]
+    L.trimeg_scatter_static.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp]
     L.trimeg_field_upload_aux.argtypes = [vp, i32, vp, i32, vp]
     L.trimeg_rhs_em.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp, vp, vp, vp, vp, vp]
     L.trimeg_pullback.argtypes = [vp, C.POINTER(trimeg_markers), sz, vp]
@@ -326,6 +328,15 @@ class Context:
             out = torch.empty((self.n_modes, self.n_vert, 6), dtype=torch.complex128, device=m["R"].device)
         _check(self.L.trimeg_scatter(self.h, C.byref(ms), n, _ptr(out, torch.complex128) if self.n_modes else C.c_void_p(0),
                                      _stream(stream)), "trimeg_scatter")
+        return out
+
+    def scatter_static(self, m: Dict[str, torch.Tensor], out: torch.Tensor, n: Optional[int] = None, stream=None) -> torch.Tensor:
+        """trimeg_scatter_static: the projection with all scratch in the library's static device array -- no allocation
+        anywhere, so `out` (complex128 [n_modes][n_vert][6]) is the caller's."""
+        n = m["R"].numel() if n is None else int(n)
+        ms = _markers(m, n)
+        _check(self.L.trimeg_scatter_static(self.h, C.byref(ms), n, _ptr(out, torch.complex128) if self.n_modes else C.c_void_p(0),
+                                            _stream(stream)), "trimeg_scatter_static")
         return out
 
     def sort(self, m: Dict[str, torch.Tensor], want_perm: bool = False, n: Optional[int] = None,

@@ -1286,6 +1286,7 @@ const char *trimeg_strerror(int code)
     case TRIMEG_ERR_CUDA: return "CUDA error";
     case TRIMEG_ERR_ALLOC: return "allocation failed";
     case TRIMEG_ERR_UNSUPPORTED: return "not defined for the loaded field's toroidal basis";
+    case TRIMEG_ERR_CAPACITY: return "problem larger than the static scratch of trimeg_scatter_static (TRIMEG_SCATTER_STATIC_BYTES): use trimeg_scatter";
     default: return "unknown error";
     }
 }

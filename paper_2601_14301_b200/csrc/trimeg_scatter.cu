@@ -15,6 +15,8 @@
 // divided among the lanes that share the modes.  (2) uses the same fixed right inverse and edge bubbles as the library's Bell
 // expansion (bell_kernel), transposed -- no linear solve.  (3) runs by vertex over a precomputed vertex -> triangle
 // adjacency: no atomics, and the result does not depend on the order of the triangles.
+#include <mutex>
+
 #include "trimeg_internal.h"
 #include "trimeg_mesh.cuh"
 #include "bell_tables.inc"
@@ -274,3 +276,84 @@ cudaError_t launch_scatter(trimeg_ctx *c, const trimeg_markers &m, size_t n, dou
 }
 
 }  // namespace trimeg
+
+// ------------------------------------------------------------------------------------ scatter without any allocation
+// trimeg_scatter_static (include/trimeg.h): the same kernels in the same order as launch_scatter, with ALL scratch -- the
+// histogram bins / cursors, the two int32 index arrays and the per-triangle results -- in one file-scope device array of
+// TRIMEG_SCATTER_STATIC_BYTES.  Every GPU that loads the library holds the array until the process exits.  In host code the
+// array's name is a host-side stand-in, not a device address: its address is fetched with cudaGetSymbolAddress once per
+// device, with that device current, and handed to the kernels as an ordinary pointer.
+namespace {
+
+static __device__ __align__(256) unsigned char g_scatter_static[TRIMEG_SCATTER_STATIC_BYTES];
+
+constexpr int SCS_MAX_DEVICES = 64;
+std::mutex g_scs_mutex;
+unsigned char *g_scs_addr[SCS_MAX_DEVICES];              // device address of g_scatter_static on device k, nullptr = not looked up yet
+
+inline size_t scs_align(size_t x) { return (x + 255) / 256 * 256; }
+
+}  // namespace
+
+extern "C" int trimeg_scatter_static(trimeg_ctx *c, const trimeg_markers *m, size_t n, void *rhs_dev, trimeg_stream stream)
+{
+    using namespace trimeg;
+    if (!c || n > 0x7fffffffULL) return TRIMEG_ERR_INVALID_ARG;
+    if (n > 0 && (!m || !m->R || !m->Z || !m->phi || !m->w || !m->cell)) return TRIMEG_ERR_INVALID_ARG;
+    if (!c->has_field) return TRIMEG_ERR_NO_FIELD;
+    if (c->field.n_phi > 0) return TRIMEG_ERR_UNSUPPORTED;
+    const int n_modes = c->field.n_modes;
+    if (n_modes == 0) return TRIMEG_OK;
+    if (!rhs_dev) return TRIMEG_ERR_INVALID_ARG;
+    // layout of the static array: bins | cell | perm | per-triangle results
+    const size_t off_cell = scs_align(sizeof(int) * ((size_t)c->n_tri + 8));
+    const size_t off_perm = off_cell + scs_align(sizeof(int32_t) * (n ? n : 1));
+    const size_t off_tri = off_perm + scs_align(sizeof(int32_t) * (n ? n : 1));
+    const size_t need = off_tri + sizeof(double2) * 18 * (size_t)c->n_tri * n_modes;
+    if (need > (size_t)TRIMEG_SCATTER_STATIC_BYTES) return TRIMEG_ERR_CAPACITY;
+    if (c->device < 0 || c->device >= SCS_MAX_DEVICES) return TRIMEG_ERR_CAPACITY;
+    int cur = -1;
+    if (cudaGetDevice(&cur) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_CUDA; }
+    if (cur != c->device && cudaSetDevice(c->device) != cudaSuccess) { cudaGetLastError(); return TRIMEG_ERR_CUDA; }
+    int rc = TRIMEG_OK;
+    unsigned char *base = nullptr;
+    {
+        std::lock_guard<std::mutex> lock(g_scs_mutex);
+        if (!g_scs_addr[c->device]) {                    // set-up, once per device, with that device current
+            void *p = nullptr;
+            if (cudaGetSymbolAddress(&p, g_scatter_static) != cudaSuccess || !p) { cudaGetLastError(); rc = TRIMEG_ERR_CUDA; }
+            else g_scs_addr[c->device] = (unsigned char *)p;
+        }
+        base = g_scs_addr[c->device];
+    }
+    if (rc == TRIMEG_OK) {
+        cudaStream_t s = (cudaStream_t)stream;
+        int *bins = (int *)base;
+        int32_t *cell = (int32_t *)(base + off_cell), *perm = (int32_t *)(base + off_perm);
+        double2 *tri_rhs = (double2 *)(base + off_tri);
+        // the array keeps the last call's contents: the bins must start at zero; cell, perm and the per-triangle results are
+        // written in full before they are read (scatter_moments_kernel writes every triangle's block, zeros for an empty one)
+        cudaError_t e = cudaMemsetAsync(bins, 0, sizeof(int) * ((size_t)c->n_tri + 2), s);
+        if (e == cudaSuccess) {
+            if (n > 0) {
+                const unsigned grid = (unsigned)((n + 255) / 256);
+                scatter_locate_kernel<<<grid, 256, 0, s>>>(c->mesh, n, m->R, m->Z, m->cell, cell);
+                scatter_hist_kernel<<<grid, 256, 0, s>>>(n, cell, c->n_tri, bins);
+                launch_scan(bins, c->n_tri + 1, s);
+                scatter_index_kernel<<<grid, 256, 0, s>>>(n, cell, c->n_tri, bins, perm);
+                c->n_launches += 4;
+            }
+            const double *nul = nullptr;
+            scatter_moments_kernel<<<c->n_tri, SC_THREADS, 0, s>>>(c->mesh, c->field, c->n_theta, c->d_tri, c->d_vR, c->d_vZ, n ? m->R : nul,
+                                                                  n ? m->Z : nul, n ? m->phi : nul, n ? m->w : nul, perm, bins, tri_rhs);
+            const size_t work = (size_t)n_modes * c->n_vert * 6;
+            scatter_assemble_kernel<<<(unsigned)((work + 255) / 256), 256, 0, s>>>(c->n_vert, n_modes, c->d_adj_off, c->d_adj, tri_rhs,
+                                                                                   (double2 *)rhs_dev);
+            c->n_launches += 2;
+            e = cudaGetLastError();
+        }
+        if (e != cudaSuccess) { cudaGetLastError(); rc = TRIMEG_ERR_CUDA; }
+    }
+    if (cur != c->device) cudaSetDevice(cur);
+    return rc;
+}
