@@ -19,7 +19,7 @@ struct Fld3 { FieldVal phi, as, ah; };
 __device__ __forceinline__ Rates rhs_point_em(const PhysDev &p, double R, double Z, double upar, double mu, double w, const Fld3 &F)
 {
     if (TRIMEG_HAS_EQTAB(p)) return rhs_from_eq<true>(p, eq_table(p.eq, R, Z), R, upar, mu, w, F.phi, F.as, F.ah);
-    if (p.eom_variant == 2) return rhs_point_reduced<true>(p, R, Z, upar, mu, w, F.phi, F.as, F.ah);   // row f4, A.19-A.29
+    if (TRIMEG_IS_REDUCED(p)) return rhs_point_reduced<true>(p, R, Z, upar, mu, w, F.phi, F.as, F.ah);   // row f4, A.19-A.29
     const double x = R - p.R0;
     const double s = fma(x, x, Z * Z);
     const double qb = fma(p.qs, s, p.q0);
@@ -147,16 +147,25 @@ __global__ void __launch_bounds__(256) pullback_kernel(MeshDev M, FieldDev F, co
 
 }  // namespace
 
+#ifdef TRIMEG_CORE_ONLY
+cudaError_t launch_rhs_em_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP, double *dU, double *dW,
+                               cudaStream_t s)
+#else
 cudaError_t launch_rhs_em(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP, double *dU, double *dW,
                           cudaStream_t s)
+#endif
 {
     if (n == 0) return cudaSuccess;
+#ifndef TRIMEG_CORE_ONLY
+    if (core_case(c)) return launch_rhs_em_core(c, m, n, dR, dZ, dP, dU, dW, s);   // the same kernel without the branches of row f4
+#endif
     rhs_em_kernel<<<(unsigned)((n + 127) / 128), 128, 0, s>>>(c->mesh, c->field, c->d_coef_aux[0], c->d_coef_aux[1], c->phys, m, n, dR, dZ, dP,
                                                              dU, dW);
     c->n_launches++;
     return cudaGetLastError();
 }
 
+#ifndef TRIMEG_CORE_ONLY
 cudaError_t launch_pullback(trimeg_ctx *c, const trimeg_markers &m, size_t n, cudaStream_t s)
 {
     if (n == 0 || c->d_coef_aux[1] == nullptr) return cudaSuccess;       // no dA^h: nothing to pull back
@@ -164,5 +173,7 @@ cudaError_t launch_pullback(trimeg_ctx *c, const trimeg_markers &m, size_t n, cu
     c->n_launches++;
     return cudaGetLastError();
 }
+
+#endif
 
 }  // namespace trimeg

@@ -124,5 +124,7 @@ constexpr size_t GATHER_LANE_MIN = 1 << 18;     // below, two more kernel launch
 cudaError_t launch_rhs_em(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP, double *dU, double *dW,
                           cudaStream_t s);
 cudaError_t launch_pullback(trimeg_ctx *c, const trimeg_markers &m, size_t n, cudaStream_t s);
+cudaError_t launch_rhs_em_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double *dR, double *dZ, double *dP, double *dU, double *dW,
+                               cudaStream_t s);
 
 }  // namespace trimeg
