@@ -1,6 +1,8 @@
 // trimeg_multi.cuh -- row a3 for P markers of ONE triangle per thread: every coefficient is loaded
-// once and feeds P Horner recurrences from a register (a warp-wide 16-byte
-// load costs the register-file write port as much as two DFMAs, so the loads per FMA must drop).
+// once and feeds P Horner recurrences from a register.  The many-mode push kernel ran on this form
+// until the lane pairs of trimeg_push_wcache.cu (one marker per lane and evaluation, two lanes on one
+// record) replaced it; it is kept as form A of the mode-loop study (modeloop_bench.cu,
+// profiles/r02_mode_loop.md) and is not part of libtrimeg.so any more.
 // The arithmetic of every marker (order of operations, fused multiply-adds) is that of
 // eval_quintic() / gather() in trimeg_device.cuh.
 #pragma once

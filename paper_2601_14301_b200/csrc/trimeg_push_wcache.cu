@@ -5,9 +5,9 @@
 // warps in lock-step (two block barriers per RK4 stage), so its latency-bound phases -- binning, scan, equations -- never
 // hide under the Horner loop of another warp: 30 % of its time.  The warp-autonomous kernel has no barrier but reads the
 // records through L1, which neither holds them all nor delivers them cheaply.  This kernel takes the warp-autonomous
-// schedule (every warp owns 32 P - SLACK markers for the whole call, groups them by triangle with ballots -- anew only at
-// a stage where one of them has changed its triangle, else the slots of the last stage stand --, evaluates P markers of
-// one triangle per lane, finishes and re-locates them) and gives the CTA's warps ONE shared,
+// schedule (every warp owns 32 P - SLACK markers for the whole call, groups them by triangle with ballots into evaluation
+// slots -- anew only at a stage where one of them has changed its triangle, else the slots of the last stage stand --,
+// evaluates the slots 32 at a time, one marker per lane, finishes and re-locates them) and gives the CTA's warps ONE shared,
 // insert-only hash table of records in shared memory:
 //   * the first warp that meets a triangle claims a bin (atomicCAS on the tag), copies the record (coefficients + geometry
 //     row) global -> shared with all its lanes, fences, and publishes it (state READY);
@@ -17,7 +17,7 @@
 //     (the bench fuses 10 steps per call: no barrier at all; meeting every step costs 4 %, every third step 2 %).
 // Everything else -- the arithmetic per marker, the locator rule, lost-marker handling -- is that of the other push kernels.
 #include "trimeg_internal.h"
-#include "trimeg_multi.cuh"
+#include "trimeg_lane.cuh"
 #include "trimeg_rk4.cuh"
 
 namespace trimeg {
@@ -98,9 +98,15 @@ __device__ __forceinline__ int wc_lookup(int tl, int lane, int *tag, volatile in
     return rec;
 }
 
+// Evaluation: P passes; in pass k lane l evaluates slot 32 k + l, one marker, in the two-phase form of trimeg_lane.cuh (2.21
+// cycles per FP64 instruction; two markers of one triangle per lane off one load per coefficient, the form of round 1 and
+// of trimeg_multi.cuh, cost 2.65).  Every group of slots (one triangle) starts at an even slot, so the lanes 2j, 2j+1 of a
+// pass read the same record: a warp-wide 16-byte shared-memory load whose addresses agree in such lane pairs costs 2
+// wavefronts of the data pipe instead of 4 (profiles/r02_mode_loop.md) -- per marker as much as one load for two markers.
+// zero: a run-time 0 the compiler cannot see through (trimeg_lane.cuh).
 template <int P, int WARPS, int SLACK>
 __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, FieldDev F, PhysDev Ph, trimeg_markers m, size_t n,
-                                                                    double dt, int nsteps, Stats *st, int nslot)
+                                                                    double dt, int nsteps, Stats *st, int nslot, int zero)
 {
     using Cfg = WCacheCfg<P, SLACK>;
     constexpr int NW = Cfg::NW, NE = Cfg::NE;
@@ -225,21 +231,23 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                     int rec = __shfl_sync(FULL, known, __ffs(rl) - 1);
                     if (rec == -1) rec = wc_lookup(tl, lane, tag, state, rec_of, counters, nslot, M, F, REC, rec_len, rec_stride, n_copied);
                     else if (rec == -2) rec = -1;
-                    const int room = (rec >= 0) ? NE - n_ev : 0;   // no record: the triangle's markers keep slot -1
+                    const int start = (n_ev + 1) & ~1;            // a group starts at an even slot (lane pairs read one record)
+                    const int room = (rec >= 0) ? NE - start : 0;  // no record: the triangle's markers keep slot -1
                     int count = 0;
 #pragma unroll
                     for (int p = 0; p < P; ++p) {
                         const bool mine = (t[p] == tl);
                         const unsigned mm = __ballot_sync(FULL, mine);
                         const int rank = count + __popc(mm & lt_mask);
-                        if (mine && rank < room) { slot[p] = n_ev + rank; recp[p] = rec; }
+                        if (mine && rank < room) { slot[p] = start + rank; recp[p] = rec; }
                         count += __popc(mm);
                         rem[p] &= ~mm;
                     }
                     count = min(count, room);
-                    const int padded = (count + P - 1) / P * P;
-                    if (lane < padded - count) ev_own[n_ev + count + lane] = -1;
-                    n_ev += padded;
+                    if (count > 0) {
+                        if (lane == 0 && start > n_ev) ev_own[n_ev] = -1;          // the padding slot in front of the group
+                        n_ev = start + count;
+                    }
                     ++nb;
                 }
 #pragma unroll
@@ -252,42 +260,28 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
             if (lane == 0) { TRIMEG_PHASE_CLOCK(0) ++n_stages; }
 
             // ------------------------------------------------------------ 2 + 3: batched evaluation, equations (slot role)
-            if (lane * P < n_ev) {
-                const int e0 = lane * P;
-                const double2 *recp0 = REC + (size_t)ev_rec[e0] * rec_stride;         // first slot of a group is real
-                int own[P];
-#pragma unroll
-                for (int p = 0; p < P; ++p) own[p] = ev_own[e0 + p];
-                TriGeom tg;
-                tg.t = cell[own[0]];
-                tg.v0 = recp0[rec_len]; tg.gx = recp0[rec_len + 1]; tg.ge = recp0[rec_len + 2];
-                const double2 v0 = tg.v0, gx = tg.gx, ge = tg.ge;
-                double xi[P], eta[P], phi[P], f[P], fx[P], fe[P], fp[P];
-#pragma unroll
-                for (int p = 0; p < P; ++p) {
-                    xi[p] = eta[p] = phi[p] = 0.0;
-                    if (own[p] >= 0) {                 // local coordinates exactly as bary_rn() (rule L2)
-                        const double dx = __dsub_rn(S[S_R * NW + own[p]], v0.x), dz = __dsub_rn(S[S_Z * NW + own[p]], v0.y);
-                        xi[p] = __dadd_rn(__dmul_rn(gx.x, dx), __dmul_rn(gx.y, dz));
-                        eta[p] = __dadd_rn(__dmul_rn(ge.x, dx), __dmul_rn(ge.y, dz));
-                        phi[p] = S[S_P * NW + own[p]];
-                    }
-                }
-                gather_multi<P, false>(F, recp0, xi, eta, phi, f, fx, fe, fp);
 #pragma unroll 1
-                for (int p = 0; p < P; ++p) {
-                    int q = -1;                                                      // select without dynamic register indexing
+            for (int pass = 0; pass < P; ++pass) {
+                const int e = 32 * pass + lane;
+                const int own1 = (e < n_ev) ? ev_own[e] : -1;
+                if (own1 >= 0) {
+                    const double2 *recp1 = REC + (size_t)ev_rec[e] * rec_stride;
+                    TriGeom tg;
+                    tg.t = cell[own1];
+                    tg.v0 = recp1[rec_len]; tg.gx = recp1[rec_len + 1]; tg.ge = recp1[rec_len + 2];
+                    // local coordinates exactly as bary_rn() (rule L2)
+                    const double dx = __dsub_rn(S[S_R * NW + own1], tg.v0.x), dz = __dsub_rn(S[S_Z * NW + own1], tg.v0.y);
+                    const double xi1 = __dadd_rn(__dmul_rn(tg.gx.x, dx), __dmul_rn(tg.gx.y, dz));
+                    const double eta1 = __dadd_rn(__dmul_rn(tg.ge.x, dx), __dmul_rn(tg.ge.y, dz));
+                    double f1, fx1, fe1, fp1;
+                    gather_lane_harmonic(F, recp1, xi1, eta1, S[S_P * NW + own1], zero, f1, fx1, fe1, fp1);
                     FieldVal fv;
-                    fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
-#pragma unroll
-                    for (int pp = 0; pp < P; ++pp)
-                        if (pp == p) {
-                            q = own[pp]; fv.f = f[pp]; fv.fphi = fp[pp];
-                            fv.fR = fma(gx.x, fx[pp], ge.x * fe[pp]);                // d/dR
-                            fv.fZ = fma(gx.y, fx[pp], ge.y * fe[pp]);                // d/dZ
-                        }
-                    if (q >= 0) advance(M, Ph, S, NW, cell, flags, q, stage, fv, dt, hdt, dt6, &tg);
+                    fv.f = f1; fv.fphi = fp1;
+                    fv.fR = fma(tg.gx.x, fx1, tg.ge.x * fe1);                    // d/dR
+                    fv.fZ = fma(tg.gx.y, fx1, tg.ge.y * fe1);                    // d/dZ
+                    advance(M, Ph, S, NW, cell, flags, own1, stage, fv, dt, hdt, dt6, &tg);
                 }
+                __syncwarp();
             }
             __syncwarp();
             if (lane == 0) { TRIMEG_PHASE_CLOCK(1) }
@@ -372,7 +366,7 @@ cudaError_t launch_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n, doub
     const size_t shm = fixed + (size_t)nslot * rec_bytes;
     const size_t per_cta = (size_t)Cfg::NW * WARPS;
     const size_t ctas = (n + per_cta - 1) / per_cta;
-    push_wcache_kernel<P, WARPS, SLACK><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats, nslot);
+    push_wcache_kernel<P, WARPS, SLACK><<<(unsigned)ctas, 32 * WARPS, shm, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats, nslot, 0);
     c->n_launches++;
     return cudaGetLastError();
 }
