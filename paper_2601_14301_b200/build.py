@@ -7,7 +7,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libtrimeg.so")
 SOURCES = ["trimeg_lib.cu", "trimeg_push.cu", "trimeg_push_wcache.cu", "trimeg_push_lane.cu", "trimeg_push_wcache_core.cu",
-           "trimeg_push_lane_core.cu", "trimeg_scatter.cu", "trimeg_em.cu", "trimeg_em_core.cu"]
+           "trimeg_push_lane_core.cu", "trimeg_push_lane_spline.cu", "trimeg_scatter.cu", "trimeg_em.cu", "trimeg_em_core.cu"]
 DEPS = SOURCES + ["trimeg_device.cuh", "trimeg_lane.cuh", "trimeg_rk4.cuh", "trimeg_internal.h", "trimeg_mesh.cuh", "bell_tables.inc", os.path.join("..", "..", "include", "trimeg.h")]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-ffp-contract=off", "-shared"]

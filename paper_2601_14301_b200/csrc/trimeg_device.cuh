@@ -33,8 +33,15 @@ constexpr double LOC_GAP_TOL = 1e-12;   // reading G31
 // A translation unit compiled with TRIMEG_CORE_ONLY (trimeg_push_*_core.cu) holds the hot kernels for the core case alone --
 // ring x sector mesh, harmonic field, rigorous equations -- without the branches of rows f3 / f4 (they cost 0.9 % of the push
 // although never taken: code size and register allocation); the launchers pick it when the context is in that case.
-#ifdef TRIMEG_CORE_ONLY
+// TRIMEG_SPLINE_ONLY (trimeg_push_lane_spline.cu): the same for row f3 -- ring x sector mesh, field on B-spline planes,
+// rigorous equations, analytic equilibrium (the general build of the lane kernel spills with row f4's branches in it).
+#if defined(TRIMEG_CORE_ONLY)
 #define TRIMEG_HAS_SPL(F) false
+#define TRIMEG_IS_REDUCED(p) false
+#define TRIMEG_IS_UNS(M) false
+#define TRIMEG_HAS_EQTAB(p) false
+#elif defined(TRIMEG_SPLINE_ONLY)
+#define TRIMEG_HAS_SPL(F) true
 #define TRIMEG_IS_REDUCED(p) false
 #define TRIMEG_IS_UNS(M) false
 #define TRIMEG_HAS_EQTAB(p) false

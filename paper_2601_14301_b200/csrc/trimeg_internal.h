@@ -110,9 +110,15 @@ cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, d
 // trimeg_push_*_core.cu: the same two kernels compiled without the branches of rows f3 / f4
 cudaError_t launch_push_wcache_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 cudaError_t launch_push_lane_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
+// trimeg_push_lane_spline.cu: the lane kernel for a B-spline field on the ring x sector mesh, rigorous equations, analytic equilibrium
+cudaError_t launch_push_lane_spline(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s);
 inline bool core_case(const trimeg_ctx *c)
 {
     return c->field.n_phi == 0 && c->params.eom_variant != 2 && c->mesh.n_r > 0 && c->phys.eq == nullptr;
+}
+inline bool spline_core_case(const trimeg_ctx *c)
+{
+    return c->field.n_phi > 0 && c->params.eom_variant != 2 && c->mesh.n_r > 0 && c->phys.eq == nullptr;
 }
 
 // trimeg_push_lane.cu: the gather alone for cell-sorted markers; gate / want: runs iff (*gate * 16 <= n) == want

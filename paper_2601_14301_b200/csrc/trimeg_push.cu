@@ -215,7 +215,9 @@ cudaError_t launch_push(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
     const int variant = effective_push_kernel(c);
-    if (variant == TRIMEG_PUSH_KERNEL_LANE) return core_case(c) ? launch_push_lane_core(c, m, n, dt, nsteps, s) : launch_push_lane(c, m, n, dt, nsteps, s);
+    if (variant == TRIMEG_PUSH_KERNEL_LANE)
+        return core_case(c) ? launch_push_lane_core(c, m, n, dt, nsteps, s)
+                            : spline_core_case(c) ? launch_push_lane_spline(c, m, n, dt, nsteps, s) : launch_push_lane(c, m, n, dt, nsteps, s);
     if (variant == TRIMEG_PUSH_KERNEL_WCACHE) return core_case(c) ? launch_push_wcache_core(c, m, n, dt, nsteps, s) : launch_push_wcache(c, m, n, dt, nsteps, s);
     push_kernel<<<grid_for(n, PUSH_BLOCK), PUSH_BLOCK, 0, s>>>(c->mesh, c->field, c->phys, m, n, dt, nsteps, c->d_stats);
     c->n_launches++;

@@ -447,7 +447,7 @@ cudaError_t launch_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double
 
 }  // namespace
 
-#ifndef TRIMEG_CORE_ONLY
+#if !defined(TRIMEG_CORE_ONLY) && !defined(TRIMEG_SPLINE_ONLY)
 cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const double *Z, const double *phi, const int32_t *hint,
                                double *f, double *fR, double *fZ, double *fP, const int *gate, int want, cudaStream_t s)
 {
@@ -471,8 +471,10 @@ cudaError_t launch_gather_lane(trimeg_ctx *c, size_t n, const double *R, const d
 
 #endif
 
-#ifdef TRIMEG_CORE_ONLY
+#if defined(TRIMEG_CORE_ONLY)
 cudaError_t launch_push_lane_core(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
+#elif defined(TRIMEG_SPLINE_ONLY)
+cudaError_t launch_push_lane_spline(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 #else
 cudaError_t launch_push_lane(trimeg_ctx *c, const trimeg_markers &m, size_t n, double dt, int nsteps, cudaStream_t s)
 #endif
