@@ -307,9 +307,10 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *         register operand per cycle); the coefficient records of the CTA's triangles sit in a shared,
  *         insert-only hash table in shared memory; 16 warps per CTA, one CTA per SM; no block barrier inside a 10-step call;
  *  TRIMEG_PUSH_KERNEL_WCACHE   every warp owns 59 markers, groups them by triangle with ballots (anew only at a stage where
- *         one of them has changed its triangle) into evaluation slots, and a lane evaluates 2 markers of one triangle off a
- *         single load of each coefficient -- from about eight modes on the shared-memory pipe cannot deliver a coefficient
- *         per marker; same record table; 12 warps per CTA.
+ *         one of them has changed its triangle) into 64 evaluation slots, every group starting at an even slot, and evaluates
+ *         32 slots per pass, one marker per lane in the same two phases: the lanes 2j, 2j+1 read one record, and a warp-wide
+ *         16-byte shared-memory load whose addresses agree in such pairs costs 2 wavefronts instead of 4 -- from about eight
+ *         modes on the shared-memory pipe cannot deliver a coefficient per marker at 4; same record table; 12 warps per CTA.
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX.  (Schedules of earlier rounds that lost everywhere were
  * removed: lock-step CTA tiles -- commit 3003ca4 --, warp kernels reading the records through L1 -- commit a10a1dc.) */
