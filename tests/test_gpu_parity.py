@@ -642,6 +642,32 @@ def test_push_many_modes_few_record_slots(B, inputs, variant):
     _assert_state_close(got, want, 1e-10, 1e-4)
 
 
+def test_schedules_agree_bit_for_bit_on_the_many_mode_config(B, inputs):
+    """The three schedules put every marker through the same operations in the same order (the
+    two-phase mode loop of trimeg_lane.cuh, the grouping and the lane pairs of the many-mode kernel change which lane
+    evaluates a marker and what its loads cost, not its arithmetic): on the cfg5 mesh with its 16 modes, cell-sorted
+    markers, 3 RK4 steps, the states are bit-identical."""
+    wl, o, ctx, _, _ = _setup(B, inputs, "cfg5")
+    assert ctx.get_push_kernel() == B.PUSH_KERNEL_WCACHE
+    m = inputs.markers(wl, n=40009)
+    results = []
+    for variant in (B.PUSH_KERNEL_THREAD, B.PUSH_KERNEL_LANE, B.PUSH_KERNEL_WCACHE):
+        ctx.set_push_kernel(variant)
+        d = _dev(B, m)
+        ctx.locate(d["R"], d["Z"], cell=d["cell"])
+        perm = ctx.sort(d, want_perm=True).cpu().numpy()    # the order inside a triangle follows an atomic cursor: undo it
+        ctx.push(d, wl.dt, 3)
+        h = _host(d)
+        back = {}
+        for k, v in h.items():
+            back[k] = np.empty_like(v)
+            back[k][perm] = v
+        results.append(back)
+    for other in results[1:]:
+        for k in ("R", "Z", "phi", "vpar", "w", "mu", "cell"):
+            assert np.array_equal(results[0][k], other[k]), k
+
+
 # ----------------------------------------------------------------------------- configs at their own sizes and step counts
 def test_cfg3_full_size_sampled_parity(B, inputs):
     """BASELINE.json configs[2] at full size: 2^26 markers (3.5 GB) in memory order as drawn (unsorted), automatic
