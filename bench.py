@@ -312,6 +312,9 @@ class PushRun:
         k = self.ctx.get_push_kernel()
         if self.n_phi and k == 1:
             return "push_lane_kernel<16> (B-spline plane records)"
+        core = not (self.n_phi or self.eom_variant == 2 or self.umesh is not None or getattr(self, "eq_tab", None) is not None)
+        if k == 2 and len(self.wl.modes) <= 14 and core:
+            return "push_wcache_kernel<2,16,5>"                    # TRIMEG_WCACHE_16_MAX_MODES, core build
         return PUSH_KERNEL_NAMES.get(k, "push kernel")
 
     def flops_unit(self):

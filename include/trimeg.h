@@ -299,7 +299,7 @@ int trimeg_compact(trimeg_ctx *ctx, trimeg_markers *m, size_t n, int64_t *perm_d
 int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nsteps,
                 trimeg_stream stream);
 /* Schedule used by trimeg_push / trimeg_push_host (same results, different kernels):
- *  TRIMEG_PUSH_KERNEL_AUTO (the default)  LANE for a field of up to 7 toroidal modes, WCACHE above;
+ *  TRIMEG_PUSH_KERNEL_AUTO (the default)  LANE for a field of up to 6 toroidal modes, WCACHE above;
  *  TRIMEG_PUSH_KERNEL_THREAD   one thread per marker, state in registers, coefficients through L1 (the plain schedule);
  *  TRIMEG_PUSH_KERNEL_LANE     lane-owned markers: every warp owns 64 markers, lane l the markers l and l + 32, for the
  *         whole call (state in shared memory; no grouping, no evaluation slots); one marker per evaluation in two phases
@@ -309,8 +309,9 @@ int trimeg_push(trimeg_ctx *ctx, trimeg_markers *m, size_t n, double dt, int nst
  *  TRIMEG_PUSH_KERNEL_WCACHE   every warp owns 59 markers, groups them by triangle with ballots (anew only at a stage where
  *         one of them has changed its triangle) into 64 evaluation slots, every group starting at an even slot, and evaluates
  *         32 slots per pass, one marker per lane in the same two phases: the lanes 2j, 2j+1 read one record, and a warp-wide
- *         16-byte shared-memory load whose addresses agree in such pairs costs 2 wavefronts instead of 4 -- from about eight
- *         modes on the shared-memory pipe cannot deliver a coefficient per marker at 4; same record table; 12 warps per CTA.
+ *         16-byte shared-memory load whose addresses agree in such pairs costs 2 wavefronts instead of 4 -- from about seven
+ *         modes on the shared-memory pipe cannot deliver a coefficient per marker at 4; same record table; 16 warps per CTA up to
+ *         14 modes (128 registers), 12 above (the larger records need the room).
  * Fastest when the markers are cell-sorted (trimeg_sort); any order is correct.
  * INVALID_ARG for a variant outside -1..TRIMEG_PUSH_KERNEL_MAX.  (Schedules of earlier rounds that lost everywhere were
  * removed: lock-step CTA tiles -- commit 3003ca4 --, warp kernels reading the records through L1 -- commit a10a1dc.) */

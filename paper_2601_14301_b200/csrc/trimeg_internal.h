@@ -8,8 +8,10 @@
 #include "trimeg_device.cuh"
 
 #ifndef TRIMEG_AUTO_SMALL_MAX_MODES
-#define TRIMEG_AUTO_SMALL_MAX_MODES 7
+#define TRIMEG_AUTO_SMALL_MAX_MODES 6
 #endif
+#define TRIMEG_WCACHE_16_MAX_MODES 14      /* many-mode kernel: 16 warps per CTA up to here, 12 above (trimeg_push_wcache.cu) */
+#define TRIMEG_GATHER_LANE_MAX_MODES 7     /* the gather alone: lane kernel for cell-sorted markers up to here */
 
 namespace trimeg {
 
@@ -65,10 +67,11 @@ namespace trimeg {
 
 // TRIMEG_PUSH_KERNEL_AUTO (measurements: DESIGN.md section 5).  Few toroidal modes: the per-stage work around the mode
 // loop (equations, locate, bookkeeping) weighs as much as the loop, and the kernel with lane-owned markers -- no grouping by
-// triangle, no evaluation slots, 16 warps per SM -- wins although it loads every coefficient once per marker.  From about
-// eight modes on the shared-memory pipe cannot deliver a coefficient per marker any more (a warp-wide 16-byte load is four
-// wavefronts), two markers of one triangle have to share each load, and the warp kernel with evaluation slots and the
-// CTA-shared record table wins (also beyond 26 modes, where only a dozen records fit).
+// triangle, no evaluation slots, 16 warps per SM -- wins although its loads cost twice the shared-memory wavefronts (markers
+// that have left their triangle sit at arbitrary lanes).  From seven modes on the shared-memory pipe cannot deliver a
+// coefficient per marker at that price, and the kernel that groups its markers by triangle (lane pairs on one record, the
+// CTA-shared record table) wins: with 16 warps while its records are small, with 12 from 15 modes on (also beyond 26 modes,
+// where only a dozen records fit).
 inline int auto_push_kernel(int n_modes)
 {
     return (n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES) ? TRIMEG_PUSH_KERNEL_LANE : TRIMEG_PUSH_KERNEL_WCACHE;

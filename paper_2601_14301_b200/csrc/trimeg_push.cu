@@ -173,7 +173,7 @@ cudaError_t launch_gather(trimeg_ctx *c, size_t n, const double *R, const double
 {
     if (n == 0) return cudaSuccess;
     int *gate = nullptr;
-    const bool two = hint && n >= GATHER_LANE_MIN && c->field.n_modes > 0 && c->field.n_modes <= TRIMEG_AUTO_SMALL_MAX_MODES;
+    const bool two = hint && n >= GATHER_LANE_MIN && c->field.n_modes > 0 && c->field.n_modes <= TRIMEG_GATHER_LANE_MAX_MODES;
     if (two) {
         // Large batches with hints: cell-sorted markers (hinted cells that never decrease; up to n / 16 exceptions are
         // tolerated) take the lane kernel (records in shared memory, inputs prefetched), anything else the thread-per-marker

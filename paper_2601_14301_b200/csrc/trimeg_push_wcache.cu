@@ -380,6 +380,13 @@ cudaError_t launch_push_wcache(trimeg_ctx *c, const trimeg_markers &m, size_t n,
 #endif
 {
     if (n == 0 || nsteps <= 0) return cudaSuccess;
+    // 16 warps at 128 registers while enough of the smaller records fit beside their state (cfg5 mesh, 2^24 markers, 12 / 16
+    // warps: 7 modes 3.29e9 / 3.43e9, 10 modes 2.62e9 / 2.70e9, 14 modes 2.05e9 / 2.07e9, 16 modes 1.843e9 / 1.839e9 -- 17
+    // record slots for 944 markers there, 2.6 times the markers without a slot)
+    // (the core build only: with the branches of rows f3 / f4 the kernel does not fit 128 registers without spilling)
+#ifdef TRIMEG_CORE_ONLY
+    if (c->field.n_modes <= TRIMEG_WCACHE_16_MAX_MODES) return launch_wcache<2, 16, 5>(c, m, n, dt, nsteps, s);
+#endif
     return launch_wcache<2, 12, 5>(c, m, n, dt, nsteps, s);
 }
 
