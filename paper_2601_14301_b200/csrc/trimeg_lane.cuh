@@ -120,10 +120,10 @@ __device__ __forceinline__ void gather_lane_impl(const FieldDev &F, const double
         m = 1; c += NCOEF;
     }
 #pragma unroll 1
-    for (; m < n_modes; ++m, c += NCOEF) {
-        if (!AP) { nn = (double)__ldg(F.mode_n + m); sincos(nn * phi, &Ei, &Er); }
+    for (int left = n_modes - m; left > 0; --left, c += NCOEF) {      // counts down: the loop test needs no bound from the constant bank
+        if (!AP) { nn = (double)__ldg(F.mode_n + (n_modes - left)); sincos(nn * phi, &Ei, &Er); }
         double pr, pi, pxr, pxi, per, pei;
-        eval_quintic_2ph(c, xi, eta, m + zero, pr, pi, pxr, pxi, per, pei);
+        eval_quintic_2ph(c, xi, eta, left + zero, pr, pi, pxr, pxi, per, pei);
         f = fma(pr, Er, fma(-pi, Ei, f));
         fx = fma(pxr, Er, fma(-pxi, Ei, fx));
         fe = fma(per, Er, fma(-pei, Ei, fe));
