@@ -174,6 +174,7 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
 #pragma unroll 1
         for (int stage = 0; stage < 4; ++stage) {
             // ------------------------------------------------------------ 1: grouping by triangle (home role) + record lookup
+            const int ps = (stage == 0) ? Y_R : S_R;   // stage 0 is evaluated at the start-of-step state itself (no copy Y -> S)
             int t[P];
             unsigned rem[P];
             bool same = true;
@@ -183,10 +184,6 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                 const bool act = (q < NW) && (flags[q] & FL_ACTIVE);
                 t[p] = act ? cell[q] : -1;
                 same = same && (t[p] == t_last[p]);
-                if (act && stage == 0) {
-#pragma unroll
-                    for (int k = 0; k < 5; ++k) S[(S_R + k) * NW + q] = S[(Y_R + k) * NW + q];
-                }
             }
             // no marker of the warp has changed its triangle since the last stage: the slots of that stage stand
             if (has_field && !__all_sync(FULL, same)) {
@@ -270,11 +267,11 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                     tg.t = cell[own1];
                     tg.v0 = recp1[rec_len]; tg.gx = recp1[rec_len + 1]; tg.ge = recp1[rec_len + 2];
                     // local coordinates exactly as bary_rn() (rule L2)
-                    const double dx = __dsub_rn(S[S_R * NW + own1], tg.v0.x), dz = __dsub_rn(S[S_Z * NW + own1], tg.v0.y);
+                    const double dx = __dsub_rn(S[(ps + 0) * NW + own1], tg.v0.x), dz = __dsub_rn(S[(ps + 1) * NW + own1], tg.v0.y);
                     const double xi1 = __dadd_rn(__dmul_rn(tg.gx.x, dx), __dmul_rn(tg.gx.y, dz));
                     const double eta1 = __dadd_rn(__dmul_rn(tg.ge.x, dx), __dmul_rn(tg.ge.y, dz));
                     double f1, fx1, fe1, fp1;
-                    gather_lane_harmonic(F, recp1, xi1, eta1, S[S_P * NW + own1], zero, f1, fx1, fe1, fp1);
+                    gather_lane_harmonic(F, recp1, xi1, eta1, S[(ps + 2) * NW + own1], zero, f1, fx1, fe1, fp1);
                     FieldVal fv;
                     fv.f = f1; fv.fphi = fp1;
                     fv.fR = fma(tg.gx.x, fx1, tg.ge.x * fe1);                    // d/dR
@@ -297,8 +294,8 @@ __global__ void __launch_bounds__(32 * WARPS, 1) push_wcache_kernel(MeshDev M, F
                 FieldVal fv;
                 fv.f = fv.fR = fv.fZ = fv.fphi = 0.0;
                 if (has_field) {
-                    const Bary b = bary_rn(M, tt, S[S_R * NW + q], S[S_Z * NW + q]);
-                    fv = gather(F, tt, b, S[S_P * NW + q]);
+                    const Bary b = bary_rn(M, tt, S[(ps + 0) * NW + q], S[(ps + 1) * NW + q]);
+                    fv = gather(F, tt, b, S[(ps + 2) * NW + q]);
                     ++n_fallback;
                 }
                 advance(M, Ph, S, NW, cell, flags, q, stage, fv, dt, hdt, dt6);
